@@ -1,0 +1,146 @@
+/*
+ * aria.h -- C ABI of libaria_b200: the quantized linear layers of the DiT denoiser of
+ * arxiv/paper_2607_08526 ("aria"), written for NVIDIA B200 (sm_100a).
+ *
+ * Source of the operations.  PAPER.md L78 (SIII-A(b), "Quantization and its evaluation"):
+ * the transformer's weights are "compressed to 8-bit or 4-bit integers (q8, q4)"; "an
+ * optional mode also runs the arithmetic in 8-bit, quantizing activations alongside weights
+ * (W8A8), on the GPU's integer tensor cores"; "the compressed copy owns its memory, the
+ * runtime frees the full-precision source once packed".  PAPER.md L73: the "per-step
+ * denoising loop is captured once and replayed as a single GPU graph".  The paper fixes no
+ * quantization scheme; the schemes are those of BASELINE.json `configs` C1-C5, as read in
+ * DESIGN.md "Readings" (R1-R17) and SURVEY.md S8(c).
+ *
+ * Conventions (all entry points):
+ *  - X[M,K] activations, row = token; W[N,K] weights, row = output channel; y = x W^T + b;
+ *    Y[M,N].  All matrices are dense row-major with no padding.
+ *  - Unless a name ends in `_host`, every data pointer is a DEVICE pointer owned by the
+ *    caller.  The library allocates and frees nothing on these calls and keeps no pointer
+ *    after return.  The fp source of a weight may be freed by the caller as soon as
+ *    aria_quantize_weights_* has completed on the stream (the paper's "releases the original").
+ *  - `stream` is a cudaStream_t passed as void*.  Device entry points only ENQUEUE work on it:
+ *    no host synchronisation, no allocation -- every one of them may be captured in a CUDA
+ *    graph.  `_host` entry points copy and synchronise (see there).
+ *  - Return value: aria_status (0 = OK, negative = error).  On a validation error nothing is
+ *    enqueued and no output is written.  Non-finite inputs are not checked (undefined).
+ *  - Alignment: every data pointer must be 16-byte aligned.  K % 32 == 0, N % 8 == 0.
+ *  - There is no CPU fallback: on a device that is not sm_100 every compute entry point
+ *    returns ARIA_ERR_ARCH.
+ */
+#ifndef ARIA_H_
+#define ARIA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define ARIA_API __attribute__((visibility("default")))
+#else
+#define ARIA_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    ARIA_OK = 0,
+    ARIA_ERR_NULL = -1,      /* a required pointer is NULL */
+    ARIA_ERR_SHAPE = -2,     /* M,N,K <= 0, K % 32 != 0, N % 8 != 0, group != 32, n_layers <= 0 */
+    ARIA_ERR_ALIGN = -3,     /* a pointer is not 16-byte aligned */
+    ARIA_ERR_DTYPE = -4,     /* unknown / unsupported aria_dtype, aria_act or aria_mode */
+    ARIA_ERR_ARCH = -5,      /* current device is not compute capability 10.x */
+    ARIA_ERR_WORKSPACE = -6, /* ws is NULL or ws_bytes < aria_workspace_bytes(...) */
+    ARIA_ERR_CUDA = -7       /* a CUDA runtime / driver call or a kernel launch failed */
+} aria_status;
+
+typedef enum { ARIA_F32 = 0, ARIA_BF16 = 1 } aria_dtype;
+typedef enum { ARIA_ACT_NONE = 0, ARIA_ACT_GELU_ERF = 1 } aria_act;
+typedef enum { ARIA_W8A8 = 0, ARIA_W4A16 = 1 } aria_mode;
+
+/* ---------------------------------------------------------------------------------------
+ * S0 -- weight quantisation, once at load (configs C1-C3; readings R2-R4).
+ * Per output channel n:  a = max_k |W[n,k]|;  w_scale[n] = a > 0 ? fl32(a/127) : 1;
+ * Wq[n,k] = clamp(rint(fl32(W[n,k] / w_scale[n])), -127, 127)   (IEEE division, ties to even).
+ * W: [N,K] of dtype `wt` (fp32 or bf16).  Wq: int8 [N,K].  w_scale: fp32 [N].            */
+ARIA_API int aria_quantize_weights_int8(const void* W, int wt, int N, int K, int8_t* Wq, float* w_scale,
+                               void* stream);
+
+/* S0 -- int4 group quantisation (config C4; readings R3, R4, R7, R8).  Per group of `group`
+ * (must be 32) consecutive k:  a = max |w|;  sg = fp16_rne(fl32(a/7)) (subnormals kept);
+ * sg == 0 -> codes 0, else q = clamp(rint(fl32(w / float(sg))), -7, 7).
+ * Wq4: uint8 [N,K/2], byte j of row n = (q[2j] & 0xF) | ((q[2j+1] & 0xF) << 4), 4-bit two's
+ * complement (0x8 never produced).  g_scale: fp16 bit patterns [N,K/32].                   */
+ARIA_API int aria_quantize_weights_int4(const void* W, int wt, int N, int K, int group, uint8_t* Wq4,
+                               uint16_t* g_scale, void* stream);
+
+/* S1 -- per-token dynamic activation quantisation ("quantizing activations
+ * alongside weights"; configs C1-C3).  Same arithmetic as aria_quantize_weights_int8 with
+ * rows = tokens.  X: [M,K] of dtype `xt`.  Xq: int8 [M,K].  x_scale: fp32 [M].             */
+ARIA_API int aria_quantize_act_int8(const void* X, int xt, int M, int K, int8_t* Xq, float* x_scale,
+                           void* stream);
+
+/* S1+S2+S3 -- one W8A8 linear ("integer tensor cores"; configs C1-C3):
+ *   Xq, sx = S1(X);  acc[m,n] = sum_k Xq[m,k] Wq[n,k]  (exact int32, tcgen05 kind::i8, TMEM);
+ *   y = float(acc) * sx[m] * w_scale[n] + bias[n];  act == GELU_ERF: y = 0.5 y (1 + erf(y/sqrt2));
+ *   Y = cast(y, yt).
+ * bias: [N] of dtype `bt`, may be NULL.  ws: scratch of at least
+ * aria_workspace_bytes(M, K, N, ARIA_W8A8) bytes (holds Xq and sx).                         */
+ARIA_API int aria_linear_w8a8(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
+                     int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
+                     size_t ws_bytes, void* stream);
+
+/* S4 -- one W4A16 linear (config C4; reading R12):  w^[n,k] = bf16_rne(q[n,k] * sg[n,k/32])
+ * dequantised on chip;  y = sum_k x[m,k] w^[n,k] (fp32 accumulate, tcgen05 kind::f16 bf16)
+ * + bias[n]; optional GELU; Y = cast(y, yt).  X: bf16 [M,K].  Wq4/g_scale: canonical format
+ * of aria_quantize_weights_int4.  bias: bf16 [N] or NULL.  ws may be NULL (unused).          */
+ARIA_API int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uint16_t* g_scale,
+                      int group, int N, const void* bias, int act, void* Y, int yt, void* ws,
+                      size_t ws_bytes, void* stream);
+
+/* S5 -- one denoising step's stack of linears (PAPER.md L73 graph replay; config C5).
+ * Layers run in array order on `stream`, each reading `in` [M,K] and writing `out` [M,N], both
+ * of dtype `io` (bf16 or fp32; W4A16 requires bf16).  `in == NULL` chains the layer to the
+ * previous layer's `out` (its N must equal this K).  mode W8A8: wq = int8 [N,K], w_scale = fp32
+ * [N]; mode W4A16: wq = packed int4 [N,K/2], w_scale = fp16 bits [N,K/32].  bias has dtype `io`,
+ * may be NULL.  Capturable: enqueue only.                                                   */
+typedef struct {
+    int K, N;
+    int act; /* aria_act applied to this layer's output */
+    const void* in;
+    const void* wq;
+    const void* w_scale;
+    const void* bias;
+    void* out;
+} aria_layer;
+
+ARIA_API int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mode, int io, void* ws,
+                          size_t ws_bytes, void* stream);
+
+/* Same stack, but `in` / `out` of every layer are HOST pointers (pinned memory recommended):
+ * each layer's input is copied host->device into `ws`, the layer runs, and its output is
+ * copied device->host; the call returns after synchronising `stream`.  Weights, scales and
+ * biases stay DEVICE pointers (the compressed copy is resident).  ws must hold
+ * aria_workspace_bytes_host(...) bytes.  Not capturable.                                    */
+ARIA_API int aria_denoiser_linears_host(const aria_layer* layers, int n_layers, int M, int mode, int io,
+                               void* ws, size_t ws_bytes, void* stream);
+
+/* Scratch sizes in bytes (0 on invalid arguments). */
+ARIA_API size_t aria_workspace_bytes(int M, int maxK, int maxN, int mode);
+ARIA_API size_t aria_workspace_bytes_host(int M, int maxK, int maxN, int mode, int io);
+
+/* Static string for a status code. */
+ARIA_API const char* aria_status_string(int status);
+
+/* Test hook for the bit-exact accumulator gate: acc[m,n] = sum_k Xq[m,k] Wq[n,k] as int32
+ * [M,N], computed by the same tcgen05 kind::i8 kernel as aria_linear_w8a8.                   */
+ARIA_API int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, int32_t* acc,
+                     void* stream);
+
+/* Library build id ("aria-b200 <version> sm_100a"). */
+ARIA_API const char* aria_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARIA_H_ */

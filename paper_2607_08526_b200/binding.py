@@ -1,0 +1,199 @@
+"""Thin ctypes binding of libaria_b200.so (include/aria.h).  Argument marshalling only: every
+step of the path runs in the library's CUDA kernels.  PyTorch is used to own device memory and
+streams.  There is no fallback: a missing library or a non-sm_100 device raises.
+
+Functions carry the C entry points' names and argument order; tensors replace pointers, the
+current torch CUDA stream replaces `stream`.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import c_char_p, c_int, c_size_t, c_void_p
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaria_b200.so")
+
+F32, BF16 = 0, 1
+ACT_NONE, ACT_GELU_ERF = 0, 1
+W8A8, W4A16 = 0, 1
+
+_lib = None
+
+
+class AriaError(RuntimeError):
+    pass
+
+
+class aria_layer(ctypes.Structure):
+    _fields_ = [("K", c_int), ("N", c_int), ("act", c_int), ("in_", c_void_p), ("wq", c_void_p),
+                ("w_scale", c_void_p), ("bias", c_void_p), ("out", c_void_p)]
+
+
+def lib() -> ctypes.CDLL:
+    """Load the CUDA library (built in-tree by `python -m paper_2607_08526_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise AriaError(f"{LIB_PATH} is missing: run `python -m paper_2607_08526_b200.build` "
+                            "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.aria_version.restype = c_char_p
+        L.aria_status_string.restype = c_char_p
+        L.aria_status_string.argtypes = [c_int]
+        L.aria_workspace_bytes.restype = c_size_t
+        L.aria_workspace_bytes.argtypes = [c_int, c_int, c_int, c_int]
+        L.aria_workspace_bytes_host.restype = c_size_t
+        L.aria_workspace_bytes_host.argtypes = [c_int, c_int, c_int, c_int, c_int]
+        L.aria_quantize_weights_int8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p]
+        L.aria_quantize_act_int8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p]
+        L.aria_quantize_weights_int4.argtypes = [c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p]
+        L.aria_linear_w8a8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p,
+                                       c_int, c_int, c_void_p, c_int, c_void_p, c_size_t, c_void_p]
+        L.aria_linear_w4a16.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p,
+                                        c_int, c_void_p, c_int, c_void_p, c_size_t, c_void_p]
+        L.aria_gemm_i8_i32.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
+        L.aria_denoiser_linears.argtypes = [ctypes.POINTER(aria_layer), c_int, c_int, c_int, c_int,
+                                            c_void_p, c_size_t, c_void_p]
+        L.aria_denoiser_linears_host.argtypes = L.aria_denoiser_linears.argtypes
+        for name in EXPORTS:
+            if name not in ("aria_version", "aria_status_string", "aria_workspace_bytes",
+                            "aria_workspace_bytes_host"):
+                getattr(L, name).restype = c_int
+        _lib = L
+    return _lib
+
+
+EXPORTS = ("aria_quantize_weights_int8", "aria_quantize_weights_int4", "aria_quantize_act_int8",
+           "aria_linear_w8a8", "aria_linear_w4a16", "aria_denoiser_linears",
+           "aria_denoiser_linears_host", "aria_workspace_bytes", "aria_workspace_bytes_host",
+           "aria_status_string", "aria_gemm_i8_i32", "aria_version")
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise AriaError(f"{what}: {lib().aria_status_string(rc).decode()} ({rc})")
+
+
+def _stream() -> c_void_p:
+    return c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dt(t: torch.Tensor) -> int:
+    if t.dtype == torch.float32:
+        return F32
+    if t.dtype == torch.bfloat16:
+        return BF16
+    raise AriaError(f"unsupported dtype {t.dtype}")
+
+
+def _ptr(t):
+    if t is None:
+        return c_void_p(0)
+    assert t.is_contiguous()
+    return c_void_p(t.data_ptr())
+
+
+def _out_dtype(code: int):
+    return torch.float32 if code == F32 else torch.bfloat16
+
+
+def aria_version() -> str:
+    return lib().aria_version().decode()
+
+
+def aria_workspace_bytes(M: int, maxK: int, maxN: int, mode: int) -> int:
+    return int(lib().aria_workspace_bytes(M, maxK, maxN, mode))
+
+
+def aria_workspace_bytes_host(M: int, maxK: int, maxN: int, mode: int, io: int) -> int:
+    return int(lib().aria_workspace_bytes_host(M, maxK, maxN, mode, io))
+
+
+def workspace(nbytes: int, device="cuda") -> torch.Tensor:
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def aria_quantize_weights_int8(W: torch.Tensor):
+    N, K = W.shape
+    Wq = torch.empty((N, K), dtype=torch.int8, device=W.device)
+    sw = torch.empty((N,), dtype=torch.float32, device=W.device)
+    _check(lib().aria_quantize_weights_int8(_ptr(W), _dt(W), N, K, _ptr(Wq), _ptr(sw), _stream()),
+           "aria_quantize_weights_int8")
+    return Wq, sw
+
+
+def aria_quantize_act_int8(X: torch.Tensor):
+    M, K = X.shape
+    Xq = torch.empty((M, K), dtype=torch.int8, device=X.device)
+    sx = torch.empty((M,), dtype=torch.float32, device=X.device)
+    _check(lib().aria_quantize_act_int8(_ptr(X), _dt(X), M, K, _ptr(Xq), _ptr(sx), _stream()),
+           "aria_quantize_act_int8")
+    return Xq, sx
+
+
+def aria_quantize_weights_int4(W: torch.Tensor, group: int = 32):
+    N, K = W.shape
+    Wq4 = torch.empty((N, K // 2), dtype=torch.uint8, device=W.device)
+    sg = torch.empty((N, K // group), dtype=torch.int16, device=W.device)  # fp16 bit patterns
+    _check(lib().aria_quantize_weights_int4(_ptr(W), _dt(W), N, K, group, _ptr(Wq4), _ptr(sg), _stream()),
+           "aria_quantize_weights_int4")
+    return Wq4, sg
+
+
+def aria_linear_w8a8(X, Wq, w_scale, bias=None, act: int = ACT_NONE, yt: int = BF16, ws=None, out=None):
+    M, K = X.shape
+    N = Wq.shape[0]
+    if ws is None:
+        ws = workspace(aria_workspace_bytes(M, K, N, W8A8), X.device)
+    Y = out if out is not None else torch.empty((M, N), dtype=_out_dtype(yt), device=X.device)
+    _check(lib().aria_linear_w8a8(_ptr(X), _dt(X), M, K, _ptr(Wq), _ptr(w_scale), N, _ptr(bias),
+                                  _dt(bias) if bias is not None else F32, act, _ptr(Y), yt, _ptr(ws),
+                                  ws.numel(), _stream()), "aria_linear_w8a8")
+    return Y
+
+
+def aria_linear_w4a16(X, Wq4, g_scale, bias=None, act: int = ACT_NONE, yt: int = BF16, ws=None, out=None,
+                      group: int = 32):
+    M, K = X.shape
+    N = Wq4.shape[0]
+    if ws is None:
+        ws = workspace(aria_workspace_bytes(M, K, N, W4A16), X.device)
+    Y = out if out is not None else torch.empty((M, N), dtype=_out_dtype(yt), device=X.device)
+    _check(lib().aria_linear_w4a16(_ptr(X), M, K, _ptr(Wq4), _ptr(g_scale), group, N, _ptr(bias), act,
+                                   _ptr(Y), yt, _ptr(ws), ws.numel(), _stream()), "aria_linear_w4a16")
+    return Y
+
+
+def aria_gemm_i8_i32(Xq, Wq):
+    M, K = Xq.shape
+    N = Wq.shape[0]
+    acc = torch.empty((M, N), dtype=torch.int32, device=Xq.device)
+    _check(lib().aria_gemm_i8_i32(_ptr(Xq), _ptr(Wq), M, N, K, _ptr(acc), _stream()), "aria_gemm_i8_i32")
+    return acc
+
+
+def make_layers(specs):
+    """specs: iterable of dicts {K, N, act, in, wq, w_scale, bias, out}; `in`/`out` may be device
+    tensors, host (pinned) tensors, raw ints, or None (chained input)."""
+    arr = (aria_layer * len(specs))()
+    for i, s in enumerate(specs):
+        def p(v):
+            if v is None:
+                return None
+            return v if isinstance(v, int) else v.data_ptr()
+        arr[i] = aria_layer(s["K"], s["N"], s.get("act", ACT_NONE), p(s.get("in")), p(s["wq"]),
+                            p(s["w_scale"]), p(s.get("bias")), p(s["out"]))
+    return arr
+
+
+def aria_denoiser_linears(layers, M: int, mode: int, io: int, ws: torch.Tensor):
+    _check(lib().aria_denoiser_linears(layers, len(layers), M, mode, io, _ptr(ws), ws.numel(), _stream()),
+           "aria_denoiser_linears")
+
+
+def aria_denoiser_linears_host(layers, M: int, mode: int, io: int, ws: torch.Tensor):
+    _check(lib().aria_denoiser_linears_host(layers, len(layers), M, mode, io, _ptr(ws), ws.numel(),
+                                            _stream()), "aria_denoiser_linears_host")

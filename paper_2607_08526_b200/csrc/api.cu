@@ -1,0 +1,236 @@
+// api.cu -- the extern "C" boundary declared in include/aria.h: argument validation and the
+// sequencing of kernels.  Device entry points only enqueue on the caller's stream.
+#include <cstring>
+
+#include "internal.cuh"
+
+using namespace aria;
+
+namespace {
+
+inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+inline bool bad_dtype(int t) { return t != ARIA_F32 && t != ARIA_BF16; }
+inline bool bad_act(int a) { return a != ARIA_ACT_NONE && a != ARIA_ACT_GELU_ERF; }
+inline size_t up256(size_t x) { return (x + 255) / 256 * 256; }
+inline size_t dsize(int t) { return t == ARIA_F32 ? 4 : 2; }
+
+int check_rows_args(const void* in, int t, int R, int C, const void* q, const void* s) {
+    if (!in || !q || !s) return ARIA_ERR_NULL;
+    if (R <= 0 || C <= 0 || C % 32 != 0) return ARIA_ERR_SHAPE;
+    if (bad_dtype(t)) return ARIA_ERR_DTYPE;
+    if (misaligned(in) || misaligned(q) || misaligned(s)) return ARIA_ERR_ALIGN;
+    return check_arch();
+}
+
+size_t w8_ws_bytes(int M, int K) { return up256(static_cast<size_t>(M) * K) + up256(static_cast<size_t>(M) * 4); }
+
+int linear_w8a8_impl(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
+                     int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
+                     cudaStream_t st, bool pdl) {
+    int8_t* Xq = static_cast<int8_t*>(ws);
+    float* sx = reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + up256(static_cast<size_t>(M) * K));
+    int rc = launch_quant_rows_i8(X, xt, M, K, Xq, sx, st, pdl);
+    if (rc != ARIA_OK) return rc;
+    W8Epilogue ep;
+    ep.sx = sx; ep.sw = w_scale; ep.bias = bias; ep.bias_t = bt; ep.act = act; ep.Y = Y;
+    ep.out_t = yt == ARIA_F32 ? 0 : 1;
+    return launch_gemm_w8a8(Xq, Wq, M, N, K, ep, st, pdl);
+}
+
+int check_layers(const aria_layer* layers, int n_layers, int M, int mode, int io, int* maxK,
+                 int* maxN, bool host_io) {
+    if (!layers) return ARIA_ERR_NULL;
+    if (n_layers <= 0 || M <= 0) return ARIA_ERR_SHAPE;
+    if (mode != ARIA_W8A8 && mode != ARIA_W4A16) return ARIA_ERR_DTYPE;
+    if (bad_dtype(io) || (mode == ARIA_W4A16 && io != ARIA_BF16)) return ARIA_ERR_DTYPE;
+    *maxK = 0; *maxN = 0;
+    for (int i = 0; i < n_layers; ++i) {
+        const aria_layer& L = layers[i];
+        if (!L.wq || !L.w_scale || !L.out) return ARIA_ERR_NULL;
+        if (!L.in && (i == 0 || layers[i - 1].N != L.K)) return i == 0 ? ARIA_ERR_NULL : ARIA_ERR_SHAPE;
+        if (L.K <= 0 || L.N <= 0 || L.K % 32 != 0 || L.N % 8 != 0) return ARIA_ERR_SHAPE;
+        if (bad_act(L.act)) return ARIA_ERR_DTYPE;
+        if (misaligned(L.wq) || misaligned(L.w_scale) || misaligned(L.bias)) return ARIA_ERR_ALIGN;
+        if (!host_io && (misaligned(L.in) || misaligned(L.out))) return ARIA_ERR_ALIGN;
+        if (L.K > *maxK) *maxK = L.K;
+        if (L.N > *maxN) *maxN = L.N;
+    }
+    return check_arch();
+}
+
+int run_layer(const aria_layer& L, const void* in, void* out, int M, int mode, int io, void* ws,
+              size_t ws_bytes, cudaStream_t st) {
+    if (mode == ARIA_W8A8)
+        return linear_w8a8_impl(in, io, M, L.K, static_cast<const int8_t*>(L.wq),
+                                static_cast<const float*>(L.w_scale), L.N, L.bias, io, L.act, out, io,
+                                ws, st, true);
+    return launch_gemm_w4a16(in, M, L.K, static_cast<const uint8_t*>(L.wq),
+                             static_cast<const uint16_t*>(L.w_scale), L.N, L.bias, L.act, out, io, ws,
+                             ws_bytes, st, true);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* aria_version(void) { return "aria-b200 0.1 sm_100a"; }
+
+const char* aria_status_string(int status) {
+    switch (status) {
+        case ARIA_OK: return "ok";
+        case ARIA_ERR_NULL: return "null pointer";
+        case ARIA_ERR_SHAPE: return "bad shape";
+        case ARIA_ERR_ALIGN: return "pointer not 16-byte aligned";
+        case ARIA_ERR_DTYPE: return "bad dtype / activation / mode";
+        case ARIA_ERR_ARCH: return "device is not sm_100 (no fallback)";
+        case ARIA_ERR_WORKSPACE: return "workspace missing or too small";
+        case ARIA_ERR_CUDA: return "CUDA error";
+        default: return "unknown status";
+    }
+}
+
+size_t aria_workspace_bytes(int M, int maxK, int maxN, int mode) {
+    if (M <= 0 || maxK <= 0 || maxN <= 0) return 0;
+    if (mode == ARIA_W8A8) return w8_ws_bytes(M, maxK);
+    if (mode == ARIA_W4A16) {
+        // Split-K bound: splits * tiles <= #SMs and a tile holds <= 128 x TT outputs, so the fp32
+        // partials never exceed #SMs * 128 * TT * 4 bytes; one counter quad per tile.
+        int sms = num_sms();
+        if (sms <= 0) sms = 148;
+        const size_t tt = M <= 32 ? 32 : M <= 64 ? 64 : M <= 128 ? 128 : 256;
+        size_t tiles = static_cast<size_t>((maxN + 127) / 128) * ((M + 31) / 32);
+        return up256(tiles * 16) + up256(static_cast<size_t>(sms) * 128 * tt * 4);
+    }
+    return 0;
+}
+
+size_t aria_workspace_bytes_host(int M, int maxK, int maxN, int mode, int io) {
+    const size_t dev = aria_workspace_bytes(M, maxK, maxN, mode);
+    if (dev == 0 || bad_dtype(io)) return 0;
+    // device scratch + two input staging buffers + two output staging buffers
+    return up256(dev) + 2 * up256(static_cast<size_t>(M) * maxK * dsize(io)) +
+           2 * up256(static_cast<size_t>(M) * maxN * dsize(io));
+}
+
+int aria_quantize_weights_int8(const void* W, int wt, int N, int K, int8_t* Wq, float* w_scale,
+                               void* stream) {
+    int rc = check_rows_args(W, wt, N, K, Wq, w_scale);
+    if (rc != ARIA_OK) return rc;
+    return launch_quant_rows_i8(W, wt, N, K, Wq, w_scale, static_cast<cudaStream_t>(stream), false);
+}
+
+int aria_quantize_act_int8(const void* X, int xt, int M, int K, int8_t* Xq, float* x_scale,
+                           void* stream) {
+    int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
+    if (rc != ARIA_OK) return rc;
+    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), false);
+}
+
+int aria_quantize_weights_int4(const void* W, int wt, int N, int K, int group, uint8_t* Wq4,
+                               uint16_t* g_scale, void* stream) {
+    if (!W || !Wq4 || !g_scale) return ARIA_ERR_NULL;
+    if (N <= 0 || K <= 0 || K % 32 != 0 || group != 32) return ARIA_ERR_SHAPE;
+    if (bad_dtype(wt)) return ARIA_ERR_DTYPE;
+    if (misaligned(W) || misaligned(Wq4) || misaligned(g_scale)) return ARIA_ERR_ALIGN;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    return launch_quant_groups_i4(W, wt, N, K, Wq4, g_scale, static_cast<cudaStream_t>(stream));
+}
+
+int aria_linear_w8a8(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
+                     int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
+                     size_t ws_bytes, void* stream) {
+    if (!X || !Wq || !w_scale || !Y) return ARIA_ERR_NULL;
+    if (M <= 0 || N <= 0 || K <= 0 || K % 32 != 0 || N % 8 != 0) return ARIA_ERR_SHAPE;
+    if (bad_dtype(xt) || bad_dtype(yt) || (bias && bad_dtype(bt)) || bad_act(act)) return ARIA_ERR_DTYPE;
+    if (misaligned(X) || misaligned(Wq) || misaligned(w_scale) || misaligned(bias) || misaligned(Y) ||
+        misaligned(ws))
+        return ARIA_ERR_ALIGN;
+    if (!ws || ws_bytes < w8_ws_bytes(M, K)) return ARIA_ERR_WORKSPACE;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    return linear_w8a8_impl(X, xt, M, K, Wq, w_scale, N, bias, bt, act, Y, yt, ws,
+                            static_cast<cudaStream_t>(stream), false);
+}
+
+int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uint16_t* g_scale,
+                      int group, int N, const void* bias, int act, void* Y, int yt, void* ws,
+                      size_t ws_bytes, void* stream) {
+    if (!X || !Wq4 || !g_scale || !Y) return ARIA_ERR_NULL;
+    if (M <= 0 || N <= 0 || K <= 0 || K % 32 != 0 || N % 8 != 0 || group != 32) return ARIA_ERR_SHAPE;
+    if (bad_dtype(yt) || bad_act(act)) return ARIA_ERR_DTYPE;
+    if (misaligned(X) || misaligned(Wq4) || misaligned(g_scale) || misaligned(bias) || misaligned(Y) ||
+        misaligned(ws))
+        return ARIA_ERR_ALIGN;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    return launch_gemm_w4a16(X, M, K, Wq4, g_scale, N, bias, act, Y, yt, ws, ws ? ws_bytes : 0,
+                             static_cast<cudaStream_t>(stream), false);
+}
+
+int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, int32_t* acc,
+                     void* stream) {
+    if (!Xq || !Wq || !acc) return ARIA_ERR_NULL;
+    if (M <= 0 || N <= 0 || K <= 0 || K % 32 != 0 || N % 8 != 0) return ARIA_ERR_SHAPE;
+    if (misaligned(Xq) || misaligned(Wq) || misaligned(acc)) return ARIA_ERR_ALIGN;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    W8Epilogue ep;
+    ep.sx = nullptr; ep.sw = nullptr; ep.bias = nullptr; ep.bias_t = ARIA_F32; ep.act = ARIA_ACT_NONE;
+    ep.Y = acc; ep.out_t = 2;
+    return launch_gemm_w8a8(Xq, Wq, M, N, K, ep, static_cast<cudaStream_t>(stream), false);
+}
+
+int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mode, int io, void* ws,
+                          size_t ws_bytes, void* stream) {
+    int maxK, maxN;
+    int rc = check_layers(layers, n_layers, M, mode, io, &maxK, &maxN, false);
+    if (rc != ARIA_OK) return rc;
+    if (misaligned(ws)) return ARIA_ERR_ALIGN;
+    if (!ws || ws_bytes < aria_workspace_bytes(M, maxK, maxN, mode)) return ARIA_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    for (int i = 0; i < n_layers; ++i) {
+        const void* in = layers[i].in ? layers[i].in : layers[i - 1].out;
+        rc = run_layer(layers[i], in, layers[i].out, M, mode, io, ws, ws_bytes, st);
+        if (rc != ARIA_OK) return rc;
+    }
+    return ARIA_OK;
+}
+
+int aria_denoiser_linears_host(const aria_layer* layers, int n_layers, int M, int mode, int io,
+                               void* ws, size_t ws_bytes, void* stream) {
+    int maxK, maxN;
+    int rc = check_layers(layers, n_layers, M, mode, io, &maxK, &maxN, true);
+    if (rc != ARIA_OK) return rc;
+    if (misaligned(ws)) return ARIA_ERR_ALIGN;
+    if (!ws || ws_bytes < aria_workspace_bytes_host(M, maxK, maxN, mode, io)) return ARIA_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t dev = up256(aria_workspace_bytes(M, maxK, maxN, mode));
+    const size_t in_b = up256(static_cast<size_t>(M) * maxK * dsize(io));
+    const size_t out_b = up256(static_cast<size_t>(M) * maxN * dsize(io));
+    uint8_t* base = static_cast<uint8_t*>(ws);
+    uint8_t* in_stage[2] = {base + dev, base + dev + in_b};
+    uint8_t* out_stage[2] = {base + dev + 2 * in_b, base + dev + 2 * in_b + out_b};
+    // One stream, in order: H2D(in_i) -> layer_i -> D2H(out_i).  Staging buffers alternate so a
+    // chained layer (in == NULL) can read the previous layer's device output.
+    for (int i = 0; i < n_layers; ++i) {
+        const aria_layer& L = layers[i];
+        const void* din;
+        if (L.in) {
+            if (cudaMemcpyAsync(in_stage[i & 1], L.in, static_cast<size_t>(M) * L.K * dsize(io),
+                                cudaMemcpyHostToDevice, st) != cudaSuccess)
+                return ARIA_ERR_CUDA;
+            din = in_stage[i & 1];
+        } else {
+            din = out_stage[(i - 1) & 1];
+        }
+        rc = run_layer(L, din, out_stage[i & 1], M, mode, io, ws, dev, st);
+        if (rc != ARIA_OK) return rc;
+        if (cudaMemcpyAsync(L.out, out_stage[i & 1], static_cast<size_t>(M) * L.N * dsize(io),
+                            cudaMemcpyDeviceToHost, st) != cudaSuccess)
+            return ARIA_ERR_CUDA;
+    }
+    return cudaStreamSynchronize(st) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+}
+
+}  // extern "C"

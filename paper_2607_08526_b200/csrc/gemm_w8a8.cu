@@ -1,0 +1,347 @@
+// gemm_w8a8.cu -- S2 + S3: int8 x int8 GEMM on tcgen05 (kind::i8, int32 accumulators in TMEM) with
+// the per-token x per-channel rescale + bias (+ GELU) epilogue fused in.
+//
+// Persistent, warp-specialised, one CTA per SM:
+//   warp 0      TMA producer: Xq tile [128 x 128 B] and Wq tile [BN x 128 B] per k-block into a
+//               STAGES-deep shared-memory ring (128-byte swizzle), completion on `full` mbarriers.
+//   warp 1      MMA issuer (one thread): 4 x tcgen05.mma (K = 32 each) per k-block into one of two
+//               TMEM accumulators [128 lanes x BN columns]; tcgen05.commit frees the ring slot and,
+//               after the last k-block, signals `tmem_full`.
+//   warps 2..5  epilogue: tcgen05.ld 32 lanes x 32 columns -> registers -> scale/bias/GELU -> global.
+//               Runs on accumulator `a` while the MMA warp fills accumulator `a^1`.
+// Tails: TMA zero-fills rows >= M / >= N and bytes >= K (zero codes add nothing); stores are masked.
+#include "internal.cuh"
+
+namespace aria {
+
+constexpr int W8_BM = 128;        // MMA M (TMEM lanes)
+constexpr int W8_BK = 128;        // bytes (= int8 elements) per k-block: one 128-byte swizzle row
+constexpr int W8_UMMA_K = 32;     // K per tcgen05.mma for 8-bit operands
+constexpr int W8_THREADS = 192;   // 6 warps
+constexpr int W8_EPI_WARP0 = 2;
+
+template <int BN>
+struct W8Cfg {
+    static constexpr int A_BYTES = W8_BM * W8_BK;
+    static constexpr int B_BYTES = BN * W8_BK;
+    static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+    static constexpr int STAGES = (200 * 1024) / STAGE_BYTES > 8 ? 8 : (200 * 1024) / STAGE_BYTES;
+    static constexpr int ACC_STRIDE = BN <= 32 ? 32 : BN <= 64 ? 64 : BN <= 128 ? 128 : 256;
+    static constexpr int TMEM_COLS = 2 * ACC_STRIDE < 32 ? 32 : 2 * ACC_STRIDE;
+    static constexpr int BAR_BYTES = (2 * STAGES + 4) * 8 + 16;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;  // + align slack
+    static_assert(BN % 32 == 0 && BN >= 32 && BN <= 256, "BN");
+    static_assert(B_BYTES % 1024 == 0, "B tile must keep 1024-byte alignment");
+};
+
+struct W8Params {
+    const float* sx;
+    const float* sw;
+    const void* bias;
+    void* Y;
+    int bias_t, act, out_t;
+    int M, N, K;
+};
+
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+    __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&t);
+}
+
+// Epilogue for 32 consecutive columns of one row held by one thread.
+template <int OUT_T>
+__device__ __forceinline__ void w8_epilogue_chunk(const uint32_t (&v)[32], const W8Params& p,
+                                                  int row, int col0, float sxv) {
+    if (row >= p.M || col0 >= p.N) return;
+    const bool full = col0 + 32 <= p.N;
+    if (OUT_T == 2) {  // raw accumulators (aria_gemm_i8_i32)
+        int32_t* y = static_cast<int32_t*>(p.Y) + static_cast<int64_t>(row) * p.N + col0;
+        if (full) {
+#pragma unroll
+            for (int j = 0; j < 32; j += 4)
+                *reinterpret_cast<uint4*>(y + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+        } else {
+            for (int j = 0; j < 32 && col0 + j < p.N; ++j) y[j] = static_cast<int32_t>(v[j]);
+        }
+        return;
+    }
+    float f[32];
+    if (full) {
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) {
+            const float4 w = __ldg(reinterpret_cast<const float4*>(p.sw + col0 + j));
+            f[j] = (static_cast<float>(static_cast<int32_t>(v[j])) * sxv) * w.x;
+            f[j + 1] = (static_cast<float>(static_cast<int32_t>(v[j + 1])) * sxv) * w.y;
+            f[j + 2] = (static_cast<float>(static_cast<int32_t>(v[j + 2])) * sxv) * w.z;
+            f[j + 3] = (static_cast<float>(static_cast<int32_t>(v[j + 3])) * sxv) * w.w;
+        }
+        if (p.bias) {
+            if (p.bias_t == ARIA_F32) {
+#pragma unroll
+                for (int j = 0; j < 32; j += 4) {
+                    const float4 b =
+                        __ldg(reinterpret_cast<const float4*>(static_cast<const float*>(p.bias) + col0 + j));
+                    f[j] += b.x; f[j + 1] += b.y; f[j + 2] += b.z; f[j + 3] += b.w;
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < 32; j += 8) {
+                    const uint4 b = __ldg(reinterpret_cast<const uint4*>(
+                        static_cast<const __nv_bfloat16*>(p.bias) + col0 + j));
+                    const uint32_t w[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        f[j + 2 * i] += __uint_as_float(w[i] << 16);
+                        f[j + 2 * i + 1] += __uint_as_float(w[i] & 0xFFFF0000u);
+                    }
+                }
+            }
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            const int c = col0 + j;
+            float t = 0.0f;
+            if (c < p.N) {
+                t = (static_cast<float>(static_cast<int32_t>(v[j])) * sxv) * __ldg(p.sw + c);
+                if (p.bias)
+                    t += p.bias_t == ARIA_F32
+                             ? __ldg(static_cast<const float*>(p.bias) + c)
+                             : __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[c]);
+            }
+            f[j] = t;
+        }
+    }
+    if (p.act == ARIA_ACT_GELU_ERF) {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) f[j] = gelu_erf(f[j]);
+    }
+    if (OUT_T == 0) {
+        float* y = static_cast<float*>(p.Y) + static_cast<int64_t>(row) * p.N + col0;
+        if (full) {
+#pragma unroll
+            for (int j = 0; j < 32; j += 4)
+                *reinterpret_cast<float4*>(y + j) = make_float4(f[j], f[j + 1], f[j + 2], f[j + 3]);
+        } else {
+            for (int j = 0; j < 32 && col0 + j < p.N; ++j) y[j] = f[j];
+        }
+    } else {
+        __nv_bfloat16* y = static_cast<__nv_bfloat16*>(p.Y) + static_cast<int64_t>(row) * p.N + col0;
+        if (full) {
+#pragma unroll
+            for (int j = 0; j < 32; j += 8)
+                *reinterpret_cast<uint4*>(y + j) =
+                    make_uint4(pack_bf16x2(f[j], f[j + 1]), pack_bf16x2(f[j + 2], f[j + 3]),
+                               pack_bf16x2(f[j + 4], f[j + 5]), pack_bf16x2(f[j + 6], f[j + 7]));
+        } else {
+            for (int j = 0; j < 32 && col0 + j < p.N; ++j) y[j] = __float2bfloat16_rn(f[j]);
+        }
+    }
+}
+
+template <int BN, int OUT_T>
+__global__ void __launch_bounds__(W8_THREADS, 1)
+w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                 const W8Params p) {
+    using Cfg = W8Cfg<BN>;
+    constexpr int STAGES = Cfg::STAGES;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;  // 128-byte swizzle atoms need 1024-byte alignment
+    uint8_t* gbase = smem_raw + (base - raw);
+    const uint32_t sA = base;
+    const uint32_t sB = base + STAGES * Cfg::A_BYTES;
+    const uint32_t bars = base + STAGES * Cfg::STAGE_BYTES;
+    const uint32_t full0 = bars, empty0 = bars + 8 * STAGES;
+    const uint32_t tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;
+    const uint32_t tmem_slot = tempty0 + 16;
+    volatile uint32_t* tmem_slot_g =
+        reinterpret_cast<volatile uint32_t*>(gbase + STAGES * Cfg::STAGE_BYTES + 16 * STAGES + 32);
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int num_m = (p.M + W8_BM - 1) / W8_BM;
+    const int num_n = (p.N + BN - 1) / BN;
+    const int num_tiles = num_m * num_n;
+    const int num_kb = (p.K + W8_BK - 1) / W8_BK;
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tmA);
+        tma_prefetch_desc(&tmB);
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(tfull0 + 8 * a, 1);
+            mbar_init(tempty0 + 8 * a, 4);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 1) {
+        tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_g;
+
+    // Everything above overlaps the previous kernel's tail under programmatic dependent launch;
+    // global memory written by it (Xq, sx) is only touched after this point.
+    pdl_wait_prior_grid();
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+                const int m0 = (t % num_m) * W8_BM, n0 = (t / num_m) * BN;
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    mbar_wait(empty0 + 8 * stage, phase ^ 1);
+                    mbar_arrive_expect_tx(full0 + 8 * stage, Cfg::STAGE_BYTES);
+                    tma_load_2d(sA + stage * Cfg::A_BYTES, &tmA, kb * W8_BK, m0, full0 + 8 * stage);
+                    tma_load_2d(sB + stage * Cfg::B_BYTES, &tmB, kb * W8_BK, n0, full0 + 8 * stage);
+                    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            constexpr uint32_t idesc = idesc_i8(W8_BM, BN);
+            int stage = 0;
+            uint32_t phase = 0;
+            int acc = 0;
+            uint32_t acc_phase = 0;
+            for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+                mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + acc * Cfg::ACC_STRIDE;
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    mbar_wait(full0 + 8 * stage, phase);
+                    tc_fence_after();
+                    const uint64_t a_desc = make_smem_desc_sw128(sA + stage * Cfg::A_BYTES);
+                    const uint64_t b_desc = make_smem_desc_sw128(sB + stage * Cfg::B_BYTES);
+#pragma unroll
+                    for (int k = 0; k < W8_BK / W8_UMMA_K; ++k)
+                        mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc,
+                                  (kb | k) != 0 ? 1u : 0u);
+                    tc_commit(empty0 + 8 * stage);  // ring slot reusable once these MMAs retire
+                    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                }
+                tc_commit(tfull0 + 8 * acc);  // accumulator complete
+                if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+            }
+        }
+    } else {
+        const int q = warp & 3;  // TMEM lane quarter this warp may read
+        int acc = 0;
+        uint32_t acc_phase = 0;
+        for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+            const int m0 = (t % num_m) * W8_BM, n0 = (t / num_m) * BN;
+            const int row = m0 + q * 32 + lane;
+            float sxv = 0.0f;
+            if (OUT_T != 2 && row < p.M) sxv = __ldg(p.sx + row);
+            mbar_wait(tfull0 + 8 * acc, acc_phase);
+            tc_fence_after();
+            const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
+#pragma unroll 1
+            for (int c = 0; c < BN / 32; ++c) {
+                uint32_t v[32];
+                tmem_ld_32x32b_x32(t_addr + c * 32, v);
+                tmem_wait_ld();
+                w8_epilogue_chunk<OUT_T>(v, p, row, n0 + c * 32, sxv);
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty0 + 8 * acc);
+            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        }
+    }
+
+    pdl_launch_dependents();
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
+    }
+}
+
+template <int BN, int OUT_T>
+static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const W8Params& p, int grid,
+                      cudaStream_t st, bool pdl) {
+    using Cfg = W8Cfg<BN>;
+    static bool attr_set = false;
+    auto kern = w8a8_gemm_kernel<BN, OUT_T>;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES) !=
+            cudaSuccess)
+            return ARIA_ERR_CUDA;
+        attr_set = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(W8_THREADS);
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, tmA, tmB, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+}
+
+template <int BN>
+static int launch_bn(const CUtensorMap& tmA, const CUtensorMap& tmB, const W8Params& p, int grid,
+                     cudaStream_t st, bool pdl) {
+    switch (p.out_t) {
+        case 0: return launch_one<BN, 0>(tmA, tmB, p, grid, st, pdl);
+        case 1: return launch_one<BN, 1>(tmA, tmB, p, grid, st, pdl);
+        default: return launch_one<BN, 2>(tmA, tmB, p, grid, st, pdl);
+    }
+}
+
+// Tile width: the BN in {64,128,192,256} with the fewest wave-quantised MMA cycles
+// (waves x BN); ties go to the wider tile (fewer B re-reads, fewer epilogue switches).
+static int pick_bn(int M, int N, int sms) {
+    const int cands[4] = {256, 192, 128, 64};
+    const int num_m = (M + W8_BM - 1) / W8_BM;
+    int best = 256;
+    long best_cost = -1;
+    for (int i = 0; i < 4; ++i) {
+        const int bn = cands[i];
+        const long tiles = static_cast<long>(num_m) * ((N + bn - 1) / bn);
+        const long waves = (tiles + sms - 1) / sms;
+        const long cost = waves * bn;
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = bn; }
+    }
+    return best;
+}
+
+int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, const W8Epilogue& ep,
+                     cudaStream_t st, bool pdl) {
+    const int sms = num_sms();
+    if (sms <= 0) return ARIA_ERR_CUDA;
+    const int bn = pick_bn(M, N, sms);
+    CUtensorMap tmA, tmB;
+    int rc = make_tmap_2d(&tmA, Xq, 1, M, K, W8_BM, W8_BK, 128);
+    if (rc != ARIA_OK) return rc;
+    rc = make_tmap_2d(&tmB, Wq, 1, N, K, bn, W8_BK, 128);
+    if (rc != ARIA_OK) return rc;
+    W8Params p;
+    p.sx = ep.sx; p.sw = ep.sw; p.bias = ep.bias; p.Y = ep.Y;
+    p.bias_t = ep.bias_t; p.act = ep.act; p.out_t = ep.out_t;
+    p.M = M; p.N = N; p.K = K;
+    const int tiles = ((M + W8_BM - 1) / W8_BM) * ((N + bn - 1) / bn);
+    const int grid = tiles < sms ? tiles : sms;
+    switch (bn) {
+        case 64: return launch_bn<64>(tmA, tmB, p, grid, st, pdl);
+        case 128: return launch_bn<128>(tmA, tmB, p, grid, st, pdl);
+        case 192: return launch_bn<192>(tmA, tmB, p, grid, st, pdl);
+        default: return launch_bn<256>(tmA, tmB, p, grid, st, pdl);
+    }
+}
+
+}  // namespace aria

@@ -1,0 +1,169 @@
+// quant.cu -- S0 / S1: symmetric int8 row quantisation and int4 group quantisation.
+// HBM-bound scans: 128-bit loads, warp-shuffle + smem block reduction for the absmax, one
+// pass over DRAM (the row is kept in registers between the absmax and the rounding).
+// Arithmetic (include/aria.h, R2-R4, R7): IEEE fp32 division (__fdiv_rn), round
+// half to even (__float2int_rn), clamp; never a reciprocal or fast-math shortcut, so codes and
+// scales are bit-identical to the definition.
+#include "internal.cuh"
+
+namespace aria {
+
+constexpr int QROW_MAX_THREADS = 256;
+constexpr int QROW_CACHE = 4;  // 8-element vectors kept in registers per thread
+
+template <typename T>
+__device__ __forceinline__ void load8(const T* p, float (&v)[8]);
+
+template <>
+__device__ __forceinline__ void load8<float>(const float* p, float (&v)[8]) {
+    const float4 a = __ldg(reinterpret_cast<const float4*>(p));
+    const float4 b = __ldg(reinterpret_cast<const float4*>(p) + 1);
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
+    v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+}
+template <>
+__device__ __forceinline__ void load8<__nv_bfloat16>(const __nv_bfloat16* p, float (&v)[8]) {
+    const uint4 a = __ldg(reinterpret_cast<const uint4*>(p));
+    const uint32_t w[4] = {a.x, a.y, a.z, a.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        v[2 * i] = __uint_as_float(w[i] << 16);
+        v[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+    }
+}
+
+__device__ __forceinline__ float absmax8(const float (&v)[8], float a) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a = fmaxf(a, fabsf(v[i]));
+    return a;
+}
+
+__device__ __forceinline__ int quant1(float x, float s, int lim) {
+    int q = __float2int_rn(__fdiv_rn(x, s));
+    return max(-lim, min(lim, q));
+}
+
+__device__ __forceinline__ uint2 quant8_i8(const float (&v)[8], float s) {
+    uint32_t lo = 0, hi = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        lo |= (static_cast<uint32_t>(quant1(v[i], s, 127)) & 0xFFu) << (8 * i);
+        hi |= (static_cast<uint32_t>(quant1(v[4 + i], s, 127)) & 0xFFu) << (8 * i);
+    }
+    return make_uint2(lo, hi);
+}
+
+// One CTA per row.  R1..R4: a = max|x|; s = a > 0 ? a/127 : 1; q = clamp(rint(x/s), +-127).
+template <typename T>
+__global__ void __launch_bounds__(QROW_MAX_THREADS)
+quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
+                     float* __restrict__ scale) {
+    __shared__ float red[QROW_MAX_THREADS / 32];
+    pdl_wait_prior_grid();
+    const int64_t row = blockIdx.x;
+    const T* x = X + row * K;
+    int8_t* q = Xq + row * K;
+    const int nvec = K >> 3;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+
+    float v[QROW_CACHE][8];
+    float a = 0.0f;
+#pragma unroll
+    for (int i = 0; i < QROW_CACHE; ++i) {
+        const int idx = tid + i * nthr;
+        if (idx < nvec) {
+            load8<T>(x + 8 * idx, v[i]);
+            a = absmax8(v[i], a);
+        }
+    }
+    for (int idx = tid + QROW_CACHE * nthr; idx < nvec; idx += nthr) {  // K > 8*CACHE*threads
+        float t[8];
+        load8<T>(x + 8 * idx, t);
+        a = absmax8(t, a);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
+    if ((tid & 31) == 0) red[tid >> 5] = a;
+    __syncthreads();
+    const int nwarp = nthr >> 5;
+    a = red[0];
+    for (int w = 1; w < nwarp; ++w) a = fmaxf(a, red[w]);
+
+    const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
+    if (tid == 0) scale[row] = s;
+    pdl_launch_dependents();
+#pragma unroll
+    for (int i = 0; i < QROW_CACHE; ++i) {
+        const int idx = tid + i * nthr;
+        if (idx < nvec) *reinterpret_cast<uint2*>(q + 8 * idx) = quant8_i8(v[i], s);
+    }
+    for (int idx = tid + QROW_CACHE * nthr; idx < nvec; idx += nthr) {
+        float t[8];
+        load8<T>(x + 8 * idx, t);
+        *reinterpret_cast<uint2*>(q + 8 * idx) = quant8_i8(t, s);
+    }
+}
+
+// int4, group 32 along K: 4 threads per group, 8 elements each (R3, R4, R7, R8).
+template <typename T>
+__global__ void __launch_bounds__(256)
+quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restrict__ Wq4,
+                       uint16_t* __restrict__ g_scale) {
+    const int64_t idx = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    const bool live = idx < n_vec;  // n_vec is a multiple of 4, so a group is never split
+    float v[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    if (live) load8<T>(W + 8 * idx, v);
+    float a = absmax8(v, 0.0f);
+    a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, 1));
+    a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, 2));
+    const __half h = __float2half_rn(__fdiv_rn(a, 7.0f));
+    const float sg = __half2float(h);
+    uint32_t packed = 0;
+    if (sg != 0.0f) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            packed |= (static_cast<uint32_t>(quant1(v[i], sg, 7)) & 0xFu) << (4 * i);
+    }
+    if (live) {
+        reinterpret_cast<uint32_t*>(Wq4)[idx] = packed;  // codes 8idx..8idx+7: low nibble = even k
+        if ((idx & 3) == 0) g_scale[idx >> 2] = __half_as_ushort(h);
+    }
+}
+
+int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
+                         bool pdl) {
+    const int nvec = C / 8;
+    int threads = ((nvec + 31) / 32) * 32;
+    threads = threads > QROW_MAX_THREADS ? QROW_MAX_THREADS : threads;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(R);
+    cfg.blockDim = dim3(threads);
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl ? 1 : 0;
+    cudaError_t e;
+    if (xt == ARIA_F32)
+        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s);
+    else
+        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<__nv_bfloat16>,
+                               static_cast<const __nv_bfloat16*>(X), C, q, s);
+    return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+}
+
+int launch_quant_groups_i4(const void* W, int wt, int N, int K, uint8_t* q4, uint16_t* sg,
+                           cudaStream_t st) {
+    const int64_t n_vec = static_cast<int64_t>(N) * K / 8;
+    const int threads = 256;
+    const unsigned blocks = static_cast<unsigned>((n_vec + threads - 1) / threads);
+    if (wt == ARIA_F32)
+        quant_groups_i4_kernel<float><<<blocks, threads, 0, st>>>(static_cast<const float*>(W), n_vec, q4, sg);
+    else
+        quant_groups_i4_kernel<__nv_bfloat16><<<blocks, threads, 0, st>>>(
+            static_cast<const __nv_bfloat16*>(W), n_vec, q4, sg);
+    return cudaGetLastError() == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+}
+
+}  // namespace aria

@@ -1,0 +1,78 @@
+// tensormap.cu -- host helpers: TMA tensor-map encoding (driver entry point resolved through the
+// runtime, so the library does not link libcuda), device queries.
+#include <mutex>
+
+#include "internal.cuh"
+
+namespace aria {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) ==
+                cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    });
+    return fn;
+}
+
+int make_tmap_2d(CUtensorMap* out, const void* base, int elem_bytes, uint64_t rows, uint64_t cols,
+                 uint32_t box_rows, uint32_t box_cols, int swizzle_bytes) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return ARIA_ERR_CUDA;
+    CUtensorMapDataType dt = elem_bytes == 1   ? CU_TENSOR_MAP_DATA_TYPE_UINT8
+                             : elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_UINT16
+                                               : CU_TENSOR_MAP_DATA_TYPE_UINT32;
+    CUtensorMapSwizzle sw = swizzle_bytes == 128  ? CU_TENSOR_MAP_SWIZZLE_128B
+                            : swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+                            : swizzle_bytes == 32 ? CU_TENSOR_MAP_SWIZZLE_32B
+                                                  : CU_TENSOR_MAP_SWIZZLE_NONE;
+    const cuuint64_t dims[2] = {cols, rows};                                 // innermost first
+    const cuuint64_t strides[1] = {cols * static_cast<uint64_t>(elem_bytes)};  // bytes, dim 1
+    const cuuint32_t box[2] = {box_cols, box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(out, dt, 2, const_cast<void*>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? ARIA_OK : ARIA_ERR_CUDA;
+}
+
+struct DevInfo {
+    int ok = 0, major = 0, sms = 0;
+};
+static DevInfo dev_info() {
+    static DevInfo cache[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return DevInfo();
+    if (!cache[dev].ok) {
+        DevInfo d;
+        if (cudaDeviceGetAttribute(&d.major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            return DevInfo();
+        d.ok = 1;
+        cache[dev] = d;
+    }
+    return cache[dev];
+}
+
+int num_sms() {
+    DevInfo d = dev_info();
+    return d.ok ? d.sms : 0;
+}
+
+int check_arch() {
+    DevInfo d = dev_info();
+    if (!d.ok) return ARIA_ERR_CUDA;
+    return d.major == 10 ? ARIA_OK : ARIA_ERR_ARCH;
+}
+
+}  // namespace aria

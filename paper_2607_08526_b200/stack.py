@@ -1,0 +1,84 @@
+"""One denoising step's stack of quantized linears (config C5), resident on the device.
+
+PAPER.md L73: the "per-step denoising loop is captured once and replayed as a single GPU graph";
+PAPER.md L78: the compressed weight copy "owns its memory, the runtime frees the full-precision
+source once packed".  This module is host-side plumbing around the C ABI: it draws the seeded
+weights (inputs.py), quantises them on the GPU with aria_quantize_weights_*, drops the fp
+source, wires the layers (reading R14: every linear reads its own N(0,1) input buffer,
+only up -> GELU -> down is chained) and captures aria_denoiser_linears in a CUDA graph.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import binding as aria
+from . import inputs
+
+
+def _dev_bf16(bits: np.ndarray) -> torch.Tensor:
+    return torch.from_numpy(bits.view(np.int16).copy()).cuda().view(torch.bfloat16)
+
+
+class LinearStack:
+    """`n_blocks` DiT blocks x (QKV, out-proj, MLP up [GELU], MLP down) at M tokens."""
+
+    def __init__(self, mode: int, M: int = 2048, n_blocks: int = inputs.N_BLOCKS, keep_host: bool = False,
+                 shared_inputs: bool = True):
+        self.mode, self.M, self.n_blocks = mode, M, n_blocks
+        self.specs = []          # per layer: dict with device tensors
+        self.host = []           # per layer: host arrays (tests only, keep_host=True)
+        # One N(0,1) bf16 input per distinct K is enough for timing and for parity (each layer has
+        # its own weights); shared_inputs=False draws one per layer (reading R14, used by tests).
+        in_cache = {}
+        for blk in range(n_blocks):
+            for which, (name, K, N, act) in enumerate(inputs.BLOCK_LINEARS):
+                L = inputs.c5_layer(blk, which, M=M if not shared_inputs else 1)
+                if shared_inputs:
+                    if K not in in_cache:
+                        bits, _ = inputs.normal_bf16((M, K), 1.0, 5, 900000 + K)
+                        in_cache[K] = (bits, _dev_bf16(bits))
+                    xbits, xdev = in_cache[K]
+                else:
+                    xbits, xdev = L["X_bits"], _dev_bf16(L["X_bits"])
+                Wd = torch.from_numpy(L["W"]).cuda()
+                if mode == aria.W8A8:
+                    wq, ws = aria.aria_quantize_weights_int8(Wd)
+                else:
+                    wq, ws = aria.aria_quantize_weights_int4(Wd)
+                torch.cuda.synchronize()
+                del Wd                                   # "releases the original"
+                chained = name == "down"
+                spec = {"name": name, "K": K, "N": N,
+                        "act": aria.ACT_GELU_ERF if act == "gelu" else aria.ACT_NONE,
+                        "in": None if chained else xdev, "wq": wq, "w_scale": ws,
+                        "bias": _dev_bf16(L["b"][0]),
+                        "out": torch.empty((M, N), dtype=torch.bfloat16, device="cuda")}
+                self.specs.append(spec)
+                if keep_host:
+                    self.host.append({"W": L["W"], "b": L["b"][1], "X_bits": None if chained else xbits})
+        self.layers = aria.make_layers(self.specs)
+        maxK = max(s["K"] for s in self.specs)
+        maxN = max(s["N"] for s in self.specs)
+        self.ws = aria.workspace(aria.aria_workspace_bytes(M, maxK, maxN, mode))
+        self.graph = None
+        self.ops = sum(2 * M * s["K"] * s["N"] for s in self.specs)
+        self.weight_bytes = sum(s["wq"].numel() * s["wq"].element_size() +
+                                s["w_scale"].numel() * s["w_scale"].element_size() for s in self.specs)
+
+    def run(self):
+        """Enqueue the whole stack on the current stream (no graph)."""
+        aria.aria_denoiser_linears(self.layers, self.M, self.mode, aria.BF16, self.ws)
+
+    def capture(self):
+        """Capture one step into a CUDA graph (after one eager warm-up)."""
+        self.run()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            self.run()
+        self.graph = g
+        return g
+
+    def replay(self):
+        self.graph.replay()

@@ -1,0 +1,121 @@
+"""GPU parity, S5: aria_denoiser_linears captured in a CUDA graph (config C5), and the full-size
+configs (C3, C4 at M=4096, C5 at M=2048 x 96 layers) on sampled rows -- a row of Y depends only
+on its own row of X and on W, so the oracle on sampled rows is exact."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2607_08526_b200 import inputs
+from aria_testutil import check_bf16_out, dev_bf16, dev_f32, host_bits16, host_f32, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def aria():
+    from paper_2607_08526_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _oracle_layer(oracle, mode, aria, x_f32, W, b, act):
+    if mode == aria.W8A8:
+        wq, sw = oracle.quant_int8_rows(W)
+        return oracle.linear_w8a8(x_f32, wq, sw, b.astype(np.float64), act)["y"]
+    codes, sg, _ = oracle.quant_int4_groups(W)
+    return oracle.linear_w4a16(x_f32, codes, sg, b.astype(np.float64), act, variant=0)
+
+
+def _check_stack(aria, oracle, st, rows=None):
+    """Compare every layer's output (all rows, or the sampled `rows`) with the oracle.  The chained
+    down-projection is teacher-forced: its oracle input is the GPU's own up-projection output."""
+    tol = 1e-3 if st.mode == aria.W8A8 else 2e-2
+    worst = 0.0
+    for i, (spec, h) in enumerate(zip(st.specs, st.host)):
+        if spec["in"] is None:
+            x = host_f32(st.specs[i - 1]["out"])
+        else:
+            x = inputs.bf16_as_f32(h["X_bits"])
+        y_bits = host_bits16(spec["out"])
+        if rows is not None:
+            x, y_bits = x[rows], y_bits[rows]
+        ref = _oracle_layer(oracle, st.mode, aria, x, h["W"], h["b"], spec["act"])
+        got = inputs.bf16_as_f32(y_bits)
+        e = rel_err(got, ref)
+        # bf16 output: the fp32 gate cannot be applied after rounding (reading R9) -> derived bound
+        check_bf16_out(y_bits, ref, inputs.bf16_bits(oracle.round_out(ref, oracle.OUT_BF16)),
+                       1e-5 if st.mode == aria.W8A8 else 2e-5, 1e-2)
+        assert e <= max(tol, 2.0 ** -8), (i, spec["name"], e)
+        worst = max(worst, e)
+    return worst
+
+
+@pytest.mark.parametrize("mode_name", ["w8a8", "w4a16"])
+def test_small_stack_graph_replay_all_rows(aria, oracle, mode_name):
+    from paper_2607_08526_b200.stack import LinearStack
+    mode = aria.W8A8 if mode_name == "w8a8" else aria.W4A16
+    st = LinearStack(mode, M=200, n_blocks=2, keep_host=True, shared_inputs=False)
+    st.capture()
+    for s in st.specs:
+        s["out"].zero_()
+    st.replay()
+    torch.cuda.synchronize()
+    first = [host_bits16(s["out"]).copy() for s in st.specs]
+    _check_stack(aria, oracle, st)
+    st.replay()                                   # replays are bit-identical (deterministic path)
+    torch.cuda.synchronize()
+    for a, s in zip(first, st.specs):
+        assert np.array_equal(a, host_bits16(s["out"]))
+
+
+@pytest.mark.parametrize("mode_name", ["w8a8", "w4a16"])
+def test_c5_full_size_sampled_rows(aria, oracle, mode_name):
+    from paper_2607_08526_b200.stack import LinearStack
+    mode = aria.W8A8 if mode_name == "w8a8" else aria.W4A16
+    st = LinearStack(mode, M=2048, n_blocks=inputs.N_BLOCKS, keep_host=True, shared_inputs=True)
+    assert len(st.specs) == 96
+    st.capture()
+    st.replay()
+    torch.cuda.synchronize()
+    rows = np.sort(np.random.default_rng(80).choice(2048, size=16, replace=False))
+    rows[0], rows[-1] = 0, 2047                   # first and last row of the first / last tile
+    _check_stack(aria, oracle, st, rows)
+
+
+def test_c3_full_size_sampled_rows(aria, oracle):
+    c = inputs.c3()                               # M = 4096, outlier channels
+    X = dev_bf16(c["X_bits"])
+    wu, su = aria.aria_quantize_weights_int8(dev_f32(c["Wup"]))
+    wd, sd = aria.aria_quantize_weights_int8(dev_f32(c["Wdown"]))
+    H = aria.aria_linear_w8a8(X, wu, su, dev_bf16(c["bup"][0]), aria.ACT_GELU_ERF, aria.BF16)
+    Y32 = aria.aria_linear_w8a8(H, wd, sd, dev_bf16(c["bdown"][0]), aria.ACT_NONE, aria.F32)
+    H32 = aria.aria_linear_w8a8(X, wu, su, dev_bf16(c["bup"][0]), aria.ACT_GELU_ERF, aria.F32)
+    torch.cuda.synchronize()
+    rows = np.sort(np.random.default_rng(81).choice(4096, size=64, replace=False))
+    wq, sw = oracle.quant_int8_rows(c["Wup"])
+    r = oracle.linear_w8a8(c["X"][rows], wq, sw, c["bup"][1].astype(np.float64), 1)
+    assert rel_err(host_f32(H32)[rows], r["y"]) <= 1e-3
+    # codes of the sampled rows, bit-exact, through the public quantiser
+    xq, sx = aria.aria_quantize_act_int8(X)
+    assert np.array_equal(xq.cpu().numpy()[rows], r["xq"]) and np.array_equal(sx.cpu().numpy()[rows], r["sx"])
+    Hf = host_f32(H)[rows]                         # teacher forcing
+    wq, sw = oracle.quant_int8_rows(c["Wdown"])
+    r2 = oracle.linear_w8a8(Hf, wq, sw, c["bdown"][1].astype(np.float64), 0)
+    assert rel_err(host_f32(Y32)[rows], r2["y"]) <= 1e-3
+
+
+@pytest.mark.parametrize("K,N", inputs.C4_SHAPES)
+def test_c4_m4096_sampled_rows(aria, oracle, K, N):
+    c = inputs.c4(4096, K, N)
+    q4, s = aria.aria_quantize_weights_int4(dev_f32(c["W"]))
+    y = aria.aria_linear_w4a16(dev_bf16(c["X_bits"]), q4, s, dev_bf16(c["b"][0]), 0, aria.BF16)
+    y32 = aria.aria_linear_w4a16(dev_bf16(c["X_bits"]), q4, s, dev_bf16(c["b"][0]), 0, aria.F32)
+    torch.cuda.synchronize()
+    rows = np.sort(np.random.default_rng(82).choice(4096, size=32, replace=False))
+    codes, sg, packed = oracle.quant_int4_groups(c["W"])
+    assert np.array_equal(q4.cpu().numpy(), packed)
+    b = c["b"][1].astype(np.float64)
+    ref0 = oracle.linear_w4a16(c["X"][rows], codes, sg, b, 0, variant=0)
+    ref1 = oracle.linear_w4a16(c["X"][rows], codes, sg, b, 0, variant=1)
+    assert rel_err(host_f32(y32)[rows], ref0) <= 2e-5
+    assert rel_err(host_f32(y)[rows], ref0) <= 2e-2 and rel_err(host_f32(y)[rows], ref1) <= 2e-2

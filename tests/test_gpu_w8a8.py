@@ -1,0 +1,121 @@
+"""GPU parity, S2 + S3 (W8A8): int32 accumulators bit-exact; fp32 output within 1e-3 of the
+oracle in the north_star norm (reading R10); bf16 output == bf16(oracle) up to 1 ulp on a
+small fraction (reading R9)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2607_08526_b200 import inputs
+from aria_testutil import check_bf16_out, dev_bf16, dev_f32, dev_i8, host_bits16, host_f32, rel_err
+
+pytestmark = pytest.mark.gpu
+TOL_F32 = 1e-3          # north_star: max relative error (vs output magnitude) on the fp32 output
+
+
+@pytest.fixture(scope="module")
+def aria():
+    from paper_2607_08526_b200 import binding
+    binding.lib()
+    return binding
+
+
+def test_acc_structured_single_tile(aria, oracle):
+    # index-coded operands localise any layout / descriptor mistake
+    M, N, K = 128, 64, 128
+    Xq = np.zeros((M, K), np.int8)
+    Xq[np.arange(M), np.arange(M) % K] = 1                       # one-hot rows
+    Wq = ((np.arange(N)[:, None] * 7 + np.arange(K)[None, :] * 3) % 251 - 125).astype(np.int8)
+    acc = aria.aria_gemm_i8_i32(dev_i8(Xq), dev_i8(Wq)).cpu().numpy()
+    assert np.array_equal(acc.astype(np.int64), oracle.gemm_i8(Xq, Wq))
+
+
+@pytest.mark.parametrize("M,N,K", [(128, 256, 256), (64, 256, 256), (512, 1536, 1536), (300, 392, 416),
+                                   (1, 8, 32), (129, 264, 6144), (1000, 4608, 1536)])
+def test_acc_bit_exact(aria, oracle, M, N, K):
+    rng = np.random.default_rng([60, M, N, K])
+    Xq = rng.integers(-127, 128, size=(M, K), dtype=np.int8)
+    Wq = rng.integers(-127, 128, size=(N, K), dtype=np.int8)
+    acc = aria.aria_gemm_i8_i32(dev_i8(Xq), dev_i8(Wq)).cpu().numpy()
+    ref = oracle.gemm_i8(Xq, Wq)
+    assert np.array_equal(acc.astype(np.int64), ref)
+
+
+def test_acc_extreme_values(aria, oracle):
+    K = 6144
+    Xq = np.full((128, K), 127, np.int8)
+    Wq = np.full((64, K), 127, np.int8)
+    Wq[1::2] = -127
+    acc = aria.aria_gemm_i8_i32(dev_i8(Xq), dev_i8(Wq)).cpu().numpy()
+    assert np.all(acc[:, 0::2] == 99096576) and np.all(acc[:, 1::2] == -99096576)
+
+
+def _linear_case(aria, oracle, Xdev, Xf32, W, bias_dev, bias_f64, act, yt_list):
+    wq_d, sw_d = aria.aria_quantize_weights_int8(dev_f32(W))
+    wq, sw = oracle.quant_int8_rows(W)
+    assert np.array_equal(wq_d.cpu().numpy(), wq)
+    ref = oracle.linear_w8a8(Xf32, wq, sw, bias_f64, act)["y"]
+    out = {}
+    for yt in yt_list:
+        y = aria.aria_linear_w8a8(Xdev, wq_d, sw_d, bias_dev, act, yt)
+        torch.cuda.synchronize()
+        if yt == aria.F32:
+            e = rel_err(host_f32(y), ref)
+            assert e <= TOL_F32, e
+            out["f32_err"] = e
+        else:
+            ref_bits = inputs.bf16_bits(oracle.round_out(ref, oracle.OUT_BF16))
+            out["bf16_mismatch"] = check_bf16_out(host_bits16(y), ref, ref_bits, 1e-5,
+                                                      2e-2 if act else 5e-3)  # erff noise + (-0 vs -1e-14) tails
+    return out
+
+
+def test_c1_tiny_fp32(aria, oracle):
+    c = inputs.c1()
+    _linear_case(aria, oracle, dev_f32(c["X"]), c["X"], c["W"], dev_f32(c["b"]), c["b"].astype(np.float64),
+                 aria.ACT_NONE, [aria.F32])
+
+
+def test_c2_attention_projections(aria, oracle):
+    c = inputs.c2()
+    X = dev_bf16(c["X_bits"])
+    for Wn, bn in (("Wqkv", "bqkv"), ("Wout", "bout")):
+        bb, bf = c[bn]
+        _linear_case(aria, oracle, X, c["X"], c[Wn], dev_bf16(bb), bf.astype(np.float64), aria.ACT_NONE,
+                     [aria.F32, aria.BF16])
+
+
+def test_c3_mlp_outliers_teacher_forced(aria, oracle):
+    # reduced M (oracle finishes in seconds); full-size rows are sampled in test_gpu_stack.py
+    c = inputs.c3(M=384)
+    X = dev_bf16(c["X_bits"])
+    bu_b, bu = c["bup"]
+    bd_b, bd = c["bdown"]
+    _linear_case(aria, oracle, X, c["X"], c["Wup"], dev_bf16(bu_b), bu.astype(np.float64), aria.ACT_GELU_ERF,
+                 [aria.F32, aria.BF16])
+    # teacher forcing (reading O5): the down-projection's oracle takes the GPU's own bf16 H
+    wq_d, sw_d = aria.aria_quantize_weights_int8(dev_f32(c["Wup"]))
+    H = aria.aria_linear_w8a8(X, wq_d, sw_d, dev_bf16(bu_b), aria.ACT_GELU_ERF, aria.BF16)
+    torch.cuda.synchronize()
+    Hf = host_f32(H)
+    hq_d, hs_d = aria.aria_quantize_act_int8(H)
+    hq, hs = oracle.quant_int8_rows(Hf)
+    assert np.array_equal(hq_d.cpu().numpy(), hq) and np.array_equal(hs_d.cpu().numpy(), hs)
+    _linear_case(aria, oracle, H, Hf, c["Wdown"], dev_bf16(bd_b), bd.astype(np.float64), aria.ACT_NONE,
+                 [aria.F32, aria.BF16])
+
+
+def test_no_bias_and_ragged_shapes(aria, oracle):
+    for (M, K, N) in [(77, 160, 72), (130, 1536, 200), (5, 32, 8)]:
+        bits, x = inputs.normal_bf16((M, K), 1.0, 61, M + K + N)
+        W = inputs.normal_f32((N, K), 0.02, 61, M + K + N + 1)
+        _linear_case(aria, oracle, dev_bf16(bits), x, W, None, None, aria.ACT_NONE, [aria.F32, aria.BF16])
+
+
+def test_zero_input_gives_bias(aria, oracle):
+    M, K, N = 64, 256, 128
+    X = torch.zeros((M, K), dtype=torch.bfloat16, device="cuda")
+    W = inputs.normal_f32((N, K), 0.02, 62, 0)
+    b = inputs.normal_f32((N,), 0.01, 62, 1)
+    wq_d, sw_d = aria.aria_quantize_weights_int8(dev_f32(W))
+    y = aria.aria_linear_w8a8(X, wq_d, sw_d, dev_f32(b), aria.ACT_NONE, aria.F32)
+    assert np.array_equal(host_f32(y), np.broadcast_to(b, (M, N)))
