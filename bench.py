@@ -1,0 +1,396 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the quantized DiT linear path on B200 (BASELINE.json metric).
+
+A STEP is one pass of the whole hot path over config C5: one denoising step's 96 linears
+(24 blocks x QKV / out-proj / MLP up+GELU / MLP down, M = 2048 tokens), replayed as a CUDA graph
+once in W8A8 mode (S1 activation quantisation + S2 int8 tcgen05 GEMM + S3 rescale/bias/GELU
+epilogue) and once in W4A16 mode (S4 on-chip int4 dequant + bf16 tcgen05 GEMM).  Weights are
+quantised once at load (S0) and are resident; inputs are resident for `value`, and come from /
+return to pinned HOST buffers through aria_denoiser_linears_host for `e2e`.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--no-per-linear]
+
+One JSON line on stdout (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "quantized DiT linear throughput: W8A8 int8 TOPS + W4A16 effective bf16 TFLOPS over one C5 denoising-step stack"
+UNIT = "Top/s"
+WORKLOAD = "C5: 24 blocks x (QKV 1536->4608, out 1536->1536, MLP 1536->6144->1536), M=2048, all-W8A8 then all-W4A16, CUDA-graph replay"
+NOMINAL_INT8_OVER_BF16 = 2.0     # B200_PROFILING.md: 4.5 POP/s int8 vs 2.25 PFLOP/s bf16, dense
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_burst": d["bf16_tflops"],
+                "bf16_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                   "--format=csv,noheader,nounits", "-lms", "100"],
+                                  stdout=self.f, stderr=subprocess.DEVNULL)
+
+    def stop(self):
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons = [], 0.0, set()
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(name)
+        busy = [c for c in sm if c > 0.5 * mx] or sm
+        return {"sm_mhz": statistics.median(busy) if busy else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------ reference arm (the oracle)
+def oracle_sample(rows: int):
+    """Time the oracle, as it stands, on block 0's four linears at `rows` tokens, both modes."""
+    from oracle import oracle as orc
+    from paper_2607_08526_b200 import inputs
+    orc.build()
+    ops, t = 0, 0.0
+    for which in range(4):
+        L = inputs.c5_layer(0, which, M=rows)
+        x, W, b = L["X"], L["W"], L["b"][1].astype(np.float64)
+        act = 1 if L["act"] == "gelu" else 0
+        wq, sw = orc.quant_int8_rows(W)                      # S0 is load-time: not timed
+        codes, sg, _ = orc.quant_int4_groups(W)
+        t0 = time.perf_counter()
+        y8 = orc.linear_w8a8(x, wq, sw, b, act)["y"]         # S1 + S2 + S3
+        orc.round_out(y8, orc.OUT_BF16)
+        y4 = orc.linear_w4a16(x, codes, sg, b, act, variant=0)  # S4
+        orc.round_out(y4, orc.OUT_BF16)
+        t += time.perf_counter() - t0
+        ops += 2 * (2 * rows * L["K"] * L["N"])
+    return ops, t, orc.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    rows = 128
+    for _ in range(args.warmup):
+        oracle_sample(8)
+    tot_ops, tot_t, cores = 0, 0.0, 1
+    for _ in range(args.steps):
+        ops, t, cores = oracle_sample(rows)
+        tot_ops += ops
+        tot_t += t
+    v = tot_ops / tot_t / 1e12
+    sample = f"per step: block 0's 4 linears at {rows} tokens, W8A8 (S1-S3) + W4A16 (S4), bf16 out"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64/f64",
+        "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------ our arm
+def time_region(torch, fn, iters):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(iters):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / iters      # ms per call
+
+
+def per_linear_table(torch, aria, inputs, pk):
+    """BASELINE metric per DiT linear: C2, C3 (W8A8) and the 9 C4 cases (W4A16), each launched from
+    a CUDA graph that cycles through enough distinct weight copies to exceed 2 x L2 (HBM-cold)."""
+    out = []
+    L2 = 126e6
+
+    def dev_bf16(bits):
+        return torch.from_numpy(bits.view(np.int16).copy()).cuda().view(torch.bfloat16)
+
+    def bench_case(name, mode, M, K, N, act):
+        bits, _ = inputs.normal_bf16((M, K), 1.0, 9, M + K + N)
+        X = dev_bf16(bits)
+        W = torch.from_numpy(inputs.normal_f32((N, K), inputs.W_STD, 9, M + K + N + 1)).cuda()
+        b = dev_bf16(inputs.normal_bf16((N,), inputs.B_STD, 9, M + K + N + 2)[0])
+        if mode == "w8a8":
+            wq, sc = aria.aria_quantize_weights_int8(W)
+            wbytes = N * K + 4 * N
+        else:
+            wq, sc = aria.aria_quantize_weights_int4(W)
+            wbytes = N * K // 2 + 2 * N * K // 32
+        del W
+        ncopy = max(2, int(2 * L2 // wbytes) + 1)
+        ncopy = min(ncopy, 64)
+        wqs = [wq.clone() for _ in range(ncopy)]
+        scs = [sc.clone() for _ in range(ncopy)]
+        Y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+        ws = aria.workspace(aria.aria_workspace_bytes(M, K, N, aria.W8A8 if mode == "w8a8" else aria.W4A16))
+
+        def launch_all():
+            for i in range(ncopy):
+                if mode == "w8a8":
+                    aria.aria_linear_w8a8(X, wqs[i], scs[i], b, act, aria.BF16, ws=ws, out=Y)
+                else:
+                    aria.aria_linear_w4a16(X, wqs[i], scs[i], b, act, aria.BF16, ws=ws, out=Y)
+        launch_all()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            launch_all()
+        g.replay()
+        ms = time_region(torch, g.replay, 5) / ncopy
+        ops = 2.0 * M * N * K
+        abytes = M * K * 2 + wbytes + 2 * N + M * N * 2          # X + weights(+scales) + bias + Y
+        tput = ops / (ms * 1e-3) / 1e12
+        peak_t = pk["bf16_burst"] * (NOMINAL_INT8_OVER_BF16 if mode == "w8a8" else 1.0)
+        t_roof = max(ops / (peak_t * 1e12), abytes / (pk["hbm_gbs"] * 1e9))
+        out.append({"case": name, "mode": mode, "M": M, "K": K, "N": N, "us": round(ms * 1e3, 2),
+                    "tput": round(tput, 1), "unit": "TOPS" if mode == "w8a8" else "eff_TFLOPS",
+                    "gbs": round(abytes / (ms * 1e-3) / 1e9, 1),
+                    "bound": "tensor" if ops / (peak_t * 1e12) >= abytes / (pk["hbm_gbs"] * 1e9) else "hbm",
+                    "roofline_frac": round(t_roof / (ms * 1e-3), 3)})
+        del wqs, scs
+
+    bench_case("C2 qkv", "w8a8", 512, 1536, 4608, aria.ACT_NONE)
+    bench_case("C2 out", "w8a8", 512, 1536, 1536, aria.ACT_NONE)
+    bench_case("C3 up+gelu", "w8a8", 4096, 1536, 6144, aria.ACT_GELU_ERF)
+    bench_case("C3 down", "w8a8", 4096, 6144, 1536, aria.ACT_NONE)
+    for M in inputs.C4_MS:
+        for (K, N) in inputs.C4_SHAPES:
+            bench_case(f"C4 M={M}", "w4a16", M, K, N, aria.ACT_NONE)
+    return out
+
+
+def run_ours(args):
+    import torch
+    from paper_2607_08526_b200 import binding as aria
+    from paper_2607_08526_b200 import inputs
+    from paper_2607_08526_b200.stack import LinearStack
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    aria.lib()
+    pk = peaks()
+    M = 2048
+    t_load = time.perf_counter()
+    st8 = LinearStack(aria.W8A8, M=M)
+    st4 = LinearStack(aria.W4A16, M=M)
+    st8.capture()
+    st4.capture()
+    torch.cuda.synchronize()
+    log(f"[bench] stacks built + captured in {time.perf_counter() - t_load:.1f}s "
+        f"(W8A8 {st8.weight_bytes / 1e6:.0f} MB, W4A16 {st4.weight_bytes / 1e6:.0f} MB resident)")
+
+    def step():
+        st8.replay()
+        st4.replay()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 1)]
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev[0].record()
+    for i in range(args.steps):
+        st8.replay()
+        ev[2 * i + 1].record()
+        st4.replay()
+        ev[2 * i + 2].record()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    t8 = sum(ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)) / args.steps
+    t4 = sum(ev[2 * i + 1].elapsed_time(ev[2 * i + 2]) for i in range(args.steps)) / args.steps
+    if dist:
+        t = torch.tensor([total_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_step = total_ms / args.steps
+    ops_step = st8.ops + st4.ops
+    value = world * ops_step / (ms_step * 1e-3) / 1e12
+
+    # ---- roofline of the dominant kernel: the W8A8 tcgen05 GEMM (S2+S3), launched alone for the
+    # same 96 layers on already-quantised activations, timed with CUDA events on its stream.
+    xq = {}
+    for K in {s["K"] for s in st8.specs}:
+        X = next((s["in"] for s in st8.specs if s["K"] == K and s["in"] is not None), None)
+        if X is None:
+            X = st8.specs[2]["out"]               # the MLP hidden state feeds the down-projection
+        xq[K] = aria.aria_quantize_act_int8(X)
+
+    def gemm_only():
+        for s in st8.specs:
+            q, sx = xq[s["K"]]
+            aria.aria_linear_w8a8_q(q, sx, s["wq"], s["w_scale"], s["bias"], s["act"], aria.BF16, out=s["out"])
+    gemm_only()
+    torch.cuda.synchronize()
+    gg = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(gg):
+        gemm_only()
+    for _ in range(3):
+        gg.replay()
+    g_ms = time_region(torch, gg.replay, args.steps)
+    n_l = len(st8.specs)
+    dur = g_ms * 1e-3 / n_l
+    ach = (st8.ops / n_l) / dur / 1e12
+    peak = pk["bf16_sustained"] * NOMINAL_INT8_OVER_BF16
+    roofline = {"kernel": "w8a8_gemm_kernel (tcgen05 kind::i8 + fused epilogue)", "bound": "tensor",
+                "achieved": ach, "peak": peak, "unit": "TOP/s", "frac": ach / peak,
+                "peak_source": f"{pk['source']} bf16 sustained x {NOMINAL_INT8_OVER_BF16:g} (nominal int8/bf16)",
+                "frac_of_burst": ach / (pk["bf16_burst"] * NOMINAL_INT8_OVER_BF16),
+                "frac_of_nominal_4500": ach / 4500.0, "avg_launch_us": dur * 1e6, "launches": n_l,
+                "traffic": None}
+
+    # ---- e2e: same step through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    try:
+        e2e = run_e2e(torch, aria, st8, st4, M, min(args.steps, 5), world)
+    except Exception as ex:                      # noqa: BLE001
+        log(f"[bench] e2e failed: {ex!r}")
+    clocks = sampler.stop() if sampler else None
+
+    if rank != 0:
+        return
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        ops, t, cores = oracle_sample(1024)
+        cpu = {"value": ops / t / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"block 0's 4 linears at 1024 of the 2048 tokens, both modes, {t:.1f} s"}
+    table = None
+    if world == 1 and not args.no_per_linear:
+        table = per_linear_table(torch, aria, inputs, pk)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int8xint8->int32 / int4->bf16xbf16->f32",
+        "data": "synthetic",
+        "config": {"workload": WORKLOAD, "tokens": M, "layers": n_l, "l2": "weights 680 MB + 382 MB per step exceed the 126 MB L2",
+                   "multi_gpu": "replicas only"},
+        "modes": {"w8a8": {"ms": t8, "tops": st8.ops / (t8 * 1e-3) / 1e12,
+                           "frac_int8_peak_sustained": st8.ops / (t8 * 1e-3) / 1e12 / peak},
+                  "w4a16": {"ms": t4, "eff_tflops": st4.ops / (t4 * 1e-3) / 1e12,
+                            "frac_bf16_peak_sustained": st4.ops / (t4 * 1e-3) / 1e12 / pk["bf16_sustained"]}},
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+        "gpu_launches": args.steps * (2 * n_l + n_l), "clocks": clocks, "per_linear": table,
+    }
+    print(json.dumps(line))
+
+
+def run_e2e(torch, aria, st8, st4, M, steps, world):
+    """aria_denoiser_linears_host: every layer's input comes from pinned host memory and every
+    layer's output goes back to pinned host memory inside the timed region."""
+    host_in = {}
+    outs = {}
+    results = {}
+    h2d = d2h = 0
+    for st, tag in ((st8, "w8a8"), (st4, "w4a16")):
+        specs = []
+        for s in st.specs:
+            K, N = s["K"], s["N"]
+            if s["in"] is not None and K not in host_in:
+                host_in[K] = s["in"].cpu().pin_memory()
+            if N not in outs:
+                outs[N] = torch.empty((M, N), dtype=torch.bfloat16).pin_memory()
+            d = dict(s)
+            d["in"] = host_in[K] if s["in"] is not None else None
+            d["out"] = outs[N]
+            specs.append(d)
+            h2d += (M * K * 2) if s["in"] is not None else 0
+            d2h += M * N * 2
+        layers = aria.make_layers(specs)
+        maxK = max(s["K"] for s in specs)
+        maxN = max(s["N"] for s in specs)
+        ws = aria.workspace(aria.aria_workspace_bytes_host(M, maxK, maxN, st.mode, aria.BF16))
+        results[tag] = (layers, ws, st.mode, specs)
+    def step():
+        for tag in ("w8a8", "w4a16"):
+            layers, ws, mode, _ = results[tag]
+            aria.aria_denoiser_linears_host(layers, M, mode, aria.BF16, ws)
+    step()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / steps
+    ops = st8.ops + st4.ops
+    return {"value": world * ops / (ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": ms, "steps": steps,
+            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+            "api": "aria_denoiser_linears_host (pinned host in/out per layer, weights resident)"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-per-linear", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

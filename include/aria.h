@@ -90,6 +90,13 @@ ARIA_API int aria_linear_w8a8(const void* X, int xt, int M, int K, const int8_t*
                      int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
                      size_t ws_bytes, void* stream);
 
+/* S2+S3 only -- the same linear for activations that are ALREADY quantised (a producer that
+ * emitted int8 codes, or a caller reusing one S1 pass for several linears of the same input):
+ * Xq int8 [M,K] and x_scale fp32 [M] as produced by aria_quantize_act_int8.  No workspace.     */
+ARIA_API int aria_linear_w8a8_q(const int8_t* Xq, const float* x_scale, int M, int K, const int8_t* Wq,
+                       const float* w_scale, int N, const void* bias, int bt, int act, void* Y,
+                       int yt, void* stream);
+
 /* S4 -- one W4A16 linear (config C4; reading R12):  w^[n,k] = bf16_rne(q[n,k] * sg[n,k/32])
  * dequantised on chip;  y = sum_k x[m,k] w^[n,k] (fp32 accumulate, tcgen05 kind::f16 bf16)
  * + bias[n]; optional GELU; Y = cast(y, yt).  X: bf16 [M,K].  Wq4/g_scale: canonical format

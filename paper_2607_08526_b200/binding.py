@@ -52,6 +52,8 @@ def lib() -> ctypes.CDLL:
         L.aria_quantize_weights_int4.argtypes = [c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p]
         L.aria_linear_w8a8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p,
                                        c_int, c_int, c_void_p, c_int, c_void_p, c_size_t, c_void_p]
+        L.aria_linear_w8a8_q.argtypes = [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p,
+                                         c_int, c_int, c_void_p, c_int, c_void_p]
         L.aria_linear_w4a16.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p,
                                         c_int, c_void_p, c_int, c_void_p, c_size_t, c_void_p]
         L.aria_gemm_i8_i32.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
@@ -66,7 +68,7 @@ def lib() -> ctypes.CDLL:
     return _lib
 
 
-EXPORTS = ("aria_quantize_weights_int8", "aria_quantize_weights_int4", "aria_quantize_act_int8",
+EXPORTS = ("aria_linear_w8a8_q", "aria_quantize_weights_int8", "aria_quantize_weights_int4", "aria_quantize_act_int8",
            "aria_linear_w8a8", "aria_linear_w4a16", "aria_denoiser_linears",
            "aria_denoiser_linears_host", "aria_workspace_bytes", "aria_workspace_bytes_host",
            "aria_status_string", "aria_gemm_i8_i32", "aria_version")
@@ -152,6 +154,16 @@ def aria_linear_w8a8(X, Wq, w_scale, bias=None, act: int = ACT_NONE, yt: int = B
     _check(lib().aria_linear_w8a8(_ptr(X), _dt(X), M, K, _ptr(Wq), _ptr(w_scale), N, _ptr(bias),
                                   _dt(bias) if bias is not None else F32, act, _ptr(Y), yt, _ptr(ws),
                                   ws.numel(), _stream()), "aria_linear_w8a8")
+    return Y
+
+
+def aria_linear_w8a8_q(Xq, x_scale, Wq, w_scale, bias=None, act: int = ACT_NONE, yt: int = BF16, out=None):
+    M, K = Xq.shape
+    N = Wq.shape[0]
+    Y = out if out is not None else torch.empty((M, N), dtype=_out_dtype(yt), device=Xq.device)
+    _check(lib().aria_linear_w8a8_q(_ptr(Xq), _ptr(x_scale), M, K, _ptr(Wq), _ptr(w_scale), N, _ptr(bias),
+                                    _dt(bias) if bias is not None else F32, act, _ptr(Y), yt, _stream()),
+           "aria_linear_w8a8_q")
     return Y
 
 

@@ -153,6 +153,23 @@ int aria_linear_w8a8(const void* X, int xt, int M, int K, const int8_t* Wq, cons
                             static_cast<cudaStream_t>(stream), false);
 }
 
+int aria_linear_w8a8_q(const int8_t* Xq, const float* x_scale, int M, int K, const int8_t* Wq,
+                       const float* w_scale, int N, const void* bias, int bt, int act, void* Y,
+                       int yt, void* stream) {
+    if (!Xq || !x_scale || !Wq || !w_scale || !Y) return ARIA_ERR_NULL;
+    if (M <= 0 || N <= 0 || K <= 0 || K % 32 != 0 || N % 8 != 0) return ARIA_ERR_SHAPE;
+    if (bad_dtype(yt) || (bias && bad_dtype(bt)) || bad_act(act)) return ARIA_ERR_DTYPE;
+    if (misaligned(Xq) || misaligned(x_scale) || misaligned(Wq) || misaligned(w_scale) ||
+        misaligned(bias) || misaligned(Y))
+        return ARIA_ERR_ALIGN;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    W8Epilogue ep;
+    ep.sx = x_scale; ep.sw = w_scale; ep.bias = bias; ep.bias_t = bt; ep.act = act; ep.Y = Y;
+    ep.out_t = yt == ARIA_F32 ? 0 : 1;
+    return launch_gemm_w8a8(Xq, Wq, M, N, K, ep, static_cast<cudaStream_t>(stream), false);
+}
+
 int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uint16_t* g_scale,
                       int group, int N, const void* bias, int act, void* Y, int yt, void* ws,
                       size_t ws_bytes, void* stream) {

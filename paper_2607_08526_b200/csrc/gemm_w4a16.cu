@@ -30,6 +30,7 @@ constexpr int W4_BN = 128;      // output channels per tile = MMA M
 constexpr int W4_THREADS = 448;
 constexpr int W4_DEQ_WARP0 = 6;
 constexpr int W4_DEQ_THREADS = 256;
+constexpr int W4_DEQ_WARPS = W4_DEQ_THREADS / 32;
 
 template <int TT, int BK>
 struct W4Cfg {
@@ -157,10 +158,10 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         tma_prefetch_desc(&tmX);
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(full0 + 8 * s, 1);
-            mbar_init(empty0 + 8 * s, W4_DEQ_THREADS + 1);  // dequantisers (packed) + MMA commit (X)
+            mbar_init(empty0 + 8 * s, W4_DEQ_WARPS + 1);  // dequantiser warps (packed) + MMA commit (X)
         }
         for (int a = 0; a < NA; ++a) {
-            mbar_init(afull0 + 8 * a, W4_DEQ_THREADS);
+            mbar_init(afull0 + 8 * a, W4_DEQ_WARPS);
             mbar_init(aempty0 + 8 * a, 1);
         }
         for (int a = 0; a < 2; ++a) {
@@ -269,7 +270,6 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                     const uint32_t off = r * Cfg::P_ROW + (par + 2 * i) * 16;
                     pk[i] = lds128(ps + (off ^ (((off >> 7) & SWM) << 4)));
                 }
-                mbar_arrive(empty0 + 8 * stage);           // packed bytes are in registers
                 mbar_wait(aempty0 + 8 * ab, aphase ^ 1);   // MMAs that read this A buffer retired
                 const uint32_t as = sA + ab * Cfg::A_BYTES;
 #pragma unroll
@@ -285,7 +285,11 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                     }
                 }
                 fence_proxy_async_smem();                  // generic-proxy writes -> async proxy (MMA)
-                mbar_arrive(afull0 + 8 * ab);
+                __syncwarp();
+                if (lane == 0) {                           // one arrival per warp, not per thread
+                    mbar_arrive(afull0 + 8 * ab);
+                    mbar_arrive(empty0 + 8 * stage);       // packed bytes consumed
+                }
                 if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 if (++ab == NA) { ab = 0; aphase ^= 1; }
             }
@@ -348,13 +352,22 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 if (old == static_cast<unsigned>(S - 1)) {
                     __threadfence();
                     const int tmax = min(TT, p.M - t0);
-                    for (int j = 0; j < tmax; ++j) {
-                        const int64_t idx = static_cast<int64_t>(t0 + j) * p.N + n;
-                        if (n_ok) {
-                            float y = 0.0f;
-                            for (int s = 0; s < S; ++s)
-                                y += __ldcg(p.partials + static_cast<int64_t>(s) * p.M * p.N + idx);
-                            w4_store(p.Y, p.out_t, idx, w4_finish(y + bv, p.act));
+                    const int64_t sstride = static_cast<int64_t>(p.M) * p.N;
+                    for (int j0 = 0; j0 < tmax; j0 += 8) {   // 8 tokens x S loads in flight
+                        float y[8];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) y[j] = 0.0f;
+                        for (int s = 0; s < S; ++s) {        // fixed split order: deterministic sum
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) {
+                                const int64_t idx = static_cast<int64_t>(t0 + j0 + j) * p.N + n;
+                                if (n_ok && j0 + j < tmax) y[j] += __ldcg(p.partials + s * sstride + idx);
+                            }
+                        }
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const int64_t idx = static_cast<int64_t>(t0 + j0 + j) * p.N + n;
+                            if (n_ok && j0 + j < tmax) w4_store(p.Y, p.out_t, idx, w4_finish(y[j] + bv, p.act));
                         }
                     }
                     if (lane == 0) p.counters[tile * 4 + q] = 0;  // ready for the next launch

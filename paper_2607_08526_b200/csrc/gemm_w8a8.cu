@@ -7,9 +7,12 @@
 //   warp 1      MMA issuer (one thread): 4 x tcgen05.mma (K = 32 each) per k-block into one of two
 //               TMEM accumulators [128 lanes x BN columns]; tcgen05.commit frees the ring slot and,
 //               after the last k-block, signals `tmem_full`.
-//   warps 2..5  epilogue: tcgen05.ld 32 lanes x 32 columns -> registers -> scale/bias/GELU -> global.
-//               Runs on accumulator `a` while the MMA warp fills accumulator `a^1`.
-// Tails: TMA zero-fills rows >= M / >= N and bytes >= K (zero codes add nothing); stores are masked.
+//   warps 2..9  epilogue (two warps per TMEM lane quarter): tcgen05.ld 32 lanes x 32 columns ->
+//               registers -> x sx[m] x sw[n] + b[n] (scales/bias staged in smem per tile) -> GELU ->
+//               cast -> 64-byte-swizzled smem block -> TMA store.  Runs on accumulator `a` while the
+//               MMA warp fills accumulator `a^1`.
+// Tails: TMA zero-fills rows >= M / >= N and bytes >= K on load (zero codes add nothing) and clips
+// them on store.
 #include "internal.cuh"
 
 namespace aria {
@@ -17,8 +20,9 @@ namespace aria {
 constexpr int W8_BM = 128;        // MMA M (TMEM lanes)
 constexpr int W8_BK = 128;        // bytes (= int8 elements) per k-block: one 128-byte swizzle row
 constexpr int W8_UMMA_K = 32;     // K per tcgen05.mma for 8-bit operands
-constexpr int W8_THREADS = 192;   // 6 warps
-constexpr int W8_EPI_WARP0 = 2;
+constexpr int W8_EPI_WARPS = 8;   // two warps per TMEM lane quarter, interleaved over column chunks
+constexpr int W8_THREADS = 64 + 32 * W8_EPI_WARPS;
+constexpr int W8_STG_BYTES = 2048;  // per-warp output staging: 32 rows x 64 bytes (64-byte swizzle)
 
 template <int BN>
 struct W8Cfg {
@@ -28,18 +32,22 @@ struct W8Cfg {
     static constexpr int STAGES = (200 * 1024) / STAGE_BYTES > 8 ? 8 : (200 * 1024) / STAGE_BYTES;
     static constexpr int ACC_STRIDE = BN <= 32 ? 32 : BN <= 64 ? 64 : BN <= 128 ? 128 : 256;
     static constexpr int TMEM_COLS = 2 * ACC_STRIDE < 32 ? 32 : 2 * ACC_STRIDE;
+    static constexpr int RING_BYTES = STAGES * STAGE_BYTES;
+    static constexpr int STG_OFF = RING_BYTES;                               // [8][2 KB] staging
+    static constexpr int SWB_OFF = STG_OFF + W8_EPI_WARPS * W8_STG_BYTES;    // float sw[BN], bias[BN]
+    static constexpr int BAR_OFF = SWB_OFF + 2 * BN * 4;
     static constexpr int BAR_BYTES = (2 * STAGES + 4) * 8 + 16;
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;  // + align slack
+    static constexpr int SMEM_BYTES = BAR_OFF + BAR_BYTES + 1024;            // + alignment slack
     static_assert(BN % 32 == 0 && BN >= 32 && BN <= 256, "BN");
     static_assert(B_BYTES % 1024 == 0, "B tile must keep 1024-byte alignment");
+    static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
 struct W8Params {
     const float* sx;
     const float* sw;
     const void* bias;
-    void* Y;
-    int bias_t, act, out_t;
+    int bias_t, act;
     int M, N, K;
 };
 
@@ -47,102 +55,36 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
     __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
     return *reinterpret_cast<uint32_t*>(&t);
 }
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d)
+                 : "memory");
+}
 
-// Epilogue for 32 consecutive columns of one row held by one thread.
-template <int OUT_T>
-__device__ __forceinline__ void w8_epilogue_chunk(const uint32_t (&v)[32], const W8Params& p,
-                                                  int row, int col0, float sxv) {
-    if (row >= p.M || col0 >= p.N) return;
-    const bool full = col0 + 32 <= p.N;
-    if (OUT_T == 2) {  // raw accumulators (aria_gemm_i8_i32)
-        int32_t* y = static_cast<int32_t*>(p.Y) + static_cast<int64_t>(row) * p.N + col0;
-        if (full) {
+// Stage one warp's [32 rows x 64 bytes] block (thread = row, w[16] = its 64 bytes) in the 64-byte
+// swizzle the output tensor map expects, and hand it to the TMA store engine.  TMA clips rows >= M
+// and columns >= N, so tails need no masking.
+__device__ __forceinline__ void w8_store_block(const CUtensorMap* tmY, uint32_t stg, int lane,
+                                               const uint32_t (&w)[16], int col0, int row0) {
+    if (lane == 0) tma_store_wait_read<0>();  // the previous store has finished reading `stg`
+    __syncwarp();
+    const uint32_t rowb = stg + lane * 64;
+    const uint32_t x = (lane >> 1) & 3;
 #pragma unroll
-            for (int j = 0; j < 32; j += 4)
-                *reinterpret_cast<uint4*>(y + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
-        } else {
-            for (int j = 0; j < 32 && col0 + j < p.N; ++j) y[j] = static_cast<int32_t>(v[j]);
-        }
-        return;
-    }
-    float f[32];
-    if (full) {
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-            const float4 w = __ldg(reinterpret_cast<const float4*>(p.sw + col0 + j));
-            f[j] = (static_cast<float>(static_cast<int32_t>(v[j])) * sxv) * w.x;
-            f[j + 1] = (static_cast<float>(static_cast<int32_t>(v[j + 1])) * sxv) * w.y;
-            f[j + 2] = (static_cast<float>(static_cast<int32_t>(v[j + 2])) * sxv) * w.z;
-            f[j + 3] = (static_cast<float>(static_cast<int32_t>(v[j + 3])) * sxv) * w.w;
-        }
-        if (p.bias) {
-            if (p.bias_t == ARIA_F32) {
-#pragma unroll
-                for (int j = 0; j < 32; j += 4) {
-                    const float4 b =
-                        __ldg(reinterpret_cast<const float4*>(static_cast<const float*>(p.bias) + col0 + j));
-                    f[j] += b.x; f[j + 1] += b.y; f[j + 2] += b.z; f[j + 3] += b.w;
-                }
-            } else {
-#pragma unroll
-                for (int j = 0; j < 32; j += 8) {
-                    const uint4 b = __ldg(reinterpret_cast<const uint4*>(
-                        static_cast<const __nv_bfloat16*>(p.bias) + col0 + j));
-                    const uint32_t w[4] = {b.x, b.y, b.z, b.w};
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        f[j + 2 * i] += __uint_as_float(w[i] << 16);
-                        f[j + 2 * i + 1] += __uint_as_float(w[i] & 0xFFFF0000u);
-                    }
-                }
-            }
-        }
-    } else {
-#pragma unroll
-        for (int j = 0; j < 32; ++j) {
-            const int c = col0 + j;
-            float t = 0.0f;
-            if (c < p.N) {
-                t = (static_cast<float>(static_cast<int32_t>(v[j])) * sxv) * __ldg(p.sw + c);
-                if (p.bias)
-                    t += p.bias_t == ARIA_F32
-                             ? __ldg(static_cast<const float*>(p.bias) + c)
-                             : __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[c]);
-            }
-            f[j] = t;
-        }
-    }
-    if (p.act == ARIA_ACT_GELU_ERF) {
-#pragma unroll
-        for (int j = 0; j < 32; ++j) f[j] = gelu_erf(f[j]);
-    }
-    if (OUT_T == 0) {
-        float* y = static_cast<float*>(p.Y) + static_cast<int64_t>(row) * p.N + col0;
-        if (full) {
-#pragma unroll
-            for (int j = 0; j < 32; j += 4)
-                *reinterpret_cast<float4*>(y + j) = make_float4(f[j], f[j + 1], f[j + 2], f[j + 3]);
-        } else {
-            for (int j = 0; j < 32 && col0 + j < p.N; ++j) y[j] = f[j];
-        }
-    } else {
-        __nv_bfloat16* y = static_cast<__nv_bfloat16*>(p.Y) + static_cast<int64_t>(row) * p.N + col0;
-        if (full) {
-#pragma unroll
-            for (int j = 0; j < 32; j += 8)
-                *reinterpret_cast<uint4*>(y + j) =
-                    make_uint4(pack_bf16x2(f[j], f[j + 1]), pack_bf16x2(f[j + 2], f[j + 3]),
-                               pack_bf16x2(f[j + 4], f[j + 5]), pack_bf16x2(f[j + 6], f[j + 7]));
-        } else {
-            for (int j = 0; j < 32 && col0 + j < p.N; ++j) y[j] = __float2bfloat16_rn(f[j]);
-        }
+    for (int c = 0; c < 4; ++c)
+        sts128(rowb + ((c ^ x) << 4), w[4 * c], w[4 * c + 1], w[4 * c + 2], w[4 * c + 3]);
+    fence_proxy_async_smem();
+    __syncwarp();
+    if (lane == 0) {
+        tma_store_2d(tmY, stg, col0, row0);
+        tma_store_commit();
     }
 }
 
+// OUT_T: 0 = fp32, 1 = bf16, 2 = raw int32 accumulators.
 template <int BN, int OUT_T>
 __global__ void __launch_bounds__(W8_THREADS, 1)
 w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                 const W8Params p) {
+                 const __grid_constant__ CUtensorMap tmY, const W8Params p) {
     using Cfg = W8Cfg<BN>;
     constexpr int STAGES = Cfg::STAGES;
     extern __shared__ uint8_t smem_raw[];
@@ -151,12 +93,13 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     uint8_t* gbase = smem_raw + (base - raw);
     const uint32_t sA = base;
     const uint32_t sB = base + STAGES * Cfg::A_BYTES;
-    const uint32_t bars = base + STAGES * Cfg::STAGE_BYTES;
+    const uint32_t bars = base + Cfg::BAR_OFF;
     const uint32_t full0 = bars, empty0 = bars + 8 * STAGES;
     const uint32_t tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;
     const uint32_t tmem_slot = tempty0 + 16;
     volatile uint32_t* tmem_slot_g =
-        reinterpret_cast<volatile uint32_t*>(gbase + STAGES * Cfg::STAGE_BYTES + 16 * STAGES + 32);
+        reinterpret_cast<volatile uint32_t*>(gbase + Cfg::BAR_OFF + 16 * STAGES + 32);
+    float* swb = reinterpret_cast<float*>(gbase + Cfg::SWB_OFF);
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -168,13 +111,14 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmA);
         tma_prefetch_desc(&tmB);
+        tma_prefetch_desc(&tmY);
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(full0 + 8 * s, 1);
             mbar_init(empty0 + 8 * s, 1);
         }
         for (int a = 0; a < 2; ++a) {
             mbar_init(tfull0 + 8 * a, 1);
-            mbar_init(tempty0 + 8 * a, 4);
+            mbar_init(tempty0 + 8 * a, W8_EPI_WARPS);
         }
         fence_mbar_init();
     }
@@ -234,29 +178,90 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             }
         }
     } else {
-        const int q = warp & 3;  // TMEM lane quarter this warp may read
+        // ------------------------------------------------------------ epilogue (warps 2..9)
+        const int ew = warp - 2;
+        const int q = warp & 3;          // TMEM lane quarter this warp may read
+        const int half = ew >> 2;        // which column chunks (c % 2 == half)
+        const int et = threadIdx.x - 64; // 0..255
+        const uint32_t stg = base + Cfg::STG_OFF + ew * W8_STG_BYTES;
         int acc = 0;
         uint32_t acc_phase = 0;
         for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
             const int m0 = (t % num_m) * W8_BM, n0 = (t / num_m) * BN;
-            const int row = m0 + q * 32 + lane;
+            const int row0 = m0 + q * 32;
             float sxv = 0.0f;
-            if (OUT_T != 2 && row < p.M) sxv = __ldg(p.sx + row);
+            if (OUT_T != 2) {
+                if (row0 + lane < p.M) sxv = __ldg(p.sx + row0 + lane);
+                // per-tile column scales and bias -> shared memory (broadcast reads later)
+                named_bar_sync(1, 32 * W8_EPI_WARPS);  // previous tile's readers are done
+                for (int i = et; i < BN; i += 32 * W8_EPI_WARPS) {
+                    const int c = n0 + i;
+                    float s = 0.0f, b = 0.0f;
+                    if (c < p.N) {
+                        s = __ldg(p.sw + c);
+                        if (p.bias)
+                            b = p.bias_t == ARIA_F32
+                                    ? __ldg(static_cast<const float*>(p.bias) + c)
+                                    : __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[c]);
+                    }
+                    swb[i] = s;
+                    swb[BN + i] = b;
+                }
+                named_bar_sync(1, 32 * W8_EPI_WARPS);
+            }
             mbar_wait(tfull0 + 8 * acc, acc_phase);
             tc_fence_after();
             const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
 #pragma unroll 1
-            for (int c = 0; c < BN / 32; ++c) {
+            for (int c = half; c < BN / 32; c += 2) {
                 uint32_t v[32];
                 tmem_ld_32x32b_x32(t_addr + c * 32, v);
                 tmem_wait_ld();
-                w8_epilogue_chunk<OUT_T>(v, p, row, n0 + c * 32, sxv);
+                const int col0 = n0 + c * 32;
+                if (OUT_T == 2) {
+                    uint32_t w[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) w[j] = v[j];
+                    w8_store_block(&tmY, stg, lane, w, col0, row0);
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) w[j] = v[16 + j];
+                    w8_store_block(&tmY, stg, lane, w, col0 + 16, row0);
+                } else {
+                    float f[32];
+#pragma unroll
+                    for (int j = 0; j < 32; j += 4) {
+                        const float4 s4 = *reinterpret_cast<const float4*>(swb + c * 32 + j);
+                        const float4 b4 = *reinterpret_cast<const float4*>(swb + BN + c * 32 + j);
+                        f[j] = fmaf(static_cast<float>(static_cast<int32_t>(v[j])) * sxv, s4.x, b4.x);
+                        f[j + 1] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 1])) * sxv, s4.y, b4.y);
+                        f[j + 2] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 2])) * sxv, s4.z, b4.z);
+                        f[j + 3] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 3])) * sxv, s4.w, b4.w);
+                    }
+                    if (p.act == ARIA_ACT_GELU_ERF) {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) f[j] = gelu_erf(f[j]);
+                    }
+                    uint32_t w[16];
+                    if (OUT_T == 1) {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) w[j] = pack_bf16x2(f[2 * j], f[2 * j + 1]);
+                        w8_store_block(&tmY, stg, lane, w, col0, row0);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[j]);
+                        w8_store_block(&tmY, stg, lane, w, col0, row0);
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[16 + j]);
+                        w8_store_block(&tmY, stg, lane, w, col0 + 16, row0);
+                    }
+                }
             }
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty0 + 8 * acc);
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
         }
+        if (lane == 0) tma_store_wait<0>();  // all of this warp's output has been written
     }
 
     pdl_launch_dependents();
@@ -269,8 +274,8 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 }
 
 template <int BN, int OUT_T>
-static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const W8Params& p, int grid,
-                      cudaStream_t st, bool pdl) {
+static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmY,
+                      const W8Params& p, int grid, cudaStream_t st, bool pdl) {
     using Cfg = W8Cfg<BN>;
     static bool attr_set = false;
     auto kern = w8a8_gemm_kernel<BN, OUT_T>;
@@ -290,21 +295,22 @@ static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const W8Pa
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kern, tmA, tmB, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    return cudaLaunchKernelEx(&cfg, kern, tmA, tmB, tmY, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
 template <int BN>
-static int launch_bn(const CUtensorMap& tmA, const CUtensorMap& tmB, const W8Params& p, int grid,
-                     cudaStream_t st, bool pdl) {
-    switch (p.out_t) {
-        case 0: return launch_one<BN, 0>(tmA, tmB, p, grid, st, pdl);
-        case 1: return launch_one<BN, 1>(tmA, tmB, p, grid, st, pdl);
-        default: return launch_one<BN, 2>(tmA, tmB, p, grid, st, pdl);
+static int launch_bn(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmY,
+                     const W8Params& p, int out_t, int grid, cudaStream_t st, bool pdl) {
+    switch (out_t) {
+        case 0: return launch_one<BN, 0>(tmA, tmB, tmY, p, grid, st, pdl);
+        case 1: return launch_one<BN, 1>(tmA, tmB, tmY, p, grid, st, pdl);
+        default: return launch_one<BN, 2>(tmA, tmB, tmY, p, grid, st, pdl);
     }
 }
 
-// Tile width: the BN in {64,128,192,256} with the fewest wave-quantised MMA cycles
-// (waves x BN); ties go to the wider tile (fewer B re-reads, fewer epilogue switches).
+// Tile width: the BN in {64,128,192,256} with the fewest wave-quantised cycles.  Per 32-byte k-step a
+// tile costs max(MMA, shared-memory operand read) = max(BN/2, 32 + BN/4) cycles (128 x BN x 32 MACs at
+// 8192 MAC/clk vs (128 + BN) x 32 bytes at 128 B/clk), so narrow tiles are smem-bound; ties go wide.
 static int pick_bn(int M, int N, int sms) {
     const int cands[4] = {256, 192, 128, 64};
     const int num_m = (M + W8_BM - 1) / W8_BM;
@@ -314,7 +320,8 @@ static int pick_bn(int M, int N, int sms) {
         const int bn = cands[i];
         const long tiles = static_cast<long>(num_m) * ((N + bn - 1) / bn);
         const long waves = (tiles + sms - 1) / sms;
-        const long cost = waves * bn;
+        const long per_tile = bn / 2 > 32 + bn / 4 ? bn / 2 : 32 + bn / 4;
+        const long cost = waves * per_tile;
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = bn; }
     }
     return best;
@@ -330,17 +337,22 @@ int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, co
     if (rc != ARIA_OK) return rc;
     rc = make_tmap_2d(&tmB, Wq, 1, N, K, bn, W8_BK, 128);
     if (rc != ARIA_OK) return rc;
+    // output tensor map: [M, N] of 2- or 4-byte elements, box = 32 rows x 64 bytes, 64-byte swizzle
+    CUtensorMap tmY;
+    const int esz = ep.out_t == 1 ? 2 : 4;
+    rc = make_tmap_2d(&tmY, ep.Y, esz, M, N, 32, 64 / esz, 64);
+    if (rc != ARIA_OK) return rc;
     W8Params p;
-    p.sx = ep.sx; p.sw = ep.sw; p.bias = ep.bias; p.Y = ep.Y;
-    p.bias_t = ep.bias_t; p.act = ep.act; p.out_t = ep.out_t;
+    p.sx = ep.sx; p.sw = ep.sw; p.bias = ep.bias;
+    p.bias_t = ep.bias_t; p.act = ep.act;
     p.M = M; p.N = N; p.K = K;
     const int tiles = ((M + W8_BM - 1) / W8_BM) * ((N + bn - 1) / bn);
     const int grid = tiles < sms ? tiles : sms;
     switch (bn) {
-        case 64: return launch_bn<64>(tmA, tmB, p, grid, st, pdl);
-        case 128: return launch_bn<128>(tmA, tmB, p, grid, st, pdl);
-        case 192: return launch_bn<192>(tmA, tmB, p, grid, st, pdl);
-        default: return launch_bn<256>(tmA, tmB, p, grid, st, pdl);
+        case 64: return launch_bn<64>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
+        case 128: return launch_bn<128>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
+        case 192: return launch_bn<192>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
+        default: return launch_bn<256>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
     }
 }
 

@@ -119,3 +119,14 @@ def test_zero_input_gives_bias(aria, oracle):
     wq_d, sw_d = aria.aria_quantize_weights_int8(dev_f32(W))
     y = aria.aria_linear_w8a8(X, wq_d, sw_d, dev_f32(b), aria.ACT_NONE, aria.F32)
     assert np.array_equal(host_f32(y), np.broadcast_to(b, (M, N)))
+
+
+def test_prequantised_entry_point_matches_fused_call(aria, oracle):
+    c = inputs.c2(M=256)
+    X = dev_bf16(c["X_bits"])
+    wq_d, sw_d = aria.aria_quantize_weights_int8(dev_f32(c["Wout"]))
+    b = dev_bf16(c["bout"][0])
+    y1 = aria.aria_linear_w8a8(X, wq_d, sw_d, b, aria.ACT_NONE, aria.F32)
+    xq, sx = aria.aria_quantize_act_int8(X)
+    y2 = aria.aria_linear_w8a8_q(xq, sx, wq_d, sw_d, b, aria.ACT_NONE, aria.F32)
+    assert torch.equal(y1, y2)
