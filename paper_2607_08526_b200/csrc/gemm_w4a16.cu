@@ -5,19 +5,25 @@
 // and the token tile is the MMA's N operand (TT = 32..256 tokens), so a 32-token batch is a legal
 // N = 32 instruction and each dequantised weight feeds TT MACs.
 //
-// Persistent, warp-specialised, one CTA per SM, 14 warps:
-//   warp 0       TMA producer: per k-block the packed int4 tile [128 rows x BK/2 bytes] (32/64-byte
-//                swizzle) and the X tile [TT x BK] bf16 (128-byte swizzle) into a ring.
-//   warp 1       MMA issuer (one thread): BK/16 tcgen05.mma per k-block, A = dequantised weights,
+// Persistent, warp-specialised, one CTA per SM.  k-blocks are 64 wide (two int4 groups).  The two
+// operands travel through SEPARATE rings, because their consumers have very different latencies:
+//   warp 0       TMA producer for X: [TT x 64] bf16 tiles (128-byte swizzle), consumed directly by
+//                the MMA -> a short ring of large stages.
+//   warp 2       TMA producer for the packed weights: [128 rows x 32 bytes] tiles (32-byte swizzle),
+//                consumed by the dequantisers -> a deep ring of 4 KB stages (this is the HBM stream).
+//   warp 1       MMA issuer (one thread): 4 tcgen05.mma per k-block, A = dequantised weights,
 //                B = X, into one of two TMEM accumulators.
-//   warps 2..5   epilogue: tcgen05.ld -> (+bias, GELU, cast) -> Y, or split-K partials.
-//   warps 6..13  dequantisers (256 threads, thread = weight row x chunk parity): LDS 16 B (32 codes,
-//                one group) -> 32 exact fp32 products q*sg -> cvt.rn.bf16x2 -> STS into the
-//                128-byte-swizzled K-major A tile; fence.proxy.async; arrive on `a_full`.
+//   warps 4..7   epilogue: tcgen05.ld -> (+bias, GELU, cast) -> smem transpose -> TMA store, or
+//                split-K partials.
+//   warps 8..    G dequantiser GROUPS of 4 warps (thread = weight row).  Group g owns A buffer g and
+//                handles k-blocks g, g+G, ...: wait packed -> LDS -> 64 x (LOP3, FFMA2/2, CVT/2) into
+//                registers -> wait A buffer free -> 8 STS -> fence -> arrive.  The arithmetic is done
+//                BEFORE waiting for the buffer, so the MMA -> dequant -> MMA hand-off is short.
 // Exactness of w^ = bf16_rne(q*sg): the nibble n is placed (XOR 8 = offset binary u = q+8) at
-// mantissa bit pos in {8,12,16} of 1.0f, giving x = 1 + u*2^(pos-23); one FFMA
+// mantissa bit pos in {8,12,16} of 1.0f, giving x = 1 + u*2^(pos-23); one FMA
 // x * (2^(23-pos) sg) - (2^(23-pos)+8) sg has exactly representable addends and the exactly
 // representable result q*sg, so fp32 holds q*sg exactly and one cvt.rn rounds it to bf16.
+// The FMAs are issued as packed fma.rn.f32x2 (two elements per instruction on sm_100).
 //
 // Split-K (small M): a work unit is (tile, k-range); units of a tile write fp32 partials to the
 // workspace, the last to arrive (per 32-channel quarter, atomic counter) sums them in split order
@@ -27,30 +33,32 @@
 namespace aria {
 
 constexpr int W4_BN = 128;      // output channels per tile = MMA M
-constexpr int W4_THREADS = 448;
-constexpr int W4_DEQ_WARP0 = 6;
-constexpr int W4_DEQ_THREADS = 256;
-constexpr int W4_DEQ_WARPS = W4_DEQ_THREADS / 32;
+constexpr int W4_BK = 64;       // k-block: 64 weights = 32 packed bytes = 2 groups per row
+constexpr int W4_EPI_WARP0 = 4;
+constexpr int W4_DEQ_WARP0 = 8;
+constexpr int W4_G = 3;         // dequantiser groups = A buffers
 
-template <int TT, int BK>
+template <int TT>
 struct W4Cfg {
-    static constexpr int P_ROW = BK / 2;                       // packed bytes per row per k-block
-    static constexpr int P_BYTES = W4_BN * P_ROW;              // 4 or 8 KB
-    static constexpr int X_SUB = TT * 128;                     // one 64-column bf16 sub-tile
-    static constexpr int X_BYTES = X_SUB * (BK / 64);
-    static constexpr int STAGE_BYTES = X_BYTES + P_BYTES;
-    static constexpr int A_SUB = W4_BN * 128;                  // 16 KB: 128 rows x 64 bf16
-    static constexpr int A_BYTES = A_SUB * (BK / 64);
-    static constexpr int NA = BK == 64 ? 3 : 2;                // dequantised A buffers
-    static constexpr int STAGES_RAW = (196 * 1024 - NA * A_BYTES) / STAGE_BYTES;
-    static constexpr int STAGES = STAGES_RAW > 8 ? 8 : STAGES_RAW;
+    static constexpr int G = W4_G;
+    static constexpr int THREADS = 32 * W4_DEQ_WARP0 + 128 * G;
+    static constexpr int P_ROW = W4_BK / 2;                    // 32 packed bytes per row per k-block
+    static constexpr int P_BYTES = W4_BN * P_ROW;              // 4 KB
+    static constexpr int X_BYTES = TT * 128;                   // TT rows x 64 bf16
+    static constexpr int A_BYTES = W4_BN * 128;                // 16 KB: 128 rows x 64 bf16
+    static constexpr int STG_BYTES = 4096;                     // per epilogue warp: 32 tokens x 128 B
+    static constexpr int XS = TT == 256 ? 3 : TT == 128 ? 4 : TT == 64 ? 6 : 8;   // X ring depth
+    static constexpr int PS = TT == 256 ? 8 : TT == 128 ? 12 : 16;                // packed ring depth
+    static constexpr int X_OFF = 0;
+    static constexpr int A_OFF = X_OFF + XS * X_BYTES;
+    static constexpr int P_OFF = A_OFF + G * A_BYTES;
+    static constexpr int STG_OFF = P_OFF + PS * P_BYTES;
+    static constexpr int BAR_OFF = STG_OFF + 4 * STG_BYTES;
+    static constexpr int NBAR = 2 * XS + 2 * PS + 2 * G + 4;
+    static constexpr int SMEM_BYTES = BAR_OFF + NBAR * 8 + 16 + 1024;
     static constexpr int ACC_STRIDE = TT;
     static constexpr int TMEM_COLS = 2 * TT < 32 ? 32 : 2 * TT;
-    static constexpr int BAR_BYTES = (2 * STAGES + 2 * NA + 4) * 8 + 16;
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + NA * A_BYTES + BAR_BYTES + 1024;
     static_assert(TT == 32 || TT == 64 || TT == 128 || TT == 256, "TT");
-    static_assert(BK == 64 || BK == 128, "BK");
-    static_assert(STAGES >= 2, "ring too shallow");
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
@@ -59,47 +67,78 @@ struct W4Params {
     const void* bias;         // bf16 [N] or nullptr
     void* Y;
     float* partials;          // [splits, M, N] fp32 (split-K only)
-    unsigned* counters;       // [num_tiles * 4], zero between launches (self-resetting)
+    unsigned* counters;       // [num_tiles * 4], zeroed by a memset node before each launch
     int act, out_t;
     int M, N, K;
     int splits;
+    long long* prof;          // debug: per-CTA role timestamps (clock64), or nullptr
 };
+
+static long long* g_w4_prof = nullptr;
+void w4_set_profile_buffer(long long* p) { g_w4_prof = p; }
+
+__device__ __forceinline__ void prof_stamp(const W4Params& p, int slot, long long t0) {
+    if (p.prof) p.prof[blockIdx.x * 16 + slot] = clock64() - t0;
+}
 
 __device__ __forceinline__ uint32_t cvt_bf16x2(float lo, float hi) {
     uint32_t r;
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
+// (a & b) ^ c in one LOP3
 __device__ __forceinline__ uint32_t lop_and_xor(uint32_t a, uint32_t b, uint32_t c) {
     uint32_t r;
-    asm("lop3.b32 %0, %1, %2, %3, 0x6A;" : "=r"(r) : "r"(a), "r"(b), "r"(c));  // (a & b) ^ c
+    asm("lop3.b32 %0, %1, %2, %3, 0x6A;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
     return r;
 }
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ uint64_t pack2u(uint32_t lo, uint32_t hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+// two fp32 FMAs in one instruction (sm_100 FFMA2); result packed as bf16x2 (lo = element 0)
+__device__ __forceinline__ uint32_t fma2_to_bf16x2(uint64_t x, uint64_t s, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(x), "l"(s), "l"(c));
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+    return cvt_bf16x2(lo, hi);
+}
 
-// 8 codes of one 32-bit word -> 8 exact fp32 products q*sg -> 4 packed bf16x2 (k ascending).
+// Per-group constants, as the four (scale, offset) pairs the element pairs of a word need.
 struct GroupConst {
-    float s8, c8, s12, c12, s16, c16;
+    uint64_t s_8_12, c_8_12, s_16_12, c_16_12, s_16_8, c_16_8, s_12_16, c_12_16;
 };
 __device__ __forceinline__ GroupConst group_const(float sg) {
+    const float s8 = sg * 32768.0f, c8 = -(sg * 32776.0f);   // 2^15, 2^15 + 8
+    const float s12 = sg * 2048.0f, c12 = -(sg * 2056.0f);   // 2^11, 2^11 + 8
+    const float s16 = sg * 128.0f, c16 = -(sg * 136.0f);     // 2^7,  2^7  + 8
     GroupConst g;
-    g.s8 = sg * 32768.0f;  g.c8 = -(sg * 32776.0f);   // 2^15, 2^15 + 8
-    g.s12 = sg * 2048.0f;  g.c12 = -(sg * 2056.0f);   // 2^11, 2^11 + 8
-    g.s16 = sg * 128.0f;   g.c16 = -(sg * 136.0f);    // 2^7,  2^7  + 8
+    g.s_8_12 = pack2(s8, s12);   g.c_8_12 = pack2(c8, c12);
+    g.s_16_12 = pack2(s16, s12); g.c_16_12 = pack2(c16, c12);
+    g.s_16_8 = pack2(s16, s8);   g.c_16_8 = pack2(c16, c8);
+    g.s_12_16 = pack2(s12, s16); g.c_12_16 = pack2(c12, c16);
     return g;
 }
+// 8 codes of one 32-bit word (nibble i = code of k = 8w + i) -> 4 packed bf16x2, k ascending.
 __device__ __forceinline__ uint4 dequant_word(uint32_t w, const GroupConst& g) {
     const uint32_t wa = w << 8, wb = w >> 12;
     const uint32_t M8 = 0x00000F00u, M12 = 0x0000F000u, M16 = 0x000F0000u;
     const uint32_t X8 = 0x3F800800u, X12 = 0x3F808000u, X16 = 0x3F880000u;  // 1.0f | (8 << pos)
-    const float e0 = fmaf(__uint_as_float(lop_and_xor(wa, M8, X8)), g.s8, g.c8);
-    const float e1 = fmaf(__uint_as_float(lop_and_xor(wa, M12, X12)), g.s12, g.c12);
-    const float e2 = fmaf(__uint_as_float(lop_and_xor(wa, M16, X16)), g.s16, g.c16);
-    const float e3 = fmaf(__uint_as_float(lop_and_xor(w, M12, X12)), g.s12, g.c12);
-    const float e4 = fmaf(__uint_as_float(lop_and_xor(w, M16, X16)), g.s16, g.c16);
-    const float e5 = fmaf(__uint_as_float(lop_and_xor(wb, M8, X8)), g.s8, g.c8);
-    const float e6 = fmaf(__uint_as_float(lop_and_xor(wb, M12, X12)), g.s12, g.c12);
-    const float e7 = fmaf(__uint_as_float(lop_and_xor(wb, M16, X16)), g.s16, g.c16);
-    return make_uint4(cvt_bf16x2(e0, e1), cvt_bf16x2(e2, e3), cvt_bf16x2(e4, e5), cvt_bf16x2(e6, e7));
+    const uint32_t e0 = lop_and_xor(wa, M8, X8), e1 = lop_and_xor(wa, M12, X12);
+    const uint32_t e2 = lop_and_xor(wa, M16, X16), e3 = lop_and_xor(w, M12, X12);
+    const uint32_t e4 = lop_and_xor(w, M16, X16), e5 = lop_and_xor(wb, M8, X8);
+    const uint32_t e6 = lop_and_xor(wb, M12, X12), e7 = lop_and_xor(wb, M16, X16);
+    return make_uint4(fma2_to_bf16x2(pack2u(e0, e1), g.s_8_12, g.c_8_12),
+                      fma2_to_bf16x2(pack2u(e2, e3), g.s_16_12, g.c_16_12),
+                      fma2_to_bf16x2(pack2u(e4, e5), g.s_16_8, g.c_16_8),
+                      fma2_to_bf16x2(pack2u(e6, e7), g.s_12_16, g.c_12_16));
 }
 
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
@@ -115,9 +154,6 @@ __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
                  : "memory");
 }
 
-__device__ __forceinline__ float w4_finish(float y, int act) {
-    return act == ARIA_ACT_GELU_ERF ? gelu_erf(y) : y;
-}
 __device__ __forceinline__ void w4_store(void* Y, int out_t, int64_t idx, float y) {
     if (out_t == ARIA_F32)
         static_cast<float*>(Y)[idx] = y;
@@ -125,43 +161,48 @@ __device__ __forceinline__ void w4_store(void* Y, int out_t, int64_t idx, float 
         static_cast<__nv_bfloat16*>(Y)[idx] = __float2bfloat16_rn(y);
 }
 
-template <int TT, int BK>
-__global__ void __launch_bounds__(W4_THREADS, 1)
+template <int TT, bool GELU>
+__global__ void __launch_bounds__(W4Cfg<TT>::THREADS, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmX,
-                  const W4Params p) {
-    using Cfg = W4Cfg<TT, BK>;
-    constexpr int STAGES = Cfg::STAGES, NA = Cfg::NA;
+                  const __grid_constant__ CUtensorMap tmY, const W4Params p) {
+    using Cfg = W4Cfg<TT>;
+    constexpr int XS = Cfg::XS, PS = Cfg::PS, G = Cfg::G;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;
     uint8_t* gbase = smem_raw + (base - raw);
-    const uint32_t sStage = base;                                   // [STAGES][X | P]
-    const uint32_t sA = base + STAGES * Cfg::STAGE_BYTES;           // [NA][A]
-    const uint32_t bars = sA + NA * Cfg::A_BYTES;
-    const uint32_t full0 = bars, empty0 = full0 + 8 * STAGES;
-    const uint32_t afull0 = empty0 + 8 * STAGES, aempty0 = afull0 + 8 * NA;
-    const uint32_t tfull0 = aempty0 + 8 * NA, tempty0 = tfull0 + 16;
+    const uint32_t sX = base + Cfg::X_OFF, sA = base + Cfg::A_OFF, sP = base + Cfg::P_OFF;
+    const uint32_t bars = base + Cfg::BAR_OFF;
+    const uint32_t xfull0 = bars, xempty0 = xfull0 + 8 * XS;
+    const uint32_t pfull0 = xempty0 + 8 * XS, pempty0 = pfull0 + 8 * PS;
+    const uint32_t afull0 = pempty0 + 8 * PS, aempty0 = afull0 + 8 * G;
+    const uint32_t tfull0 = aempty0 + 8 * G, tempty0 = tfull0 + 16;
     const uint32_t tmem_slot = tempty0 + 16;
-    volatile uint32_t* tmem_slot_g = reinterpret_cast<volatile uint32_t*>(
-        gbase + STAGES * Cfg::STAGE_BYTES + NA * Cfg::A_BYTES + (2 * STAGES + 2 * NA + 4) * 8);
+    volatile uint32_t* tmem_slot_g =
+        reinterpret_cast<volatile uint32_t*>(gbase + Cfg::BAR_OFF + Cfg::NBAR * 8);
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const int num_n = (p.N + W4_BN - 1) / W4_BN;
     const int num_t = (p.M + TT - 1) / TT;
-    const int num_kb = (p.K + BK - 1) / BK;
+    const int num_kb = (p.K + W4_BK - 1) / W4_BK;
     const int S = p.splits;
     const int num_units = num_n * num_t * S;
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmP);
         tma_prefetch_desc(&tmX);
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(full0 + 8 * s, 1);
-            mbar_init(empty0 + 8 * s, W4_DEQ_WARPS + 1);  // dequantiser warps (packed) + MMA commit (X)
+        tma_prefetch_desc(&tmY);
+        for (int s = 0; s < XS; ++s) {
+            mbar_init(xfull0 + 8 * s, 1);
+            mbar_init(xempty0 + 8 * s, 1);      // MMA commit
         }
-        for (int a = 0; a < NA; ++a) {
-            mbar_init(afull0 + 8 * a, W4_DEQ_WARPS);
+        for (int s = 0; s < PS; ++s) {
+            mbar_init(pfull0 + 8 * s, 1);
+            mbar_init(pempty0 + 8 * s, 4);      // the 4 warps of the dequant group that read it
+        }
+        for (int a = 0; a < G; ++a) {
+            mbar_init(afull0 + 8 * a, 4);
             mbar_init(aempty0 + 8 * a, 1);
         }
         for (int a = 0; a < 2; ++a) {
@@ -180,28 +221,45 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     const uint32_t tmem_base = *tmem_slot_g;
 
     pdl_wait_prior_grid();
+    const long long t_start = clock64();
 
     if (warp == 0) {
-        // ------------------------------------------------------------ TMA producer
+        // ------------------------------------------------------------ TMA producer: X
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int u = blockIdx.x; u < num_units; u += gridDim.x) {
+                const int tile = u / S, sp = u % S;
+                const int t0 = (tile / num_n) * TT;
+                const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
+                for (int kb = kb0; kb < kb1; ++kb) {
+                    mbar_wait(xempty0 + 8 * stage, phase ^ 1);
+                    mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);
+                    tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
+                    if (++stage == XS) { stage = 0; phase ^= 1; }
+                }
+            }
+            prof_stamp(p, 0, t_start);
+        }
+    } else if (warp == 2) {
+        // ------------------------------------------------------------ TMA producer: packed weights
         if (lane == 0) {
             const uint64_t pol_w = policy_evict_first();  // weights are streamed once per launch
             int stage = 0;
             uint32_t phase = 0;
             for (int u = blockIdx.x; u < num_units; u += gridDim.x) {
                 const int tile = u / S, sp = u % S;
-                const int n0 = (tile % num_n) * W4_BN, t0 = (tile / num_n) * TT;
+                const int n0 = (tile % num_n) * W4_BN;
                 const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
                 for (int kb = kb0; kb < kb1; ++kb) {
-                    mbar_wait(empty0 + 8 * stage, phase ^ 1);
-                    const uint32_t st = sStage + stage * Cfg::STAGE_BYTES;
-                    mbar_arrive_expect_tx(full0 + 8 * stage, Cfg::STAGE_BYTES);
-#pragma unroll
-                    for (int j = 0; j < BK / 64; ++j)
-                        tma_load_2d(st + j * Cfg::X_SUB, &tmX, kb * BK + j * 64, t0, full0 + 8 * stage);
-                    tma_load_2d_hint(st + Cfg::X_BYTES, &tmP, kb * (BK / 2), n0, full0 + 8 * stage, pol_w);
-                    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                    mbar_wait(pempty0 + 8 * stage, phase ^ 1);
+                    mbar_arrive_expect_tx(pfull0 + 8 * stage, Cfg::P_BYTES);
+                    tma_load_2d_hint(sP + stage * Cfg::P_BYTES, &tmP, kb * Cfg::P_ROW, n0,
+                                     pfull0 + 8 * stage, pol_w);
+                    if (++stage == PS) { stage = 0; phase ^= 1; }
                 }
             }
+            prof_stamp(p, 6, t_start);
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------ MMA issuer
@@ -216,86 +274,89 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * Cfg::ACC_STRIDE;
                 for (int kb = kb0; kb < kb1; ++kb) {
-                    mbar_wait(full0 + 8 * stage, phase);    // X landed
+                    mbar_wait(xfull0 + 8 * stage, phase);   // X landed
                     mbar_wait(afull0 + 8 * ab, aphase);     // weights dequantised
                     tc_fence_after();
-                    const uint32_t xs = sStage + stage * Cfg::STAGE_BYTES;
-                    const uint32_t as = sA + ab * Cfg::A_BYTES;
+                    const uint64_t a_desc = make_smem_desc_sw128(sA + ab * Cfg::A_BYTES);
+                    const uint64_t b_desc = make_smem_desc_sw128(sX + stage * Cfg::X_BYTES);
 #pragma unroll
-                    for (int j = 0; j < BK / 64; ++j) {
-                        const uint64_t a_desc = make_smem_desc_sw128(as + j * Cfg::A_SUB);
-                        const uint64_t b_desc = make_smem_desc_sw128(xs + j * Cfg::X_SUB);
-#pragma unroll
-                        for (int k = 0; k < 4; ++k)  // 4 x (K = 16 bf16 = 32 bytes) per 64-column sub-tile
-                            mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc,
-                                       (kb != kb0 || j != 0 || k != 0) ? 1u : 0u);
-                    }
-                    tc_commit(empty0 + 8 * stage);
+                    for (int k = 0; k < 4; ++k)  // 4 x (K = 16 bf16 = 32 bytes)
+                        mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc,
+                                   (kb != kb0 || k != 0) ? 1u : 0u);
+                    tc_commit(xempty0 + 8 * stage);
                     tc_commit(aempty0 + 8 * ab);
-                    if (++stage == STAGES) { stage = 0; phase ^= 1; }
-                    if (++ab == NA) { ab = 0; aphase ^= 1; }
+                    if (++stage == XS) { stage = 0; phase ^= 1; }
+                    if (++ab == G) { ab = 0; aphase ^= 1; }
                 }
                 tc_commit(tfull0 + 8 * acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1; }
             }
+            prof_stamp(p, 1, t_start);
         }
     } else if (warp >= W4_DEQ_WARP0) {
-        // ------------------------------------------------------------ dequantisers
-        const int dt = threadIdx.x - W4_DEQ_WARP0 * 32;
-        const int r = dt & 127;        // weight row inside the tile
-        const int par = dt >> 7;       // chunk parity handled by this thread
-        constexpr int NCH = BK / 32;   // 16-byte chunks (= groups) per row per k-block
-        constexpr uint32_t SWM = Cfg::P_ROW / 16 - 1;
-        const int gpr = p.K >> 5;      // groups per weight row
-        int stage = 0, ab = 0;
-        uint32_t phase = 0, aphase = 0;
+        // ------------------------------------------------------------ dequantiser groups
+        const int dw = warp - W4_DEQ_WARP0;
+        const int g = dw >> 2;                    // group = A buffer index
+        const int r = (dw & 3) * 32 + lane;       // weight row inside the tile
+        const int gpr = p.K >> 5;                 // groups per weight row
+        const uint32_t rowb = sA + g * Cfg::A_BYTES + (r >> 3) * 1024 + (r & 7) * 128;
+        const uint32_t xr = r & 7;
+        const uint32_t off0 = r * Cfg::P_ROW;
+        const uint32_t poff0 = off0 ^ (((off0 >> 7) & 1u) << 4);          // 32-byte swizzle
+        const uint32_t poff1 = (off0 + 16) ^ (((off0 >> 7) & 1u) << 4);
+        int it = 0;                               // running k-block counter of this CTA
+        uint32_t aphase = 0;
         for (int u = blockIdx.x; u < num_units; u += gridDim.x) {
             const int tile = u / S, sp = u % S;
             const int n0 = (tile % num_n) * W4_BN;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             const bool row_ok = n0 + r < p.N;
-            const uint16_t* srow = p.g_scale + static_cast<int64_t>(row_ok ? n0 + r : 0) * gpr;
-            for (int kb = kb0; kb < kb1; ++kb) {
-                uint16_t sbits[NCH / 2];
-#pragma unroll
-                for (int i = 0; i < NCH / 2; ++i) {
-                    const int g = kb * NCH + par + 2 * i;
-                    sbits[i] = (row_ok && g < gpr) ? __ldg(srow + g) : static_cast<uint16_t>(0);
-                }
-                mbar_wait(full0 + 8 * stage, phase);
-                const uint32_t ps = sStage + stage * Cfg::STAGE_BYTES + Cfg::X_BYTES;
-                uint4 pk[NCH / 2];
-#pragma unroll
-                for (int i = 0; i < NCH / 2; ++i) {
-                    const uint32_t off = r * Cfg::P_ROW + (par + 2 * i) * 16;
-                    pk[i] = lds128(ps + (off ^ (((off >> 7) & SWM) << 4)));
-                }
-                mbar_wait(aempty0 + 8 * ab, aphase ^ 1);   // MMAs that read this A buffer retired
-                const uint32_t as = sA + ab * Cfg::A_BYTES;
-#pragma unroll
-                for (int i = 0; i < NCH / 2; ++i) {
-                    const int c = par + 2 * i;
-                    const GroupConst gc = group_const(__half2float(__ushort_as_half(sbits[i])));
-                    const uint32_t rowb = as + (c >> 1) * Cfg::A_SUB + (r >> 3) * 1024 + (r & 7) * 128;
-                    const uint32_t words[4] = {pk[i].x, pk[i].y, pk[i].z, pk[i].w};
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const uint32_t chunk = static_cast<uint32_t>((c & 1) * 4 + j) ^ (r & 7);
-                        sts128(rowb + chunk * 16, dequant_word(words[j], gc));
+            const uint32_t* srow = reinterpret_cast<const uint32_t*>(
+                p.g_scale + static_cast<int64_t>(row_ok ? n0 + r : 0) * gpr);
+            for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                if (it % G != g) continue;
+                const int stage = it % PS;
+                const uint32_t phase = (it / PS) & 1;
+                // the two fp16 group scales of this row and k-block: one aligned 32-bit load
+                uint32_t sc2 = 0;
+                if (row_ok) {
+                    if ((gpr & 1) == 0) {
+                        sc2 = __ldg(srow + kb);
+                    } else {  // odd group count: rows are only 2-byte aligned
+                        const uint16_t* s16 = reinterpret_cast<const uint16_t*>(srow);
+                        sc2 = __ldg(s16 + 2 * kb);
+                        if (2 * kb + 1 < gpr) sc2 |= static_cast<uint32_t>(__ldg(s16 + 2 * kb + 1)) << 16;
                     }
                 }
+                mbar_wait(pfull0 + 8 * stage, phase);
+                const uint32_t ps = sP + stage * Cfg::P_BYTES;
+                const uint4 pk0 = lds128(ps + poff0);
+                const uint4 pk1 = lds128(ps + poff1);
+                uint4 o[8];
+                {
+                    const GroupConst gc = group_const(__half2float(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu))));
+                    o[0] = dequant_word(pk0.x, gc); o[1] = dequant_word(pk0.y, gc);
+                    o[2] = dequant_word(pk0.z, gc); o[3] = dequant_word(pk0.w, gc);
+                }
+                {
+                    const GroupConst gc = group_const(__half2float(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16))));
+                    o[4] = dequant_word(pk1.x, gc); o[5] = dequant_word(pk1.y, gc);
+                    o[6] = dequant_word(pk1.z, gc); o[7] = dequant_word(pk1.w, gc);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(pempty0 + 8 * stage);   // packed bytes are in registers
+                mbar_wait(aempty0 + 8 * g, aphase ^ 1);            // MMAs reading this A buffer retired
+#pragma unroll
+                for (int j = 0; j < 8; ++j) sts128(rowb + ((static_cast<uint32_t>(j) ^ xr) << 4), o[j]);
                 fence_proxy_async_smem();                  // generic-proxy writes -> async proxy (MMA)
                 __syncwarp();
-                if (lane == 0) {                           // one arrival per warp, not per thread
-                    mbar_arrive(afull0 + 8 * ab);
-                    mbar_arrive(empty0 + 8 * stage);       // packed bytes consumed
-                }
-                if (++stage == STAGES) { stage = 0; phase ^= 1; }
-                if (++ab == NA) { ab = 0; aphase ^= 1; }
+                if (lane == 0) mbar_arrive(afull0 + 8 * g);        // one arrival per warp
+                aphase ^= 1;
             }
         }
-    } else {
-        // ------------------------------------------------------------ epilogue (warps 2..5)
+        if ((dw & 3) == 0 && lane == 0) prof_stamp(p, 2 + g, t_start);
+    } else if (warp >= W4_EPI_WARP0) {
+        // ------------------------------------------------------------ epilogue (warps 4..7)
         const int q = warp & 3;
         int acc = 0;
         uint32_t acc_phase = 0;
@@ -308,19 +369,43 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             if (p.bias && n_ok) bv = __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[n]);
             mbar_wait(tfull0 + 8 * acc, acc_phase);
             tc_fence_after();
+            if (q == 0 && lane == 0) prof_stamp(p, 8 + 2 * min(3, (u - blockIdx.x) / gridDim.x), t_start);
             const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
             if (S == 1) {
+                // Transpose through shared memory: this thread owns output channel n and 32 tokens
+                // of the chunk; it writes its column of the [32 tokens x 32 channels] block (rows of
+                // 64 B bf16 / 128 B fp32, swizzled as the output tensor map expects), then one TMA
+                // store writes the block -- coalesced, asynchronous, clipped at M and N.
+                const uint32_t stg = base + Cfg::STG_OFF + (warp - W4_EPI_WARP0) * Cfg::STG_BYTES;
 #pragma unroll 1
                 for (int c = 0; c < TT / 32; ++c) {
-                    uint32_t v[32];
-                    tmem_ld_32x32b_x32(t_addr + c * 32, v);
-                    tmem_wait_ld();
+                    if (lane == 0) tma_store_wait_read<0>();   // previous block left the staging buffer
+                    __syncwarp();
+#pragma unroll 1
+                    for (int gq = 0; gq < 4; ++gq) {           // 8 tokens per step keeps the code small
+                        uint32_t v[8];
+                        tmem_ld_32x32b_x8(t_addr + c * 32 + gq * 8, v);
+                        tmem_wait_ld();
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const int tok = t0 + c * 32 + j;
-                        if (n_ok && tok < p.M)
-                            w4_store(p.Y, p.out_t, static_cast<int64_t>(tok) * p.N + n,
-                                     w4_finish(__uint_as_float(v[j]) + bv, p.act));
+                        for (int jj = 0; jj < 8; ++jj) {
+                            const int j = gq * 8 + jj;         // token row inside the block
+                            float y = __uint_as_float(v[jj]) + bv;
+                            if (GELU) y = gelu_erf(y);
+                            if (p.out_t == ARIA_BF16) {
+                                const uint32_t off = j * 64 + ((((lane * 2) >> 4) ^ ((j >> 1) & 3)) << 4) + ((lane * 2) & 15);
+                                const uint16_t h = __bfloat16_as_ushort(__float2bfloat16_rn(y));
+                                asm volatile("st.shared.u16 [%0], %1;" ::"r"(stg + off), "h"(h) : "memory");
+                            } else {
+                                const uint32_t off = j * 128 + ((((lane * 4) >> 4) ^ (j & 7)) << 4) + ((lane * 4) & 15);
+                                asm volatile("st.shared.f32 [%0], %1;" ::"r"(stg + off), "f"(y) : "memory");
+                            }
+                        }
+                    }
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) {
+                        tma_store_2d(&tmY, stg, n0 + q * 32, t0 + c * 32);
+                        tma_store_commit();
                     }
                 }
                 tc_fence_before();
@@ -329,13 +414,13 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             } else {
                 float* part = p.partials + static_cast<int64_t>(sp) * p.M * p.N;
 #pragma unroll 1
-                for (int c = 0; c < TT / 32; ++c) {
-                    uint32_t v[32];
-                    tmem_ld_32x32b_x32(t_addr + c * 32, v);
+                for (int c8 = 0; c8 < TT / 8; ++c8) {
+                    uint32_t v[8];
+                    tmem_ld_32x32b_x8(t_addr + c8 * 8, v);
                     tmem_wait_ld();
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const int tok = t0 + c * 32 + j;
+                    for (int j = 0; j < 8; ++j) {
+                        const int tok = t0 + c8 * 8 + j;
                         if (n_ok && tok < p.M)
                             __stcg(part + static_cast<int64_t>(tok) * p.N + n, __uint_as_float(v[j]));
                     }
@@ -367,16 +452,17 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {
                             const int64_t idx = static_cast<int64_t>(t0 + j0 + j) * p.N + n;
-                            if (n_ok && j0 + j < tmax) w4_store(p.Y, p.out_t, idx, w4_finish(y[j] + bv, p.act));
+                            if (n_ok && j0 + j < tmax) w4_store(p.Y, p.out_t, idx, GELU ? gelu_erf(y[j] + bv) : y[j] + bv);
                         }
                     }
-                    if (lane == 0) p.counters[tile * 4 + q] = 0;  // ready for the next launch
                 }
             }
+            if (q == 0 && lane == 0) prof_stamp(p, 9 + 2 * min(3, (u - blockIdx.x) / gridDim.x), t_start);
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
         }
     }
 
+    if (warp >= W4_EPI_WARP0 && warp < W4_DEQ_WARP0 && lane == 0) tma_store_wait<0>();
     pdl_launch_dependents();
     tc_fence_before();
     __syncthreads();
@@ -386,26 +472,29 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     }
 }
 
-template <int TT, int BK>
+template <int TT, bool GELU>
 static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, const W4Params& p,
                      int grid, cudaStream_t st, bool pdl) {
-    using Cfg = W4Cfg<TT, BK>;
+    using Cfg = W4Cfg<TT>;
     static bool attr_set = false;
-    auto kern = w4a16_gemm_kernel<TT, BK>;
+    auto kern = w4a16_gemm_kernel<TT, GELU>;
     if (!attr_set) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES) !=
             cudaSuccess)
             return ARIA_ERR_CUDA;
         attr_set = true;
     }
-    CUtensorMap tmP, tmX;
+    CUtensorMap tmP, tmX, tmY;
     int rc = make_tmap_2d(&tmP, Wq4, 1, N, K / 2, W4_BN, Cfg::P_ROW, Cfg::P_ROW);
     if (rc != ARIA_OK) return rc;
     rc = make_tmap_2d(&tmX, X, 2, M, K, TT, 64, 128);
     if (rc != ARIA_OK) return rc;
+    // output: box = 32 tokens x 32 channels (64 B bf16 rows / 128 B fp32 rows)
+    rc = make_tmap_2d(&tmY, p.Y, p.out_t == ARIA_F32 ? 4 : 2, M, N, 32, 32, p.out_t == ARIA_F32 ? 128 : 64);
+    if (rc != ARIA_OK) return rc;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(W4_THREADS);
+    cfg.blockDim = dim3(Cfg::THREADS);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute at[1];
@@ -413,15 +502,14 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kern, tmP, tmX, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    return cudaLaunchKernelEx(&cfg, kern, tmP, tmX, tmY, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
-// Split-K plan shared by the launcher and aria_workspace_bytes.
-void w4_plan(int M, int N, int K, int sms, int* tt_out, int* bk_out, int* splits_out) {
+// Tile / split-K plan shared by the launcher and aria_workspace_bytes.
+void w4_plan(int M, int N, int K, int sms, int* tt_out, int* splits_out) {
     const int tt = M <= 32 ? 32 : M <= 64 ? 64 : M <= 128 ? 128 : 256;
-    const int bk = tt <= 64 ? 128 : 64;
     const int tiles = ((N + W4_BN - 1) / W4_BN) * ((M + tt - 1) / tt);
-    const int num_kb = (K + bk - 1) / bk;
+    const int num_kb = (K + W4_BK - 1) / W4_BK;
     int s = 1;
     if (tiles * 2 <= sms) {  // less than half the machine busy: split K
         s = sms / tiles;
@@ -429,12 +517,12 @@ void w4_plan(int M, int N, int K, int sms, int* tt_out, int* bk_out, int* splits
         if (s > 16) s = 16;
         if (s < 1) s = 1;
     }
-    *tt_out = tt; *bk_out = bk; *splits_out = s;
+    *tt_out = tt; *splits_out = s;
 }
 
 size_t w4_workspace_bytes(int M, int N, int K, int sms) {
-    int tt, bk, s;
-    w4_plan(M, N, K, sms, &tt, &bk, &s);
+    int tt, s;
+    w4_plan(M, N, K, sms, &tt, &s);
     const size_t tiles = static_cast<size_t>((N + W4_BN - 1) / W4_BN) * ((M + tt - 1) / tt);
     size_t counters = (tiles * 4 * sizeof(unsigned) + 255) / 256 * 256;
     size_t partials = s > 1 ? static_cast<size_t>(s) * M * N * sizeof(float) : 0;
@@ -446,12 +534,13 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
                       cudaStream_t st, bool pdl) {
     const int sms = num_sms();
     if (sms <= 0) return ARIA_ERR_CUDA;
-    int tt, bk, s;
-    w4_plan(M, N, K, sms, &tt, &bk, &s);
+    int tt, s;
+    w4_plan(M, N, K, sms, &tt, &s);
     if (s > 1 && (ws == nullptr || ws_bytes < w4_workspace_bytes(M, N, K, sms))) s = 1;
     W4Params p;
     p.g_scale = g_scale; p.bias = bias; p.Y = Y;
     p.act = act; p.out_t = yt; p.M = M; p.N = N; p.K = K; p.splits = s;
+    p.prof = g_w4_prof;
     const size_t tiles = static_cast<size_t>((N + W4_BN - 1) / W4_BN) * ((M + tt - 1) / tt);
     p.counters = static_cast<unsigned*>(ws);
     p.partials = s > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) +
@@ -461,10 +550,15 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
     const int grid = units < sms ? units : sms;
     if (s > 1 && cudaMemsetAsync(p.counters, 0, tiles * 4 * sizeof(unsigned), st) != cudaSuccess)
         return ARIA_ERR_CUDA;
-    if (tt == 32) return launch_w4<32, 128>(X, M, K, Wq4, N, p, grid, st, pdl);
-    if (tt == 64) return launch_w4<64, 128>(X, M, K, Wq4, N, p, grid, st, pdl);
-    if (tt == 128) return launch_w4<128, 64>(X, M, K, Wq4, N, p, grid, st, pdl);
-    return launch_w4<256, 64>(X, M, K, Wq4, N, p, grid, st, pdl);
+    const bool gelu = act == ARIA_ACT_GELU_ERF;
+#define ARIA_W4_LAUNCH(TTV)                                                        \
+    return gelu ? launch_w4<TTV, true>(X, M, K, Wq4, N, p, grid, st, pdl)          \
+                : launch_w4<TTV, false>(X, M, K, Wq4, N, p, grid, st, pdl)
+    if (tt == 32) { ARIA_W4_LAUNCH(32); }
+    if (tt == 64) { ARIA_W4_LAUNCH(64); }
+    if (tt == 128) { ARIA_W4_LAUNCH(128); }
+    ARIA_W4_LAUNCH(256);
+#undef ARIA_W4_LAUNCH
 }
 
 }  // namespace aria

@@ -60,28 +60,9 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, ui
                  : "memory");
 }
 
-// Stage one warp's [32 rows x 64 bytes] block (thread = row, w[16] = its 64 bytes) in the 64-byte
-// swizzle the output tensor map expects, and hand it to the TMA store engine.  TMA clips rows >= M
-// and columns >= N, so tails need no masking.
-__device__ __forceinline__ void w8_store_block(const CUtensorMap* tmY, uint32_t stg, int lane,
-                                               const uint32_t (&w)[16], int col0, int row0) {
-    if (lane == 0) tma_store_wait_read<0>();  // the previous store has finished reading `stg`
-    __syncwarp();
-    const uint32_t rowb = stg + lane * 64;
-    const uint32_t x = (lane >> 1) & 3;
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-        sts128(rowb + ((c ^ x) << 4), w[4 * c], w[4 * c + 1], w[4 * c + 2], w[4 * c + 3]);
-    fence_proxy_async_smem();
-    __syncwarp();
-    if (lane == 0) {
-        tma_store_2d(tmY, stg, col0, row0);
-        tma_store_commit();
-    }
-}
-
-// OUT_T: 0 = fp32, 1 = bf16, 2 = raw int32 accumulators.
-template <int BN, int OUT_T>
+// OUT_T: 0 = fp32, 1 = bf16, 2 = raw int32 accumulators.  GELU: apply exact-erf GELU (compiled in only
+// where used: 32 inlined erff bodies would thrash the instruction cache of every role).
+template <int BN, int OUT_T, bool GELU>
 __global__ void __launch_bounds__(W8_THREADS, 1)
 w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                  const __grid_constant__ CUtensorMap tmY, const W8Params p) {
@@ -212,47 +193,68 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             mbar_wait(tfull0 + 8 * acc, acc_phase);
             tc_fence_after();
             const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
+            // Column groups of 8: tcgen05.ld x8 -> scale/bias/GELU -> 16 B (bf16) or 32 B (fp32/int32)
+            // of this thread's row into the 64-byte-swizzled [32 rows x 64 B] staging block; every
+            // 64 B of columns one TMA store (clipped at M / N by the tensor map).
+            constexpr int GPB = OUT_T == 1 ? 4 : 2;   // 8-column groups per 64-byte block
+            const uint32_t rowb = stg + lane * 64;
+            const uint32_t xr = (lane >> 1) & 3;
 #pragma unroll 1
             for (int c = half; c < BN / 32; c += 2) {
-                uint32_t v[32];
-                tmem_ld_32x32b_x32(t_addr + c * 32, v);
-                tmem_wait_ld();
-                const int col0 = n0 + c * 32;
-                if (OUT_T == 2) {
-                    uint32_t w[16];
+#pragma unroll 1
+                for (int gq = 0; gq < 4; ++gq) {
+                    uint32_t v[8];
+                    tmem_ld_32x32b_x8(t_addr + c * 32 + gq * 8, v);
+                    tmem_wait_ld();
+                    const int cb = c * 32 + gq * 8;   // column inside the tile
+                    uint32_t w[8];
+                    if (OUT_T == 2) {
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) w[j] = v[j];
-                    w8_store_block(&tmY, stg, lane, w, col0, row0);
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) w[j] = v[16 + j];
-                    w8_store_block(&tmY, stg, lane, w, col0 + 16, row0);
-                } else {
-                    float f[32];
-#pragma unroll
-                    for (int j = 0; j < 32; j += 4) {
-                        const float4 s4 = *reinterpret_cast<const float4*>(swb + c * 32 + j);
-                        const float4 b4 = *reinterpret_cast<const float4*>(swb + BN + c * 32 + j);
-                        f[j] = fmaf(static_cast<float>(static_cast<int32_t>(v[j])) * sxv, s4.x, b4.x);
-                        f[j + 1] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 1])) * sxv, s4.y, b4.y);
-                        f[j + 2] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 2])) * sxv, s4.z, b4.z);
-                        f[j + 3] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 3])) * sxv, s4.w, b4.w);
-                    }
-                    if (p.act == ARIA_ACT_GELU_ERF) {
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) f[j] = gelu_erf(f[j]);
-                    }
-                    uint32_t w[16];
-                    if (OUT_T == 1) {
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) w[j] = pack_bf16x2(f[2 * j], f[2 * j + 1]);
-                        w8_store_block(&tmY, stg, lane, w, col0, row0);
+                        for (int j = 0; j < 8; ++j) w[j] = v[j];
                     } else {
+                        float f[8];
+                        const float4 s0 = *reinterpret_cast<const float4*>(swb + cb);
+                        const float4 s1 = *reinterpret_cast<const float4*>(swb + cb + 4);
+                        const float4 b0 = *reinterpret_cast<const float4*>(swb + BN + cb);
+                        const float4 b1 = *reinterpret_cast<const float4*>(swb + BN + cb + 4);
+                        f[0] = fmaf(static_cast<float>(static_cast<int32_t>(v[0])) * sxv, s0.x, b0.x);
+                        f[1] = fmaf(static_cast<float>(static_cast<int32_t>(v[1])) * sxv, s0.y, b0.y);
+                        f[2] = fmaf(static_cast<float>(static_cast<int32_t>(v[2])) * sxv, s0.z, b0.z);
+                        f[3] = fmaf(static_cast<float>(static_cast<int32_t>(v[3])) * sxv, s0.w, b0.w);
+                        f[4] = fmaf(static_cast<float>(static_cast<int32_t>(v[4])) * sxv, s1.x, b1.x);
+                        f[5] = fmaf(static_cast<float>(static_cast<int32_t>(v[5])) * sxv, s1.y, b1.y);
+                        f[6] = fmaf(static_cast<float>(static_cast<int32_t>(v[6])) * sxv, s1.z, b1.z);
+                        f[7] = fmaf(static_cast<float>(static_cast<int32_t>(v[7])) * sxv, s1.w, b1.w);
+                        if (GELU) {
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[j]);
-                        w8_store_block(&tmY, stg, lane, w, col0, row0);
+                            for (int j = 0; j < 8; ++j) f[j] = gelu_erf(f[j]);
+                        }
+                        if (OUT_T == 1) {
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[16 + j]);
-                        w8_store_block(&tmY, stg, lane, w, col0 + 16, row0);
+                            for (int j = 0; j < 4; ++j) w[j] = pack_bf16x2(f[2 * j], f[2 * j + 1]);
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) w[j] = __float_as_uint(f[j]);
+                        }
+                    }
+                    const int gb = gq % GPB;          // position of this group inside the 64-byte block
+                    if (gb == 0) {                    // first group of a block: staging must be free
+                        if (lane == 0) tma_store_wait_read<0>();
+                        __syncwarp();
+                    }
+                    if (OUT_T == 1) {
+                        sts128(rowb + ((static_cast<uint32_t>(gb) ^ xr) << 4), w[0], w[1], w[2], w[3]);
+                    } else {
+                        sts128(rowb + ((static_cast<uint32_t>(2 * gb) ^ xr) << 4), w[0], w[1], w[2], w[3]);
+                        sts128(rowb + ((static_cast<uint32_t>(2 * gb + 1) ^ xr) << 4), w[4], w[5], w[6], w[7]);
+                    }
+                    if (gb == GPB - 1) {              // block complete: hand it to the TMA store engine
+                        fence_proxy_async_smem();
+                        __syncwarp();
+                        if (lane == 0) {
+                            tma_store_2d(&tmY, stg, n0 + cb + 8 - 8 * GPB, row0);
+                            tma_store_commit();
+                        }
                     }
                 }
             }
@@ -273,12 +275,12 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     }
 }
 
-template <int BN, int OUT_T>
+template <int BN, int OUT_T, bool GELU>
 static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmY,
                       const W8Params& p, int grid, cudaStream_t st, bool pdl) {
     using Cfg = W8Cfg<BN>;
     static bool attr_set = false;
-    auto kern = w8a8_gemm_kernel<BN, OUT_T>;
+    auto kern = w8a8_gemm_kernel<BN, OUT_T, GELU>;
     if (!attr_set) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES) !=
             cudaSuccess)
@@ -301,10 +303,13 @@ static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUte
 template <int BN>
 static int launch_bn(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmY,
                      const W8Params& p, int out_t, int grid, cudaStream_t st, bool pdl) {
+    const bool gelu = p.act == ARIA_ACT_GELU_ERF;
     switch (out_t) {
-        case 0: return launch_one<BN, 0>(tmA, tmB, tmY, p, grid, st, pdl);
-        case 1: return launch_one<BN, 1>(tmA, tmB, tmY, p, grid, st, pdl);
-        default: return launch_one<BN, 2>(tmA, tmB, tmY, p, grid, st, pdl);
+        case 0: return gelu ? launch_one<BN, 0, true>(tmA, tmB, tmY, p, grid, st, pdl)
+                            : launch_one<BN, 0, false>(tmA, tmB, tmY, p, grid, st, pdl);
+        case 1: return gelu ? launch_one<BN, 1, true>(tmA, tmB, tmY, p, grid, st, pdl)
+                            : launch_one<BN, 1, false>(tmA, tmB, tmY, p, grid, st, pdl);
+        default: return launch_one<BN, 2, false>(tmA, tmB, tmY, p, grid, st, pdl);
     }
 }
 

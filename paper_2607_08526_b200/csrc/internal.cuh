@@ -41,5 +41,6 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
                       int N, const void* bias, int act, void* Y, int yt, void* ws, size_t ws_bytes,
                       cudaStream_t st, bool pdl);
 size_t w4_workspace_bytes(int M, int N, int K, int sms);
+void w4_set_profile_buffer(long long* p);  // debug hook: per-CTA role timestamps
 
 }  // namespace aria

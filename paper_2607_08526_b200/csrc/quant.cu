@@ -32,6 +32,30 @@ __device__ __forceinline__ void load8<__nv_bfloat16>(const __nv_bfloat16* p, flo
     }
 }
 
+// Raw (still packed) 8-element vectors: what the warp-per-row kernel keeps in registers.
+template <typename T> struct Raw8;
+template <> struct Raw8<float> { float4 a, b; };
+template <> struct Raw8<__nv_bfloat16> { uint4 a; };
+__device__ __forceinline__ void load_raw(const float* p, Raw8<float>& r) {
+    r.a = __ldg(reinterpret_cast<const float4*>(p));
+    r.b = __ldg(reinterpret_cast<const float4*>(p) + 1);
+}
+__device__ __forceinline__ void load_raw(const __nv_bfloat16* p, Raw8<__nv_bfloat16>& r) {
+    r.a = __ldg(reinterpret_cast<const uint4*>(p));
+}
+__device__ __forceinline__ void unpack8(const Raw8<float>& r, float (&v)[8]) {
+    v[0] = r.a.x; v[1] = r.a.y; v[2] = r.a.z; v[3] = r.a.w;
+    v[4] = r.b.x; v[5] = r.b.y; v[6] = r.b.z; v[7] = r.b.w;
+}
+__device__ __forceinline__ void unpack8(const Raw8<__nv_bfloat16>& r, float (&v)[8]) {
+    const uint32_t w[4] = {r.a.x, r.a.y, r.a.z, r.a.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        v[2 * i] = __uint_as_float(w[i] << 16);
+        v[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+    }
+}
+
 __device__ __forceinline__ float absmax8(const float (&v)[8], float a) {
 #pragma unroll
     for (int i = 0; i < 8; ++i) a = fmaxf(a, fabsf(v[i]));
@@ -41,6 +65,44 @@ __device__ __forceinline__ float absmax8(const float (&v)[8], float a) {
 __device__ __forceinline__ int quant1(float x, float s, int lim) {
     int q = __float2int_rn(__fdiv_rn(x, s));
     return max(-lim, min(lim, q));
+}
+
+// Exact rint(fl32(x / s)) without a division per element.  With r = RN(1/s), r_lo = r (1 - 2^-20) and
+// r_hi = r (1 + 2^-20) bracket 1/s by far more than the rounding of r, so for every x the exact
+// quotient AND its fp32 rounding lie between x*r_lo and x*r_hi.  fma(x, r_*, 1.5*2^23) rounds the
+// exact product to an integer (ties to even) in the low mantissa bits; rint is monotone, so if both
+// ends give the same integer, rint(fl32(x/s)) is that integer (a tie strictly inside the bracket
+// would separate the two ends).  Otherwise (|x/s| within ~1e-4 of a .5 boundary, probability ~2e-4)
+// the caller falls back to the IEEE division.  |x/s| <= 127 (1 + 2^-23): no clamp is needed.
+struct FastQ {
+    float r_lo, r_hi;
+    bool ok;  // false: s is outside the range where r is finite and normal -> always divide
+};
+__device__ __forceinline__ FastQ make_fastq(float s) {
+    FastQ f;
+    const float r = __frcp_rn(s);
+    f.r_lo = r * 0.99999904632568359375f;   // 1 - 2^-20
+    f.r_hi = r * 1.00000095367431640625f;   // 1 + 2^-20
+    f.ok = (s > 1e-30f) && (s < 1e30f);
+    return f;
+}
+constexpr float QMAGIC = 12582912.0f;  // 1.5 * 2^23: float bits 0x4B400000 + q
+
+// Quantise 8 values; returns false if any needs the exact-division path.
+__device__ __forceinline__ bool quant8_fast(const float (&v)[8], const FastQ& f, uint2& out) {
+    uint32_t y[8];
+    bool same = true;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const uint32_t a = __float_as_uint(fmaf(v[i], f.r_lo, QMAGIC));
+        const uint32_t b = __float_as_uint(fmaf(v[i], f.r_hi, QMAGIC));
+        same = same && (a == b);
+        y[i] = a;
+    }
+    // low byte of each y is the two's-complement code
+    out.x = __byte_perm(__byte_perm(y[0], y[1], 0x0040), __byte_perm(y[2], y[3], 0x0040), 0x5410);
+    out.y = __byte_perm(__byte_perm(y[4], y[5], 0x0040), __byte_perm(y[6], y[7], 0x0040), 0x5410);
+    return same;
 }
 
 __device__ __forceinline__ uint2 quant8_i8(const float (&v)[8], float s) {
@@ -92,15 +154,69 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
     const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
     if (tid == 0) scale[row] = s;
     pdl_launch_dependents();
+    const FastQ f = make_fastq(s);
 #pragma unroll
     for (int i = 0; i < QROW_CACHE; ++i) {
         const int idx = tid + i * nthr;
-        if (idx < nvec) *reinterpret_cast<uint2*>(q + 8 * idx) = quant8_i8(v[i], s);
+        if (idx < nvec) {
+            uint2 o;
+            if (!f.ok || !quant8_fast(v[i], f, o)) o = quant8_i8(v[i], s);
+            *reinterpret_cast<uint2*>(q + 8 * idx) = o;
+        }
     }
     for (int idx = tid + QROW_CACHE * nthr; idx < nvec; idx += nthr) {
         float t[8];
         load8<T>(x + 8 * idx, t);
-        *reinterpret_cast<uint2*>(q + 8 * idx) = quant8_i8(t, s);
+        uint2 o;
+        if (!f.ok || !quant8_fast(t, f, o)) o = quant8_i8(t, s);
+        *reinterpret_cast<uint2*>(q + 8 * idx) = o;
+    }
+}
+
+// One WARP per row (K <= 8 * 32 * VPL): every lane issues all its 16-byte loads up front, the
+// absmax is a pure shuffle reduction, no shared memory and no block barrier.
+template <typename T, int VPL>
+__global__ void __launch_bounds__(256)
+quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restrict__ Xq,
+                          float* __restrict__ scale) {
+    pdl_wait_prior_grid();
+    const int lane = threadIdx.x & 31;
+    const int64_t row = static_cast<int64_t>(blockIdx.x) * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= R) return;
+    const T* x = X + row * K;
+    int8_t* q = Xq + row * K;
+    const int nvec = K >> 3;
+    Raw8<T> raw[VPL];
+#pragma unroll
+    for (int i = 0; i < VPL; ++i) {
+        const int idx = lane + 32 * i;
+        if (idx < nvec) load_raw(x + 8 * idx, raw[i]);
+    }
+    float a = 0.0f;
+#pragma unroll
+    for (int i = 0; i < VPL; ++i) {
+        if (lane + 32 * i < nvec) {
+            float v[8];
+            unpack8(raw[i], v);
+            a = absmax8(v, a);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
+    const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
+    if (lane == 0) scale[row] = s;
+    pdl_launch_dependents();
+    const FastQ f = make_fastq(s);
+#pragma unroll
+    for (int i = 0; i < VPL; ++i) {
+        const int idx = lane + 32 * i;
+        if (idx < nvec) {
+            float v[8];
+            unpack8(raw[i], v);
+            uint2 o;
+            if (!f.ok || !quant8_fast(v, f, o)) o = quant8_i8(v, s);
+            *reinterpret_cast<uint2*>(q + 8 * idx) = o;
+        }
     }
 }
 
@@ -130,9 +246,42 @@ quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restri
     }
 }
 
+template <typename T, int VPL>
+static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, float* s,
+                                    cudaLaunchConfig_t& cfg) {
+    cfg.blockDim = dim3(256);
+    cfg.gridDim = dim3((R + 7) / 8);
+    return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s);
+}
+
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
                          bool pdl) {
     const int nvec = C / 8;
+    {   // warp-per-row variants: bf16 rows up to 6144, fp32 rows up to 3072 elements
+        cudaLaunchConfig_t cfg = {};
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = pdl ? 1 : 0;
+        const int vpl = (nvec + 31) / 32;
+        cudaError_t e = cudaErrorInvalidValue;
+        bool done = true;
+        if (xt == ARIA_BF16) {
+            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg);
+            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg);
+            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg);
+            else if (vpl <= 24) e = launch_warp_rows<__nv_bfloat16, 24>(X, R, C, q, s, cfg);
+            else done = false;
+        } else {
+            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg);
+            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg);
+            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg);
+            else done = false;
+        }
+        if (done) return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    }
     int threads = ((nvec + 31) / 32) * 32;
     threads = threads > QROW_MAX_THREADS ? QROW_MAX_THREADS : threads;
     cudaLaunchConfig_t cfg = {};
