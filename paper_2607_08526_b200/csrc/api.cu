@@ -201,6 +201,8 @@ int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, in
 /* Debug hook (not in aria.h): per-CTA role timestamps of the W4A16 kernel, 16 int64 per CTA. */
 __attribute__((visibility("default"))) void aria_debug_w4_profile(long long* buf) { w4_set_profile_buffer(buf); }
 
+__attribute__((visibility("default"))) void aria_debug_w8_profile(long long* buf) { w8_set_profile_buffer(buf); }
+
 int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mode, int io, void* ws,
                           size_t ws_bytes, void* stream) {
     int maxK, maxN;

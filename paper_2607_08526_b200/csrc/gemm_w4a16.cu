@@ -221,6 +221,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     const uint32_t tmem_base = *tmem_slot_g;
 
     pdl_wait_prior_grid();
+    pdl_launch_dependents();   // the next kernel may become resident now; it blocks in its own wait
     const long long t_start = clock64();
 
     if (warp == 0) {
@@ -463,7 +464,6 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     }
 
     if (warp >= W4_EPI_WARP0 && warp < W4_DEQ_WARP0 && lane == 0) tma_store_wait<0>();
-    pdl_launch_dependents();
     tc_fence_before();
     __syncthreads();
     if (warp == 1) {

@@ -35,6 +35,8 @@ struct W8Epilogue {
 int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, const W8Epilogue& ep,
                      cudaStream_t st, bool pdl);
 
+void w8_set_profile_buffer(long long* p);  // debug hook: per-CTA role timestamps
+
 // ---- gemm_w4a16.cu
 // ws: split-K partials + tile counters (w4_workspace_bytes); too small / null -> no split-K.
 int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uint16_t* g_scale,

@@ -180,6 +180,7 @@ __global__ void __launch_bounds__(256)
 quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restrict__ Xq,
                           float* __restrict__ scale) {
     pdl_wait_prior_grid();
+    pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
     const int64_t row = static_cast<int64_t>(blockIdx.x) * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (row >= R) return;
@@ -205,7 +206,6 @@ quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restr
     for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
     const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
     if (lane == 0) scale[row] = s;
-    pdl_launch_dependents();
     const FastQ f = make_fastq(s);
 #pragma unroll
     for (int i = 0; i < VPL; ++i) {
