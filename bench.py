@@ -294,7 +294,9 @@ def run_ours(args):
                 "peak_source": f"{pk['source']} bf16 sustained x {NOMINAL_INT8_OVER_BF16:g} (nominal int8/bf16)",
                 "frac_of_burst": ach / (pk["bf16_burst"] * NOMINAL_INT8_OVER_BF16),
                 "frac_of_nominal_4500": ach / 4500.0, "avg_launch_us": dur * 1e6, "launches": n_l,
-                "traffic": None}
+                # dram__bytes_read.sum + dram__bytes_write.sum per launch, mean of the 4 consecutive layers
+                # captured with `ncu --set full` in profiles/r1b_w8a8_full.md (10.28, 5.54, 12.66, 22.06 MB)
+                "traffic": 12.64e6, "traffic_unit": "bytes/launch (ncu, profiles/r1b_w8a8_full.md)"}
 
     # ---- e2e: same step through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
