@@ -129,6 +129,16 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------ our arm
+def max_over_ranks(value: float, dist, device="cuda") -> float:
+    """Replicas only: the job's step time is the slowest rank's; no data-path collective."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def time_region(torch, fn, iters):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
@@ -256,10 +266,7 @@ def run_ours(args):
     total_ms = ev[0].elapsed_time(ev[-1])
     t8 = sum(ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)) / args.steps
     t4 = sum(ev[2 * i + 1].elapsed_time(ev[2 * i + 2]) for i in range(args.steps)) / args.steps
-    if dist:
-        t = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist)
     ms_step = total_ms / args.steps
     ops_step = st8.ops + st4.ops
     value = world * ops_step / (ms_step * 1e-3) / 1e12

@@ -1,5 +1,6 @@
 // api.cu -- the extern "C" boundary declared in include/aria.h: argument validation and the
 // sequencing of kernels.  Device entry points only enqueue on the caller's stream.
+#include <cstdlib>
 #include <cstring>
 
 #include "internal.cuh"
@@ -60,13 +61,14 @@ int check_layers(const aria_layer* layers, int n_layers, int M, int mode, int io
 
 int run_layer(const aria_layer& L, const void* in, void* out, int M, int mode, int io, void* ws,
               size_t ws_bytes, cudaStream_t st) {
+    static const bool pdl = getenv("ARIA_NO_PDL") == nullptr;   // debug switch
     if (mode == ARIA_W8A8)
         return linear_w8a8_impl(in, io, M, L.K, static_cast<const int8_t*>(L.wq),
                                 static_cast<const float*>(L.w_scale), L.N, L.bias, io, L.act, out, io,
-                                ws, st, true);
+                                ws, st, pdl);
     return launch_gemm_w4a16(in, M, L.K, static_cast<const uint8_t*>(L.wq),
                              static_cast<const uint16_t*>(L.w_scale), L.N, L.bias, L.act, out, io, ws,
-                             ws_bytes, st, true);
+                             ws_bytes, st, pdl);
 }
 
 }  // namespace
@@ -97,9 +99,8 @@ size_t aria_workspace_bytes(int M, int maxK, int maxN, int mode) {
         // partials never exceed #SMs * 128 * TT * 4 bytes; one counter quad per tile.
         int sms = num_sms();
         if (sms <= 0) sms = 148;
-        const size_t tt = M <= 32 ? 32 : M <= 64 ? 64 : M <= 128 ? 128 : 256;
         size_t tiles = static_cast<size_t>((maxN + 127) / 128) * ((M + 31) / 32);
-        return up256(tiles * 16) + up256(static_cast<size_t>(sms) * 128 * tt * 4);
+        return up256(tiles * 16) + up256(static_cast<size_t>(sms) * 128 * 256 * 4);
     }
     return 0;
 }

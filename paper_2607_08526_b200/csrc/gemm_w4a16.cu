@@ -15,8 +15,8 @@
 //                B = X, into one of two TMEM accumulators.
 //   warps 4..7   epilogue: tcgen05.ld -> (+bias, GELU, cast) -> smem transpose -> TMA store, or
 //                split-K partials.
-//   warps 8..    G dequantiser GROUPS of 4 warps (thread = weight row).  Group g owns A buffer g and
-//                handles k-blocks g, g+G, ...: wait packed -> LDS -> 64 x (LOP3, FFMA2/2, CVT/2) into
+//   warps 8..    G dequantiser GROUPS of 4 warps (thread = weight row).  Group g handles k-blocks
+//                g, g+G, ... (A buffer = k-block index mod NB): wait packed -> LDS -> 64 x (LOP3, FFMA2/2, CVT/2) into
 //                registers -> wait A buffer free -> 8 STS -> fence -> arrive.  The arithmetic is done
 //                BEFORE waiting for the buffer, so the MMA -> dequant -> MMA hand-off is short.
 // Exactness of w^ = bf16_rne(q*sg): the nibble n is placed (XOR 8 = offset binary u = q+8) at
@@ -28,6 +28,8 @@
 // Split-K (small M): a work unit is (tile, k-range); units of a tile write fp32 partials to the
 // workspace, the last to arrive (per 32-channel quarter, atomic counter) sums them in split order
 // -- deterministic -- and finishes the epilogue.
+#include <cstdlib>
+
 #include "internal.cuh"
 
 namespace aria {
@@ -38,23 +40,28 @@ constexpr int W4_EPI_WARP0 = 4;
 constexpr int W4_DEQ_WARP0 = 8;
 constexpr int W4_G = 3;         // dequantiser groups = A buffers
 
-template <int TT>
+// CTAS = 2: a CTA PAIR (cta_group::2) computes 256 output channels x TT tokens; each CTA dequantises its
+// own 128 weight rows and stages only HALF of the X tile, which halves the X traffic through shared
+// memory (TMA write + MMA read) -- the dominant term of the smem-bound k-block time.
+template <int TT, int CTAS = 1>
 struct W4Cfg {
     static constexpr int G = W4_G;
+    static constexpr int NB = CTAS == 2 ? 5 : G;               // dequantised A buffers (pair: deeper, see kernel)
     static constexpr int THREADS = 32 * W4_DEQ_WARP0 + 128 * G;
     static constexpr int P_ROW = W4_BK / 2;                    // 32 packed bytes per row per k-block
     static constexpr int P_BYTES = W4_BN * P_ROW;              // 4 KB
-    static constexpr int X_BYTES = TT * 128;                   // TT rows x 64 bf16
+    static constexpr int X_ROWS = TT / CTAS;                   // token rows staged by one CTA
+    static constexpr int X_BYTES = X_ROWS * 128;               // x 64 bf16
     static constexpr int A_BYTES = W4_BN * 128;                // 16 KB: 128 rows x 64 bf16
     static constexpr int STG_BYTES = 4096;                     // per epilogue warp: 32 tokens x 128 B
-    static constexpr int XS = TT == 256 ? 3 : TT == 128 ? 4 : TT == 64 ? 6 : 8;   // X ring depth
+    static constexpr int XS = X_ROWS == 256 ? 3 : X_ROWS == 128 ? 4 : X_ROWS == 64 ? 6 : 8;   // X ring depth
     static constexpr int PS = TT == 256 ? 8 : TT == 128 ? 12 : 16;                // packed ring depth
     static constexpr int X_OFF = 0;
     static constexpr int A_OFF = X_OFF + XS * X_BYTES;
-    static constexpr int P_OFF = A_OFF + G * A_BYTES;
+    static constexpr int P_OFF = A_OFF + NB * A_BYTES;
     static constexpr int STG_OFF = P_OFF + PS * P_BYTES;
     static constexpr int BAR_OFF = STG_OFF + 4 * STG_BYTES;
-    static constexpr int NBAR = 2 * XS + 2 * PS + 2 * G + 4;
+    static constexpr int NBAR = 2 * XS + 2 * PS + 3 * NB + 4;
     static constexpr int SMEM_BYTES = BAR_OFF + NBAR * 8 + 16 + 1024;
     static constexpr int ACC_STRIDE = TT;
     static constexpr int TMEM_COLS = 2 * TT < 32 ? 32 : 2 * TT;
@@ -161,12 +168,12 @@ __device__ __forceinline__ void w4_store(void* Y, int out_t, int64_t idx, float 
         static_cast<__nv_bfloat16*>(Y)[idx] = __float2bfloat16_rn(y);
 }
 
-template <int TT, bool GELU>
-__global__ void __launch_bounds__(W4Cfg<TT>::THREADS, 1)
+template <int TT, bool GELU, int CTAS>
+__global__ void __launch_bounds__(W4Cfg<TT, CTAS>::THREADS, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmX,
                   const __grid_constant__ CUtensorMap tmY, const W4Params p) {
-    using Cfg = W4Cfg<TT>;
-    constexpr int XS = Cfg::XS, PS = Cfg::PS, G = Cfg::G;
+    using Cfg = W4Cfg<TT, CTAS>;
+    constexpr int XS = Cfg::XS, PS = Cfg::PS, G = Cfg::G, NB = Cfg::NB;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;
@@ -175,19 +182,23 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     const uint32_t bars = base + Cfg::BAR_OFF;
     const uint32_t xfull0 = bars, xempty0 = xfull0 + 8 * XS;
     const uint32_t pfull0 = xempty0 + 8 * XS, pempty0 = pfull0 + 8 * PS;
-    const uint32_t afull0 = pempty0 + 8 * PS, aempty0 = afull0 + 8 * G;
-    const uint32_t tfull0 = aempty0 + 8 * G, tempty0 = tfull0 + 16;
+    const uint32_t afull0 = pempty0 + 8 * PS, aempty0 = afull0 + 8 * NB;
+    const uint32_t afwd0 = aempty0 + 8 * NB;                   // pair mode, peer CTA: local "A ready"
+    const uint32_t tfull0 = afwd0 + 8 * NB, tempty0 = tfull0 + 16;
     const uint32_t tmem_slot = tempty0 + 16;
     volatile uint32_t* tmem_slot_g =
         reinterpret_cast<volatile uint32_t*>(gbase + Cfg::BAR_OFF + Cfg::NBAR * 8);
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const int num_n = (p.N + W4_BN - 1) / W4_BN;
+    const uint32_t rank = CTAS == 2 ? cluster_ctarank() : 0u;   // position in the CTA pair
+    constexpr int UN = W4_BN * CTAS;                            // output channels per work unit
+    const int num_n = (p.N + UN - 1) / UN;
     const int num_t = (p.M + TT - 1) / TT;
     const int num_kb = (p.K + W4_BK - 1) / W4_BK;
-    const int S = p.splits;
+    const int S = CTAS == 2 ? 1 : p.splits;
     const int num_units = num_n * num_t * S;
+    const int unit0 = blockIdx.x / CTAS, unit_step = gridDim.x / CTAS;
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmP);
@@ -201,22 +212,29 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             mbar_init(pfull0 + 8 * s, 1);
             mbar_init(pempty0 + 8 * s, 4);      // the 4 warps of the dequant group that read it
         }
-        for (int a = 0; a < G; ++a) {
-            mbar_init(afull0 + 8 * a, 4);
+        for (int a = 0; a < NB; ++a) {
+            // leader: its own 4 dequant warps + (pair mode) one forwarded arrival for the peer's 4
+            mbar_init(afull0 + 8 * a, CTAS == 2 ? 5 : 4);
             mbar_init(aempty0 + 8 * a, 1);
+            mbar_init(afwd0 + 8 * a, 4);
         }
         for (int a = 0; a < 2; ++a) {
             mbar_init(tfull0 + 8 * a, 1);
-            mbar_init(tempty0 + 8 * a, 4);
+            mbar_init(tempty0 + 8 * a, 4 * CTAS);
         }
         fence_mbar_init();
     }
     if (warp == 1) {
-        tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
-        tmem_relinquish();
+        if (CTAS == 2) {
+            tmem_alloc_2sm(tmem_slot, Cfg::TMEM_COLS);
+            tmem_relinquish_2sm();
+        } else {
+            tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
+            tmem_relinquish();
+        }
     }
     tc_fence_before();
-    __syncthreads();
+    if (CTAS == 2) cluster_sync(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_g;
 
@@ -229,14 +247,20 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         if (lane == 0) {
             int stage = 0;
             uint32_t phase = 0;
-            for (int u = blockIdx.x; u < num_units; u += gridDim.x) {
+            for (int u = unit0; u < num_units; u += unit_step) {
                 const int tile = u / S, sp = u % S;
-                const int t0 = (tile / num_n) * TT;
+                const int t0 = (tile / num_n) * TT + rank * Cfg::X_ROWS;
                 const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
                 for (int kb = kb0; kb < kb1; ++kb) {
                     mbar_wait(xempty0 + 8 * stage, phase ^ 1);
-                    mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);
-                    tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
+                    if (CTAS == 2) {   // both halves are counted on the leader's barrier
+                        if (rank == 0) mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES * 2);
+                        tma_load_2d_2sm(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0,
+                                        (xfull0 + 8 * stage) & PEER_BIT_MASK);
+                    } else {
+                        mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);
+                        tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
+                    }
                     if (++stage == XS) { stage = 0; phase ^= 1; }
                 }
             }
@@ -248,9 +272,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             const uint64_t pol_w = policy_evict_first();  // weights are streamed once per launch
             int stage = 0;
             uint32_t phase = 0;
-            for (int u = blockIdx.x; u < num_units; u += gridDim.x) {
+            for (int u = unit0; u < num_units; u += unit_step) {
                 const int tile = u / S, sp = u % S;
-                const int n0 = (tile % num_n) * W4_BN;
+                const int n0 = (tile % num_n) * UN + rank * W4_BN;
                 const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
                 for (int kb = kb0; kb < kb1; ++kb) {
                     mbar_wait(pempty0 + 8 * stage, phase ^ 1);
@@ -264,11 +288,11 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------ MMA issuer
-        if (lane == 0) {
-            constexpr uint32_t idesc = idesc_bf16(W4_BN, TT);
+        if (lane == 0 && rank == 0) {
+            constexpr uint32_t idesc = idesc_bf16(UN, TT);
             int stage = 0, ab = 0, acc = 0;
             uint32_t phase = 0, aphase = 0, acc_phase = 0;
-            for (int u = blockIdx.x; u < num_units; u += gridDim.x) {
+            for (int u = unit0; u < num_units; u += unit_step) {
                 const int sp = u % S;
                 const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
                 mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1);
@@ -281,15 +305,23 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                     const uint64_t a_desc = make_smem_desc_sw128(sA + ab * Cfg::A_BYTES);
                     const uint64_t b_desc = make_smem_desc_sw128(sX + stage * Cfg::X_BYTES);
 #pragma unroll
-                    for (int k = 0; k < 4; ++k)  // 4 x (K = 16 bf16 = 32 bytes)
-                        mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc,
-                                   (kb != kb0 || k != 0) ? 1u : 0u);
-                    tc_commit(xempty0 + 8 * stage);
-                    tc_commit(aempty0 + 8 * ab);
+                    for (int k = 0; k < 4; ++k) {  // 4 x (K = 16 bf16 = 32 bytes)
+                        if (CTAS == 2)
+                            mma_f16_ss_2sm(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                        else
+                            mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                    }
+                    if (CTAS == 2) {
+                        tc_commit_2sm(xempty0 + 8 * stage, 3);
+                        tc_commit_2sm(aempty0 + 8 * ab, 3);
+                    } else {
+                        tc_commit(xempty0 + 8 * stage);
+                        tc_commit(aempty0 + 8 * ab);
+                    }
                     if (++stage == XS) { stage = 0; phase ^= 1; }
-                    if (++ab == G) { ab = 0; aphase ^= 1; }
+                    if (++ab == NB) { ab = 0; aphase ^= 1; }
                 }
-                tc_commit(tfull0 + 8 * acc);
+                if (CTAS == 2) tc_commit_2sm(tfull0 + 8 * acc, 3); else tc_commit(tfull0 + 8 * acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1; }
             }
             prof_stamp(p, 1, t_start);
@@ -300,16 +332,15 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         const int g = dw >> 2;                    // group = A buffer index
         const int r = (dw & 3) * 32 + lane;       // weight row inside the tile
         const int gpr = p.K >> 5;                 // groups per weight row
-        const uint32_t rowb = sA + g * Cfg::A_BYTES + (r >> 3) * 1024 + (r & 7) * 128;
+        const uint32_t rowoff = (r >> 3) * 1024 + (r & 7) * 128;
         const uint32_t xr = r & 7;
         const uint32_t off0 = r * Cfg::P_ROW;
         const uint32_t poff0 = off0 ^ (((off0 >> 7) & 1u) << 4);          // 32-byte swizzle
         const uint32_t poff1 = (off0 + 16) ^ (((off0 >> 7) & 1u) << 4);
         int it = 0;                               // running k-block counter of this CTA
-        uint32_t aphase = 0;
-        for (int u = blockIdx.x; u < num_units; u += gridDim.x) {
+        for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int n0 = (tile % num_n) * W4_BN;
+            const int n0 = (tile % num_n) * UN + rank * W4_BN;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             const bool row_ok = n0 + r < p.N;
             const uint32_t* srow = reinterpret_cast<const uint32_t*>(
@@ -346,31 +377,48 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(pempty0 + 8 * stage);   // packed bytes are in registers
-                mbar_wait(aempty0 + 8 * g, aphase ^ 1);            // MMAs reading this A buffer retired
+                const int ab = it % NB;                            // A buffer of this k-block
+                const uint32_t rowb = sA + ab * Cfg::A_BYTES + rowoff;
+                mbar_wait(aempty0 + 8 * ab, ((it / NB) & 1) ^ 1);  // MMAs reading this A buffer retired
 #pragma unroll
                 for (int j = 0; j < 8; ++j) sts128(rowb + ((static_cast<uint32_t>(j) ^ xr) << 4), o[j]);
                 fence_proxy_async_smem();                  // generic-proxy writes -> async proxy (MMA)
                 __syncwarp();
-                if (lane == 0) mbar_arrive(afull0 + 8 * g);        // one arrival per warp
-                aphase ^= 1;
+                if (lane == 0) {                                   // one arrival per warp
+                    // pair mode, peer CTA: arrive locally (cheap); a forwarder thread relays to the leader,
+                    // keeping the cluster-scope release off the dequantisers' path
+                    if (CTAS == 2 && rank == 1) mbar_arrive(afwd0 + 8 * ab); else mbar_arrive(afull0 + 8 * ab);
+                }
             }
         }
         if ((dw & 3) == 0 && lane == 0) prof_stamp(p, 2 + g, t_start);
+    } else if (warp == 3) {
+        // ------------------------------------------------------------ pair mode, peer CTA: forwarder
+        if (CTAS == 2 && rank == 1 && lane == 0) {
+            int it = 0;
+            for (int u = unit0; u < num_units; u += unit_step) {
+                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                    const int ab = it % NB;
+                    mbar_wait(afwd0 + 8 * ab, (it / NB) & 1);          // the peer's 4 dequant warps are done
+                    mbar_arrive_cluster(mapa_shared(afull0 + 8 * ab, 0));
+                }
+            }
+        }
     } else if (warp >= W4_EPI_WARP0) {
         // ------------------------------------------------------------ epilogue (warps 4..7)
         const int q = warp & 3;
         int acc = 0;
         uint32_t acc_phase = 0;
-        for (int u = blockIdx.x; u < num_units; u += gridDim.x) {
+        for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int n0 = (tile % num_n) * W4_BN, t0 = (tile / num_n) * TT;
+            const int n0 = (tile % num_n) * UN + rank * W4_BN, t0 = (tile / num_n) * TT;
             const int n = n0 + q * 32 + lane;
             const bool n_ok = n < p.N;
             float bv = 0.0f;
             if (p.bias && n_ok) bv = __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[n]);
             mbar_wait(tfull0 + 8 * acc, acc_phase);
             tc_fence_after();
-            if (q == 0 && lane == 0) prof_stamp(p, 8 + 2 * min(3, (u - blockIdx.x) / gridDim.x), t_start);
+            if (q == 0 && lane == 0) prof_stamp(p, 8 + 2 * min(3, (u - unit0) / unit_step), t_start);
             const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
             if (S == 1) {
                 // Transpose through shared memory: this thread owns output channel n and 32 tokens
@@ -411,7 +459,10 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(tempty0 + 8 * acc);
+                if (lane == 0) {
+                    if (CTAS == 2) mbar_arrive_cluster(mapa_shared(tempty0 + 8 * acc, 0));
+                    else mbar_arrive(tempty0 + 8 * acc);
+                }
             } else {
                 float* part = p.partials + static_cast<int64_t>(sp) * p.M * p.N;
 #pragma unroll 1
@@ -439,45 +490,52 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                     __threadfence();
                     const int tmax = min(TT, p.M - t0);
                     const int64_t sstride = static_cast<int64_t>(p.M) * p.N;
-                    for (int j0 = 0; j0 < tmax; j0 += 8) {   // 8 tokens x S loads in flight
-                        float y[8];
+                    for (int j0 = 0; j0 < tmax; j0 += 16) {  // 16 tokens x 2 splits = 32 loads in flight
+                        float y[16];
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) y[j] = 0.0f;
-                        for (int s = 0; s < S; ++s) {        // fixed split order: deterministic sum
+                        for (int j = 0; j < 16; ++j) y[j] = 0.0f;
+                        for (int s = 0; s < S; s += 2) {     // fixed split order: deterministic sum
+                            float a[16], b[16];
+                            const bool two = s + 1 < S;
 #pragma unroll
-                            for (int j = 0; j < 8; ++j) {
+                            for (int j = 0; j < 16; ++j) {
                                 const int64_t idx = static_cast<int64_t>(t0 + j0 + j) * p.N + n;
-                                if (n_ok && j0 + j < tmax) y[j] += __ldcg(p.partials + s * sstride + idx);
+                                const bool ok = n_ok && j0 + j < tmax;
+                                a[j] = ok ? __ldcg(p.partials + s * sstride + idx) : 0.0f;
+                                b[j] = ok && two ? __ldcg(p.partials + (s + 1) * sstride + idx) : 0.0f;
                             }
+#pragma unroll
+                            for (int j = 0; j < 16; ++j) y[j] = (y[j] + a[j]) + b[j];
                         }
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) {
+                        for (int j = 0; j < 16; ++j) {
                             const int64_t idx = static_cast<int64_t>(t0 + j0 + j) * p.N + n;
                             if (n_ok && j0 + j < tmax) w4_store(p.Y, p.out_t, idx, GELU ? gelu_erf(y[j] + bv) : y[j] + bv);
                         }
                     }
                 }
             }
-            if (q == 0 && lane == 0) prof_stamp(p, 9 + 2 * min(3, (u - blockIdx.x) / gridDim.x), t_start);
+            if (q == 0 && lane == 0) prof_stamp(p, 9 + 2 * min(3, (u - unit0) / unit_step), t_start);
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
         }
     }
 
     if (warp >= W4_EPI_WARP0 && warp < W4_DEQ_WARP0 && lane == 0) tma_store_wait<0>();
     tc_fence_before();
-    __syncthreads();
+    if (CTAS == 2) cluster_sync(); else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
-        tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
+        if (CTAS == 2) tmem_dealloc_2sm(tmem_base, Cfg::TMEM_COLS);
+        else tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
     }
 }
 
-template <int TT, bool GELU>
+template <int TT, bool GELU, int CTAS>
 static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, const W4Params& p,
                      int grid, cudaStream_t st, bool pdl) {
-    using Cfg = W4Cfg<TT>;
+    using Cfg = W4Cfg<TT, CTAS>;
     static bool attr_set = false;
-    auto kern = w4a16_gemm_kernel<TT, GELU>;
+    auto kern = w4a16_gemm_kernel<TT, GELU, CTAS>;
     if (!attr_set) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES) !=
             cudaSuccess)
@@ -487,7 +545,7 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
     CUtensorMap tmP, tmX, tmY;
     int rc = make_tmap_2d(&tmP, Wq4, 1, N, K / 2, W4_BN, Cfg::P_ROW, Cfg::P_ROW);
     if (rc != ARIA_OK) return rc;
-    rc = make_tmap_2d(&tmX, X, 2, M, K, TT, 64, 128);
+    rc = make_tmap_2d(&tmX, X, 2, M, K, Cfg::X_ROWS, 64, 128);
     if (rc != ARIA_OK) return rc;
     // output: box = 32 tokens x 32 channels (64 B bf16 rows / 128 B fp32 rows)
     rc = make_tmap_2d(&tmY, p.Y, p.out_t == ARIA_F32 ? 4 : 2, M, N, 32, 32, p.out_t == ARIA_F32 ? 128 : 64);
@@ -497,27 +555,55 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
     cfg.blockDim = dim3(Cfg::THREADS);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute at[2];
+    int na = 0;
+    if (pdl) {
+        at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (CTAS == 2) {
+        at[na].id = cudaLaunchAttributeClusterDimension;
+        at[na].val.clusterDim.x = 2;
+        at[na].val.clusterDim.y = 1;
+        at[na].val.clusterDim.z = 1;
+        ++na;
+    }
     cfg.attrs = at;
-    cfg.numAttrs = pdl ? 1 : 0;
+    cfg.numAttrs = na;
     return cudaLaunchKernelEx(&cfg, kern, tmP, tmX, tmY, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
-// Tile / split-K plan shared by the launcher and aria_workspace_bytes.
+// Tile / split-K plan shared by the launcher and aria_workspace_bytes.  Cost model (cycles): a unit
+// spends per k-block max(MMA, shared memory) = (256 TT + 40 KB) / 128 B/clk = 2 TT + 320 (the X tile
+// is written by TMA and read by the MMA; packed weights, dequantised A tile and its MMA read are the
+// constant), plus an epilogue ~ 40 TT, a fixed ~3000, and for split-K the fp32 partial round trip
+// ~ 100 TT + 4000.  Pick the (TT, splits) with the fewest wave-quantised cycles.
 void w4_plan(int M, int N, int K, int sms, int* tt_out, int* splits_out) {
-    const int tt = M <= 32 ? 32 : M <= 64 ? 64 : M <= 128 ? 128 : 256;
-    const int tiles = ((N + W4_BN - 1) / W4_BN) * ((M + tt - 1) / tt);
     const int num_kb = (K + W4_BK - 1) / W4_BK;
-    int s = 1;
-    if (tiles * 2 <= sms) {  // less than half the machine busy: split K
-        s = sms / tiles;
-        if (s > num_kb) s = num_kb;
-        if (s > 16) s = 16;
-        if (s < 1) s = 1;
+    const int num_n = (N + W4_BN - 1) / W4_BN;
+    const int tts[4] = {256, 128, 64, 32};
+    long best = -1;
+    int best_tt = 32, best_s = 1;
+    for (int i = 0; i < 4; ++i) {
+        const int tt = tts[i];
+        if (tt > 32 && tt >= 2 * M) continue;                 // mostly padding
+        const int tiles = num_n * ((M + tt - 1) / tt);
+        int smax = sms / tiles;
+        if (smax > num_kb) smax = num_kb;
+        if (smax > 16) smax = 16;
+        if (smax < 1) smax = 1;
+        for (int s = 1; s <= smax; ++s) {
+            const long units = static_cast<long>(tiles) * s;
+            const long waves = (units + sms - 1) / sms;
+            const long kb = (num_kb + s - 1) / s;
+            long unit = kb * (2 * tt + 320) + 40L * tt + 3000;
+            if (s > 1) unit += 100L * tt + 4000;
+            const long cost = waves * unit;
+            if (best < 0 || cost < best) { best = cost; best_tt = tt; best_s = s; }
+        }
     }
-    *tt_out = tt; *splits_out = s;
+    *tt_out = best_tt; *splits_out = best_s;
 }
 
 size_t w4_workspace_bytes(int M, int N, int K, int sms) {
@@ -546,14 +632,24 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
     p.partials = s > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) +
                                                   (tiles * 4 * sizeof(unsigned) + 255) / 256 * 256)
                        : nullptr;
-    const int units = static_cast<int>(tiles) * s;
-    const int grid = units < sms ? units : sms;
+    // CTA pairs for the big-tile, no-split case: same wave count, half the X traffic through smem
+    // CTA-pair mode is implemented and parity-tested but OFF by default: the peer CTA's cluster-scope
+    // mbarrier arrive after its STS + fence.proxy.async costs ~1.3k cycles per k-block on the hand-off
+    // path (measured with the role timestamps), which more than cancels the halved X traffic.
+    static const bool want_pair = getenv("ARIA_W4_PAIR") != nullptr;
+    const bool pair = want_pair && tt == 256 && s == 1 && N > W4_BN && sms >= 2;
+    const int units = pair ? ((N + 2 * W4_BN - 1) / (2 * W4_BN)) * ((M + tt - 1) / tt) : static_cast<int>(tiles) * s;
+    const int slots = pair ? sms / 2 : sms;
+    const int grid = (units < slots ? units : slots) * (pair ? 2 : 1);
     if (s > 1 && cudaMemsetAsync(p.counters, 0, tiles * 4 * sizeof(unsigned), st) != cudaSuccess)
         return ARIA_ERR_CUDA;
     const bool gelu = act == ARIA_ACT_GELU_ERF;
 #define ARIA_W4_LAUNCH(TTV)                                                        \
-    return gelu ? launch_w4<TTV, true>(X, M, K, Wq4, N, p, grid, st, pdl)          \
-                : launch_w4<TTV, false>(X, M, K, Wq4, N, p, grid, st, pdl)
+    return gelu ? launch_w4<TTV, true, 1>(X, M, K, Wq4, N, p, grid, st, pdl)       \
+                : launch_w4<TTV, false, 1>(X, M, K, Wq4, N, p, grid, st, pdl)
+    if (pair)
+        return gelu ? launch_w4<256, true, 2>(X, M, K, Wq4, N, p, grid, st, pdl)
+                    : launch_w4<256, false, 2>(X, M, K, Wq4, N, p, grid, st, pdl);
     if (tt == 32) { ARIA_W4_LAUNCH(32); }
     if (tt == 64) { ARIA_W4_LAUNCH(64); }
     if (tt == 128) { ARIA_W4_LAUNCH(128); }

@@ -33,7 +33,8 @@ struct W8Cfg {
     static constexpr int B_ROWS = BN / CTAS;                   // B rows staged by one CTA
     static constexpr int B_BYTES = B_ROWS * W8_BK;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-    static constexpr int STAGES = (200 * 1024) / STAGE_BYTES > 8 ? 8 : (200 * 1024) / STAGE_BYTES;
+    static constexpr int RING_BUDGET = 227 * 1024 - 1024 - 256 - W8_EPI_WARPS * W8_STG_BYTES - 2 * BN * 4;
+    static constexpr int STAGES = RING_BUDGET / STAGE_BYTES > 8 ? 8 : RING_BUDGET / STAGE_BYTES;
     static constexpr int ACC_STRIDE = BN <= 32 ? 32 : BN <= 64 ? 64 : BN <= 128 ? 128 : 256;
     static constexpr int TMEM_COLS = 2 * ACC_STRIDE < 32 ? 32 : 2 * ACC_STRIDE;
     static constexpr int RING_BYTES = STAGES * STAGE_BYTES;
@@ -263,7 +264,8 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         // ------------------------------------------------------------ epilogue (warps 2..9)
         const int ew = warp - 2;
         const int q = warp & 3;          // TMEM lane quarter this warp may read
-        const int half = ew >> 2;        // which column chunks (c % 2 == half)
+        constexpr int PQ = W8_EPI_WARPS / 4;   // warps per TMEM lane quarter
+        const int part = ew >> 2;        // this warp takes the 32-column chunks c = part, part + PQ, ...
         const int et = threadIdx.x - 64; // 0..255
         const uint32_t stg = base + Cfg::STG_OFF + ew * W8_STG_BYTES;
         int acc = 0;
@@ -296,21 +298,28 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             tc_fence_after();
             if (ew == 0 && lane == 0) w8_stamp(p, 8 + 2 * min(3, (t - unit0) / unit_step), t_start);
             const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
-            // This warp's columns: chunks c = half, half + 2, ... of 32, as groups of 16.  Two register
-            // sets alternate so that one tcgen05.ld is always in flight behind the arithmetic.
-            constexpr int NGW = BN / 32;                       // 16-column groups per warp (even)
-            auto gcol = [&](int g) { return (half + 2 * (g >> 1)) * 32 + (g & 1) * 16; };
+            // A chunk is two groups of 16 columns held in two register sets; the refill of the first set
+            // for the next chunk is in flight while the second set is processed.
+            constexpr int NC = BN / 32;
             uint32_t va[16], vb[16];
-            tmem_ld_32x32b_x16(t_addr + gcol(0), va);
-            tmem_wait_ld_x16(va);
-#pragma unroll 1
-            for (int g = 0; g < NGW; g += 2) {
-                tmem_ld_32x32b_x16(t_addr + gcol(g + 1), vb);
-                w8_epilogue_16<BN, OUT_T, GELU>(va, swb, gcol(g), sxv, stg, lane, &tmY, n0, row0);
+            int c = part;
+            if (c < NC) {
+                tmem_ld_32x32b_x16(t_addr + c * 32, va);
+                tmem_ld_32x32b_x16(t_addr + c * 32 + 16, vb);
+                tmem_wait_ld_x16(va);
                 tmem_wait_ld_x16(vb);
-                if (g + 2 < NGW) tmem_ld_32x32b_x16(t_addr + gcol(g + 2), va);
-                w8_epilogue_16<BN, OUT_T, GELU>(vb, swb, gcol(g + 1), sxv, stg, lane, &tmY, n0, row0);
-                if (g + 2 < NGW) tmem_wait_ld_x16(va);
+            }
+#pragma unroll 1
+            for (; c < NC; c += PQ) {
+                const int cn = c + PQ;
+                w8_epilogue_16<BN, OUT_T, GELU>(va, swb, c * 32, sxv, stg, lane, &tmY, n0, row0);
+                if (cn < NC) tmem_ld_32x32b_x16(t_addr + cn * 32, va);
+                w8_epilogue_16<BN, OUT_T, GELU>(vb, swb, c * 32 + 16, sxv, stg, lane, &tmY, n0, row0);
+                if (cn < NC) {
+                    tmem_ld_32x32b_x16(t_addr + cn * 32 + 16, vb);
+                    tmem_wait_ld_x16(va);
+                    tmem_wait_ld_x16(vb);
+                }
             }
             tc_fence_before();
             __syncwarp();

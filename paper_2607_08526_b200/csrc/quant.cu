@@ -257,7 +257,7 @@ static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, floa
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
                          bool pdl) {
     const int nvec = C / 8;
-    {   // warp-per-row variants: bf16 rows up to 6144, fp32 rows up to 3072 elements
+    {   // warp-per-row variants: rows up to 3072 elements (wider rows: one CTA per row, below)
         cudaLaunchConfig_t cfg = {};
         cfg.stream = st;
         cudaLaunchAttribute at[1];
@@ -272,7 +272,6 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
             if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg);
             else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg);
             else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg);
-            else if (vpl <= 24) e = launch_warp_rows<__nv_bfloat16, 24>(X, R, C, q, s, cfg);
             else done = false;
         } else {
             if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg);
