@@ -242,17 +242,18 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     pdl_launch_dependents();   // the next kernel may become resident now; it blocks in its own wait
     const long long t_start = clock64();
 
+    // Producer / MMA warps: warp-uniform loops, one elected lane issues (see gemm_w8a8.cu).
     if (warp == 0) {
         // ------------------------------------------------------------ TMA producer: X
-        if (lane == 0) {
-            int stage = 0;
-            uint32_t phase = 0;
-            for (int u = unit0; u < num_units; u += unit_step) {
-                const int tile = u / S, sp = u % S;
-                const int t0 = (tile / num_n) * TT + rank * Cfg::X_ROWS;
-                const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
-                for (int kb = kb0; kb < kb1; ++kb) {
-                    mbar_wait(xempty0 + 8 * stage, phase ^ 1);
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int u = unit0; u < num_units; u += unit_step) {
+            const int tile = u / S, sp = u % S;
+            const int t0 = (tile / num_n) * TT + rank * Cfg::X_ROWS;
+            const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
+            for (int kb = kb0; kb < kb1; ++kb) {
+                mbar_wait(xempty0 + 8 * stage, phase ^ 1);
+                if (elect_one()) {
                     if (CTAS == 2) {   // both halves are counted on the leader's barrier
                         if (rank == 0) mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES * 2);
                         tma_load_2d_2sm(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0,
@@ -261,70 +262,76 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                         mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);
                         tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
                     }
-                    if (++stage == XS) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == XS) { stage = 0; phase ^= 1; }
             }
-            prof_stamp(p, 0, t_start);
         }
+        if (lane == 0) prof_stamp(p, 0, t_start);
     } else if (warp == 2) {
         // ------------------------------------------------------------ TMA producer: packed weights
-        if (lane == 0) {
-            const uint64_t pol_w = policy_evict_first();  // weights are streamed once per launch
-            int stage = 0;
-            uint32_t phase = 0;
-            for (int u = unit0; u < num_units; u += unit_step) {
-                const int tile = u / S, sp = u % S;
-                const int n0 = (tile % num_n) * UN + rank * W4_BN;
-                const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
-                for (int kb = kb0; kb < kb1; ++kb) {
-                    mbar_wait(pempty0 + 8 * stage, phase ^ 1);
+        const uint64_t pol_w = policy_evict_first();  // weights are streamed once per launch
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int u = unit0; u < num_units; u += unit_step) {
+            const int tile = u / S, sp = u % S;
+            const int n0 = (tile % num_n) * UN + rank * W4_BN;
+            const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
+            for (int kb = kb0; kb < kb1; ++kb) {
+                mbar_wait(pempty0 + 8 * stage, phase ^ 1);
+                if (elect_one()) {
                     mbar_arrive_expect_tx(pfull0 + 8 * stage, Cfg::P_BYTES);
                     tma_load_2d_hint(sP + stage * Cfg::P_BYTES, &tmP, kb * Cfg::P_ROW, n0,
                                      pfull0 + 8 * stage, pol_w);
-                    if (++stage == PS) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == PS) { stage = 0; phase ^= 1; }
             }
-            prof_stamp(p, 6, t_start);
         }
+        if (lane == 0) prof_stamp(p, 6, t_start);
     } else if (warp == 1) {
         // ------------------------------------------------------------ MMA issuer
-        if (lane == 0 && rank == 0) {
+        if (rank == 0) {
             constexpr uint32_t idesc = idesc_bf16(UN, TT);
+            const uint64_t desc_hi = make_smem_desc_sw128(0);
             int stage = 0, ab = 0, acc = 0;
             uint32_t phase = 0, aphase = 0, acc_phase = 0;
             for (int u = unit0; u < num_units; u += unit_step) {
                 const int sp = u % S;
                 const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
                 mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1);
-                tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * Cfg::ACC_STRIDE;
                 for (int kb = kb0; kb < kb1; ++kb) {
                     mbar_wait(xfull0 + 8 * stage, phase);   // X landed
                     mbar_wait(afull0 + 8 * ab, aphase);     // weights dequantised
                     tc_fence_after();
-                    const uint64_t a_desc = make_smem_desc_sw128(sA + ab * Cfg::A_BYTES);
-                    const uint64_t b_desc = make_smem_desc_sw128(sX + stage * Cfg::X_BYTES);
+                    const uint64_t a_desc = desc_hi | (((sA + ab * Cfg::A_BYTES) & 0x3FFFF) >> 4);
+                    const uint64_t b_desc = desc_hi | (((sX + stage * Cfg::X_BYTES) & 0x3FFFF) >> 4);
+                    if (elect_one()) {
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {  // 4 x (K = 16 bf16 = 32 bytes)
-                        if (CTAS == 2)
-                            mma_f16_ss_2sm(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
-                        else
-                            mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                        for (int k = 0; k < 4; ++k) {  // 4 x (K = 16 bf16 = 32 bytes)
+                            if (CTAS == 2)
+                                mma_f16_ss_2sm(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                            else
+                                mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                        }
+                        if (CTAS == 2) {
+                            tc_commit_2sm(xempty0 + 8 * stage, 3);
+                            tc_commit_2sm(aempty0 + 8 * ab, 3);
+                            if (kb == kb1 - 1) tc_commit_2sm(tfull0 + 8 * acc, 3);
+                        } else {
+                            tc_commit(xempty0 + 8 * stage);
+                            tc_commit(aempty0 + 8 * ab);
+                            if (kb == kb1 - 1) tc_commit(tfull0 + 8 * acc);
+                        }
                     }
-                    if (CTAS == 2) {
-                        tc_commit_2sm(xempty0 + 8 * stage, 3);
-                        tc_commit_2sm(aempty0 + 8 * ab, 3);
-                    } else {
-                        tc_commit(xempty0 + 8 * stage);
-                        tc_commit(aempty0 + 8 * ab);
-                    }
+                    __syncwarp();
                     if (++stage == XS) { stage = 0; phase ^= 1; }
                     if (++ab == NB) { ab = 0; aphase ^= 1; }
                 }
-                if (CTAS == 2) tc_commit_2sm(tfull0 + 8 * acc, 3); else tc_commit(tfull0 + 8 * acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1; }
             }
-            prof_stamp(p, 1, t_start);
+            if (lane == 0) prof_stamp(p, 1, t_start);
         }
     } else if (warp >= W4_DEQ_WARP0) {
         // ------------------------------------------------------------ dequantiser groups

@@ -13,6 +13,8 @@
 //               MMA warp fills accumulator `a^1`.
 // Tails: TMA zero-fills rows >= M / >= N and bytes >= K on load (zero codes add nothing) and clips
 // them on store.
+#include <cstdlib>
+
 #include "internal.cuh"
 
 namespace aria {
@@ -33,18 +35,26 @@ struct W8Cfg {
     static constexpr int B_ROWS = BN / CTAS;                   // B rows staged by one CTA
     static constexpr int B_BYTES = B_ROWS * W8_BK;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-    static constexpr int RING_BUDGET = 227 * 1024 - 1024 - 256 - W8_EPI_WARPS * W8_STG_BYTES - 2 * BN * 4;
+    static constexpr int SWB_BYTES = 2 * 2 * BN * 4;           // double-buffered float sw[BN], bias[BN]
+    static constexpr int FIXED = 1024 + 256 + SWB_BYTES;       // alignment slack + barriers + scales
+    // Output staging: every epilogue warp rotates through NBUF blocks of [32 rows x 64 B]; a block is
+    // only rewritten after the TMA store issued NBUF stores earlier has read it, so the stores of a
+    // whole tile stay in flight.  4 blocks if the operand ring keeps >= 4 stages, else 2.
+    static constexpr int BUDGET4 = 227 * 1024 - FIXED - W8_EPI_WARPS * 4 * W8_STG_BYTES;
+    static constexpr int NBUF = BUDGET4 / STAGE_BYTES >= 4 ? 4 : 2;
+    static constexpr int RING_BUDGET = 227 * 1024 - FIXED - W8_EPI_WARPS * NBUF * W8_STG_BYTES;
     static constexpr int STAGES = RING_BUDGET / STAGE_BYTES > 8 ? 8 : RING_BUDGET / STAGE_BYTES;
     static constexpr int ACC_STRIDE = BN <= 32 ? 32 : BN <= 64 ? 64 : BN <= 128 ? 128 : 256;
     static constexpr int TMEM_COLS = 2 * ACC_STRIDE < 32 ? 32 : 2 * ACC_STRIDE;
     static constexpr int RING_BYTES = STAGES * STAGE_BYTES;
-    static constexpr int STG_OFF = RING_BYTES;                               // [8][2 KB] staging
-    static constexpr int SWB_OFF = STG_OFF + W8_EPI_WARPS * W8_STG_BYTES;    // float sw[BN], bias[BN]
-    static constexpr int BAR_OFF = SWB_OFF + 2 * BN * 4;
+    static constexpr int STG_OFF = RING_BYTES;                                      // [8][NBUF][2 KB]
+    static constexpr int SWB_OFF = STG_OFF + W8_EPI_WARPS * NBUF * W8_STG_BYTES;
+    static constexpr int BAR_OFF = SWB_OFF + SWB_BYTES;
     static constexpr int BAR_BYTES = (2 * STAGES + 4) * 8 + 16;
     static constexpr int SMEM_BYTES = BAR_OFF + BAR_BYTES + 1024;            // + alignment slack
     static_assert(BN % 32 == 0 && BN >= 32 && BN <= 256, "BN");
     static_assert(B_BYTES % 1024 == 0, "B tile must keep 1024-byte alignment");
+    static_assert(STAGES >= 2, "ring too shallow");
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
@@ -60,7 +70,7 @@ struct W8Params {
 static long long* g_w8_prof = nullptr;
 void w8_set_profile_buffer(long long* p) { g_w8_prof = p; }
 __device__ __forceinline__ void w8_stamp(const W8Params& p, int slot, long long t0) {
-    if (p.prof) p.prof[blockIdx.x * 16 + slot] = clock64() - t0;
+    if (p.prof) p.prof[blockIdx.x * 20 + slot] = clock64() - t0;
 }
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
@@ -73,13 +83,14 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, ui
 }
 
 // Epilogue for 16 accumulator columns of this thread's row: x sx[m] x sw[n] + b[n] -> GELU -> cast ->
-// 32 B (bf16) or 64 B (fp32 / int32) into the warp's 64-byte-swizzled [32 rows x 64 B] staging block;
-// each completed 64-byte block goes out as one TMA store (clipped at M / N by the tensor map).
-template <int BN, int OUT_T, bool GELU>
+// 32 B (bf16) or 64 B (fp32 / int32) into one of the warp's 64-byte-swizzled [32 rows x 64 B] staging
+// blocks; each completed block goes out as one TMA store (clipped at M / N by the tensor map) and the
+// warp moves on to its next block.  The arithmetic is issued as packed f32x2 instructions.
+template <int BN, int OUT_T, bool GELU, int NBUF>
 __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const float* swb, int cb, float sxv,
-                                               uint32_t stg, int lane, const CUtensorMap* tmY, int n0,
-                                               int row0) {
-    const uint32_t rowb = stg + lane * 64;
+                                               uint32_t stg0, int& sbuf, int lane, const CUtensorMap* tmY,
+                                               int n0, int row0) {
+    const uint32_t rowb = stg0 + sbuf * W8_STG_BYTES + lane * 64;
     const uint32_t xr = (lane >> 1) & 3;
     const bool first = OUT_T != 1 || (cb & 16) == 0;   // first group of a 64-byte block
     const bool last = OUT_T != 1 || (cb & 16) != 0;    // block complete after this group
@@ -89,18 +100,21 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
         for (int j = 0; j < 16; ++j) w[j] = v[j];
     } else {
         float f[16];
+        const uint64_t sx2 = pack_f2(sxv, sxv);
 #pragma unroll
         for (int j = 0; j < 16; j += 4) {
             const float4 s4 = *reinterpret_cast<const float4*>(swb + cb + j);
             const float4 b4 = *reinterpret_cast<const float4*>(swb + BN + cb + j);
-            f[j] = fmaf(static_cast<float>(static_cast<int32_t>(v[j])) * sxv, s4.x, b4.x);
-            f[j + 1] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 1])) * sxv, s4.y, b4.y);
-            f[j + 2] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 2])) * sxv, s4.z, b4.z);
-            f[j + 3] = fmaf(static_cast<float>(static_cast<int32_t>(v[j + 3])) * sxv, s4.w, b4.w);
+            const uint64_t t01 = mul2(pack_f2(static_cast<float>(static_cast<int32_t>(v[j])),
+                                              static_cast<float>(static_cast<int32_t>(v[j + 1]))), sx2);
+            const uint64_t t23 = mul2(pack_f2(static_cast<float>(static_cast<int32_t>(v[j + 2])),
+                                              static_cast<float>(static_cast<int32_t>(v[j + 3]))), sx2);
+            unpack_f2(fma2(t01, pack_f2(s4.x, s4.y), pack_f2(b4.x, b4.y)), f[j], f[j + 1]);
+            unpack_f2(fma2(t23, pack_f2(s4.z, s4.w), pack_f2(b4.z, b4.w)), f[j + 2], f[j + 3]);
         }
         if (GELU) {
 #pragma unroll
-            for (int j = 0; j < 16; ++j) f[j] = gelu_erf(f[j]);
+            for (int j = 0; j < 16; j += 2) gelu_erf2(f[j], f[j + 1]);
         }
         if (OUT_T == 1) {
 #pragma unroll
@@ -110,8 +124,8 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
             for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[j]);
         }
     }
-    if (first) {   // the previous TMA store must have finished reading the staging block
-        if (lane == 0) tma_store_wait_read<0>();
+    if (first) {   // the TMA store issued NBUF blocks ago must have finished reading this block
+        if (elect_one()) tma_store_wait_read<NBUF - 1>();
         __syncwarp();
     }
     if (OUT_T == 1) {
@@ -126,10 +140,11 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
     if (last) {
         fence_proxy_async_smem();
         __syncwarp();
-        if (lane == 0) {
-            tma_store_2d(tmY, stg, n0 + (OUT_T == 1 ? (cb & ~31) : cb), row0);
+        if (elect_one()) {
+            tma_store_2d(tmY, stg0 + sbuf * W8_STG_BYTES, n0 + (OUT_T == 1 ? (cb & ~31) : cb), row0);
             tma_store_commit();
         }
+        sbuf = sbuf + 1 == NBUF ? 0 : sbuf + 1;
     }
 }
 
@@ -153,8 +168,9 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     const uint32_t tmem_slot = tempty0 + 16;
     volatile uint32_t* tmem_slot_g =
         reinterpret_cast<volatile uint32_t*>(gbase + Cfg::BAR_OFF + 16 * STAGES + 32);
-    float* swb = reinterpret_cast<float*>(gbase + Cfg::SWB_OFF);
+    float* swb_all = reinterpret_cast<float*>(gbase + Cfg::SWB_OFF);   // [2][2 * BN]
 
+    const long long t_entry = clock64();
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const uint32_t rank = CTAS == 2 ? cluster_ctarank() : 0u;   // position in the CTA pair
@@ -198,19 +214,30 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     pdl_wait_prior_grid();
     pdl_launch_dependents();   // the next kernel may become resident now; it blocks in its own wait
     const long long t_start = clock64();
+    if (threadIdx.x == 0 && p.prof) {
+        p.prof[blockIdx.x * 20 + 16] = t_start - t_entry;
+        unsigned long long gt;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+        p.prof[blockIdx.x * 20 + 18] = static_cast<long long>(gt);
+    }
 
+    // Producer and MMA warps run their loops WARP-UNIFORMLY (all 32 lanes execute the control flow and
+    // the barrier waits; one elected lane issues the TMA / tcgen05 instructions).  With the loop inside
+    // an `if (lane == 0)` the compiler cannot keep descriptors and barrier addresses in uniform registers
+    // and wraps every UTMALDG / UTCIMMA in a vote loop -- measured at ~155 clk per MMA instead of the
+    // tensor pipe's 128 (BN = 256).
     if (warp == 0) {
         // ------------------------------------------------------------ TMA producer (every CTA)
-        if (lane == 0) {
-            int stage = 0;
-            uint32_t phase = 0;
-            for (int t = unit0; t < num_tiles; t += unit_step) {
-                const int m0 = (t % num_m) * UM + rank * W8_BM;
-                const int n0 = (t / num_m) * BN + rank * Cfg::B_ROWS;
-                for (int kb = 0; kb < num_kb; ++kb) {
-                    mbar_wait(empty0 + 8 * stage, phase ^ 1);
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int t = unit0; t < num_tiles; t += unit_step) {
+            const int m0 = (t % num_m) * UM + rank * W8_BM;
+            const int n0 = (t / num_m) * BN + rank * Cfg::B_ROWS;
+            for (int kb = 0; kb < num_kb; ++kb) {
+                mbar_wait(empty0 + 8 * stage, phase ^ 1);
+                if (elect_one()) {
                     if (CTAS == 2) {
-                        // both CTAs' bytes are counted on the LEADER's barrier, where the MMA thread waits
+                        // both CTAs' bytes are counted on the LEADER's barrier, where the MMA warp waits
                         const uint32_t lbar = (full0 + 8 * stage) & PEER_BIT_MASK;
                         if (rank == 0) mbar_arrive_expect_tx(full0 + 8 * stage, Cfg::STAGE_BYTES * 2);
                         tma_load_2d_2sm(sA + stage * Cfg::A_BYTES, &tmA, kb * W8_BK, m0, lbar);
@@ -220,102 +247,117 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                         tma_load_2d(sA + stage * Cfg::A_BYTES, &tmA, kb * W8_BK, m0, full0 + 8 * stage);
                         tma_load_2d(sB + stage * Cfg::B_BYTES, &tmB, kb * W8_BK, n0, full0 + 8 * stage);
                     }
-                    if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == STAGES) { stage = 0; phase ^= 1; }
             }
-            w8_stamp(p, 0, t_start);
         }
+        if (lane == 0) w8_stamp(p, 0, t_start);
     } else if (warp == 1) {
         // ------------------------------------------------------------ MMA issuer (leader CTA only)
-        if (lane == 0 && rank == 0) {
+        if (rank == 0) {
             constexpr uint32_t idesc = idesc_i8(UM, BN);
+            const uint64_t desc_hi = make_smem_desc_sw128(0);
             int stage = 0;
             uint32_t phase = 0;
             int acc = 0;
             uint32_t acc_phase = 0;
             for (int t = unit0; t < num_tiles; t += unit_step) {
                 mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1);
-                tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * Cfg::ACC_STRIDE;
                 for (int kb = 0; kb < num_kb; ++kb) {
                     mbar_wait(full0 + 8 * stage, phase);
                     tc_fence_after();
-                    const uint64_t a_desc = make_smem_desc_sw128(sA + stage * Cfg::A_BYTES);
-                    const uint64_t b_desc = make_smem_desc_sw128(sB + stage * Cfg::B_BYTES);
+                    const uint64_t a_desc = desc_hi | (((sA + stage * Cfg::A_BYTES) & 0x3FFFF) >> 4);
+                    const uint64_t b_desc = desc_hi | (((sB + stage * Cfg::B_BYTES) & 0x3FFFF) >> 4);
+                    if (elect_one()) {
 #pragma unroll
-                    for (int k = 0; k < W8_BK / W8_UMMA_K; ++k) {
-                        if (CTAS == 2)
-                            mma_i8_ss_2sm(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
-                        else
-                            mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+                        for (int k = 0; k < W8_BK / W8_UMMA_K; ++k) {
+                            if (CTAS == 2)
+                                mma_i8_ss_2sm(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+                            else
+                                mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+                        }
+                        // ring slot reusable (in both CTAs) once these MMAs retire
+                        if (CTAS == 2) tc_commit_2sm(empty0 + 8 * stage, 3); else tc_commit(empty0 + 8 * stage);
+                        // accumulator complete: wake the epilogue warps of both CTAs
+                        if (kb == num_kb - 1) {
+                            if (CTAS == 2) tc_commit_2sm(tfull0 + 8 * acc, 3); else tc_commit(tfull0 + 8 * acc);
+                        }
                     }
-                    // ring slot reusable (in both CTAs) once these MMAs retire
-                    if (CTAS == 2) tc_commit_2sm(empty0 + 8 * stage, 3); else tc_commit(empty0 + 8 * stage);
+                    __syncwarp();
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
-                // accumulator complete: wake the epilogue warps of both CTAs
-                if (CTAS == 2) tc_commit_2sm(tfull0 + 8 * acc, 3); else tc_commit(tfull0 + 8 * acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1; }
-                w8_stamp(p, 2 + min(5, (t - unit0) / unit_step), t_start);
+                if (lane == 0) w8_stamp(p, 2 + min(5, (t - unit0) / unit_step), t_start);
             }
-            w8_stamp(p, 1, t_start);
+            if (lane == 0) w8_stamp(p, 1, t_start);
         }
     } else {
         // ------------------------------------------------------------ epilogue (warps 2..9)
         const int ew = warp - 2;
         const int q = warp & 3;          // TMEM lane quarter this warp may read
         constexpr int PQ = W8_EPI_WARPS / 4;   // warps per TMEM lane quarter
-        const int part = ew >> 2;        // this warp takes the 32-column chunks c = part, part + PQ, ...
-        const int et = threadIdx.x - 64; // 0..255
-        const uint32_t stg = base + Cfg::STG_OFF + ew * W8_STG_BYTES;
+        constexpr int NBUF = Cfg::NBUF;
+        constexpr int NC = BN / 32;            // 32-column chunks per tile
+        constexpr int CPW = (NC + PQ - 1) / PQ;   // contiguous chunks per warp
+        const int part = ew >> 2;        // this warp takes chunks [part * CPW, part * CPW + CPW)
+        const int c_beg = part * CPW, c_end = min(NC, c_beg + CPW);
+        const int et = threadIdx.x - 64; // 0..255: column index whose scale / bias this thread stages
+        const uint32_t stg0 = base + Cfg::STG_OFF + ew * (NBUF * W8_STG_BYTES);
+        int sbuf = 0;
         int acc = 0;
         uint32_t acc_phase = 0;
         const uint32_t tempty_leader = CTAS == 2 ? mapa_shared(tempty0, 0) : 0u;
-        for (int t = unit0; t < num_tiles; t += unit_step) {
+        // per-tile column scales and bias live in shared memory (broadcast reads), double buffered:
+        // the next tile's values are fetched into registers while this tile is processed.
+        auto fetch_swb = [&](int t, float& sv, float& bv) {
+            sv = 0.0f; bv = 0.0f;
+            const int c = (t / num_m) * BN + et;
+            if (OUT_T != 2 && et < BN && t < num_tiles && c < p.N) {
+                sv = __ldg(p.sw + c);
+                if (p.bias)
+                    bv = p.bias_t == ARIA_F32 ? __ldg(static_cast<const float*>(p.bias) + c)
+                                              : __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[c]);
+            }
+        };
+        if (OUT_T != 2) {
+            float sv, bv;
+            fetch_swb(unit0, sv, bv);
+            if (et < BN) { swb_all[et] = sv; swb_all[BN + et] = bv; }
+            named_bar_sync(1, 32 * W8_EPI_WARPS);
+        }
+        int it = 0;
+        for (int t = unit0; t < num_tiles; t += unit_step, ++it) {
             const int m0 = (t % num_m) * UM + rank * W8_BM, n0 = (t / num_m) * BN;
             const int row0 = m0 + q * 32;
-            float sxv = 0.0f;
+            const float* swb = swb_all + (it & 1) * 2 * BN;
+            float sxv = 0.0f, nsv = 0.0f, nbv = 0.0f;
             if (OUT_T != 2) {
                 if (row0 + lane < p.M) sxv = __ldg(p.sx + row0 + lane);
-                // per-tile column scales and bias -> shared memory (broadcast reads later)
-                named_bar_sync(1, 32 * W8_EPI_WARPS);  // previous tile's readers are done
-                for (int i = et; i < BN; i += 32 * W8_EPI_WARPS) {
-                    const int c = n0 + i;
-                    float s = 0.0f, b = 0.0f;
-                    if (c < p.N) {
-                        s = __ldg(p.sw + c);
-                        if (p.bias)
-                            b = p.bias_t == ARIA_F32
-                                    ? __ldg(static_cast<const float*>(p.bias) + c)
-                                    : __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[c]);
-                    }
-                    swb[i] = s;
-                    swb[BN + i] = b;
-                }
-                named_bar_sync(1, 32 * W8_EPI_WARPS);
+                fetch_swb(t + unit_step, nsv, nbv);
             }
             mbar_wait(tfull0 + 8 * acc, acc_phase);
             tc_fence_after();
-            if (ew == 0 && lane == 0) w8_stamp(p, 8 + 2 * min(3, (t - unit0) / unit_step), t_start);
+            if (ew == 0 && lane == 0) w8_stamp(p, 8 + 2 * min(3, it), t_start);
             const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
             // A chunk is two groups of 16 columns held in two register sets; the refill of the first set
             // for the next chunk is in flight while the second set is processed.
-            constexpr int NC = BN / 32;
             uint32_t va[16], vb[16];
-            int c = part;
-            if (c < NC) {
+            int c = c_beg;
+            if (c < c_end) {
                 tmem_ld_32x32b_x16(t_addr + c * 32, va);
                 tmem_ld_32x32b_x16(t_addr + c * 32 + 16, vb);
                 tmem_wait_ld_x16(va);
                 tmem_wait_ld_x16(vb);
             }
 #pragma unroll 1
-            for (; c < NC; c += PQ) {
-                const int cn = c + PQ;
-                w8_epilogue_16<BN, OUT_T, GELU>(va, swb, c * 32, sxv, stg, lane, &tmY, n0, row0);
-                if (cn < NC) tmem_ld_32x32b_x16(t_addr + cn * 32, va);
-                w8_epilogue_16<BN, OUT_T, GELU>(vb, swb, c * 32 + 16, sxv, stg, lane, &tmY, n0, row0);
-                if (cn < NC) {
+            for (; c < c_end; ++c) {
+                const int cn = c + 1;
+                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(va, swb, c * 32, sxv, stg0, sbuf, lane, &tmY, n0, row0);
+                if (cn < c_end) tmem_ld_32x32b_x16(t_addr + cn * 32, va);
+                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(vb, swb, c * 32 + 16, sxv, stg0, sbuf, lane, &tmY, n0, row0);
+                if (cn < c_end) {
                     tmem_ld_32x32b_x16(t_addr + cn * 32 + 16, vb);
                     tmem_wait_ld_x16(va);
                     tmem_wait_ld_x16(vb);
@@ -327,10 +369,16 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                 if (CTAS == 2) mbar_arrive_cluster(tempty_leader + 8 * acc);   // leader's barrier
                 else mbar_arrive(tempty0 + 8 * acc);
             }
-            if (ew == 0 && lane == 0) w8_stamp(p, 9 + 2 * min(3, (t - unit0) / unit_step), t_start);
+            if (ew == 0 && lane == 0) w8_stamp(p, 9 + 2 * min(3, it), t_start);
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+            if (OUT_T != 2) {   // publish the next tile's scales / bias; everyone is done reading that buffer
+                float* nx = swb_all + ((it + 1) & 1) * 2 * BN;
+                if (et < BN) { nx[et] = nsv; nx[BN + et] = nbv; }
+                named_bar_sync(1, 32 * W8_EPI_WARPS);
+            }
         }
-        if (lane == 0) tma_store_wait<0>();  // all of this warp's output has been written
+        if (elect_one()) tma_store_wait<0>();  // all of this warp's output has been written
+        __syncwarp();
     }
 
     tc_fence_before();
@@ -339,6 +387,12 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         tc_fence_after();
         if (CTAS == 2) tmem_dealloc_2sm(tmem_base, Cfg::TMEM_COLS);
         else tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
+    }
+    if (threadIdx.x == 32 && p.prof) {
+        p.prof[blockIdx.x * 20 + 17] = clock64() - t_start;
+        unsigned long long gt;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+        p.prof[blockIdx.x * 20 + 19] = static_cast<long long>(gt);
     }
 }
 
@@ -422,7 +476,12 @@ int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, co
                      cudaStream_t st, bool pdl) {
     const int sms = num_sms();
     if (sms <= 0) return ARIA_ERR_CUDA;
-    const W8Plan plan = pick_plan(M, N, sms);
+    W8Plan plan = pick_plan(M, N, sms);
+    if (const char* e = getenv("ARIA_W8_PLAN")) {   // debug override: "bn,ctas"
+        int b = 0, c = 0;
+        if (sscanf(e, "%d,%d", &b, &c) == 2 && (c == 1 || (c == 2 && M > W8_BM && b >= 128)) &&
+            (b == 64 || b == 128 || b == 192 || b == 256)) { plan.bn = b; plan.ctas = c; }
+    }
     const int bn = plan.bn, ctas = plan.ctas;
     CUtensorMap tmA, tmB;
     int rc = make_tmap_2d(&tmA, Xq, 1, M, K, W8_BM, W8_BK, 128);
