@@ -124,6 +124,29 @@ typedef struct {
 ARIA_API int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mode, int io, void* ws,
                           size_t ws_bytes, void* stream);
 
+/* S5 with a PLAN (SURVEY S8(b) "a plan variant that pre-encodes TMA tensor maps is allowed").
+ * aria_stack_plan_create validates the list exactly like aria_denoiser_linears, copies it, and
+ * ALLOCATES the plan's own device scratch (tensor maps, schedule, split-K partials, flags): it
+ * may synchronise and is not capturable.  The plan keeps the layers' device pointers (weights,
+ * scales, biases, in/out buffers), which must stay valid until aria_stack_plan_destroy.
+ * aria_stack_plan_run only ENQUEUES one step on `stream` (capturable) and computes
+ * exactly what aria_denoiser_linears computes for the same list.  For mode W4A16 with M <= 32,
+ * bf16 I/O, every K % 256 == 0 and no output buffer overlapping another output or an earlier
+ * input, the step is ONE persistent weight-streaming kernel over all layers (HBM bound; layers
+ * whose input is not an earlier layer's output may overlap, results are identical to array
+ * order); there the dequantised weight is w^ = fp16_rn(q * sg) (fp16 operand x bf16 activations
+ * in the same tcgen05 kind::f16 MMA; needs sg <= 127), or bf16_rne(q * sg) as in
+ * aria_linear_w4a16 when the environment variable ARIA_W4_F16A=0 is set at plan creation.
+ * Any other list runs the per-layer path.  A plan's scratch serves ONE step at a time: do not
+ * run the same plan concurrently on two streams.  aria_stack_plan_is_streaming: 1 if the plan
+ * uses the stream kernel.                                                                   */
+typedef struct aria_stack_plan aria_stack_plan;
+ARIA_API int aria_stack_plan_create(const aria_layer* layers, int n_layers, int M, int mode, int io,
+                                    aria_stack_plan** plan);
+ARIA_API int aria_stack_plan_run(const aria_stack_plan* plan, void* stream);
+ARIA_API int aria_stack_plan_is_streaming(const aria_stack_plan* plan);
+ARIA_API void aria_stack_plan_destroy(aria_stack_plan* plan);
+
 /* Same stack, but `in` / `out` of every layer are HOST pointers (pinned memory recommended):
  * each layer's input is copied host->device into `ws`, the layer runs, and its output is
  * copied device->host; the call returns after synchronising `stream`.  Weights, scales and

@@ -60,9 +60,15 @@ def lib() -> ctypes.CDLL:
         L.aria_denoiser_linears.argtypes = [ctypes.POINTER(aria_layer), c_int, c_int, c_int, c_int,
                                             c_void_p, c_size_t, c_void_p]
         L.aria_denoiser_linears_host.argtypes = L.aria_denoiser_linears.argtypes
+        L.aria_stack_plan_create.argtypes = [ctypes.POINTER(aria_layer), c_int, c_int, c_int, c_int,
+                                             ctypes.POINTER(c_void_p)]
+        L.aria_stack_plan_run.argtypes = [c_void_p, c_void_p]
+        L.aria_stack_plan_is_streaming.argtypes = [c_void_p]
+        L.aria_stack_plan_destroy.argtypes = [c_void_p]
+        L.aria_stack_plan_destroy.restype = None
         for name in EXPORTS:
             if name not in ("aria_version", "aria_status_string", "aria_workspace_bytes",
-                            "aria_workspace_bytes_host"):
+                            "aria_workspace_bytes_host", "aria_stack_plan_destroy"):
                 getattr(L, name).restype = c_int
         _lib = L
     return _lib
@@ -71,7 +77,8 @@ def lib() -> ctypes.CDLL:
 EXPORTS = ("aria_linear_w8a8_q", "aria_quantize_weights_int8", "aria_quantize_weights_int4", "aria_quantize_act_int8",
            "aria_linear_w8a8", "aria_linear_w4a16", "aria_denoiser_linears",
            "aria_denoiser_linears_host", "aria_workspace_bytes", "aria_workspace_bytes_host",
-           "aria_status_string", "aria_gemm_i8_i32", "aria_version")
+           "aria_status_string", "aria_gemm_i8_i32", "aria_version", "aria_stack_plan_create",
+           "aria_stack_plan_run", "aria_stack_plan_is_streaming", "aria_stack_plan_destroy")
 
 
 def _check(rc: int, what: str):
@@ -209,3 +216,24 @@ def aria_denoiser_linears(layers, M: int, mode: int, io: int, ws: torch.Tensor):
 def aria_denoiser_linears_host(layers, M: int, mode: int, io: int, ws: torch.Tensor):
     _check(lib().aria_denoiser_linears_host(layers, len(layers), M, mode, io, _ptr(ws), ws.numel(),
                                             _stream()), "aria_denoiser_linears_host")
+
+
+def aria_stack_plan_create(layers, M: int, mode: int, io: int) -> c_void_p:
+    """Returns the opaque plan handle; the caller keeps the layers' tensors alive and calls
+    aria_stack_plan_destroy."""
+    plan = c_void_p(0)
+    _check(lib().aria_stack_plan_create(layers, len(layers), M, mode, io, ctypes.byref(plan)),
+           "aria_stack_plan_create")
+    return plan
+
+
+def aria_stack_plan_run(plan: c_void_p):
+    _check(lib().aria_stack_plan_run(plan, _stream()), "aria_stack_plan_run")
+
+
+def aria_stack_plan_is_streaming(plan: c_void_p) -> bool:
+    return bool(lib().aria_stack_plan_is_streaming(plan))
+
+
+def aria_stack_plan_destroy(plan: c_void_p):
+    lib().aria_stack_plan_destroy(plan)

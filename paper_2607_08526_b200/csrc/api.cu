@@ -2,6 +2,8 @@
 // sequencing of kernels.  Device entry points only enqueue on the caller's stream.
 #include <cstdlib>
 #include <cstring>
+#include <new>
+#include <vector>
 
 #include "internal.cuh"
 
@@ -72,6 +74,14 @@ int run_layer(const aria_layer& L, const void* in, void* out, int M, int mode, i
 }
 
 }  // namespace
+
+struct aria_stack_plan {
+    std::vector<aria_layer> layers;
+    int M = 0, mode = 0, io = 0;
+    WsPlan* ws_plan = nullptr;      // small-M W4A16: the persistent stream kernel (w4a16_stream.cu)
+    void* d_ws = nullptr;           // otherwise: scratch of the per-layer path
+    size_t ws_bytes = 0;
+};
 
 extern "C" {
 
@@ -202,6 +212,8 @@ int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, in
 /* Debug hook (not in aria.h): per-CTA role timestamps of the W4A16 kernel, 16 int64 per CTA. */
 __attribute__((visibility("default"))) void aria_debug_w4_profile(long long* buf) { w4_set_profile_buffer(buf); }
 
+__attribute__((visibility("default"))) void aria_debug_ws_profile(long long* buf) { ws_set_profile_buffer(buf); }
+
 __attribute__((visibility("default"))) void aria_debug_w8_profile(long long* buf) { w8_set_profile_buffer(buf); }
 
 int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mode, int io, void* ws,
@@ -218,6 +230,48 @@ int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mod
         if (rc != ARIA_OK) return rc;
     }
     return ARIA_OK;
+}
+
+int aria_stack_plan_create(const aria_layer* layers, int n_layers, int M, int mode, int io,
+                           aria_stack_plan** plan_out) {
+    if (!plan_out) return ARIA_ERR_NULL;
+    *plan_out = nullptr;
+    int maxK, maxN;
+    int rc = check_layers(layers, n_layers, M, mode, io, &maxK, &maxN, false);
+    if (rc != ARIA_OK) return rc;
+    aria_stack_plan* plan = new (std::nothrow) aria_stack_plan;
+    if (!plan) return ARIA_ERR_CUDA;
+    plan->layers.assign(layers, layers + n_layers);
+    plan->M = M; plan->mode = mode; plan->io = io;
+    if (ws_eligible(layers, n_layers, M, mode, io)) {
+        rc = ws_plan_create(layers, n_layers, M, io, &plan->ws_plan);
+    } else {
+        plan->ws_bytes = aria_workspace_bytes(M, maxK, maxN, mode);
+        rc = cudaMalloc(&plan->d_ws, plan->ws_bytes) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    }
+    if (rc != ARIA_OK) {
+        aria_stack_plan_destroy(plan);
+        return rc;
+    }
+    *plan_out = plan;
+    return ARIA_OK;
+}
+
+int aria_stack_plan_run(const aria_stack_plan* plan, void* stream) {
+    if (!plan) return ARIA_ERR_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (plan->ws_plan) return ws_plan_run(plan->ws_plan, st);
+    return aria_denoiser_linears(plan->layers.data(), static_cast<int>(plan->layers.size()), plan->M,
+                                 plan->mode, plan->io, plan->d_ws, plan->ws_bytes, stream);
+}
+
+int aria_stack_plan_is_streaming(const aria_stack_plan* plan) { return plan && plan->ws_plan ? 1 : 0; }
+
+void aria_stack_plan_destroy(aria_stack_plan* plan) {
+    if (!plan) return;
+    ws_plan_destroy(plan->ws_plan);
+    cudaFree(plan->d_ws);
+    delete plan;
 }
 
 int aria_denoiser_linears_host(const aria_layer* layers, int n_layers, int M, int mode, int io,

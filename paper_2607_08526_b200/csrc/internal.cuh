@@ -45,4 +45,12 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
 size_t w4_workspace_bytes(int M, int N, int K, int sms);
 void w4_set_profile_buffer(long long* p);  // debug hook: per-CTA role timestamps
 
+// ---- w4a16_stream.cu: persistent weight-streaming kernel for a list of W4A16 linears at M <= 32
+struct WsPlan;
+bool ws_eligible(const aria_layer* layers, int n_layers, int M, int mode, int io);
+int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan** out);
+int ws_plan_run(const WsPlan* plan, cudaStream_t st);
+void ws_plan_destroy(WsPlan* plan);
+void ws_set_profile_buffer(long long* p);  // debug hook: per-CTA role timestamps (read at plan creation)
+
 }  // namespace aria

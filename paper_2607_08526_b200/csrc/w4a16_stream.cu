@@ -1,0 +1,633 @@
+// w4a16_stream.cu -- S4 at small M (<= 32 tokens): ONE persistent weight-streaming kernel for a whole
+// list of W4A16 linears (a denoising step's stack, or a batch of independent linears).
+//
+// At M <= 32 a linear moves ~4-5 MB of packed weights and does ~0.2 us of tensor work: it is bound by
+// HBM, and a kernel per layer cannot even ramp the memory system up (0.7 us of data per launch).  Here
+// the weight stream of ALL layers runs back to back through one deep TMA ring per SM; nothing in it
+// depends on activations, so it keeps flowing while a layer waits for its input.
+//
+// Work unit = (layer, 128 output channels, ALL of K); a stage is 256 k-values of 128 weight rows:
+// 16 KB of packed int4 (128-byte rows, SWIZZLE_128B) + 2 KB of fp16 group scales.  There is no
+// split-K: a cross-CTA reduction costs a chain of ~6 global round trips per unit (partials, fence,
+// counter, re-read) -- measured 4k-25k cycles per unit against ~2.7k cycles of dequantisation, the
+// reason the per-layer kernel is latency bound at M = 32.  Instead the host deals the units of ALL
+// layers to the CTAs at plan time (in layer order, always to the least-loaded CTA), so every CTA
+// streams the same number of stages and a layer with few tiles simply overlaps its neighbours.
+// Roles (768 threads, 1 CTA / SM):
+//   warp 0      X producer: [32 tokens x 64 k] bf16 tiles by TMA (L2 resident), after the unit's
+//               dependency (a chained layer waits for its producer layer's completion counter).
+//   warp 2      weight producer: packed + scale tiles by TMA, evict-first (the HBM stream).
+//   warp 1      MMA issuer: tcgen05.mma kind::f16, A = dequantised weights IN TENSOR MEMORY
+//               (128 rows x 16 k per instruction), B = X tile in shared memory, D = fp32 in TMEM.
+//   warps 4-7   epilogue: tcgen05.ld -> + bias, GELU, cast -> coalesced stores; a layer that feeds a
+//               later layer also bumps its completion counter (release).
+//   warps 8-23  four dequantiser groups (thread = weight row; group g = 64-k sub-block g of every
+//               stage): LDS -> registers -> tcgen05.st into a ring of TMEM A slots.  The dequantised
+//               tile never touches shared memory: per weight shared memory sees 0.5 B (TMA write)
+//               + 0.5 B (LDS) instead of 4.5 B with an smem A tile, which would cap the stream at
+//               ~28 weights/clk/SM -- below the ~41 weights/clk/SM that HBM delivers.
+// Dequantisation (AF16): the offset-binary nibble u = q + 8 in a byte 0x0u IS the e4m3 number
+// u * 2^-9; cvt.rn.f16x2.e4m3x2 turns two of them into fp16 and one HFMA2
+// (u 2^-9)(512 sg) - 8 sg = fp16_rn(q sg) finishes: w^ is the correctly rounded fp16 value of the
+// dequantised weight, 13 instructions per 8 weights (the exact-bf16 path of gemm_w4a16.cu needs 18
+// and saturates the ALU pipe at 24.6 weights/clk/SM).  The MMA takes A as fp16 and B (activations)
+// as bf16 -- both formats of kind::f16.  AF16 = false keeps w^ = bf16_rne(q sg) (slower).
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "internal.cuh"
+
+namespace aria {
+
+constexpr int WS_TT = 32;        // tokens per tile = MMA N
+constexpr int WS_ROWS = 128;     // output channels per tile = MMA M
+constexpr int WS_SBK = 256;      // k-values per stage
+constexpr int WS_PS = 7;         // weight ring depth (stages of 18 KB)
+constexpr int WS_XS = 3;         // X ring depth (stages of 16 KB)
+constexpr int WS_NA = 8;         // TMEM A slots (32 columns = 128 rows x 64 k each)
+constexpr int WS_G = 4;          // dequantiser groups
+constexpr int WS_EPI_WARP0 = 4;
+constexpr int WS_DEQ_WARP0 = 8;
+constexpr int WS_THREADS = 32 * WS_DEQ_WARP0 + 128 * WS_G;   // 768
+constexpr int WS_P_BYTES = WS_ROWS * 128;                    // 16 KB
+constexpr int WS_S_BYTES = WS_ROWS * 16;                     // 2 KB
+constexpr int WS_X_BYTES = 4 * WS_TT * 128;                  // 16 KB: 4 sub-tiles [32 x 64] bf16
+constexpr int WS_P_OFF = 0;
+constexpr int WS_X_OFF = WS_P_OFF + WS_PS * WS_P_BYTES;
+constexpr int WS_S_OFF = WS_X_OFF + WS_XS * WS_X_BYTES;
+constexpr int WS_BAR_OFF = WS_S_OFF + WS_PS * WS_S_BYTES;
+constexpr int WS_NBAR = 2 * WS_PS + 2 * WS_XS + 2 * WS_NA + 4;
+constexpr int WS_SMEM_BYTES = WS_BAR_OFF + WS_NBAR * 8 + 16 + 1024;
+constexpr int WS_ACC_COL0 = 0;                               // two fp32 accumulators of 32 columns
+constexpr int WS_A_COL0 = 64;
+constexpr int WS_TMEM_COLS = 512;
+static_assert(WS_SMEM_BYTES <= 227 * 1024, "shared memory");
+static_assert(WS_A_COL0 + WS_NA * 32 <= WS_TMEM_COLS, "tensor memory");
+
+// One linear of the list, as the kernel sees it (device memory; tensor maps need 64-byte alignment).
+struct alignas(128) WsLayer {
+    CUtensorMap tmP;          // packed int4 [N, K/2] u8, box 128 rows x 128 B, SWIZZLE_128B
+    CUtensorMap tmS;          // group scales [N, K/32] fp16, box 128 rows x 8, no swizzle
+    CUtensorMap tmX;          // activations [M, K] bf16, box 32 rows x 64, SWIZZLE_128B
+    const void* bias;         // bf16 [N] or nullptr
+    void* Y;                  // [M, N] bf16 / fp32
+    int N, K;
+    int num_n, num_sb;        // 128-row tiles, 256-k stages
+    int act, out_t;
+    int dep;                  // layer whose completion this layer's input needs, or -1
+    int notify;               // 1 if a later layer depends on this one (epilogue bumps done[l])
+    unsigned done_target;     // num_n * 4 quarter-tiles complete the layer
+    int pad_[3];
+};
+
+struct WsParams {
+    const WsLayer* layers;    // [n_layers]
+    const int* sched;         // units (layer << 16 | tile), CTA b owns sched[sched_off[b] .. sched_off[b+1])
+    const int* sched_off;     // [grid + 1]
+    unsigned* done;           // [n_layers] completion counters   (zeroed before each launch)
+    int n_layers, M;
+    long long* prof;          // debug: per-CTA role timestamps (16 per CTA), or nullptr
+};
+
+static long long* g_ws_prof = nullptr;
+void ws_set_profile_buffer(long long* p) { g_ws_prof = p; }
+#define WS_STAMP(slot) do { if (p.prof) p.prof[blockIdx.x * 16 + (slot)] = clock64() - t_start; } while (0)
+
+__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// Spin until a completion counter reaches its target.  Producers are earlier units of CTAs that are
+// resident (grid <= #SMs, 1 CTA/SM); a watchdog turns a scheduling bug into a trap, not a hang.
+__device__ __forceinline__ void wait_counter(const unsigned* p, unsigned target) {
+    if (ld_acquire(p) >= target) return;
+    const long long t0 = clock64();
+    while (ld_acquire(p) < target) {
+        __nanosleep(64);
+        if (clock64() - t0 > 4000000000LL) {
+            printf("aria: stream-kernel dependency watchdog (block %d)\n", blockIdx.x);
+            __trap();
+        }
+    }
+}
+__device__ __forceinline__ void fence_proxy_async_all() {
+    asm volatile("fence.proxy.async;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_st_32x32b_x32(uint32_t taddr, const uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+        "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
+        "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
+        "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() {
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]^T
+__device__ __forceinline__ void mma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc,
+                                           uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+// ---- dequantisation, 8 codes of one 32-bit word (nibble i = code of k = 8w + i) -> 4 packed pairs
+__device__ __forceinline__ uint32_t ws_lop_and_xor(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, 0x6A;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+__device__ __forceinline__ void cvt_e4m3x4_f16(uint32_t v, uint32_t& lo, uint32_t& hi) {
+    asm("{\n\t.reg .b16 l, h;\n\tmov.b32 {l, h}, %2;\n\t"
+        "cvt.rn.f16x2.e4m3x2 %0, l;\n\tcvt.rn.f16x2.e4m3x2 %1, h;\n\t}"
+        : "=r"(lo), "=r"(hi)
+        : "r"(v));
+}
+__device__ __forceinline__ uint32_t hfma2_u32(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+// fp16 path: S2 = (512 sg, 512 sg), C2 = (-8 sg, -8 sg), both exact in fp16 unless 512 sg overflows
+// (sg > 127.9, i.e. |w| > 895: such a group takes the value inf -- documented limit of the fp16 path).
+__device__ __forceinline__ void dequant_word_f16(uint32_t w, uint32_t S2, uint32_t C2, uint32_t* o) {
+    const uint32_t t = w >> 4;
+    const uint32_t lo = ws_lop_and_xor(__byte_perm(w, t, 0x5140), 0x0F0F0F0Fu, 0x08080808u);  // k0..k3
+    const uint32_t hi = ws_lop_and_xor(__byte_perm(w, t, 0x7362), 0x0F0F0F0Fu, 0x08080808u);  // k4..k7
+    uint32_t a, b, c, d;
+    cvt_e4m3x4_f16(lo, a, b);
+    cvt_e4m3x4_f16(hi, c, d);
+    o[0] = hfma2_u32(a, S2, C2);
+    o[1] = hfma2_u32(b, S2, C2);
+    o[2] = hfma2_u32(c, S2, C2);
+    o[3] = hfma2_u32(d, S2, C2);
+}
+// exact bf16 path (same arithmetic as gemm_w4a16.cu): nibble at mantissa bit pos of 1.0f, one FMA
+// with exactly representable addends, one cvt.rn.bf16x2.
+__device__ __forceinline__ uint32_t ws_fma2_bf16x2(uint32_t e0, uint32_t e1, uint64_t s, uint64_t c) {
+    uint64_t x, d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "r"(e0), "r"(e1));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(x), "l"(s), "l"(c));
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+__device__ __forceinline__ void dequant_word_bf16(uint32_t w, float sg, uint32_t* o) {
+    const float s8 = sg * 32768.0f, c8 = -(sg * 32776.0f);
+    const float s12 = sg * 2048.0f, c12 = -(sg * 2056.0f);
+    const float s16 = sg * 128.0f, c16 = -(sg * 136.0f);
+    const uint32_t wa = w << 8, wb = w >> 12;
+    const uint32_t M8 = 0x00000F00u, M12 = 0x0000F000u, M16 = 0x000F0000u;
+    const uint32_t X8 = 0x3F800800u, X12 = 0x3F808000u, X16 = 0x3F880000u;
+    o[0] = ws_fma2_bf16x2(ws_lop_and_xor(wa, M8, X8), ws_lop_and_xor(wa, M12, X12), pack_f2(s8, s12), pack_f2(c8, c12));
+    o[1] = ws_fma2_bf16x2(ws_lop_and_xor(wa, M16, X16), ws_lop_and_xor(w, M12, X12), pack_f2(s16, s12), pack_f2(c16, c12));
+    o[2] = ws_fma2_bf16x2(ws_lop_and_xor(w, M16, X16), ws_lop_and_xor(wb, M8, X8), pack_f2(s16, s8), pack_f2(c16, c8));
+    o[3] = ws_fma2_bf16x2(ws_lop_and_xor(wb, M12, X12), ws_lop_and_xor(wb, M16, X16), pack_f2(s12, s16), pack_f2(c12, c16));
+}
+
+__device__ __forceinline__ uint4 ws_lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint32_t ws_lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
+// Walks this CTA's unit list; every role runs an identical copy.
+struct UnitIter {
+    const int* sched;
+    int i, end;
+    int l, tile, sb0, sb1;
+    bool first;
+    __device__ __forceinline__ UnitIter(const WsParams& p)
+        : sched(p.sched), i(p.sched_off[blockIdx.x]), end(p.sched_off[blockIdx.x + 1]), first(true) {}
+    __device__ __forceinline__ bool valid() const { return i < end; }
+    __device__ __forceinline__ void locate(const WsParams& p) {   // call when valid()
+        const int e = __ldg(sched + i);
+        l = e >> 16;
+        tile = e & 0xFFFF;
+        sb0 = 0;
+        sb1 = p.layers[l].num_sb;
+    }
+    __device__ __forceinline__ void next() { ++i; first = false; }
+};
+
+template <bool AF16>
+__global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;
+    uint8_t* gbase = smem_raw + (base - raw);
+    const uint32_t sP = base + WS_P_OFF, sX = base + WS_X_OFF, sS = base + WS_S_OFF;
+    const uint32_t bars = base + WS_BAR_OFF;
+    const uint32_t pfull0 = bars, pempty0 = pfull0 + 8 * WS_PS;
+    const uint32_t xfull0 = pempty0 + 8 * WS_PS, xempty0 = xfull0 + 8 * WS_XS;
+    const uint32_t afull0 = xempty0 + 8 * WS_XS, aempty0 = afull0 + 8 * WS_NA;
+    const uint32_t tfull0 = aempty0 + 8 * WS_NA, tempty0 = tfull0 + 16;
+    const uint32_t tmem_slot = tempty0 + 16;
+    volatile uint32_t* tmem_slot_g =
+        reinterpret_cast<volatile uint32_t*>(gbase + WS_BAR_OFF + WS_NBAR * 8);
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+
+    if (warp == 0 && lane == 0) {
+        for (int s = 0; s < WS_PS; ++s) {
+            mbar_init(pfull0 + 8 * s, 1);
+            mbar_init(pempty0 + 8 * s, 4 * WS_G);     // every dequantiser warp reads every stage
+        }
+        for (int s = 0; s < WS_XS; ++s) {
+            mbar_init(xfull0 + 8 * s, 1);
+            mbar_init(xempty0 + 8 * s, 1);            // MMA commit
+        }
+        for (int a = 0; a < WS_NA; ++a) {
+            mbar_init(afull0 + 8 * a, 4);             // the 4 warps of the group that filled it
+            mbar_init(aempty0 + 8 * a, 1);            // MMA commit
+        }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(tfull0 + 8 * a, 1);
+            mbar_init(tempty0 + 8 * a, 4);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 1) {
+        tmem_alloc(tmem_slot, WS_TMEM_COLS);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_g;
+    const long long t_start = clock64();
+
+    if (warp == 0) {
+        // ------------------------------------------------------------ X producer
+        int stage = 0;
+        uint32_t phase = 0;
+        for (UnitIter it(p); it.valid(); it.next()) {
+            it.locate(p);
+            const WsLayer& L = p.layers[it.l];
+            if (L.dep >= 0) {       // chained layer: the producer layer must be complete
+                if (lane == 0) {
+                    wait_counter(p.done + L.dep, p.layers[L.dep].done_target);
+                    fence_proxy_async_all();   // generic-proxy stores of other SMs -> this TMA read
+                }
+                __syncwarp();
+            }
+            for (int sb = it.sb0; sb < it.sb1; ++sb) {
+                mbar_wait(xempty0 + 8 * stage, phase ^ 1);
+                if (elect_one()) {
+                    mbar_arrive_expect_tx(xfull0 + 8 * stage, WS_X_BYTES);
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        tma_load_2d(sX + stage * WS_X_BYTES + j * (WS_TT * 128), &L.tmX,
+                                    sb * WS_SBK + j * 64, 0, xfull0 + 8 * stage);
+                }
+                __syncwarp();
+                if (++stage == WS_XS) { stage = 0; phase ^= 1; }
+            }
+        }
+        if (lane == 0) WS_STAMP(0);
+    } else if (warp == 2) {
+        // ------------------------------------------------------------ weight producer (the HBM stream)
+        const uint64_t pol_w = policy_evict_first();
+        int stage = 0;
+        uint32_t phase = 0;
+        for (UnitIter it(p); it.valid(); it.next()) {
+            it.locate(p);
+            const WsLayer& L = p.layers[it.l];
+            const int n0 = it.tile * WS_ROWS;
+            for (int sb = it.sb0; sb < it.sb1; ++sb) {
+                mbar_wait(pempty0 + 8 * stage, phase ^ 1);
+                if (elect_one()) {
+                    mbar_arrive_expect_tx(pfull0 + 8 * stage, WS_P_BYTES + WS_S_BYTES);
+                    tma_load_2d_hint(sP + stage * WS_P_BYTES, &L.tmP, sb * 128, n0, pfull0 + 8 * stage, pol_w);
+                    tma_load_2d_hint(sS + stage * WS_S_BYTES, &L.tmS, sb * 8, n0, pfull0 + 8 * stage, pol_w);
+                }
+                __syncwarp();
+                if (++stage == WS_PS) { stage = 0; phase ^= 1; }
+            }
+        }
+        if (lane == 0) WS_STAMP(1);
+    } else if (warp == 1) {
+        // ------------------------------------------------------------ MMA issuer
+        constexpr uint32_t idesc = make_idesc(1, AF16 ? 0u : 1u, 1, WS_ROWS, WS_TT);
+        const uint64_t desc_hi = make_smem_desc_sw128(0);
+        int xs = 0, slot = 0, acc = 0;
+        uint32_t xphase = 0, aphase = 0, acc_phase = 0;
+        for (UnitIter it(p); it.valid(); it.next()) {
+            it.locate(p);
+            mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1);
+            tc_fence_after();
+            const uint32_t d_tmem = tmem_base + WS_ACC_COL0 + acc * WS_TT;
+            for (int sb = it.sb0; sb < it.sb1; ++sb) {
+                mbar_wait(xfull0 + 8 * xs, xphase);
+                for (int j = 0; j < 4; ++j) {
+                    mbar_wait(afull0 + 8 * slot, aphase);
+                    tc_fence_after();
+                    if (lane == 0 && it.first && sb == it.sb0 && j == 0) WS_STAMP(2);
+                    const uint32_t a_tmem = tmem_base + WS_A_COL0 + slot * 32;
+                    const uint64_t b_desc =
+                        desc_hi | (((sX + xs * WS_X_BYTES + j * (WS_TT * 128)) & 0x3FFFF) >> 4);
+                    if (elect_one()) {
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            mma_f16_ts(d_tmem, a_tmem + k * 8, b_desc + 2 * k, idesc,
+                                       (sb != it.sb0 || j != 0 || k != 0) ? 1u : 0u);
+                        tc_commit(aempty0 + 8 * slot);
+                        if (j == 3) tc_commit(xempty0 + 8 * xs);
+                        if (j == 3 && sb == it.sb1 - 1) tc_commit(tfull0 + 8 * acc);
+                    }
+                    __syncwarp();
+                    if (++slot == WS_NA) { slot = 0; aphase ^= 1; }
+                }
+                if (++xs == WS_XS) { xs = 0; xphase ^= 1; }
+            }
+            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        }
+        if (lane == 0) WS_STAMP(3);
+    } else if (warp >= WS_DEQ_WARP0) {
+        // ------------------------------------------------------------ dequantiser groups
+        const int dw = warp - WS_DEQ_WARP0;
+        const int g = dw >> 2;                    // group = 64-k sub-block of the stage
+        const int q = dw & 3;                     // TMEM lane quarter (== warp % 4)
+        const int r = q * 32 + lane;              // weight row inside the tile
+        const uint32_t xr = r & 7;
+        const uint32_t poff0 = r * 128 + (((2 * g) ^ xr) << 4);        // 128-byte swizzle
+        const uint32_t poff1 = r * 128 + (((2 * g + 1) ^ xr) << 4);
+        const uint32_t soff = r * 16 + g * 4;
+        const uint32_t a_lane = static_cast<uint32_t>(q * 32) << 16;
+        int stage = 0;
+        uint32_t phase = 0;
+        int half = 0;                             // A slot = half * 4 + g
+        uint32_t aphase = 0;
+        for (UnitIter it(p); it.valid(); it.next()) {
+            it.locate(p);
+            for (int sb = it.sb0; sb < it.sb1; ++sb) {
+                mbar_wait(pfull0 + 8 * stage, phase);
+                if (dw == 0 && lane == 0 && it.first && sb == it.sb0) WS_STAMP(4);
+                const uint32_t sc2 = ws_lds32(sS + stage * WS_S_BYTES + soff);
+                const uint4 pk0 = ws_lds128(sP + stage * WS_P_BYTES + poff0);
+                const uint4 pk1 = ws_lds128(sP + stage * WS_P_BYTES + poff1);
+                uint32_t o[32];
+                if (AF16) {
+                    const __half2 k512 = __floats2half2_rn(512.0f, 512.0f), km8 = __floats2half2_rn(-8.0f, -8.0f);
+                    {
+                        const __half2 s = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
+                        const __half2 S = __hmul2(s, k512), C = __hmul2(s, km8);
+                        const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&S), C2 = *reinterpret_cast<const uint32_t*>(&C);
+                        dequant_word_f16(pk0.x, S2, C2, o + 0);  dequant_word_f16(pk0.y, S2, C2, o + 4);
+                        dequant_word_f16(pk0.z, S2, C2, o + 8);  dequant_word_f16(pk0.w, S2, C2, o + 12);
+                    }
+                    {
+                        const __half2 s = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
+                        const __half2 S = __hmul2(s, k512), C = __hmul2(s, km8);
+                        const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&S), C2 = *reinterpret_cast<const uint32_t*>(&C);
+                        dequant_word_f16(pk1.x, S2, C2, o + 16); dequant_word_f16(pk1.y, S2, C2, o + 20);
+                        dequant_word_f16(pk1.z, S2, C2, o + 24); dequant_word_f16(pk1.w, S2, C2, o + 28);
+                    }
+                } else {
+                    const float s0 = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
+                    const float s1 = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
+                    dequant_word_bf16(pk0.x, s0, o + 0);  dequant_word_bf16(pk0.y, s0, o + 4);
+                    dequant_word_bf16(pk0.z, s0, o + 8);  dequant_word_bf16(pk0.w, s0, o + 12);
+                    dequant_word_bf16(pk1.x, s1, o + 16); dequant_word_bf16(pk1.y, s1, o + 20);
+                    dequant_word_bf16(pk1.z, s1, o + 24); dequant_word_bf16(pk1.w, s1, o + 28);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(pempty0 + 8 * stage);       // packed bytes are in registers
+                const int slot = half * 4 + g;
+                mbar_wait(aempty0 + 8 * slot, aphase ^ 1);             // MMAs reading this slot retired
+                tc_fence_after();
+                tmem_st_32x32b_x32(tmem_base + WS_A_COL0 + slot * 32 + a_lane, o);
+                tmem_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(afull0 + 8 * slot);
+                if (++stage == WS_PS) { stage = 0; phase ^= 1; }
+                if (++half == 2) { half = 0; aphase ^= 1; }
+            }
+        }
+        if (dw == 0 && lane == 0) WS_STAMP(5);
+    } else if (warp >= WS_EPI_WARP0) {
+        // ------------------------------------------------------------ epilogue (warps 4..7)
+        const int q = warp & 3;
+        int acc = 0;
+        uint32_t acc_phase = 0;
+        for (UnitIter it(p); it.valid(); it.next()) {
+            it.locate(p);
+            const WsLayer& L = p.layers[it.l];
+            const int N = L.N, M = p.M;
+            const int n = it.tile * WS_ROWS + q * 32 + lane;
+            const bool n_ok = n < N;
+            mbar_wait(tfull0 + 8 * acc, acc_phase);
+            tc_fence_after();
+            if (q == 0 && lane == 0 && it.first) WS_STAMP(6);
+            uint32_t v[32];
+            tmem_ld_32x32b_x32(tmem_base + WS_ACC_COL0 + acc * WS_TT + (static_cast<uint32_t>(q * 32) << 16), v);
+            tmem_wait_ld();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty0 + 8 * acc);             // accumulator is in registers
+            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+
+            if (n_ok) {
+                const float bv = L.bias ? __bfloat162float(static_cast<const __nv_bfloat16*>(L.bias)[n]) : 0.0f;
+                const bool gelu = L.act == ARIA_ACT_GELU_ERF;
+#pragma unroll
+                for (int t = 0; t < WS_TT; ++t) {
+                    if (t < M) {
+                        float y = __uint_as_float(v[t]) + bv;
+                        if (gelu) y = gelu_erf(y);
+                        const size_t idx = static_cast<size_t>(t) * N + n;   // a warp writes 32 consecutive n
+                        if (L.out_t == ARIA_F32) static_cast<float*>(L.Y)[idx] = y;
+                        else static_cast<__nv_bfloat16*>(L.Y)[idx] = __float2bfloat16_rn(y);
+                    }
+                }
+            }
+            if (L.notify) {                 // a later layer reads this output: publish the quarter-tile
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) atomicAdd(p.done + it.l, 1u);
+            }
+            if (q == 0 && lane == 0 && it.first) WS_STAMP(7);
+        }
+        if (q == 0 && lane == 0) WS_STAMP(8);
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc(tmem_base, WS_TMEM_COLS);
+    }
+}
+
+}  // namespace aria
+
+// ------------------------------------------------------------------------------------------------
+// Host side: pre-encoded tensor maps, the unit schedule and the scratch of one layer list.
+namespace aria {
+
+struct WsPlan {
+    bool a_f16 = true;
+    WsLayer* d_layers = nullptr;
+    int* d_sched = nullptr;         // unit lists + offsets
+    unsigned* d_done = nullptr;
+    size_t done_bytes = 0;
+    WsParams params{};
+    int grid = 0;
+};
+
+void ws_plan_destroy(WsPlan* p) {
+    if (!p) return;
+    cudaFree(p->d_layers);
+    cudaFree(p->d_sched);
+    cudaFree(p->d_done);
+    delete p;
+}
+
+static bool overlaps(const void* a, size_t an, const void* b, size_t bn) {
+    const uintptr_t a0 = reinterpret_cast<uintptr_t>(a), b0 = reinterpret_cast<uintptr_t>(b);
+    return a0 < b0 + bn && b0 < a0 + an;
+}
+
+// The stream kernel runs layers concurrently where the list allows it, so it is used only when
+// running them in array order cannot be told apart: bf16 I/O, M <= 32, K % 256 == 0 (16-byte pitch of
+// the scale tensor map), and no output buffer that overlaps another layer's output or an EARLIER
+// layer's input (a later layer reading an earlier output is the chained case and is tracked).
+bool ws_eligible(const aria_layer* layers, int n_layers, int M, int mode, int io) {
+    if (mode != ARIA_W4A16 || io != ARIA_BF16 || M > WS_TT) return false;
+    if (getenv("ARIA_NO_STREAM")) return false;
+    for (int i = 0; i < n_layers; ++i) {
+        if (layers[i].K % WS_SBK != 0) return false;
+        const size_t ob = static_cast<size_t>(M) * layers[i].N * 2;
+        for (int j = 0; j < n_layers; ++j) {
+            if (j == i) continue;
+            if (overlaps(layers[i].out, ob, layers[j].out, static_cast<size_t>(M) * layers[j].N * 2)) return false;
+            if (j < i && layers[j].in &&
+                overlaps(layers[i].out, ob, layers[j].in, static_cast<size_t>(M) * layers[j].K * 2))
+                return false;
+        }
+    }
+    return true;
+}
+
+int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan** out) {
+    *out = nullptr;
+    WsPlan* plan = new (std::nothrow) WsPlan;
+    if (!plan) return ARIA_ERR_CUDA;
+    // default: the fp16 operand (see the header comment); ARIA_W4_F16A=0 keeps w^ = bf16_rne(q sg),
+    // the slower exact-bf16 path.  Read per plan so tests can build both.
+    const char* e = getenv("ARIA_W4_F16A");
+    plan->a_f16 = e == nullptr || e[0] != '0';
+    const int sms = num_sms();
+    if (sms <= 0) { ws_plan_destroy(plan); return ARIA_ERR_CUDA; }
+    std::vector<WsLayer> h(n_layers);
+    int total_units = 0;
+    for (int i = 0; i < n_layers; ++i) {
+        const aria_layer& L = layers[i];
+        WsLayer& w = h[i];
+        memset(&w, 0, sizeof(w));
+        const void* in = L.in ? L.in : layers[i - 1].out;
+        if (make_tmap_2d(&w.tmP, L.wq, 1, L.N, L.K / 2, WS_ROWS, 128, 128) != ARIA_OK ||
+            make_tmap_2d(&w.tmS, L.w_scale, 2, L.N, L.K / 32, WS_ROWS, 8, 0) != ARIA_OK ||
+            make_tmap_2d(&w.tmX, in, 2, M, L.K, WS_TT, 64, 128) != ARIA_OK) {
+            ws_plan_destroy(plan);
+            return ARIA_ERR_CUDA;
+        }
+        w.bias = L.bias; w.Y = L.out; w.N = L.N; w.K = L.K;
+        w.num_n = (L.N + WS_ROWS - 1) / WS_ROWS;
+        w.num_sb = L.K / WS_SBK;
+        w.act = L.act; w.out_t = io;
+        // dependency: an input that overlaps an earlier layer's output waits for that layer
+        w.dep = -1;
+        for (int j = i - 1; j >= 0; --j)
+            if (overlaps(in, static_cast<size_t>(M) * L.K * 2, layers[j].out, static_cast<size_t>(M) * layers[j].N * 2)) {
+                w.dep = j;
+                h[j].notify = 1;
+                break;
+            }
+        w.done_target = static_cast<unsigned>(w.num_n * 4);
+        total_units += w.num_n;
+        if (w.num_n > 0xFFFF || n_layers > 0x7FFF) { ws_plan_destroy(plan); return ARIA_ERR_SHAPE; }
+    }
+    // Schedule: layers in order, each tile to the CTA with the least work so far (cost = stages + a
+    // per-unit constant for the accumulator hand-off), so every CTA's list is in layer order (a
+    // dependency always points to a unit that is earlier in some CTA's list: no deadlock) and all
+    // CTAs stream the same number of stages.
+    const int grid = total_units < sms ? total_units : sms;
+    std::vector<std::vector<int>> lists(grid);
+    std::vector<long> load(grid, 0);
+    for (int i = 0; i < n_layers; ++i)
+        for (int t = 0; t < h[i].num_n; ++t) {
+            int best = 0;
+            for (int c = 1; c < grid; ++c)
+                if (load[c] < load[best]) best = c;
+            lists[best].push_back((i << 16) | t);
+            load[best] += 2 * h[i].num_sb + 1;
+        }
+    std::vector<int> sched;
+    std::vector<int> off(grid + 1, 0);
+    for (int c = 0; c < grid; ++c) {
+        off[c] = static_cast<int>(sched.size());
+        sched.insert(sched.end(), lists[c].begin(), lists[c].end());
+    }
+    off[grid] = static_cast<int>(sched.size());
+    const size_t sched_n = sched.size();
+    sched.insert(sched.end(), off.begin(), off.end());
+    plan->done_bytes = static_cast<size_t>(n_layers) * sizeof(unsigned);
+    if (cudaMalloc(&plan->d_layers, h.size() * sizeof(WsLayer)) != cudaSuccess ||
+        cudaMalloc(&plan->d_sched, sched.size() * sizeof(int)) != cudaSuccess ||
+        cudaMalloc(&plan->d_done, plan->done_bytes) != cudaSuccess ||
+        cudaMemcpy(plan->d_layers, h.data(), h.size() * sizeof(WsLayer), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(plan->d_sched, sched.data(), sched.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+        ws_plan_destroy(plan);
+        return ARIA_ERR_CUDA;
+    }
+    plan->params.layers = plan->d_layers;
+    plan->params.sched = plan->d_sched;
+    plan->params.sched_off = plan->d_sched + sched_n;
+    plan->params.done = plan->d_done;
+    plan->params.n_layers = n_layers;
+    plan->params.M = M;
+    plan->params.prof = g_ws_prof;
+    plan->grid = grid;
+    *out = plan;
+    return ARIA_OK;
+}
+
+int ws_plan_run(const WsPlan* plan, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(w4a16_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM_BYTES) != cudaSuccess ||
+            cudaFuncSetAttribute(w4a16_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM_BYTES) != cudaSuccess)
+            return ARIA_ERR_CUDA;
+        attr_set = true;
+    }
+    if (cudaMemsetAsync(plan->d_done, 0, plan->done_bytes, st) != cudaSuccess) return ARIA_ERR_CUDA;
+    if (plan->a_f16)
+        w4a16_stream_kernel<true><<<plan->grid, WS_THREADS, WS_SMEM_BYTES, st>>>(plan->params);
+    else
+        w4a16_stream_kernel<false><<<plan->grid, WS_THREADS, WS_SMEM_BYTES, st>>>(plan->params);
+    return cudaGetLastError() == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+}
+
+}  // namespace aria

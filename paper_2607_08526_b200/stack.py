@@ -24,8 +24,9 @@ class LinearStack:
     """`n_blocks` DiT blocks x (QKV, out-proj, MLP up [GELU], MLP down) at M tokens."""
 
     def __init__(self, mode: int, M: int = 2048, n_blocks: int = inputs.N_BLOCKS, keep_host: bool = False,
-                 shared_inputs: bool = True):
+                 shared_inputs: bool = True, use_plan: bool = False):
         self.mode, self.M, self.n_blocks = mode, M, n_blocks
+        self.plan = None
         self.specs = []          # per layer: dict with device tensors
         self.host = []           # per layer: host arrays (tests only, keep_host=True)
         # One N(0,1) bf16 input per distinct K is enough for timing and for parity (each layer has
@@ -62,13 +63,23 @@ class LinearStack:
         maxN = max(s["N"] for s in self.specs)
         self.ws = aria.workspace(aria.aria_workspace_bytes(M, maxK, maxN, mode))
         self.graph = None
+        if use_plan:     # aria_stack_plan_*: at M <= 32 in W4A16 one persistent weight-streaming kernel
+            self.plan = aria.aria_stack_plan_create(self.layers, M, mode, aria.BF16)
         self.ops = sum(2 * M * s["K"] * s["N"] for s in self.specs)
         self.weight_bytes = sum(s["wq"].numel() * s["wq"].element_size() +
                                 s["w_scale"].numel() * s["w_scale"].element_size() for s in self.specs)
 
     def run(self):
         """Enqueue the whole stack on the current stream (no graph)."""
-        aria.aria_denoiser_linears(self.layers, self.M, self.mode, aria.BF16, self.ws)
+        if self.plan is not None:
+            aria.aria_stack_plan_run(self.plan)
+        else:
+            aria.aria_denoiser_linears(self.layers, self.M, self.mode, aria.BF16, self.ws)
+
+    def __del__(self):
+        if getattr(self, "plan", None) is not None:
+            aria.aria_stack_plan_destroy(self.plan)
+            self.plan = None
 
     def capture(self):
         """Capture one step into a CUDA graph (after one eager warm-up)."""
