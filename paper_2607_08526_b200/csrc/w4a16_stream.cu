@@ -30,8 +30,11 @@
 // u * 2^-9; cvt.rn.f16x2.e4m3x2 turns two of them into fp16 and one HFMA2
 // (u 2^-9)(512 sg) - 8 sg = fp16_rn(q sg) finishes: w^ is the correctly rounded fp16 value of the
 // dequantised weight, 13 instructions per 8 weights (the exact-bf16 path of gemm_w4a16.cu needs 18
-// and saturates the ALU pipe at 24.6 weights/clk/SM).  The MMA takes A as fp16 and B (activations)
-// as bf16 -- both formats of kind::f16.  AF16 = false keeps w^ = bf16_rne(q sg) (slower).
+// and saturates the ALU pipe at 24.6 weights/clk/SM -- 60% of what HBM delivers).  kind::f16 takes
+// fp16 x fp16 or bf16 x bf16 but not a mix (illegal instruction on sm_100a), so the bf16 activations
+// are converted to fp16 too: external inputs once per launch by the otherwise idle warps, chained
+// outputs by the producing epilogue (exact for 2^-14 <= |x| <= 65504).  AF16 = false keeps
+// w^ = bf16_rne(q sg) and bf16 activations (slower).
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -44,9 +47,9 @@ namespace aria {
 constexpr int WS_TT = 32;        // tokens per tile = MMA N
 constexpr int WS_ROWS = 128;     // output channels per tile = MMA M
 constexpr int WS_SBK = 256;      // k-values per stage
-constexpr int WS_PS = 7;         // weight ring depth (stages of 18 KB)
-constexpr int WS_XS = 3;         // X ring depth (stages of 16 KB)
-constexpr int WS_NA = 8;         // TMEM A slots (32 columns = 128 rows x 64 k each)
+constexpr int WS_PS = 8;         // weight ring depth (stages of 18 KB)
+constexpr int WS_XS = 3;         // X ring depth (stages of 16 KB): X must be requested BEFORE the weights of its stage
+constexpr int WS_NA = 3;         // TMEM A slots, one STAGE each (128 columns = 128 rows x 256 k)
 constexpr int WS_G = 4;          // dequantiser groups
 constexpr int WS_EPI_WARP0 = 4;
 constexpr int WS_DEQ_WARP0 = 8;
@@ -60,11 +63,15 @@ constexpr int WS_S_OFF = WS_X_OFF + WS_XS * WS_X_BYTES;
 constexpr int WS_BAR_OFF = WS_S_OFF + WS_PS * WS_S_BYTES;
 constexpr int WS_NBAR = 2 * WS_PS + 2 * WS_XS + 2 * WS_NA + 4;
 constexpr int WS_SMEM_BYTES = WS_BAR_OFF + WS_NBAR * 8 + 16 + 1024;
-constexpr int WS_ACC_COL0 = 0;                               // two fp32 accumulators of 32 columns
-constexpr int WS_A_COL0 = 64;
+// Accumulators (WS_NACC > 1 would spread the k-steps over independent accumulators that the epilogue
+// adds; measured: no gain -- back-to-back N = 32 MMAs into one accumulator do not serialise).
+constexpr int WS_NACC = 1;
+constexpr int WS_ACC_COL0 = 0;                               // 2 buffers x 4 fp32 accumulators x 32 columns
+constexpr int WS_A_COL0 = 2 * WS_NACC * WS_TT;
 constexpr int WS_TMEM_COLS = 512;
 static_assert(WS_SMEM_BYTES <= 227 * 1024, "shared memory");
-static_assert(WS_A_COL0 + WS_NA * 32 <= WS_TMEM_COLS, "tensor memory");
+static_assert((WS_PS & (WS_PS - 1)) == 0, "weight ring depth must be a power of two");
+static_assert(WS_A_COL0 + WS_NA * 128 <= WS_TMEM_COLS, "tensor memory");
 
 // One linear of the list, as the kernel sees it (device memory; tensor maps need 64-byte alignment).
 struct alignas(128) WsLayer {
@@ -73,27 +80,40 @@ struct alignas(128) WsLayer {
     CUtensorMap tmX;          // activations [M, K] bf16, box 32 rows x 64, SWIZZLE_128B
     const void* bias;         // bf16 [N] or nullptr
     void* Y;                  // [M, N] bf16 / fp32
+    void* Y16;                // fp16 copy of the bf16 output for the layers that read it (AF16), or nullptr
     int N, K;
     int num_n, num_sb;        // 128-row tiles, 256-k stages
     int act, out_t;
     int dep;                  // layer whose completion this layer's input needs, or -1
     int notify;               // 1 if a later layer depends on this one (epilogue bumps done[l])
     unsigned done_target;     // num_n * 4 quarter-tiles complete the layer
-    int pad_[3];
+    int pad_[1];
+};
+
+// AF16: external bf16 inputs are converted once per launch to fp16 (the MMA needs both operands in
+// the same 16-bit format); segment i covers 16-byte chunks [chunk0, chunk0 + chunks).
+struct WsConv {
+    const uint4* src;         // bf16, 8 per chunk
+    uint4* dst;               // fp16
+    int chunk0, chunks;
 };
 
 struct WsParams {
     const WsLayer* layers;    // [n_layers]
+    const WsConv* conv;       // [n_conv] (AF16)
+    int n_conv, conv_chunks;
     const int* sched;         // units (layer << 16 | tile), CTA b owns sched[sched_off[b] .. sched_off[b+1])
     const int* sched_off;     // [grid + 1]
-    unsigned* done;           // [n_layers] completion counters   (zeroed before each launch)
+    unsigned* done;           // [n_layers] completion counters + [n_layers] = CTAs done converting (zeroed before each launch)
     int n_layers, M;
     long long* prof;          // debug: per-CTA role timestamps (16 per CTA), or nullptr
+    int dbg;                  // debug experiments (ARIA_WS_DBG): 1 = skip dequant math, 2 = skip MMAs
 };
 
 static long long* g_ws_prof = nullptr;
 void ws_set_profile_buffer(long long* p) { g_ws_prof = p; }
-#define WS_STAMP(slot) do { if (p.prof) p.prof[blockIdx.x * 16 + (slot)] = clock64() - t_start; } while (0)
+#define WS_TIMED(accum, stmt) do { if (PROF) { const long long t_ = clock64(); stmt; accum += clock64() - t_; } else { stmt; } } while (0)
+#define WS_STAMP(slot) do { if (PROF) p.prof[blockIdx.x * 16 + (slot)] = clock64() - t_start; } while (0)
 
 __device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
     unsigned v;
@@ -113,6 +133,12 @@ __device__ __forceinline__ void wait_counter(const unsigned* p, unsigned target)
         }
     }
 }
+__device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t v) {
+    const float lo = __uint_as_float(v << 16), hi = __uint_as_float(v & 0xFFFF0000u);
+    uint32_t r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
 __device__ __forceinline__ void fence_proxy_async_all() {
     asm volatile("fence.proxy.async;" ::: "memory");
 }
@@ -125,6 +151,14 @@ __device__ __forceinline__ void tmem_st_32x32b_x32(uint32_t taddr, const uint32_
         "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
         "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
         "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st_32x32b_x16(uint32_t taddr, const uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+        "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
         : "memory");
 }
 __device__ __forceinline__ void tmem_wait_st() {
@@ -229,7 +263,7 @@ struct UnitIter {
     __device__ __forceinline__ void next() { ++i; first = false; }
 };
 
-template <bool AF16>
+template <bool AF16, bool PROF>
 __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsParams p) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
@@ -258,7 +292,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             mbar_init(xempty0 + 8 * s, 1);            // MMA commit
         }
         for (int a = 0; a < WS_NA; ++a) {
-            mbar_init(afull0 + 8 * a, 4);             // the 4 warps of the group that filled it
+            mbar_init(afull0 + 8 * a, 4 * WS_G);      // every dequantiser warp fills its part of the slot
             mbar_init(aempty0 + 8 * a, 1);            // MMA commit
         }
         for (int a = 0; a < 2; ++a) {
@@ -277,8 +311,38 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
     const uint32_t tmem_base = *tmem_slot_g;
     const long long t_start = clock64();
 
+    if (AF16 && p.n_conv > 0 && warp >= WS_EPI_WARP0) {
+        // bf16 -> fp16 of the external inputs (exact for 2^-14 <= |x| <= 65504, saturating above,
+        // absolute error <= 2^-25 below); the producers and the MMA warp start streaming meanwhile.
+        constexpr int CT = WS_THREADS - 32 * WS_EPI_WARP0;
+        const int ctid = threadIdx.x - 32 * WS_EPI_WARP0;
+        for (int c = blockIdx.x * CT + ctid; c < p.conv_chunks; c += gridDim.x * CT) {
+            int lo = 0, hi = p.n_conv - 1;         // segment of chunk c
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (__ldg(&p.conv[mid].chunk0) <= c) lo = mid; else hi = mid - 1;
+            }
+            const WsConv cv = p.conv[lo];
+            const uint4 v = __ldg(cv.src + (c - cv.chunk0));
+            uint4 o;
+            o.x = bf16x2_to_f16x2(v.x); o.y = bf16x2_to_f16x2(v.y);
+            o.z = bf16x2_to_f16x2(v.z); o.w = bf16x2_to_f16x2(v.w);
+            cv.dst[c - cv.chunk0] = o;
+        }
+        __threadfence();
+        named_bar_sync(1, CT);
+        if (ctid == 0) atomicAdd(p.done + p.n_layers, 1u);
+    }
+
     if (warp == 0) {
         // ------------------------------------------------------------ X producer
+        if (AF16 && p.n_conv > 0) {
+            if (lane == 0) {
+                wait_counter(p.done + p.n_layers, gridDim.x);
+                fence_proxy_async_all();
+            }
+            __syncwarp();
+        }
         int stage = 0;
         uint32_t phase = 0;
         for (UnitIter it(p); it.valid(); it.next()) {
@@ -294,10 +358,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             for (int sb = it.sb0; sb < it.sb1; ++sb) {
                 mbar_wait(xempty0 + 8 * stage, phase ^ 1);
                 if (elect_one()) {
-                    mbar_arrive_expect_tx(xfull0 + 8 * stage, WS_X_BYTES);
+                    mbar_arrive_expect_tx(xfull0 + 8 * stage, (PROF && (p.dbg & 8)) ? WS_X_BYTES / 4 : WS_X_BYTES);
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
-                        tma_load_2d(sX + stage * WS_X_BYTES + j * (WS_TT * 128), &L.tmX,
+                        if (j == 0 || !(PROF && (p.dbg & 8))) tma_load_2d(sX + stage * WS_X_BYTES + j * (WS_TT * 128), &L.tmX,
                                     sb * WS_SBK + j * 64, 0, xfull0 + 8 * stage);
                 }
                 __syncwarp();
@@ -317,9 +381,9 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             for (int sb = it.sb0; sb < it.sb1; ++sb) {
                 mbar_wait(pempty0 + 8 * stage, phase ^ 1);
                 if (elect_one()) {
-                    mbar_arrive_expect_tx(pfull0 + 8 * stage, WS_P_BYTES + WS_S_BYTES);
+                    mbar_arrive_expect_tx(pfull0 + 8 * stage, WS_P_BYTES + ((PROF && (p.dbg & 4)) ? 0 : WS_S_BYTES));
                     tma_load_2d_hint(sP + stage * WS_P_BYTES, &L.tmP, sb * 128, n0, pfull0 + 8 * stage, pol_w);
-                    tma_load_2d_hint(sS + stage * WS_S_BYTES, &L.tmS, sb * 8, n0, pfull0 + 8 * stage, pol_w);
+                    if (!(PROF && (p.dbg & 4))) tma_load_2d_hint(sS + stage * WS_S_BYTES, &L.tmS, sb * 8, n0, pfull0 + 8 * stage, pol_w);
                 }
                 __syncwarp();
                 if (++stage == WS_PS) { stage = 0; phase ^= 1; }
@@ -328,104 +392,142 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         if (lane == 0) WS_STAMP(1);
     } else if (warp == 1) {
         // ------------------------------------------------------------ MMA issuer
-        constexpr uint32_t idesc = make_idesc(1, AF16 ? 0u : 1u, 1, WS_ROWS, WS_TT);
+        constexpr uint32_t idesc = make_idesc(1, AF16 ? 0u : 1u, AF16 ? 0u : 1u, WS_ROWS, WS_TT);
         const uint64_t desc_hi = make_smem_desc_sw128(0);
         int xs = 0, slot = 0, acc = 0;
         uint32_t xphase = 0, aphase = 0, acc_phase = 0;
+        long long w_t = 0, w_x = 0, w_a = 0;
         for (UnitIter it(p); it.valid(); it.next()) {
             it.locate(p);
-            mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1);
+            WS_TIMED(w_t, mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1));
             tc_fence_after();
-            const uint32_t d_tmem = tmem_base + WS_ACC_COL0 + acc * WS_TT;
+            const uint32_t d_tmem = tmem_base + WS_ACC_COL0 + acc * (WS_NACC * WS_TT);
             for (int sb = it.sb0; sb < it.sb1; ++sb) {
-                mbar_wait(xfull0 + 8 * xs, xphase);
-                for (int j = 0; j < 4; ++j) {
-                    mbar_wait(afull0 + 8 * slot, aphase);
-                    tc_fence_after();
-                    if (lane == 0 && it.first && sb == it.sb0 && j == 0) WS_STAMP(2);
-                    const uint32_t a_tmem = tmem_base + WS_A_COL0 + slot * 32;
-                    const uint64_t b_desc =
-                        desc_hi | (((sX + xs * WS_X_BYTES + j * (WS_TT * 128)) & 0x3FFFF) >> 4);
-                    if (elect_one()) {
+                WS_TIMED(w_x, mbar_wait(xfull0 + 8 * xs, xphase));
+                WS_TIMED(w_a, mbar_wait(afull0 + 8 * slot, aphase));       // all 4 sub-blocks of the stage dequantised
+                tc_fence_after();
+                if (lane == 0 && it.first && sb == it.sb0) WS_STAMP(2);
+                const uint32_t a_tmem = tmem_base + WS_A_COL0 + slot * 128;
+                const uint64_t b_desc = desc_hi | (((sX + xs * WS_X_BYTES) & 0x3FFFF) >> 4);
+                if (elect_one()) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)             // 64-k sub-tile of X: 4 KB apart
 #pragma unroll
                         for (int k = 0; k < 4; ++k)
-                            mma_f16_ts(d_tmem, a_tmem + k * 8, b_desc + 2 * k, idesc,
-                                       (sb != it.sb0 || j != 0 || k != 0) ? 1u : 0u);
-                        tc_commit(aempty0 + 8 * slot);
-                        if (j == 3) tc_commit(xempty0 + 8 * xs);
-                        if (j == 3 && sb == it.sb1 - 1) tc_commit(tfull0 + 8 * acc);
-                    }
-                    __syncwarp();
-                    if (++slot == WS_NA) { slot = 0; aphase ^= 1; }
+                            if (!(PROF && (p.dbg & 2)))
+                                mma_f16_ts(d_tmem + (k % WS_NACC) * WS_TT, a_tmem + j * 32 + k * 8,
+                                           b_desc + j * (WS_TT * 128 / 16) + 2 * k, idesc,
+                                           (sb != it.sb0 || j * 4 + k >= WS_NACC) ? 1u : 0u);
+                    tc_commit(aempty0 + 8 * slot);
+                    tc_commit(xempty0 + 8 * xs);
+                    if (sb == it.sb1 - 1) tc_commit(tfull0 + 8 * acc);
                 }
+                __syncwarp();
+                if (++slot == WS_NA) { slot = 0; aphase ^= 1; }
                 if (++xs == WS_XS) { xs = 0; xphase ^= 1; }
             }
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
         }
-        if (lane == 0) WS_STAMP(3);
+        if (lane == 0) { WS_STAMP(3); if (PROF) { p.prof[blockIdx.x * 16 + 9] = w_t; p.prof[blockIdx.x * 16 + 10] = w_x; p.prof[blockIdx.x * 16 + 11] = w_a; } }
     } else if (warp >= WS_DEQ_WARP0) {
         // ------------------------------------------------------------ dequantiser groups
+        // The dequantisers do not care about unit boundaries: they see one sequence of `total` stages.
+        // Software pipelined per warp: the packed bytes of stage s+1 are loaded before the arithmetic
+        // of stage s, each half (32 k) goes to TMEM as soon as its 16 registers are ready, and the
+        // "A slot full" signal of stage s is sent in the middle of stage s+1 (its stores have long
+        // landed by then) -- the four warps that share an SM sub-partition hit their barriers at the
+        // same time, so latency that is not overlapped inside a warp is not overlapped at all.  The
+        // loop is issue bound (~120 arithmetic instructions per warp and sub-block): everything else in
+        // it is kept to a minimum.
         const int dw = warp - WS_DEQ_WARP0;
         const int g = dw >> 2;                    // group = 64-k sub-block of the stage
         const int q = dw & 3;                     // TMEM lane quarter (== warp % 4)
         const int r = q * 32 + lane;              // weight row inside the tile
         const uint32_t xr = r & 7;
-        const uint32_t poff0 = r * 128 + (((2 * g) ^ xr) << 4);        // 128-byte swizzle
-        const uint32_t poff1 = r * 128 + (((2 * g + 1) ^ xr) << 4);
-        const uint32_t soff = r * 16 + g * 4;
-        const uint32_t a_lane = static_cast<uint32_t>(q * 32) << 16;
-        int stage = 0;
-        uint32_t phase = 0;
-        int half = 0;                             // A slot = half * 4 + g
+        const uint32_t pa0 = sP + r * 128 + (((2 * g) ^ xr) << 4);        // 128-byte swizzle
+        const uint32_t pa1 = sP + r * 128 + (((2 * g + 1) ^ xr) << 4);
+        const uint32_t sa = sS + r * 16 + g * 4;
+        const uint32_t a_base = tmem_base + WS_A_COL0 + g * 32 + (static_cast<uint32_t>(q * 32) << 16);
+        int total = 0;                            // stages of this CTA
+        for (int i = p.sched_off[blockIdx.x]; i < p.sched_off[blockIdx.x + 1]; ++i)
+            total += __ldg(&p.layers[__ldg(p.sched + i) >> 16].num_sb);
+        uint4 pk0 = make_uint4(0, 0, 0, 0), pk1 = pk0;
+        uint32_t sc2 = 0;
+        if (total > 0) {
+            mbar_wait(pfull0, 0);
+            if (PROF && dw == 0 && lane == 0) WS_STAMP(4);
+            sc2 = ws_lds32(sa);
+            pk0 = ws_lds128(pa0);
+            pk1 = ws_lds128(pa1);
+        }
+        int slot = 0;
         uint32_t aphase = 0;
-        for (UnitIter it(p); it.valid(); it.next()) {
-            it.locate(p);
-            for (int sb = it.sb0; sb < it.sb1; ++sb) {
-                mbar_wait(pfull0 + 8 * stage, phase);
-                if (dw == 0 && lane == 0 && it.first && sb == it.sb0) WS_STAMP(4);
-                const uint32_t sc2 = ws_lds32(sS + stage * WS_S_BYTES + soff);
-                const uint4 pk0 = ws_lds128(sP + stage * WS_P_BYTES + poff0);
-                const uint4 pk1 = ws_lds128(sP + stage * WS_P_BYTES + poff1);
-                uint32_t o[32];
-                if (AF16) {
-                    const __half2 k512 = __floats2half2_rn(512.0f, 512.0f), km8 = __floats2half2_rn(-8.0f, -8.0f);
-                    {
-                        const __half2 s = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
-                        const __half2 S = __hmul2(s, k512), C = __hmul2(s, km8);
-                        const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&S), C2 = *reinterpret_cast<const uint32_t*>(&C);
-                        dequant_word_f16(pk0.x, S2, C2, o + 0);  dequant_word_f16(pk0.y, S2, C2, o + 4);
-                        dequant_word_f16(pk0.z, S2, C2, o + 8);  dequant_word_f16(pk0.w, S2, C2, o + 12);
-                    }
-                    {
-                        const __half2 s = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
-                        const __half2 S = __hmul2(s, k512), C = __hmul2(s, km8);
-                        const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&S), C2 = *reinterpret_cast<const uint32_t*>(&C);
-                        dequant_word_f16(pk1.x, S2, C2, o + 16); dequant_word_f16(pk1.y, S2, C2, o + 20);
-                        dequant_word_f16(pk1.z, S2, C2, o + 24); dequant_word_f16(pk1.w, S2, C2, o + 28);
-                    }
-                } else {
-                    const float s0 = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
-                    const float s1 = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
-                    dequant_word_bf16(pk0.x, s0, o + 0);  dequant_word_bf16(pk0.y, s0, o + 4);
-                    dequant_word_bf16(pk0.z, s0, o + 8);  dequant_word_bf16(pk0.w, s0, o + 12);
-                    dequant_word_bf16(pk1.x, s1, o + 16); dequant_word_bf16(pk1.y, s1, o + 20);
-                    dequant_word_bf16(pk1.z, s1, o + 24); dequant_word_bf16(pk1.w, s1, o + 28);
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(pempty0 + 8 * stage);       // packed bytes are in registers
-                const int slot = half * 4 + g;
-                mbar_wait(aempty0 + 8 * slot, aphase ^ 1);             // MMAs reading this slot retired
-                tc_fence_after();
-                tmem_st_32x32b_x32(tmem_base + WS_A_COL0 + slot * 32 + a_lane, o);
-                tmem_wait_st();
+        long long w_p = 0, w_e = 0, w_s = 0;
+#pragma unroll 2
+        for (int s = 0; s < total; ++s) {
+            // ---- start the loads of the next stage
+            uint4 nk0 = pk0, nk1 = pk1;
+            uint32_t nsc = sc2;
+            if (s + 1 < total) {
+                const int ns = (s + 1) & (WS_PS - 1);
+                WS_TIMED(w_p, mbar_wait(pfull0 + 8 * ns, ((s + 1) / WS_PS) & 1));
+                nsc = ws_lds32(sa + ns * WS_S_BYTES);
+                nk0 = ws_lds128(pa0 + ns * WS_P_BYTES);
+                nk1 = ws_lds128(pa1 + ns * WS_P_BYTES);
+            }
+            uint32_t o[16];
+            // ---- first half: k 0..31 of the sub-block
+            if (PROF && (p.dbg & 1)) {
+#pragma unroll
+                for (int i = 0; i < 16; ++i) o[i] = pk0.x + i;
+            } else if (AF16) {
+                const __half2 sh = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
+                const __half2 S = __hmul2(sh, __floats2half2_rn(512.0f, 512.0f)), C = __hmul2(sh, __floats2half2_rn(-8.0f, -8.0f));
+                const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&S), C2 = *reinterpret_cast<const uint32_t*>(&C);
+                dequant_word_f16(pk0.x, S2, C2, o + 0);  dequant_word_f16(pk0.y, S2, C2, o + 4);
+                dequant_word_f16(pk0.z, S2, C2, o + 8);  dequant_word_f16(pk0.w, S2, C2, o + 12);
+            } else {
+                const float s0 = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
+                dequant_word_bf16(pk0.x, s0, o + 0);  dequant_word_bf16(pk0.y, s0, o + 4);
+                dequant_word_bf16(pk0.z, s0, o + 8);  dequant_word_bf16(pk0.w, s0, o + 12);
+            }
+            if (s > 0) {                           // publish the previous stage's sub-block
+                WS_TIMED(w_s, tmem_wait_st());
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(afull0 + 8 * slot);
-                if (++stage == WS_PS) { stage = 0; phase ^= 1; }
-                if (++half == 2) { half = 0; aphase ^= 1; }
+                if (lane == 0) mbar_arrive(afull0 + 8 * (slot == 0 ? WS_NA - 1 : slot - 1));
             }
+            WS_TIMED(w_e, mbar_wait(aempty0 + 8 * slot, aphase ^ 1));   // MMAs reading this slot retired
+            tc_fence_after();
+            tmem_st_32x32b_x16(a_base + slot * 128, o);
+            // ---- second half: k 32..63
+            if (PROF && (p.dbg & 1)) {
+#pragma unroll
+                for (int i = 0; i < 16; ++i) o[i] = pk1.x + i;
+            } else if (AF16) {
+                const __half2 sh = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
+                const __half2 S = __hmul2(sh, __floats2half2_rn(512.0f, 512.0f)), C = __hmul2(sh, __floats2half2_rn(-8.0f, -8.0f));
+                const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&S), C2 = *reinterpret_cast<const uint32_t*>(&C);
+                dequant_word_f16(pk1.x, S2, C2, o + 0);  dequant_word_f16(pk1.y, S2, C2, o + 4);
+                dequant_word_f16(pk1.z, S2, C2, o + 8);  dequant_word_f16(pk1.w, S2, C2, o + 12);
+            } else {
+                const float s1 = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
+                dequant_word_bf16(pk1.x, s1, o + 0);  dequant_word_bf16(pk1.y, s1, o + 4);
+                dequant_word_bf16(pk1.z, s1, o + 8);  dequant_word_bf16(pk1.w, s1, o + 12);
+            }
+            tmem_st_32x32b_x16(a_base + slot * 128 + 16, o);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(pempty0 + 8 * (s & (WS_PS - 1)));   // this stage's packed bytes are consumed
+            pk0 = nk0; pk1 = nk1; sc2 = nsc;
+            if (++slot == WS_NA) { slot = 0; aphase ^= 1; }
         }
-        if (dw == 0 && lane == 0) WS_STAMP(5);
+        if (total > 0) {
+            tmem_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(afull0 + 8 * (slot == 0 ? WS_NA - 1 : slot - 1));
+        }
+        if (PROF && dw == 0 && lane == 0) { WS_STAMP(5); p.prof[blockIdx.x * 16 + 12] = w_p; p.prof[blockIdx.x * 16 + 13] = w_e; p.prof[blockIdx.x * 16 + 14] = w_s; }
     } else if (warp >= WS_EPI_WARP0) {
         // ------------------------------------------------------------ epilogue (warps 4..7)
         const int q = warp & 3;
@@ -433,36 +535,70 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         uint32_t acc_phase = 0;
         for (UnitIter it(p); it.valid(); it.next()) {
             it.locate(p);
-            const WsLayer& L = p.layers[it.l];
-            const int N = L.N, M = p.M;
+            // layer fields into registers FIRST: the compiler must assume the output stores below may
+            // alias the layer table and would otherwise re-load them from L2 after every store
+            // (measured: 10k cycles per epilogue instead of a few hundred)
+            const WsLayer* Lp = p.layers + it.l;
+            const int N = __ldg(&Lp->N), M = p.M;
+            const int act = __ldg(&Lp->act), out_t = __ldg(&Lp->out_t), notify = __ldg(&Lp->notify);
+            const __nv_bfloat16* bias = static_cast<const __nv_bfloat16*>(
+                reinterpret_cast<const void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->bias))));
+            void* const Yp = reinterpret_cast<void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->Y)));
+            void* const Y16p = reinterpret_cast<void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->Y16)));
             const int n = it.tile * WS_ROWS + q * 32 + lane;
             const bool n_ok = n < N;
+            const float bv = bias && n_ok ? __bfloat162float(bias[n]) : 0.0f;
             mbar_wait(tfull0 + 8 * acc, acc_phase);
             tc_fence_after();
             if (q == 0 && lane == 0 && it.first) WS_STAMP(6);
             uint32_t v[32];
-            tmem_ld_32x32b_x32(tmem_base + WS_ACC_COL0 + acc * WS_TT + (static_cast<uint32_t>(q * 32) << 16), v);
-            tmem_wait_ld();
+            {
+                const uint32_t t_addr = tmem_base + WS_ACC_COL0 + acc * (WS_NACC * WS_TT) + (static_cast<uint32_t>(q * 32) << 16);
+                tmem_ld_32x32b_x32(t_addr, v);
+                tmem_wait_ld();
+#pragma unroll
+                for (int a = 1; a < WS_NACC; ++a) {          // fixed order: deterministic
+                    uint32_t w[32];
+                    tmem_ld_32x32b_x32(t_addr + a * WS_TT, w);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int t = 0; t < WS_TT; ++t) v[t] = __float_as_uint(__uint_as_float(v[t]) + __uint_as_float(w[t]));
+                }
+            }
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty0 + 8 * acc);             // accumulator is in registers
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
 
             if (n_ok) {
-                const float bv = L.bias ? __bfloat162float(static_cast<const __nv_bfloat16*>(L.bias)[n]) : 0.0f;
-                const bool gelu = L.act == ARIA_ACT_GELU_ERF;
+                const bool gelu = act == ARIA_ACT_GELU_ERF;
+                if (out_t == ARIA_F32) {
+                    float* Y = static_cast<float*>(Yp) + n;
 #pragma unroll
-                for (int t = 0; t < WS_TT; ++t) {
-                    if (t < M) {
-                        float y = __uint_as_float(v[t]) + bv;
-                        if (gelu) y = gelu_erf(y);
-                        const size_t idx = static_cast<size_t>(t) * N + n;   // a warp writes 32 consecutive n
-                        if (L.out_t == ARIA_F32) static_cast<float*>(L.Y)[idx] = y;
-                        else static_cast<__nv_bfloat16*>(L.Y)[idx] = __float2bfloat16_rn(y);
+                    for (int t = 0; t < WS_TT; ++t) {
+                        if (t < M) {
+                            float y = __uint_as_float(v[t]) + bv;
+                            if (gelu) y = gelu_erf(y);
+                            Y[static_cast<size_t>(t) * N] = y;           // a warp writes 32 consecutive n
+                        }
+                    }
+                } else {
+                    __nv_bfloat16* Y = static_cast<__nv_bfloat16*>(Yp) + n;
+                    __half* Y16 = AF16 && Y16p ? static_cast<__half*>(Y16p) + n : nullptr;
+#pragma unroll
+                    for (int t = 0; t < WS_TT; ++t) {
+                        if (t < M) {
+                            float y = __uint_as_float(v[t]) + bv;
+                            if (gelu) y = gelu_erf(y);
+                            const __nv_bfloat16 yb = __float2bfloat16_rn(y);
+                            Y[static_cast<size_t>(t) * N] = yb;
+                            // what the dependent layer's MMA reads: the bf16 value, as fp16
+                            if (AF16 && Y16) Y16[static_cast<size_t>(t) * N] = __float2half_rn(__bfloat162float(yb));
+                        }
                     }
                 }
             }
-            if (L.notify) {                 // a later layer reads this output: publish the quarter-tile
+            if (notify) {                   // a later layer reads this output: publish the quarter-tile
                 __threadfence();
                 __syncwarp();
                 if (lane == 0) atomicAdd(p.done + it.l, 1u);
@@ -492,6 +628,8 @@ struct WsPlan {
     int* d_sched = nullptr;         // unit lists + offsets
     unsigned* d_done = nullptr;
     size_t done_bytes = 0;
+    WsConv* d_conv = nullptr;
+    void* d_x16 = nullptr;          // fp16 copies of external inputs and of chained outputs
     WsParams params{};
     int grid = 0;
 };
@@ -501,6 +639,8 @@ void ws_plan_destroy(WsPlan* p) {
     cudaFree(p->d_layers);
     cudaFree(p->d_sched);
     cudaFree(p->d_done);
+    cudaFree(p->d_conv);
+    cudaFree(p->d_x16);
     delete p;
 }
 
@@ -542,17 +682,17 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     if (sms <= 0) { ws_plan_destroy(plan); return ARIA_ERR_CUDA; }
     std::vector<WsLayer> h(n_layers);
     int total_units = 0;
+    // pass 1: shapes, dependencies; fp16 scratch layout (AF16)
+    std::vector<const void*> ext_src;          // distinct external inputs
+    std::vector<size_t> ext_elems, ext_off;
+    std::vector<size_t> y16_off(n_layers, 0);
+    std::vector<int> in_ext(n_layers, -1);
+    size_t x16_elems = 0;
     for (int i = 0; i < n_layers; ++i) {
         const aria_layer& L = layers[i];
         WsLayer& w = h[i];
         memset(&w, 0, sizeof(w));
         const void* in = L.in ? L.in : layers[i - 1].out;
-        if (make_tmap_2d(&w.tmP, L.wq, 1, L.N, L.K / 2, WS_ROWS, 128, 128) != ARIA_OK ||
-            make_tmap_2d(&w.tmS, L.w_scale, 2, L.N, L.K / 32, WS_ROWS, 8, 0) != ARIA_OK ||
-            make_tmap_2d(&w.tmX, in, 2, M, L.K, WS_TT, 64, 128) != ARIA_OK) {
-            ws_plan_destroy(plan);
-            return ARIA_ERR_CUDA;
-        }
         w.bias = L.bias; w.Y = L.out; w.N = L.N; w.K = L.K;
         w.num_n = (L.N + WS_ROWS - 1) / WS_ROWS;
         w.num_sb = L.K / WS_SBK;
@@ -562,12 +702,55 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
         for (int j = i - 1; j >= 0; --j)
             if (overlaps(in, static_cast<size_t>(M) * L.K * 2, layers[j].out, static_cast<size_t>(M) * layers[j].N * 2)) {
                 w.dep = j;
-                h[j].notify = 1;
                 break;
             }
+        if (w.dep >= 0) {
+            // the fp16 path reads the producer's fp16 copy, which has the producer's exact geometry
+            if (plan->a_f16 && (in != layers[w.dep].out || layers[w.dep].N != L.K)) plan->a_f16 = false;
+            h[w.dep].notify = 1;
+        } else {
+            size_t e = 0;
+            while (e < ext_src.size() && !(ext_src[e] == in && ext_elems[e] == static_cast<size_t>(M) * L.K)) ++e;
+            if (e == ext_src.size()) { ext_src.push_back(in); ext_elems.push_back(static_cast<size_t>(M) * L.K); }
+            in_ext[i] = static_cast<int>(e);
+        }
         w.done_target = static_cast<unsigned>(w.num_n * 4);
         total_units += w.num_n;
-        if (w.num_n > 0xFFFF || n_layers > 0x7FFF) { ws_plan_destroy(plan); return ARIA_ERR_SHAPE; }
+        if (w.num_n > 0xFFFF || n_layers > 0x7FFF || (static_cast<size_t>(M) * L.K) % 8 != 0) { ws_plan_destroy(plan); return ARIA_ERR_SHAPE; }
+    }
+    std::vector<WsConv> conv;
+    if (plan->a_f16) {
+        for (size_t e = 0; e < ext_src.size(); ++e) { ext_off.push_back(x16_elems); x16_elems += (ext_elems[e] + 127) / 128 * 128; }
+        for (int i = 0; i < n_layers; ++i)
+            if (h[i].notify) { y16_off[i] = x16_elems; x16_elems += (static_cast<size_t>(M) * layers[i].N + 127) / 128 * 128; }
+        if (cudaMalloc(&plan->d_x16, x16_elems * 2 + 256) != cudaSuccess) { ws_plan_destroy(plan); return ARIA_ERR_CUDA; }
+        int chunk0 = 0;
+        for (size_t e = 0; e < ext_src.size(); ++e) {
+            WsConv c;
+            c.src = static_cast<const uint4*>(ext_src[e]);
+            c.dst = reinterpret_cast<uint4*>(static_cast<uint16_t*>(plan->d_x16) + ext_off[e]);
+            c.chunk0 = chunk0; c.chunks = static_cast<int>(ext_elems[e] / 8);
+            chunk0 += c.chunks;
+            conv.push_back(c);
+        }
+        plan->params.conv_chunks = chunk0;
+    }
+    // pass 2: tensor maps
+    for (int i = 0; i < n_layers; ++i) {
+        const aria_layer& L = layers[i];
+        WsLayer& w = h[i];
+        const void* in = L.in ? L.in : layers[i - 1].out;
+        if (plan->a_f16) {
+            uint16_t* x16 = static_cast<uint16_t*>(plan->d_x16);
+            in = w.dep >= 0 ? x16 + y16_off[w.dep] : x16 + ext_off[in_ext[i]];
+            if (w.notify) w.Y16 = x16 + y16_off[i];
+        }
+        if (make_tmap_2d(&w.tmP, L.wq, 1, L.N, L.K / 2, WS_ROWS, 128, 128) != ARIA_OK ||
+            make_tmap_2d(&w.tmS, L.w_scale, 2, L.N, L.K / 32, WS_ROWS, 8, 0) != ARIA_OK ||
+            make_tmap_2d(&w.tmX, in, 2, M, L.K, WS_TT, 64, 128) != ARIA_OK) {
+            ws_plan_destroy(plan);
+            return ARIA_ERR_CUDA;
+        }
     }
     // Schedule: layers in order, each tile to the CTA with the least work so far (cost = stages + a
     // per-unit constant for the accumulator hand-off), so every CTA's list is in layer order (a
@@ -593,12 +776,14 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     off[grid] = static_cast<int>(sched.size());
     const size_t sched_n = sched.size();
     sched.insert(sched.end(), off.begin(), off.end());
-    plan->done_bytes = static_cast<size_t>(n_layers) * sizeof(unsigned);
+    plan->done_bytes = (static_cast<size_t>(n_layers) + 1) * sizeof(unsigned);
     if (cudaMalloc(&plan->d_layers, h.size() * sizeof(WsLayer)) != cudaSuccess ||
         cudaMalloc(&plan->d_sched, sched.size() * sizeof(int)) != cudaSuccess ||
         cudaMalloc(&plan->d_done, plan->done_bytes) != cudaSuccess ||
         cudaMemcpy(plan->d_layers, h.data(), h.size() * sizeof(WsLayer), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(plan->d_sched, sched.data(), sched.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaMemcpy(plan->d_sched, sched.data(), sched.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess ||
+        (!conv.empty() && (cudaMalloc(&plan->d_conv, conv.size() * sizeof(WsConv)) != cudaSuccess ||
+                           cudaMemcpy(plan->d_conv, conv.data(), conv.size() * sizeof(WsConv), cudaMemcpyHostToDevice) != cudaSuccess))) {
         ws_plan_destroy(plan);
         return ARIA_ERR_CUDA;
     }
@@ -606,28 +791,35 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     plan->params.sched = plan->d_sched;
     plan->params.sched_off = plan->d_sched + sched_n;
     plan->params.done = plan->d_done;
+    plan->params.conv = plan->d_conv;
+    plan->params.n_conv = static_cast<int>(conv.size());
     plan->params.n_layers = n_layers;
     plan->params.M = M;
     plan->params.prof = g_ws_prof;
+    plan->params.dbg = getenv("ARIA_WS_DBG") ? atoi(getenv("ARIA_WS_DBG")) : 0;
     plan->grid = grid;
     *out = plan;
     return ARIA_OK;
 }
 
-int ws_plan_run(const WsPlan* plan, cudaStream_t st) {
+template <bool AF16, bool PROF>
+static int ws_launch(const WsPlan* plan, cudaStream_t st) {
     static bool attr_set = false;
+    auto kern = w4a16_stream_kernel<AF16, PROF>;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(w4a16_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM_BYTES) != cudaSuccess ||
-            cudaFuncSetAttribute(w4a16_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM_BYTES) != cudaSuccess)
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM_BYTES) != cudaSuccess)
             return ARIA_ERR_CUDA;
         attr_set = true;
     }
-    if (cudaMemsetAsync(plan->d_done, 0, plan->done_bytes, st) != cudaSuccess) return ARIA_ERR_CUDA;
-    if (plan->a_f16)
-        w4a16_stream_kernel<true><<<plan->grid, WS_THREADS, WS_SMEM_BYTES, st>>>(plan->params);
-    else
-        w4a16_stream_kernel<false><<<plan->grid, WS_THREADS, WS_SMEM_BYTES, st>>>(plan->params);
+    kern<<<plan->grid, WS_THREADS, WS_SMEM_BYTES, st>>>(plan->params);
     return cudaGetLastError() == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+}
+
+int ws_plan_run(const WsPlan* plan, cudaStream_t st) {
+    if (cudaMemsetAsync(plan->d_done, 0, plan->done_bytes, st) != cudaSuccess) return ARIA_ERR_CUDA;
+    const bool prof = plan->params.prof != nullptr || plan->params.dbg != 0;   // debug build of the kernel
+    if (plan->a_f16) return prof ? ws_launch<true, true>(plan, st) : ws_launch<true, false>(plan, st);
+    return prof ? ws_launch<false, true>(plan, st) : ws_launch<false, false>(plan, st);
 }
 
 }  // namespace aria
