@@ -267,6 +267,8 @@ void oracle_epilogue_w8a8(const int64_t *acc, const float *sx, const float *sw, 
 /* W4A16 linear (config C4; readings R12):
  *   variant 0: w^ = bf16_rne(float(q) * float(sg))   (product exact in fp32)
  *   variant 1: w^ = q * sg  exactly (not rounded to bf16)
+ *   variant 2: w^ = fp16_rne(float(q) * float(sg))   (reading R12b: the small-M
+ *              weight-streaming path feeds the tensor core fp16 operands)
  *   y = sum_k (double)x[m,k] * (double)w^[n,k] + (double)b[n]  (fp64)
  * X is fp32 holding bf16 values exactly.  codes[N,K] int8, sg_bits[N,K/G]. */
 void oracle_linear_w4a16(const float *X, const int8_t *codes, const uint16_t *sg_bits,
@@ -282,6 +284,8 @@ void oracle_linear_w4a16(const float *X, const int8_t *codes, const uint16_t *sg
             float prod = (float)codes[n * K + k] * sg; /* exact: 3-bit x 11-bit */
             if (variant == 0)
                 wrow[k] = (double)oracle_bf16_bits_to_f32(oracle_f64_to_bf16_bits((double)prod));
+            else if (variant == 2)
+                wrow[k] = (double)oracle_fp16_bits_to_f32(oracle_f32_to_fp16_bits(prod));
             else
                 wrow[k] = (double)prod;
         }
@@ -298,7 +302,7 @@ void oracle_linear_w4a16(const float *X, const int8_t *codes, const uint16_t *sg
     }
 }
 
-/* Dequantised weight matrix of variant 0/1 as fp64 [N,K] (for the pin that
+/* Dequantised weight matrix of variant 0/1/2 as fp64 [N,K] (for the pin that
  * reduces O4 to numpy.matmul). */
 void oracle_dequant_int4(const int8_t *codes, const uint16_t *sg_bits, int variant, int64_t N,
                          int64_t K, int G, double *What)
@@ -310,6 +314,8 @@ void oracle_dequant_int4(const int8_t *codes, const uint16_t *sg_bits, int varia
             float prod = (float)codes[n * K + k] * sg;
             What[n * K + k] = variant == 0
                                   ? (double)oracle_bf16_bits_to_f32(oracle_f64_to_bf16_bits(prod))
+                              : variant == 2
+                                  ? (double)oracle_fp16_bits_to_f32(oracle_f32_to_fp16_bits(prod))
                                   : (double)prod;
         }
 }

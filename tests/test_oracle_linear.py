@@ -156,11 +156,13 @@ def test_o4_reduces_to_numpy_matmul(oracle):
     W = inputs.normal_f32((40, 256), 0.02, 78, 1)
     b = inputs.normal_f32((40,), 0.01, 78, 2).astype(np.float64)
     codes, sg, packed = oracle.quant_int4_groups(W)
-    for variant in (0, 1):
+    for variant in (0, 1, 2):
         # independent dequantisation: numpy fp16 decode, exact product, ml_dtypes bf16 rounding
+        # (variant 0) / numpy float16 rounding (variant 2, the fp16-operand reading R12b)
         s = np.repeat(sg.view(np.float16).astype(np.float32), 32, axis=1)
         prod = codes.astype(np.float32) * s
-        what = prod.astype(ml_dtypes.bfloat16).astype(np.float64) if variant == 0 else prod.astype(np.float64)
+        what = (prod.astype(ml_dtypes.bfloat16).astype(np.float64) if variant == 0 else
+                prod.astype(np.float16).astype(np.float64) if variant == 2 else prod.astype(np.float64))
         assert np.array_equal(oracle.dequant_int4(codes, sg, variant), what)
         ref = X.astype(np.float64) @ what.T + b
         y = oracle.linear_w4a16(X, codes, sg, b, variant=variant)
@@ -169,6 +171,9 @@ def test_o4_reduces_to_numpy_matmul(oracle):
     y0 = oracle.linear_w4a16(X, codes, sg, variant=0)
     y1 = oracle.linear_w4a16(X, codes, sg, variant=1)
     assert 0 < np.abs(y0 - y1).max() < 2e-2 * np.abs(y1).max()
+    # fp16 rounding of w^ (11 significant bits) sits 8x closer to the exact product than bf16 rounding
+    y2 = oracle.linear_w4a16(X, codes, sg, variant=2)
+    assert 0 < np.abs(y2 - y1).max() < 0.25 * np.abs(y0 - y1).max()
 
 
 def test_o4_quantisation_noise_level(oracle):
