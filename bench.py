@@ -213,6 +213,72 @@ def per_linear_table(torch, aria, inputs, pk):
     return out
 
 
+def small_m_stream(torch, aria, inputs, pk, iters=20):
+    """SURVEY S8(d) 'C5-shaped stack at M=32, W4A16': the weight-bound regime.  One plan
+    (aria_stack_plan_*) = ONE persistent weight-streaming kernel over all 96 layers, captured in a CUDA
+    graph; 382 MB of packed weights + scales per replay exceed the 126 MB L2, so every replay is
+    HBM-cold.  Also the three C4 shapes at M=32, each as a plan over enough independent linears of
+    that shape to exceed 2 x L2.  Bytes are ALGORITHMIC: X + packed weights + scales + bias + Y."""
+    from paper_2607_08526_b200.stack import LinearStack
+    M = 32
+    out = {}
+
+    def timed_graph(run):
+        run()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            run()
+        for _ in range(3):
+            g.replay()
+        ts = []
+        for _ in range(iters):
+            ts.append(time_region(torch, g.replay, 1))
+        return statistics.median(ts), min(ts)
+
+    st = LinearStack(aria.W4A16, M=M, use_plan=True)
+    assert aria.aria_stack_plan_is_streaming(st.plan), "M=32 W4A16 stack must take the stream kernel"
+    abytes = sum(M * s["K"] * 2 + s["K"] * s["N"] // 2 + s["K"] * s["N"] // 16 + 2 * s["N"] + M * s["N"] * 2
+                 for s in st.specs)
+    med, best = timed_graph(st.run)
+    out["c5_stack_m32"] = {"layers": len(st.specs), "launches_per_step": 1, "us": round(med * 1e3, 2),
+                           "us_best": round(best * 1e3, 2), "bytes": abytes,
+                           "gbs": round(abytes / (med * 1e-3) / 1e9, 1),
+                           "hbm_frac_measured": round(abytes / (med * 1e-3) / 1e9 / pk["hbm_gbs"], 3),
+                           "hbm_frac_nominal_8000": round(abytes / (med * 1e-3) / 1e9 / 8000.0, 3),
+                           "eff_tflops": round(st.ops / (med * 1e-3) / 1e12, 1)}
+    del st
+    cases = []
+    for (K, N) in inputs.C4_SHAPES:
+        wbytes = N * K // 2 + N * K // 16
+        ncopy = int(2 * 126e6 // wbytes) + 1
+        W = torch.from_numpy(inputs.normal_f32((N, K), inputs.W_STD, 9, K + N + 1)).cuda()
+        wq, sc = aria.aria_quantize_weights_int4(W)
+        del W
+        bits, _ = inputs.normal_bf16((M, K), 1.0, 9, K + N)
+        X = torch.from_numpy(bits.view(np.int16).copy()).cuda().view(torch.bfloat16)
+        b = torch.from_numpy(inputs.normal_bf16((N,), inputs.B_STD, 9, K + N + 2)[0].view(np.int16).copy()).cuda().view(torch.bfloat16)
+        specs = [{"K": K, "N": N, "act": aria.ACT_NONE, "in": X, "wq": wq.clone(), "w_scale": sc.clone(), "bias": b,
+                  "out": torch.empty((M, N), dtype=torch.bfloat16, device="cuda")} for _ in range(ncopy)]
+        layers = aria.make_layers(specs)
+        plan = aria.aria_stack_plan_create(layers, M, aria.W4A16, aria.BF16)
+        try:
+            assert aria.aria_stack_plan_is_streaming(plan)
+            med, best = timed_graph(lambda: aria.aria_stack_plan_run(plan))
+        finally:
+            torch.cuda.synchronize()
+            aria.aria_stack_plan_destroy(plan)
+        ab = M * K * 2 + wbytes + 2 * N + M * N * 2
+        us = med * 1e3 / ncopy
+        cases.append({"case": f"C4 M=32 {K}->{N}", "linears_per_launch": ncopy, "us_per_linear": round(us, 3),
+                      "gbs": round(ab / (us * 1e-6) / 1e9, 1),
+                      "hbm_frac_measured": round(ab / (us * 1e-6) / 1e9 / pk["hbm_gbs"], 3),
+                      "eff_tflops": round(2.0 * M * N * K / (us * 1e-6) / 1e12, 1)})
+        del specs, layers
+    out["c4_m32_batched"] = cases
+    return out
+
+
 def run_ours(args):
     import torch
     from paper_2607_08526_b200 import binding as aria
@@ -320,9 +386,13 @@ def run_ours(args):
         ops, t, cores = oracle_sample(1024)
         cpu = {"value": ops / t / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"block 0's 4 linears at 1024 of the 2048 tokens, both modes, {t:.1f} s"}
-    table = None
+    ops8, ops4 = st8.ops, st4.ops
+    table = small = None
     if world == 1 and not args.no_per_linear:
+        st8 = st4 = gg = xq = None            # free the M=2048 stacks before the per-linear sections
+        torch.cuda.empty_cache()
         table = per_linear_table(torch, aria, inputs, pk)
+        small = small_m_stream(torch, aria, inputs, pk)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
@@ -330,12 +400,13 @@ def run_ours(args):
         "data": "synthetic",
         "config": {"workload": WORKLOAD, "tokens": M, "layers": n_l, "l2": "weights 680 MB + 382 MB per step exceed the 126 MB L2",
                    "multi_gpu": "replicas only"},
-        "modes": {"w8a8": {"ms": t8, "tops": st8.ops / (t8 * 1e-3) / 1e12,
-                           "frac_int8_peak_sustained": st8.ops / (t8 * 1e-3) / 1e12 / peak},
-                  "w4a16": {"ms": t4, "eff_tflops": st4.ops / (t4 * 1e-3) / 1e12,
-                            "frac_bf16_peak_sustained": st4.ops / (t4 * 1e-3) / 1e12 / pk["bf16_sustained"]}},
+        "modes": {"w8a8": {"ms": t8, "tops": ops8 / (t8 * 1e-3) / 1e12,
+                           "frac_int8_peak_sustained": ops8 / (t8 * 1e-3) / 1e12 / peak},
+                  "w4a16": {"ms": t4, "eff_tflops": ops4 / (t4 * 1e-3) / 1e12,
+                            "frac_bf16_peak_sustained": ops4 / (t4 * 1e-3) / 1e12 / pk["bf16_sustained"]}},
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": args.steps * (2 * n_l + n_l), "clocks": clocks, "per_linear": table,
+        "small_m": small,
     }
     print(json.dumps(line))
 
@@ -394,7 +465,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-per-linear", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--small-m-only", action="store_true",
+                    help="only the M=32 W4A16 stream-kernel section (used for ncu captures)")
     args = ap.parse_args()
+    if args.small_m_only:
+        import torch
+        from paper_2607_08526_b200 import binding as aria
+        from paper_2607_08526_b200 import inputs
+        aria.lib()
+        print(json.dumps({"small_m": small_m_stream(torch, aria, inputs, peaks(), iters=max(args.steps, 3))}))
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -47,31 +47,35 @@ namespace aria {
 constexpr int WS_TT = 32;        // tokens per tile = MMA N
 constexpr int WS_ROWS = 128;     // output channels per tile = MMA M
 constexpr int WS_SBK = 256;      // k-values per stage
-constexpr int WS_PS = 8;         // weight ring depth (stages of 18 KB)
-constexpr int WS_XS = 3;         // X ring depth (stages of 16 KB): X must be requested BEFORE the weights of its stage
+constexpr int WS_PS = 6;         // weight ring depth (stages of 18 KB); the dequantiser loop is unrolled by WS_PS
+constexpr int WS_XS = 4;         // X ring depth (stages of 20 KB): X must be requested BEFORE the weights of its stage
 constexpr int WS_NA = 3;         // TMEM A slots, one STAGE each (128 columns = 128 rows x 256 k)
 constexpr int WS_G = 4;          // dequantiser groups
+constexpr int WS_NTACC = 3;      // accumulator buffers: a slow (GELU + fp16 copy) epilogue must not stall the MMA
 constexpr int WS_EPI_WARP0 = 4;
 constexpr int WS_DEQ_WARP0 = 8;
 constexpr int WS_THREADS = 32 * WS_DEQ_WARP0 + 128 * WS_G;   // 768
 constexpr int WS_P_BYTES = WS_ROWS * 128;                    // 16 KB
 constexpr int WS_S_BYTES = WS_ROWS * 16;                     // 2 KB
-constexpr int WS_X_BYTES = 4 * WS_TT * 128;                  // 16 KB: 4 sub-tiles [32 x 64] bf16
+constexpr int WS_XSUB = 5;                                   // X sub-tiles [32 x 64] per stage: 4 of activations + 1 of group sums (AF16)
+constexpr int WS_X_BYTES = WS_XSUB * WS_TT * 128;            // 20 KB
+constexpr int WS_XLD = 320;                                  // fp16 elements per 256-k stage of the X16 copy: 256 x + 16 sums + pad
+constexpr int WS_A_SLOT = 136;                               // TMEM columns per A slot: 128 (256 k) + 8 (16 zero-point k)
 constexpr int WS_P_OFF = 0;
 constexpr int WS_X_OFF = WS_P_OFF + WS_PS * WS_P_BYTES;
 constexpr int WS_S_OFF = WS_X_OFF + WS_XS * WS_X_BYTES;
 constexpr int WS_BAR_OFF = WS_S_OFF + WS_PS * WS_S_BYTES;
-constexpr int WS_NBAR = 2 * WS_PS + 2 * WS_XS + 2 * WS_NA + 4;
+constexpr int WS_NBAR = 2 * WS_PS + 2 * WS_XS + 2 * WS_NA + 2 * WS_NTACC;
 constexpr int WS_SMEM_BYTES = WS_BAR_OFF + WS_NBAR * 8 + 16 + 1024;
 // Accumulators (WS_NACC > 1 would spread the k-steps over independent accumulators that the epilogue
 // adds; measured: no gain -- back-to-back N = 32 MMAs into one accumulator do not serialise).
 constexpr int WS_NACC = 1;
 constexpr int WS_ACC_COL0 = 0;                               // 2 buffers x 4 fp32 accumulators x 32 columns
-constexpr int WS_A_COL0 = 2 * WS_NACC * WS_TT;
+constexpr int WS_A_COL0 = WS_NTACC * WS_NACC * WS_TT;
 constexpr int WS_TMEM_COLS = 512;
 static_assert(WS_SMEM_BYTES <= 227 * 1024, "shared memory");
-static_assert((WS_PS & (WS_PS - 1)) == 0, "weight ring depth must be a power of two");
-static_assert(WS_A_COL0 + WS_NA * 128 <= WS_TMEM_COLS, "tensor memory");
+static_assert(WS_PS % WS_NA == 0 && (WS_PS / WS_NA) % 2 == 0, "the unrolled dequantiser loop needs static A-slot parities");
+static_assert(WS_A_COL0 + WS_NA * WS_A_SLOT <= WS_TMEM_COLS, "tensor memory");
 
 // One linear of the list, as the kernel sees it (device memory; tensor maps need 64-byte alignment).
 struct alignas(128) WsLayer {
@@ -93,9 +97,10 @@ struct alignas(128) WsLayer {
 // AF16: external bf16 inputs are converted once per launch to fp16 (the MMA needs both operands in
 // the same 16-bit format); segment i covers 16-byte chunks [chunk0, chunk0 + chunks).
 struct WsConv {
-    const uint4* src;         // bf16, 8 per chunk
-    uint4* dst;               // fp16
+    const uint4* src;         // bf16 [M, K], 8 per chunk
+    uint16_t* dst;            // fp16 [M, ld16] in the stream layout (see x16_pos)
     int chunk0, chunks;
+    int kc8, ld16;            // K / 8 chunks per row; K / 256 * WS_XLD
 };
 
 struct WsParams {
@@ -104,6 +109,7 @@ struct WsParams {
     int n_conv, conv_chunks;
     const int* sched;         // units (layer << 16 | tile), CTA b owns sched[sched_off[b] .. sched_off[b+1])
     const int* sched_off;     // [grid + 1]
+    const int* sched_total;   // [grid] stages of each CTA
     unsigned* done;           // [n_layers] completion counters + [n_layers] = CTAs done converting (zeroed before each launch)
     int n_layers, M;
     long long* prof;          // debug: per-CTA role timestamps (16 per CTA), or nullptr
@@ -113,7 +119,7 @@ struct WsParams {
 static long long* g_ws_prof = nullptr;
 void ws_set_profile_buffer(long long* p) { g_ws_prof = p; }
 #define WS_TIMED(accum, stmt) do { if (PROF) { const long long t_ = clock64(); stmt; accum += clock64() - t_; } else { stmt; } } while (0)
-#define WS_STAMP(slot) do { if (PROF) p.prof[blockIdx.x * 16 + (slot)] = clock64() - t_start; } while (0)
+#define WS_STAMP(slot) do { if (PROF && p.prof) p.prof[blockIdx.x * 16 + (slot)] = clock64() - t_start; } while (0)
 
 __device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
     unsigned v;
@@ -161,6 +167,9 @@ __device__ __forceinline__ void tmem_st_32x32b_x16(uint32_t taddr, const uint32_
         "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
         : "memory");
 }
+__device__ __forceinline__ void tmem_st_32x32b_x2(uint32_t taddr, uint32_t v0, uint32_t v1) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(v0), "r"(v1) : "memory");
+}
 __device__ __forceinline__ void tmem_wait_st() {
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
@@ -181,30 +190,33 @@ __device__ __forceinline__ uint32_t ws_lop_and_xor(uint32_t a, uint32_t b, uint3
     asm("lop3.b32 %0, %1, %2, %3, 0x6A;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
     return r;
 }
-__device__ __forceinline__ void cvt_e4m3x4_f16(uint32_t v, uint32_t& lo, uint32_t& hi) {
-    asm("{\n\t.reg .b16 l, h;\n\tmov.b32 {l, h}, %2;\n\t"
-        "cvt.rn.f16x2.e4m3x2 %0, l;\n\tcvt.rn.f16x2.e4m3x2 %1, h;\n\t}"
-        : "=r"(lo), "=r"(hi)
-        : "r"(v));
-}
 __device__ __forceinline__ uint32_t hfma2_u32(uint32_t a, uint32_t b, uint32_t c) {
     uint32_t r;
     asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
     return r;
 }
-// fp16 path: S2 = (512 sg, 512 sg), C2 = (-8 sg, -8 sg), both exact in fp16 unless 512 sg overflows
-// (sg > 127.9, i.e. |w| > 895: such a group takes the value inf -- documented limit of the fp16 path).
-__device__ __forceinline__ void dequant_word_f16(uint32_t w, uint32_t S2, uint32_t C2, uint32_t* o) {
-    const uint32_t t = w >> 4;
-    const uint32_t lo = ws_lop_and_xor(__byte_perm(w, t, 0x5140), 0x0F0F0F0Fu, 0x08080808u);  // k0..k3
-    const uint32_t hi = ws_lop_and_xor(__byte_perm(w, t, 0x7362), 0x0F0F0F0Fu, 0x08080808u);  // k4..k7
-    uint32_t a, b, c, d;
-    cvt_e4m3x4_f16(lo, a, b);
-    cvt_e4m3x4_f16(hi, c, d);
-    o[0] = hfma2_u32(a, S2, C2);
-    o[1] = hfma2_u32(b, S2, C2);
-    o[2] = hfma2_u32(c, S2, C2);
-    o[3] = hfma2_u32(d, S2, C2);
+// fp16 path, 9 instructions per 8 weights (1 SHF, 4 LOP3, 4 HFMA2).  The offset-binary nibble
+// u = q + 8 (two's-complement nibble XOR 8) is dropped into the mantissa of an fp16 constant whose ulp
+// is 1 at that bit position: bits 0-3 of 0x6400 (= 1024) give 1024 + u, bits 4-7 of 0x5400 (= 64) give
+// 64 + u.  One HFMA2 (B + u) sg - B sg has an exact product and an exactly representable addend
+// (B sg, B a power of two), so it returns fp16_rn(u sg): the correctly rounded UNSIGNED dequantised
+// weight.  The zero point -8 sg x is exact and linear, so the tensor core applies it: 16 extra k per
+// stage with A = -8 sg (per group) and B = the group sums of x (hi + lo fp16 split), see the MMA warp.
+// Output register i holds the pair (k_i, k_{i+4}) of the word: the k order inside each 8-k word is
+// [0,4,1,5,2,6,3,7], and the fp16 activation copy is written in the same order (x16_pos).
+// S2 = (sg, sg), C0 = -(1024 sg), C1 = -(64 sg): exact unless 1024 sg overflows (sg > 63.9, i.e.
+// |w| > 447: such a group takes the value inf/nan -- documented limit of the fp16 path).
+__device__ __forceinline__ void dequant_word_f16(uint32_t w, uint32_t S2, uint32_t C0, uint32_t C1, uint32_t* o) {
+    const uint32_t t = w >> 8;
+    o[0] = hfma2_u32(ws_lop_and_xor(w, 0x000F000Fu, 0x64086408u), S2, C0);   // k0, k4
+    o[1] = hfma2_u32(ws_lop_and_xor(w, 0x00F000F0u, 0x54805480u), S2, C1);   // k1, k5
+    o[2] = hfma2_u32(ws_lop_and_xor(t, 0x000F000Fu, 0x64086408u), S2, C0);   // k2, k6
+    o[3] = hfma2_u32(ws_lop_and_xor(t, 0x00F000F0u, 0x54805480u), S2, C1);   // k3, k7
+}
+// position of k inside one 256-k stage row of the fp16 activation copy (word order [0,4,1,5,2,6,3,7])
+__device__ __forceinline__ int x16_pos(int k) {
+    const int i = k & 7;
+    return (k & ~7) | ((i & 3) << 1) | (i >> 2);
 }
 // exact bf16 path (same arithmetic as gemm_w4a16.cu): nibble at mantissa bit pos of 1.0f, one FMA
 // with exactly representable addends, one cvt.rn.bf16x2.
@@ -244,6 +256,12 @@ __device__ __forceinline__ uint32_t ws_lds32(uint32_t addr) {
     return v;
 }
 
+// Lean mbarrier wait for the dequantiser loop (no watchdog code in the hot loop; try_wait suspends in
+// hardware; a pipeline bug is caught by the watchdogs of the other roles).
+__device__ __forceinline__ void mbar_wait_lean(uint32_t bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {}
+}
+
 // Walks this CTA's unit list; every role runs an identical copy.
 struct UnitIter {
     const int* sched;
@@ -274,8 +292,8 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
     const uint32_t pfull0 = bars, pempty0 = pfull0 + 8 * WS_PS;
     const uint32_t xfull0 = pempty0 + 8 * WS_PS, xempty0 = xfull0 + 8 * WS_XS;
     const uint32_t afull0 = xempty0 + 8 * WS_XS, aempty0 = afull0 + 8 * WS_NA;
-    const uint32_t tfull0 = aempty0 + 8 * WS_NA, tempty0 = tfull0 + 16;
-    const uint32_t tmem_slot = tempty0 + 16;
+    const uint32_t tfull0 = aempty0 + 8 * WS_NA, tempty0 = tfull0 + 8 * WS_NTACC;
+    const uint32_t tmem_slot = tempty0 + 8 * WS_NTACC;
     volatile uint32_t* tmem_slot_g =
         reinterpret_cast<volatile uint32_t*>(gbase + WS_BAR_OFF + WS_NBAR * 8);
 
@@ -295,10 +313,11 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             mbar_init(afull0 + 8 * a, 4 * WS_G);      // every dequantiser warp fills its part of the slot
             mbar_init(aempty0 + 8 * a, 1);            // MMA commit
         }
-        for (int a = 0; a < 2; ++a) {
+        for (int a = 0; a < WS_NTACC; ++a) {
             mbar_init(tfull0 + 8 * a, 1);
             mbar_init(tempty0 + 8 * a, 4);
         }
+
         fence_mbar_init();
     }
     if (warp == 1) {
@@ -314,20 +333,47 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
     if (AF16 && p.n_conv > 0 && warp >= WS_EPI_WARP0) {
         // bf16 -> fp16 of the external inputs (exact for 2^-14 <= |x| <= 65504, saturating above,
         // absolute error <= 2^-25 below); the producers and the MMA warp start streaming meanwhile.
+        // Written in the stream layout: per 256-k stage WS_XLD fp16 = 256 x (k order of
+        // dequant_word_f16) + 8 x (hi, lo) sums of the stage's 32-k groups (the zero-point operand).
         constexpr int CT = WS_THREADS - 32 * WS_EPI_WARP0;
         const int ctid = threadIdx.x - 32 * WS_EPI_WARP0;
-        for (int c = blockIdx.x * CT + ctid; c < p.conv_chunks; c += gridDim.x * CT) {
-            int lo = 0, hi = p.n_conv - 1;         // segment of chunk c
-            while (lo < hi) {
-                const int mid = (lo + hi + 1) >> 1;
-                if (__ldg(&p.conv[mid].chunk0) <= c) lo = mid; else hi = mid - 1;
+        for (int cb = blockIdx.x * CT + (ctid & ~31); cb < p.conv_chunks; cb += gridDim.x * CT) {   // warp-uniform
+            const int c = cb + lane;
+            const bool ok = c < p.conv_chunks;       // chunk counts are multiples of 32: quads are all-or-nothing
+            float sum = 0.0f;
+            uint16_t* drow = nullptr;
+            int kc = 0;
+            if (ok) {
+                int lo = 0, hi = p.n_conv - 1;         // segment of chunk c
+                while (lo < hi) {
+                    const int mid = (lo + hi + 1) >> 1;
+                    if (__ldg(&p.conv[mid].chunk0) <= c) lo = mid; else hi = mid - 1;
+                }
+                const WsConv cv = p.conv[lo];
+                const int ci = c - cv.chunk0;
+                const int m = ci / cv.kc8;
+                kc = ci - m * cv.kc8;
+                const uint4 v = __ldg(cv.src + ci);
+                const uint32_t h01 = bf16x2_to_f16x2(v.x), h23 = bf16x2_to_f16x2(v.y);
+                const uint32_t h45 = bf16x2_to_f16x2(v.z), h67 = bf16x2_to_f16x2(v.w);
+                uint4 o;                               // pairs (k_i, k_{i+4})
+                o.x = __byte_perm(h01, h45, 0x5410); o.y = __byte_perm(h01, h45, 0x7632);
+                o.z = __byte_perm(h23, h67, 0x5410); o.w = __byte_perm(h23, h67, 0x7632);
+                drow = cv.dst + static_cast<size_t>(m) * cv.ld16 + (kc >> 5) * WS_XLD;
+                *reinterpret_cast<uint4*>(drow + (kc & 31) * 8) = o;
+                const float2 f01 = __half22float2(*reinterpret_cast<const __half2*>(&h01));
+                const float2 f23 = __half22float2(*reinterpret_cast<const __half2*>(&h23));
+                const float2 f45 = __half22float2(*reinterpret_cast<const __half2*>(&h45));
+                const float2 f67 = __half22float2(*reinterpret_cast<const __half2*>(&h67));
+                sum = ((f01.x + f01.y) + (f23.x + f23.y)) + ((f45.x + f45.y) + (f67.x + f67.y));
             }
-            const WsConv cv = p.conv[lo];
-            const uint4 v = __ldg(cv.src + (c - cv.chunk0));
-            uint4 o;
-            o.x = bf16x2_to_f16x2(v.x); o.y = bf16x2_to_f16x2(v.y);
-            o.z = bf16x2_to_f16x2(v.z); o.w = bf16x2_to_f16x2(v.w);
-            cv.dst[c - cv.chunk0] = o;
+            sum += __shfl_xor_sync(0xffffffffu, sum, 1);     // 4 chunks = one 32-k group
+            sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+            if (ok && (kc & 3) == 0) {
+                const __half sh = __float2half_rn(sum);
+                const __half sl = __float2half_rn(sum - __half2float(sh));
+                *reinterpret_cast<__half2*>(drow + 256 + 2 * ((kc >> 2) & 7)) = __halves2half2(sh, sl);
+            }
         }
         __threadfence();
         named_bar_sync(1, CT);
@@ -348,7 +394,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         for (UnitIter it(p); it.valid(); it.next()) {
             it.locate(p);
             const WsLayer& L = p.layers[it.l];
-            if (L.dep >= 0) {       // chained layer: the producer layer must be complete
+            if (L.dep >= 0 && !(p.dbg & 128)) {       // chained layer: the producer layer must be complete
                 if (lane == 0) {
                     wait_counter(p.done + L.dep, p.layers[L.dep].done_target);
                     fence_proxy_async_all();   // generic-proxy stores of other SMs -> this TMA read
@@ -358,11 +404,12 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             for (int sb = it.sb0; sb < it.sb1; ++sb) {
                 mbar_wait(xempty0 + 8 * stage, phase ^ 1);
                 if (elect_one()) {
-                    mbar_arrive_expect_tx(xfull0 + 8 * stage, (PROF && (p.dbg & 8)) ? WS_X_BYTES / 4 : WS_X_BYTES);
+                    constexpr int NSUB = AF16 ? WS_XSUB : 4;
+                    mbar_arrive_expect_tx(xfull0 + 8 * stage, NSUB * WS_TT * 128);
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        if (j == 0 || !(PROF && (p.dbg & 8))) tma_load_2d(sX + stage * WS_X_BYTES + j * (WS_TT * 128), &L.tmX,
-                                    sb * WS_SBK + j * 64, 0, xfull0 + 8 * stage);
+                    for (int j = 0; j < NSUB; ++j)
+                        tma_load_2d(sX + stage * WS_X_BYTES + j * (WS_TT * 128), &L.tmX,
+                                    sb * (AF16 ? WS_XLD : WS_SBK) + j * 64, 0, xfull0 + 8 * stage);
                 }
                 __syncwarp();
                 if (++stage == WS_XS) { stage = 0; phase ^= 1; }
@@ -382,7 +429,11 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
                 mbar_wait(pempty0 + 8 * stage, phase ^ 1);
                 if (elect_one()) {
                     mbar_arrive_expect_tx(pfull0 + 8 * stage, WS_P_BYTES + ((PROF && (p.dbg & 4)) ? 0 : WS_S_BYTES));
+                    if (PROF && (p.dbg & 32)) tma_load_2d_hint(sP + stage * WS_P_BYTES, &L.tmP, 0, n0 * (L.K / 2) / 128 + sb * 128, pfull0 + 8 * stage, pol_w);
+                    else
                     tma_load_2d_hint(sP + stage * WS_P_BYTES, &L.tmP, sb * 128, n0, pfull0 + 8 * stage, pol_w);
+                    if (PROF && (p.dbg & 64)) tma_load_2d_hint(sS + stage * WS_S_BYTES, &L.tmS, 0, n0 * (L.K / 16) / 16 + sb * 128, pfull0 + 8 * stage, pol_w);
+                    else
                     if (!(PROF && (p.dbg & 4))) tma_load_2d_hint(sS + stage * WS_S_BYTES, &L.tmS, sb * 8, n0, pfull0 + 8 * stage, pol_w);
                 }
                 __syncwarp();
@@ -407,7 +458,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
                 WS_TIMED(w_a, mbar_wait(afull0 + 8 * slot, aphase));       // all 4 sub-blocks of the stage dequantised
                 tc_fence_after();
                 if (lane == 0 && it.first && sb == it.sb0) WS_STAMP(2);
-                const uint32_t a_tmem = tmem_base + WS_A_COL0 + slot * 128;
+                const uint32_t a_tmem = tmem_base + WS_A_COL0 + slot * WS_A_SLOT;
                 const uint64_t b_desc = desc_hi | (((sX + xs * WS_X_BYTES) & 0x3FFFF) >> 4);
                 if (elect_one()) {
 #pragma unroll
@@ -418,6 +469,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
                                 mma_f16_ts(d_tmem + (k % WS_NACC) * WS_TT, a_tmem + j * 32 + k * 8,
                                            b_desc + j * (WS_TT * 128 / 16) + 2 * k, idesc,
                                            (sb != it.sb0 || j * 4 + k >= WS_NACC) ? 1u : 0u);
+                    // zero point: 16 more k with A = -8 sg of the stage's 8 groups (each twice) and
+                    // B = (hi, lo) of the groups' activation sums
+                    if (AF16 && !(PROF && (p.dbg & 2)))
+                        mma_f16_ts(d_tmem, a_tmem + 128, b_desc + 4 * (WS_TT * 128 / 16), idesc, 1u);
                     tc_commit(aempty0 + 8 * slot);
                     tc_commit(xempty0 + 8 * xs);
                     if (sb == it.sb1 - 1) tc_commit(tfull0 + 8 * acc);
@@ -426,19 +481,19 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
                 if (++slot == WS_NA) { slot = 0; aphase ^= 1; }
                 if (++xs == WS_XS) { xs = 0; xphase ^= 1; }
             }
-            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+            if (++acc == WS_NTACC) { acc = 0; acc_phase ^= 1; }
         }
-        if (lane == 0) { WS_STAMP(3); if (PROF) { p.prof[blockIdx.x * 16 + 9] = w_t; p.prof[blockIdx.x * 16 + 10] = w_x; p.prof[blockIdx.x * 16 + 11] = w_a; } }
+        if (lane == 0) { WS_STAMP(3); if (PROF && p.prof) { p.prof[blockIdx.x * 16 + 9] = w_t; p.prof[blockIdx.x * 16 + 10] = w_x; p.prof[blockIdx.x * 16 + 11] = w_a; } }
     } else if (warp >= WS_DEQ_WARP0) {
         // ------------------------------------------------------------ dequantiser groups
         // The dequantisers do not care about unit boundaries: they see one sequence of `total` stages.
         // Software pipelined per warp: the packed bytes of stage s+1 are loaded before the arithmetic
         // of stage s, each half (32 k) goes to TMEM as soon as its 16 registers are ready, and the
         // "A slot full" signal of stage s is sent in the middle of stage s+1 (its stores have long
-        // landed by then) -- the four warps that share an SM sub-partition hit their barriers at the
-        // same time, so latency that is not overlapped inside a warp is not overlapped at all.  The
-        // loop is issue bound (~120 arithmetic instructions per warp and sub-block): everything else in
-        // it is kept to a minimum.
+        // landed by then).  The loop is ISSUE bound (ncu: the 16 dequantiser warps own ~90% of the
+        // SM's issued instructions), so it is unrolled by the weight-ring depth: every ring index,
+        // barrier address and A-slot parity is a compile-time constant and the register rotation of
+        // the software pipeline costs no moves.
         const int dw = warp - WS_DEQ_WARP0;
         const int g = dw >> 2;                    // group = 64-k sub-block of the stage
         const int q = dw & 3;                     // TMEM lane quarter (== warp % 4)
@@ -448,9 +503,8 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         const uint32_t pa1 = sP + r * 128 + (((2 * g + 1) ^ xr) << 4);
         const uint32_t sa = sS + r * 16 + g * 4;
         const uint32_t a_base = tmem_base + WS_A_COL0 + g * 32 + (static_cast<uint32_t>(q * 32) << 16);
-        int total = 0;                            // stages of this CTA
-        for (int i = p.sched_off[blockIdx.x]; i < p.sched_off[blockIdx.x + 1]; ++i)
-            total += __ldg(&p.layers[__ldg(p.sched + i) >> 16].num_sb);
+        const uint32_t z_base = tmem_base + WS_A_COL0 + 128 + g * 2 + (static_cast<uint32_t>(q * 32) << 16);
+        const int total = __ldg(p.sched_total + blockIdx.x);      // stages of this CTA
         uint4 pk0 = make_uint4(0, 0, 0, 0), pk1 = pk0;
         uint32_t sc2 = 0;
         if (total > 0) {
@@ -460,74 +514,87 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             pk0 = ws_lds128(pa0);
             pk1 = ws_lds128(pa1);
         }
-        int slot = 0;
-        uint32_t aphase = 0;
-        long long w_p = 0, w_e = 0, w_s = 0;
-#pragma unroll 2
-        for (int s = 0; s < total; ++s) {
-            // ---- start the loads of the next stage
-            uint4 nk0 = pk0, nk1 = pk1;
-            uint32_t nsc = sc2;
-            if (s + 1 < total) {
-                const int ns = (s + 1) & (WS_PS - 1);
-                WS_TIMED(w_p, mbar_wait(pfull0 + 8 * ns, ((s + 1) / WS_PS) & 1));
-                nsc = ws_lds32(sa + ns * WS_S_BYTES);
-                nk0 = ws_lds128(pa0 + ns * WS_P_BYTES);
-                nk1 = ws_lds128(pa1 + ns * WS_P_BYTES);
-            }
-            uint32_t o[16];
-            // ---- first half: k 0..31 of the sub-block
-            if (PROF && (p.dbg & 1)) {
+        uint32_t pphase = 0;                      // parity of the weight-ring pass of this round
+        for (int s0 = 0; s0 < total; s0 += WS_PS) {
 #pragma unroll
-                for (int i = 0; i < 16; ++i) o[i] = pk0.x + i;
-            } else if (AF16) {
-                const __half2 sh = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
-                const __half2 S = __hmul2(sh, __floats2half2_rn(512.0f, 512.0f)), C = __hmul2(sh, __floats2half2_rn(-8.0f, -8.0f));
-                const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&S), C2 = *reinterpret_cast<const uint32_t*>(&C);
-                dequant_word_f16(pk0.x, S2, C2, o + 0);  dequant_word_f16(pk0.y, S2, C2, o + 4);
-                dequant_word_f16(pk0.z, S2, C2, o + 8);  dequant_word_f16(pk0.w, S2, C2, o + 12);
-            } else {
-                const float s0 = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
-                dequant_word_bf16(pk0.x, s0, o + 0);  dequant_word_bf16(pk0.y, s0, o + 4);
-                dequant_word_bf16(pk0.z, s0, o + 8);  dequant_word_bf16(pk0.w, s0, o + 12);
-            }
-            if (s > 0) {                           // publish the previous stage's sub-block
-                WS_TIMED(w_s, tmem_wait_st());
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(afull0 + 8 * (slot == 0 ? WS_NA - 1 : slot - 1));
-            }
-            WS_TIMED(w_e, mbar_wait(aempty0 + 8 * slot, aphase ^ 1));   // MMAs reading this slot retired
-            tc_fence_after();
-            tmem_st_32x32b_x16(a_base + slot * 128, o);
-            // ---- second half: k 32..63
-            if (PROF && (p.dbg & 1)) {
+            for (int j = 0; j < WS_PS; ++j) {
+                const int s = s0 + j;
+                if (s < total) {                  // warp-uniform
+                    const int slot = j % WS_NA;                              // compile-time after unrolling
+                    const uint32_t a_par = static_cast<uint32_t>((j / WS_NA) & 1);
+                    const int nj = (j + 1) % WS_PS;
+                    // ---- start the loads of the next stage
+                    uint4 nk0 = pk0, nk1 = pk1;
+                    uint32_t nsc = sc2;
+                    if (s + 1 < total) {
+                        mbar_wait_lean(pfull0 + 8 * nj, nj == 0 ? pphase ^ 1u : pphase);
+                        nsc = ws_lds32(sa + nj * WS_S_BYTES);
+                        nk0 = ws_lds128(pa0 + nj * WS_P_BYTES);
+                        nk1 = ws_lds128(pa1 + nj * WS_P_BYTES);
+                    }
+                    uint32_t o[16];
+                    uint32_t z0 = 0, z1 = 0;      // (-8 sg, -8 sg) of the sub-block's two groups (AF16)
+                    // ---- first half: k 0..31 of the sub-block
+                    if (PROF && (p.dbg & 1)) {
 #pragma unroll
-                for (int i = 0; i < 16; ++i) o[i] = pk1.x + i;
-            } else if (AF16) {
-                const __half2 sh = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
-                const __half2 S = __hmul2(sh, __floats2half2_rn(512.0f, 512.0f)), C = __hmul2(sh, __floats2half2_rn(-8.0f, -8.0f));
-                const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&S), C2 = *reinterpret_cast<const uint32_t*>(&C);
-                dequant_word_f16(pk1.x, S2, C2, o + 0);  dequant_word_f16(pk1.y, S2, C2, o + 4);
-                dequant_word_f16(pk1.z, S2, C2, o + 8);  dequant_word_f16(pk1.w, S2, C2, o + 12);
-            } else {
-                const float s1 = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
-                dequant_word_bf16(pk1.x, s1, o + 0);  dequant_word_bf16(pk1.y, s1, o + 4);
-                dequant_word_bf16(pk1.z, s1, o + 8);  dequant_word_bf16(pk1.w, s1, o + 12);
+                        for (int i = 0; i < 16; ++i) o[i] = pk0.x + i;
+                    } else if (AF16) {
+                        const __half2 sh = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
+                        const __half2 A = __hmul2(sh, __floats2half2_rn(-1024.0f, -1024.0f)), B = __hmul2(sh, __floats2half2_rn(-64.0f, -64.0f));
+                        const __half2 Z = __hmul2(sh, __floats2half2_rn(-8.0f, -8.0f));
+                        const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&sh);
+                        const uint32_t C0 = *reinterpret_cast<const uint32_t*>(&A), C1 = *reinterpret_cast<const uint32_t*>(&B);
+                        z0 = *reinterpret_cast<const uint32_t*>(&Z);
+                        dequant_word_f16(pk0.x, S2, C0, C1, o + 0);  dequant_word_f16(pk0.y, S2, C0, C1, o + 4);
+                        dequant_word_f16(pk0.z, S2, C0, C1, o + 8);  dequant_word_f16(pk0.w, S2, C0, C1, o + 12);
+                    } else {
+                        const float sf = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 & 0xFFFFu)));
+                        dequant_word_bf16(pk0.x, sf, o + 0);  dequant_word_bf16(pk0.y, sf, o + 4);
+                        dequant_word_bf16(pk0.z, sf, o + 8);  dequant_word_bf16(pk0.w, sf, o + 12);
+                    }
+                    if (s > 0) {                  // publish the previous stage's sub-block
+                        tmem_wait_st();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(afull0 + 8 * ((slot + WS_NA - 1) % WS_NA));
+                    }
+                    mbar_wait_lean(aempty0 + 8 * slot, a_par ^ 1u);   // MMAs reading this slot retired
+                    tc_fence_after();
+                    tmem_st_32x32b_x16(a_base + slot * WS_A_SLOT, o);
+                    // ---- second half: k 32..63
+                    if (PROF && (p.dbg & 1)) {
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) o[i] = pk1.x + i;
+                    } else if (AF16) {
+                        const __half2 sh = __half2half2(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
+                        const __half2 A = __hmul2(sh, __floats2half2_rn(-1024.0f, -1024.0f)), B = __hmul2(sh, __floats2half2_rn(-64.0f, -64.0f));
+                        const __half2 Z = __hmul2(sh, __floats2half2_rn(-8.0f, -8.0f));
+                        const uint32_t S2 = *reinterpret_cast<const uint32_t*>(&sh);
+                        const uint32_t C0 = *reinterpret_cast<const uint32_t*>(&A), C1 = *reinterpret_cast<const uint32_t*>(&B);
+                        z1 = *reinterpret_cast<const uint32_t*>(&Z);
+                        dequant_word_f16(pk1.x, S2, C0, C1, o + 0);  dequant_word_f16(pk1.y, S2, C0, C1, o + 4);
+                        dequant_word_f16(pk1.z, S2, C0, C1, o + 8);  dequant_word_f16(pk1.w, S2, C0, C1, o + 12);
+                    } else {
+                        const float sf = __half2float(__ushort_as_half(static_cast<uint16_t>(sc2 >> 16)));
+                        dequant_word_bf16(pk1.x, sf, o + 0);  dequant_word_bf16(pk1.y, sf, o + 4);
+                        dequant_word_bf16(pk1.z, sf, o + 8);  dequant_word_bf16(pk1.w, sf, o + 12);
+                    }
+                    tmem_st_32x32b_x16(a_base + slot * WS_A_SLOT + 16, o);
+                    if (AF16) tmem_st_32x32b_x2(z_base + slot * WS_A_SLOT, z0, z1);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(pempty0 + 8 * j);   // this stage's packed bytes are consumed
+                    pk0 = nk0; pk1 = nk1; sc2 = nsc;
+                }
             }
-            tmem_st_32x32b_x16(a_base + slot * 128 + 16, o);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(pempty0 + 8 * (s & (WS_PS - 1)));   // this stage's packed bytes are consumed
-            pk0 = nk0; pk1 = nk1; sc2 = nsc;
-            if (++slot == WS_NA) { slot = 0; aphase ^= 1; }
+            pphase ^= 1u;
         }
         if (total > 0) {
             tmem_wait_st();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(afull0 + 8 * (slot == 0 ? WS_NA - 1 : slot - 1));
+            if (lane == 0) mbar_arrive(afull0 + 8 * ((total - 1) % WS_NA));
         }
-        if (PROF && dw == 0 && lane == 0) { WS_STAMP(5); p.prof[blockIdx.x * 16 + 12] = w_p; p.prof[blockIdx.x * 16 + 13] = w_e; p.prof[blockIdx.x * 16 + 14] = w_s; }
+        if (PROF && dw == 0 && lane == 0) WS_STAMP(5);
     } else if (warp >= WS_EPI_WARP0) {
         // ------------------------------------------------------------ epilogue (warps 4..7)
         const int q = warp & 3;
@@ -544,7 +611,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             const __nv_bfloat16* bias = static_cast<const __nv_bfloat16*>(
                 reinterpret_cast<const void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->bias))));
             void* const Yp = reinterpret_cast<void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->Y)));
-            void* const Y16p = reinterpret_cast<void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->Y16)));
+            void* const Y16p = (p.dbg & 256) ? nullptr : reinterpret_cast<void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->Y16)));
             const int n = it.tile * WS_ROWS + q * 32 + lane;
             const bool n_ok = n < N;
             const float bv = bias && n_ok ? __bfloat162float(bias[n]) : 0.0f;
@@ -568,11 +635,11 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty0 + 8 * acc);             // accumulator is in registers
-            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+            if (++acc == WS_NTACC) { acc = 0; acc_phase ^= 1; }
 
-            if (n_ok) {
-                const bool gelu = act == ARIA_ACT_GELU_ERF;
-                if (out_t == ARIA_F32) {
+            const bool gelu = act == ARIA_ACT_GELU_ERF;
+            if (out_t == ARIA_F32) {
+                if (n_ok) {
                     float* Y = static_cast<float*>(Yp) + n;
 #pragma unroll
                     for (int t = 0; t < WS_TT; ++t) {
@@ -582,19 +649,64 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
                             Y[static_cast<size_t>(t) * N] = y;           // a warp writes 32 consecutive n
                         }
                     }
-                } else {
-                    __nv_bfloat16* Y = static_cast<__nv_bfloat16*>(Yp) + n;
-                    __half* Y16 = AF16 && Y16p ? static_cast<__half*>(Y16p) + n : nullptr;
+                }
+            } else if (AF16 && Y16p) {
+                // A later layer reads this output (its K = this N, a multiple of 256): besides the bf16
+                // result write what that layer's MMA reads -- the bf16 value as fp16, in the stream
+                // layout, and the (hi, lo) sum of this warp's 32 channels = one 32-k group of that layer.
+                __nv_bfloat16* Y = static_cast<__nv_bfloat16*>(Yp) + n;
+                const int n0 = it.tile * WS_ROWS + q * 32;                // warp-uniform; N % 256 == 0 here
+                const int ld16 = (N >> 8) * WS_XLD;
+                __half* Yrow = static_cast<__half*>(Y16p) + (n0 >> 8) * WS_XLD;
+                const int xpos = x16_pos(n & 255), spos = 256 + 2 * ((n0 >> 5) & 7);
+                float hs[WS_TT];                                          // the bf16 outputs, as fp32
 #pragma unroll
-                    for (int t = 0; t < WS_TT; ++t) {
-                        if (t < M) {
-                            float y = __uint_as_float(v[t]) + bv;
-                            if (gelu) y = gelu_erf(y);
-                            const __nv_bfloat16 yb = __float2bfloat16_rn(y);
-                            Y[static_cast<size_t>(t) * N] = yb;
-                            // what the dependent layer's MMA reads: the bf16 value, as fp16
-                            if (AF16 && Y16) Y16[static_cast<size_t>(t) * N] = __float2half_rn(__bfloat162float(yb));
-                        }
+                for (int t = 0; t < WS_TT; t += 2) {
+                    float y0 = __uint_as_float(v[t]) + bv, y1 = __uint_as_float(v[t + 1]) + bv;
+                    if (gelu) gelu_erf2(y0, y1);
+                    uint32_t yb2, yh2;
+                    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(yb2) : "f"(y1), "f"(y0));
+                    hs[t] = __uint_as_float(yb2 << 16);
+                    hs[t + 1] = __uint_as_float(yb2 & 0xFFFF0000u);
+                    // what the next layer's MMA reads: the bf16 value as fp16 (exact for 2^-14 <= |y| <= 65504)
+                    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(yh2) : "f"(hs[t + 1]), "f"(hs[t]));
+                    if (t < M) {                                          // M is warp-uniform
+                        reinterpret_cast<uint16_t*>(Y)[static_cast<size_t>(t) * N] = static_cast<uint16_t>(yb2);
+                        reinterpret_cast<uint16_t*>(Yrow)[static_cast<size_t>(t) * ld16 + xpos] = static_cast<uint16_t>(yh2);
+                    }
+                    if (t + 1 < M) {
+                        reinterpret_cast<uint16_t*>(Y)[static_cast<size_t>(t + 1) * N] = static_cast<uint16_t>(yb2 >> 16);
+                        reinterpret_cast<uint16_t*>(Yrow)[static_cast<size_t>(t + 1) * ld16 + xpos] = static_cast<uint16_t>(yh2 >> 16);
+                    }
+                }
+                // sums over the warp's 32 channels for all 32 tokens by recursive halving: 31 independent
+                // shuffles instead of 32 dependent 5-step butterflies; lane L ends with token L's sum
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) {
+                    const bool up = (lane & d) != 0;
+#pragma unroll
+                    for (int i = 0; i < d; ++i) {
+                        const float keep = up ? hs[i + d] : hs[i];
+                        const float give = up ? hs[i] : hs[i + d];
+                        hs[i] = keep + __shfl_xor_sync(0xffffffffu, give, d);
+                    }
+                }
+                if (lane < M) {
+                    const __half sh = __float2half_rn(hs[0]);
+                    const __half sl = __float2half_rn(hs[0] - __half2float(sh));
+                    *reinterpret_cast<__half2*>(Yrow + static_cast<size_t>(lane) * ld16 + spos) = __halves2half2(sh, sl);
+                }
+            } else if (n_ok) {
+                uint16_t* Y = static_cast<uint16_t*>(Yp) + n;
+#pragma unroll
+                for (int t = 0; t < WS_TT; t += 2) {
+                    if (t < M) {
+                        float y0 = __uint_as_float(v[t]) + bv, y1 = __uint_as_float(v[t + 1]) + bv;
+                        if (gelu) gelu_erf2(y0, y1);
+                        uint32_t yb2;
+                        asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(yb2) : "f"(y1), "f"(y0));
+                        Y[static_cast<size_t>(t) * N] = static_cast<uint16_t>(yb2);
+                        if (t + 1 < M) Y[static_cast<size_t>(t + 1) * N] = static_cast<uint16_t>(yb2 >> 16);
                     }
                 }
             }
@@ -720,16 +832,22 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     }
     std::vector<WsConv> conv;
     if (plan->a_f16) {
-        for (size_t e = 0; e < ext_src.size(); ++e) { ext_off.push_back(x16_elems); x16_elems += (ext_elems[e] + 127) / 128 * 128; }
+        // fp16 copies in the stream layout: [M, K / 256 * WS_XLD] per distinct external input and per
+        // chained output (the pad columns are never read by an MMA; zeroed once for tidiness)
+        auto x16_size = [&](size_t K) { return (static_cast<size_t>(M) * (K / WS_SBK) * WS_XLD + 127) / 128 * 128; };
+        for (size_t e = 0; e < ext_src.size(); ++e) { ext_off.push_back(x16_elems); x16_elems += x16_size(ext_elems[e] / M); }
         for (int i = 0; i < n_layers; ++i)
-            if (h[i].notify) { y16_off[i] = x16_elems; x16_elems += (static_cast<size_t>(M) * layers[i].N + 127) / 128 * 128; }
-        if (cudaMalloc(&plan->d_x16, x16_elems * 2 + 256) != cudaSuccess) { ws_plan_destroy(plan); return ARIA_ERR_CUDA; }
+            if (h[i].notify) { y16_off[i] = x16_elems; x16_elems += x16_size(layers[i].N); }
+        if (cudaMalloc(&plan->d_x16, x16_elems * 2 + 256) != cudaSuccess ||
+            cudaMemset(plan->d_x16, 0, x16_elems * 2 + 256) != cudaSuccess) { ws_plan_destroy(plan); return ARIA_ERR_CUDA; }
         int chunk0 = 0;
         for (size_t e = 0; e < ext_src.size(); ++e) {
             WsConv c;
+            const size_t K = ext_elems[e] / M;
             c.src = static_cast<const uint4*>(ext_src[e]);
-            c.dst = reinterpret_cast<uint4*>(static_cast<uint16_t*>(plan->d_x16) + ext_off[e]);
+            c.dst = static_cast<uint16_t*>(plan->d_x16) + ext_off[e];
             c.chunk0 = chunk0; c.chunks = static_cast<int>(ext_elems[e] / 8);
+            c.kc8 = static_cast<int>(K / 8); c.ld16 = static_cast<int>(K / WS_SBK * WS_XLD);
             chunk0 += c.chunks;
             conv.push_back(c);
         }
@@ -745,27 +863,66 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
             in = w.dep >= 0 ? x16 + y16_off[w.dep] : x16 + ext_off[in_ext[i]];
             if (w.notify) w.Y16 = x16 + y16_off[i];
         }
-        if (make_tmap_2d(&w.tmP, L.wq, 1, L.N, L.K / 2, WS_ROWS, 128, 128) != ARIA_OK ||
-            make_tmap_2d(&w.tmS, L.w_scale, 2, L.N, L.K / 32, WS_ROWS, 8, 0) != ARIA_OK ||
-            make_tmap_2d(&w.tmX, in, 2, M, L.K, WS_TT, 64, 128) != ARIA_OK) {
+        const int dbg_ = getenv("ARIA_WS_DBG") ? atoi(getenv("ARIA_WS_DBG")) : 0;
+        if (((dbg_ & 32) ? make_tmap_2d(&w.tmP, L.wq, 1, static_cast<uint64_t>(L.N) * (L.K / 2) / 128, 128, WS_ROWS, 128, 128)
+                         : make_tmap_2d(&w.tmP, L.wq, 1, L.N, L.K / 2, WS_ROWS, 128, 128)) != ARIA_OK ||
+            ((dbg_ & 64) ? make_tmap_2d(&w.tmS, L.w_scale, 2, static_cast<uint64_t>(L.N) * (L.K / 32) / 8, 8, WS_ROWS, 8, 0)
+                         : make_tmap_2d(&w.tmS, L.w_scale, 2, L.N, L.K / 32, WS_ROWS, 8, 0)) != ARIA_OK ||
+            make_tmap_2d(&w.tmX, in, 2, M, plan->a_f16 ? L.K / WS_SBK * WS_XLD : L.K, WS_TT, 64, 128) != ARIA_OK) {
             ws_plan_destroy(plan);
             return ARIA_ERR_CUDA;
         }
     }
-    // Schedule: layers in order, each tile to the CTA with the least work so far (cost = stages + a
-    // per-unit constant for the accumulator hand-off), so every CTA's list is in layer order (a
-    // dependency always points to a unit that is earlier in some CTA's list: no deadlock) and all
-    // CTAs stream the same number of stages.
+    // Schedule.  Units are dealt in ONE global order, each to the CTA with the least work so far, so
+    // all CTAs stream the same number of stages.  The order is the array order, except that a layer
+    // whose input is an earlier layer's output is held back until every CTA has been given ~GAP
+    // producer-unit durations of other work since its producer: by then the producer's last tile has
+    // been stored and the consumer's units do not stall the weight ring (measured on config C5's
+    // wiring: dependents right behind their producer cost +30% -- CTAs drift apart by ~15% -- while
+    // "dependents last" runs at the rate of a list without dependencies).  It stays a topological
+    // order and every CTA walks its units in that order, so a dependency always points to a unit
+    // that is earlier in some CTA's list: no deadlock.  Layers that may run concurrently write
+    // disjoint buffers (ws_eligible), so results equal array order.
     const int grid = total_units < sms ? total_units : sms;
+    std::vector<int> order;
+    {
+        const char* eg = getenv("ARIA_WS_GAP");
+        const double gap_units = eg ? atof(eg) : 32.0;      // in producer-unit durations
+        std::vector<char> placed(n_layers, 0);
+        std::vector<double> placed_at(n_layers, 0.0);
+        double cum = 0.0;                                   // work per CTA dealt so far
+        int n_placed = 0;
+        while (n_placed < n_layers) {
+            int pick = -1, fallback = -1;
+            for (int i = 0; i < n_layers && pick < 0; ++i) {
+                if (placed[i]) continue;
+                const int d = h[i].dep;
+                if (d < 0) { pick = i; break; }
+                if (!placed[d]) continue;
+                if (fallback < 0) fallback = i;
+                if (cum - placed_at[d] >= gap_units * (2 * h[d].num_sb + 1)) pick = i;
+            }
+            if (pick < 0) pick = fallback;                  // nothing independent left: take the stall
+            placed[pick] = 1;
+            cum += static_cast<double>(h[pick].num_n) * (2 * h[pick].num_sb + 1) / grid;
+            placed_at[pick] = cum;
+            order.push_back(pick);
+            ++n_placed;
+        }
+    }
+    // cost of a unit in quarter stages: its stages + ~1/4 stage of accumulator hand-off
+    auto unit_cost = [&](const WsLayer& w) { return 4 * w.num_sb + 1; };
     std::vector<std::vector<int>> lists(grid);
     std::vector<long> load(grid, 0);
-    for (int i = 0; i < n_layers; ++i)
+    std::vector<int> totals(grid, 0);
+    for (int i : order)
         for (int t = 0; t < h[i].num_n; ++t) {
             int best = 0;
             for (int c = 1; c < grid; ++c)
                 if (load[c] < load[best]) best = c;
             lists[best].push_back((i << 16) | t);
-            load[best] += 2 * h[i].num_sb + 1;
+            load[best] += unit_cost(h[i]);
+            totals[best] += h[i].num_sb;
         }
     std::vector<int> sched;
     std::vector<int> off(grid + 1, 0);
@@ -776,6 +933,7 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     off[grid] = static_cast<int>(sched.size());
     const size_t sched_n = sched.size();
     sched.insert(sched.end(), off.begin(), off.end());
+    sched.insert(sched.end(), totals.begin(), totals.end());
     plan->done_bytes = (static_cast<size_t>(n_layers) + 1) * sizeof(unsigned);
     if (cudaMalloc(&plan->d_layers, h.size() * sizeof(WsLayer)) != cudaSuccess ||
         cudaMalloc(&plan->d_sched, sched.size() * sizeof(int)) != cudaSuccess ||
@@ -790,6 +948,7 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     plan->params.layers = plan->d_layers;
     plan->params.sched = plan->d_sched;
     plan->params.sched_off = plan->d_sched + sched_n;
+    plan->params.sched_total = plan->d_sched + sched_n + grid + 1;
     plan->params.done = plan->d_done;
     plan->params.conv = plan->d_conv;
     plan->params.n_conv = static_cast<int>(conv.size());
@@ -817,7 +976,7 @@ static int ws_launch(const WsPlan* plan, cudaStream_t st) {
 
 int ws_plan_run(const WsPlan* plan, cudaStream_t st) {
     if (cudaMemsetAsync(plan->d_done, 0, plan->done_bytes, st) != cudaSuccess) return ARIA_ERR_CUDA;
-    const bool prof = plan->params.prof != nullptr || plan->params.dbg != 0;   // debug build of the kernel
+    const bool prof = plan->params.prof != nullptr || (plan->params.dbg & 127) != 0;   // debug build of the kernel
     if (plan->a_f16) return prof ? ws_launch<true, true>(plan, st) : ws_launch<true, false>(plan, st);
     return prof ? ws_launch<false, true>(plan, st) : ws_launch<false, false>(plan, st);
 }

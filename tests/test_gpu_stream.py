@@ -1,6 +1,6 @@
 """GPU parity, S4/S5 at small M through the PLAN API (aria_stack_plan_*): the persistent
-weight-streaming kernel (csrc/w4a16_stream.cu).  Its dequantised weight is w^ = fp16_rn(q*sg)
-(oracle variant 2, reading R12b) by default and bf16_rne(q*sg) (variant 0) with ARIA_W4_F16A=0;
+weight-streaming kernel (csrc/w4a16_stream.cu).  Its dequantised weight is w^ = fp16_rn((q+8)*sg) - 8*sg
+(oracle variant 3, reading R12c) by default and bf16_rne(q*sg) (variant 0) with ARIA_W4_F16A=0;
 outputs are bf16.  Gates: north_star 2e-2 against every oracle variant, and the tight bf16-output
 gate of reading R9 against the variant the path implements."""
 import os
@@ -58,17 +58,21 @@ def _run_plan(aria, specs, M, expect_stream=True):
 
 def _check(oracle, host, x, got_bits, variant):
     got = inputs.bf16_as_f32(got_bits)
-    refs = [oracle.linear_w4a16(x, host["codes"], host["sg"], host["b"], host["act"], variant=v) for v in (0, 1, 2)]
+    refs = [oracle.linear_w4a16(x, host["codes"], host["sg"], host["b"], host["act"], variant=v) for v in (0, 1, 2, 3)]
     for r in refs:
         assert rel_err(got, r) <= TOL
     ref = refs[variant]
-    # GELU output: tiny negative tails round differently -> looser bit-match fraction (reading R9)
+    # Bit-match fraction of the bf16 output (reading R9).  The offset-binary operand (variant 3) carries
+    # partial sums of x * u * sg with u in [1, 15] that the zero-point MMA cancels once per 256-k stage:
+    # the tensor core's fp32 accumulation error is relative to those larger partial sums (worst for
+    # non-zero-mean activations such as GELU outputs), so up to 3% of the outputs land on the
+    # neighbouring bf16 value; every element still meets the 2^-8 |ref| + 2e-5 max|ref| bound.
     check_bf16_out(got_bits, ref, inputs.bf16_bits(oracle.round_out(ref, oracle.OUT_BF16)), 2e-5,
-                   2e-2 if host["act"] else 1e-2)
+                   3e-2 if variant == 3 else (2e-2 if host["act"] else 1e-2))
 
 
 def _variant():
-    return 0 if os.environ.get("ARIA_W4_F16A", "1").startswith("0") else 2
+    return 0 if os.environ.get("ARIA_W4_F16A", "1").startswith("0") else 3
 
 
 @pytest.mark.parametrize("M,K,N", [(32, 256, 128), (32, 512, 384), (7, 256, 136), (1, 768, 8), (20, 1536, 1536)])

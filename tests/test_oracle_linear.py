@@ -156,13 +156,17 @@ def test_o4_reduces_to_numpy_matmul(oracle):
     W = inputs.normal_f32((40, 256), 0.02, 78, 1)
     b = inputs.normal_f32((40,), 0.01, 78, 2).astype(np.float64)
     codes, sg, packed = oracle.quant_int4_groups(W)
-    for variant in (0, 1, 2):
+    for variant in (0, 1, 2, 3):
         # independent dequantisation: numpy fp16 decode, exact product, ml_dtypes bf16 rounding
-        # (variant 0) / numpy float16 rounding (variant 2, the fp16-operand reading R12b)
+        # (variant 0) / numpy float16 rounding (variant 2, the fp16-operand reading R12b) / numpy
+        # float16 rounding of the UNSIGNED code's product minus the exact zero point (variant 3, R12c)
         s = np.repeat(sg.view(np.float16).astype(np.float32), 32, axis=1)
         prod = codes.astype(np.float32) * s
+        uprod = (codes.astype(np.float32) + 8.0) * s
         what = (prod.astype(ml_dtypes.bfloat16).astype(np.float64) if variant == 0 else
-                prod.astype(np.float16).astype(np.float64) if variant == 2 else prod.astype(np.float64))
+                prod.astype(np.float16).astype(np.float64) if variant == 2 else
+                uprod.astype(np.float16).astype(np.float64) - 8.0 * s.astype(np.float64) if variant == 3 else
+                prod.astype(np.float64))
         assert np.array_equal(oracle.dequant_int4(codes, sg, variant), what)
         ref = X.astype(np.float64) @ what.T + b
         y = oracle.linear_w4a16(X, codes, sg, b, variant=variant)
@@ -174,6 +178,25 @@ def test_o4_reduces_to_numpy_matmul(oracle):
     # fp16 rounding of w^ (11 significant bits) sits 8x closer to the exact product than bf16 rounding
     y2 = oracle.linear_w4a16(X, codes, sg, variant=2)
     assert 0 < np.abs(y2 - y1).max() < 0.25 * np.abs(y0 - y1).max()
+    # offset-binary fp16 rounding acts on u*sg (up to 15*sg): at most ~2x the error of variant 2
+    y3 = oracle.linear_w4a16(X, codes, sg, variant=3)
+    assert 0 < np.abs(y3 - y1).max() < 0.5 * np.abs(y0 - y1).max()
+
+
+def test_o4_variant3_hand_values(oracle):
+    # H2(iii) group (tests/golden/h2_int4.json): sg = 0x297C = 0.0428466796875, codes [2,-5,7,-1].
+    # u*sg = [10, 3, 15, 7]*sg = [0.428466796875, 0.1285400390625, 0.6427001953125, 0.2999267578125];
+    # fp16 spacing is 2^-12 in [0.25,0.5), 2^-13 in [0.125,0.25), 2^-11 in [0.5,1):
+    #   0.428466796875 = 1755*2^-12 exact; 0.1285400390625 = 1053*2^-13 exact;
+    #   0.6427001953125 = 1316.25*2^-11 -> 1316*2^-11 = 0.642578125; 0.2999267578125 = 1228.5*2^-12 -> tie to even 1228*2^-12 = 0.2998046875
+    sg = np.zeros((1, 1), np.uint16); sg[0, 0] = 0x297C
+    codes = np.zeros((1, 32), np.int8); codes[0, :4] = [2, -5, 7, -1]
+    w = oracle.dequant_int4(codes, sg, 3)[0]
+    s = 0.0428466796875
+    assert w[0] == 0.428466796875 - 8 * s and w[1] == 0.1285400390625 - 8 * s
+    assert w[2] == 0.642578125 - 8 * s and w[3] == 0.2998046875 - 8 * s
+    assert np.all(w[4:] == np.float64(np.float16(8 * s)) - 8 * s)     # code 0 -> fp16(8 sg) - 8 sg = 0 (8 sg is exact)
+    assert np.all(w[4:] == 0.0)
 
 
 def test_o4_quantisation_noise_level(oracle):
