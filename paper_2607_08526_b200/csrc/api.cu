@@ -29,10 +29,10 @@ size_t w8_ws_bytes(int M, int K) { return up256(static_cast<size_t>(M) * K) + up
 
 int linear_w8a8_impl(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
                      int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
-                     cudaStream_t st, bool pdl) {
+                     cudaStream_t st, bool pdl, bool early = false) {
     int8_t* Xq = static_cast<int8_t*>(ws);
     float* sx = reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + up256(static_cast<size_t>(M) * K));
-    int rc = launch_quant_rows_i8(X, xt, M, K, Xq, sx, st, pdl);
+    int rc = launch_quant_rows_i8(X, xt, M, K, Xq, sx, st, pdl, early);
     if (rc != ARIA_OK) return rc;
     W8Epilogue ep;
     ep.sx = sx; ep.sw = w_scale; ep.bias = bias; ep.bias_t = bt; ep.act = act; ep.Y = Y;
@@ -61,13 +61,16 @@ int check_layers(const aria_layer* layers, int n_layers, int M, int mode, int io
     return check_arch();
 }
 
+// early: W8A8 only -- this layer's activation quantiser may overlap the previous layer's GEMM (see
+// aria_denoiser_linears).
 int run_layer(const aria_layer& L, const void* in, void* out, int M, int mode, int io, void* ws,
-              size_t ws_bytes, cudaStream_t st) {
+              size_t ws_bytes, cudaStream_t st, bool early = false) {
     static const bool pdl = getenv("ARIA_NO_PDL") == nullptr;   // debug switch
+    static const bool no_early = getenv("ARIA_NO_EARLY_QUANT") != nullptr;
     if (mode == ARIA_W8A8)
         return linear_w8a8_impl(in, io, M, L.K, static_cast<const int8_t*>(L.wq),
                                 static_cast<const float*>(L.w_scale), L.N, L.bias, io, L.act, out, io,
-                                ws, st, pdl);
+                                ws, st, pdl, early && !no_early);
     return launch_gemm_w4a16(in, M, L.K, static_cast<const uint8_t*>(L.wq),
                              static_cast<const uint16_t*>(L.w_scale), L.N, L.bias, L.act, out, io, ws,
                              ws_bytes, st, pdl);
@@ -103,7 +106,7 @@ const char* aria_status_string(int status) {
 
 size_t aria_workspace_bytes(int M, int maxK, int maxN, int mode) {
     if (M <= 0 || maxK <= 0 || maxN <= 0) return 0;
-    if (mode == ARIA_W8A8) return w8_ws_bytes(M, maxK);
+    if (mode == ARIA_W8A8) return 2 * w8_ws_bytes(M, maxK);   // two (Xq, sx) buffers: see aria_denoiser_linears
     if (mode == ARIA_W4A16) {
         // Split-K bound: splits * tiles <= #SMs and a tile holds <= 128 x TT outputs, so the fp32
         // partials never exceed #SMs * 128 * TT * 4 bytes; one counter quad per tile.
@@ -224,9 +227,25 @@ int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mod
     if (misaligned(ws)) return ARIA_ERR_ALIGN;
     if (!ws || ws_bytes < aria_workspace_bytes(M, maxK, maxN, mode)) return ARIA_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // W8A8: the (Xq, sx) scratch alternates between two buffers, and the S1 pass of a layer whose
+    // input the previous layer does not write starts while that layer's GEMM is still running
+    // (programmatic dependent launch): the GEMM of layer i-1 reads buffer (i-1)&1 and writes out[i-1],
+    // the quantiser of layer i reads in[i] and writes buffer i&1.  Every kernel of the chain waits
+    // for its predecessor before it EXITS, so "kernel k complete" implies "kernels < k complete" and
+    // nothing older than layer i-1's GEMM can still be running.
+    static const bool single_buf = getenv("ARIA_W8_SINGLE_BUF") != nullptr;   // debug switch
+    const size_t half = mode == ARIA_W8A8 && !single_buf ? w8_ws_bytes(M, maxK) : 0;
     for (int i = 0; i < n_layers; ++i) {
-        const void* in = layers[i].in ? layers[i].in : layers[i - 1].out;
-        rc = run_layer(layers[i], in, layers[i].out, M, mode, io, ws, ws_bytes, st);
+        const aria_layer& L = layers[i];
+        const void* in = L.in ? L.in : layers[i - 1].out;
+        bool early = false;
+        if (mode == ARIA_W8A8 && i > 0) {
+            const uintptr_t a0 = reinterpret_cast<uintptr_t>(in), a1 = a0 + static_cast<size_t>(M) * L.K * dsize(io);
+            const uintptr_t b0 = reinterpret_cast<uintptr_t>(layers[i - 1].out),
+                            b1 = b0 + static_cast<size_t>(M) * layers[i - 1].N * dsize(io);
+            early = !single_buf && !(a0 < b1 && b0 < a1);
+        }
+        rc = run_layer(L, in, L.out, M, mode, io, static_cast<uint8_t*>(ws) + (i & 1) * half, ws_bytes - (i & 1) * half, st, early);
         if (rc != ARIA_OK) return rc;
     }
     return ARIA_OK;

@@ -334,7 +334,9 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             const float* swb = swb_all + (it & 1) * 2 * BN;
             float sxv = 0.0f, nsv = 0.0f, nbv = 0.0f;
             if (OUT_T != 2) {
-                if (row0 + lane < p.M) sxv = __ldg(p.sx + row0 + lane);
+                // sx is written by the grid before this one: an ordered load (a non-coherent load is a
+                // pure value to the compiler and may be hoisted above griddepcontrol.wait)
+                if (row0 + lane < p.M) asm volatile("ld.global.f32 %0, [%1];" : "=f"(sxv) : "l"(p.sx + row0 + lane) : "memory");
                 fetch_swb(t + unit_step, nsv, nbv);
             }
             mbar_wait(tfull0 + 8 * acc, acc_phase);

@@ -8,8 +8,10 @@
 namespace aria {
 
 // ---- quant.cu
+// early (needs pdl): the pass does not wait for the previous grid before it starts -- the caller
+// guarantees that grid neither writes X nor touches q / s -- but still waits for it before it ends.
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl);
+                         bool pdl, bool early = false);
 int launch_quant_groups_i4(const void* W, int wt, int N, int K, uint8_t* q4, uint16_t* sg,
                            cudaStream_t st);
 

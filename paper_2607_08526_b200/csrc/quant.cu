@@ -11,19 +11,31 @@ namespace aria {
 constexpr int QROW_MAX_THREADS = 256;
 constexpr int QROW_CACHE = 4;  // 8-element vectors kept in registers per thread
 
+// 16-byte global loads that stay BELOW griddepcontrol.wait: a non-coherent (ld.global.nc) load is a
+// pure value to the compiler, which hoisted it above the wait of the quantiser kernels -- under
+// programmatic dependent launch the previous grid is still writing X at that point.
+__device__ __forceinline__ uint4 ld_global_v4(const void* p) {
+    uint4 v;
+    asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ float4 ld_global_f4(const void* p) {
+    const uint4 v = ld_global_v4(p);
+    return make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
+}
 template <typename T>
 __device__ __forceinline__ void load8(const T* p, float (&v)[8]);
 
 template <>
 __device__ __forceinline__ void load8<float>(const float* p, float (&v)[8]) {
-    const float4 a = __ldg(reinterpret_cast<const float4*>(p));
-    const float4 b = __ldg(reinterpret_cast<const float4*>(p) + 1);
+    const float4 a = ld_global_f4(p);
+    const float4 b = ld_global_f4(p + 4);
     v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
     v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
 }
 template <>
 __device__ __forceinline__ void load8<__nv_bfloat16>(const __nv_bfloat16* p, float (&v)[8]) {
-    const uint4 a = __ldg(reinterpret_cast<const uint4*>(p));
+    const uint4 a = ld_global_v4(p);
     const uint32_t w[4] = {a.x, a.y, a.z, a.w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -37,11 +49,11 @@ template <typename T> struct Raw8;
 template <> struct Raw8<float> { float4 a, b; };
 template <> struct Raw8<__nv_bfloat16> { uint4 a; };
 __device__ __forceinline__ void load_raw(const float* p, Raw8<float>& r) {
-    r.a = __ldg(reinterpret_cast<const float4*>(p));
-    r.b = __ldg(reinterpret_cast<const float4*>(p) + 1);
+    r.a = ld_global_f4(p);
+    r.b = ld_global_f4(p + 4);
 }
 __device__ __forceinline__ void load_raw(const __nv_bfloat16* p, Raw8<__nv_bfloat16>& r) {
-    r.a = __ldg(reinterpret_cast<const uint4*>(p));
+    r.a = ld_global_v4(p);
 }
 __device__ __forceinline__ void unpack8(const Raw8<float>& r, float (&v)[8]) {
     v[0] = r.a.x; v[1] = r.a.y; v[2] = r.a.z; v[3] = r.a.w;
@@ -119,9 +131,12 @@ __device__ __forceinline__ uint2 quant8_i8(const float (&v)[8], float s) {
 template <typename T>
 __global__ void __launch_bounds__(QROW_MAX_THREADS)
 quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
-                     float* __restrict__ scale) {
+                     float* __restrict__ scale, int early) {
     __shared__ float red[QROW_MAX_THREADS / 32];
-    pdl_wait_prior_grid();
+    // early: X, Xq and scale are untouched by the grid before this one (the caller checked), so the
+    // pass runs concurrently with it; the wait moves to the end so that "this grid is complete" still
+    // implies "every earlier grid is complete" for whoever waits on this one.
+    if (!early) pdl_wait_prior_grid();
     const int64_t row = blockIdx.x;
     const T* x = X + row * K;
     int8_t* q = Xq + row * K;
@@ -171,6 +186,7 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
         if (!f.ok || !quant8_fast(t, f, o)) o = quant8_i8(t, s);
         *reinterpret_cast<uint2*>(q + 8 * idx) = o;
     }
+    if (early) pdl_wait_prior_grid();
 }
 
 // One WARP per row (K <= 8 * 32 * VPL): every lane issues all its 16-byte loads up front, the
@@ -178,12 +194,15 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
 template <typename T, int VPL>
 __global__ void __launch_bounds__(256)
 quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restrict__ Xq,
-                          float* __restrict__ scale) {
-    pdl_wait_prior_grid();
+                          float* __restrict__ scale, int early) {
+    if (!early) pdl_wait_prior_grid();      // early: see quant_rows_i8_kernel
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
     const int64_t row = static_cast<int64_t>(blockIdx.x) * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (row >= R) return;
+    if (row >= R) {
+        if (early) pdl_wait_prior_grid();
+        return;
+    }
     const T* x = X + row * K;
     int8_t* q = Xq + row * K;
     const int nvec = K >> 3;
@@ -218,6 +237,7 @@ quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restr
             *reinterpret_cast<uint2*>(q + 8 * idx) = o;
         }
     }
+    if (early) pdl_wait_prior_grid();
 }
 
 // int4, group 32 along K: 4 threads per group, 8 elements each (R3, R4, R7, R8).
@@ -248,15 +268,16 @@ quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restri
 
 template <typename T, int VPL>
 static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, float* s,
-                                    cudaLaunchConfig_t& cfg) {
+                                    cudaLaunchConfig_t& cfg, int early) {
     cfg.blockDim = dim3(256);
     cfg.gridDim = dim3((R + 7) / 8);
-    return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s);
+    return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s, early);
 }
 
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl) {
+                         bool pdl, bool early_) {
     const int nvec = C / 8;
+    const int early = pdl && early_ ? 1 : 0;
     {   // warp-per-row variants: rows up to 3072 elements (wider rows: one CTA per row, below)
         cudaLaunchConfig_t cfg = {};
         cfg.stream = st;
@@ -269,14 +290,14 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
         cudaError_t e = cudaErrorInvalidValue;
         bool done = true;
         if (xt == ARIA_BF16) {
-            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg);
-            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg);
-            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg);
+            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg, early);
+            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg, early);
+            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg, early);
             else done = false;
         } else {
-            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg);
-            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg);
-            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg);
+            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg, early);
+            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg, early);
+            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg, early);
             else done = false;
         }
         if (done) return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
@@ -294,10 +315,10 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
     cfg.numAttrs = pdl ? 1 : 0;
     cudaError_t e;
     if (xt == ARIA_F32)
-        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s);
+        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s, early);
     else
         e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<__nv_bfloat16>,
-                               static_cast<const __nv_bfloat16*>(X), C, q, s);
+                               static_cast<const __nv_bfloat16*>(X), C, q, s, early);
     return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
