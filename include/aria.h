@@ -85,7 +85,8 @@ ARIA_API int aria_quantize_act_int8(const void* X, int xt, int M, int K, int8_t*
  *   y = float(acc) * sx[m] * w_scale[n] + bias[n];  act == GELU_ERF: y = 0.5 y (1 + erf(y/sqrt2));
  *   Y = cast(y, yt).
  * bias: [N] of dtype `bt`, may be NULL.  ws: scratch of at least
- * aria_workspace_bytes(M, K, N, ARIA_W8A8) bytes (holds Xq and sx).                         */
+ * aria_workspace_bytes(M, K, N, ARIA_W8A8) bytes (holds Xq and sx; the size covers the two
+ * alternating buffers aria_denoiser_linears uses).                                           */
 ARIA_API int aria_linear_w8a8(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
                      int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
                      size_t ws_bytes, void* stream);
@@ -110,7 +111,9 @@ ARIA_API int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, 
  * of dtype `io` (bf16 or fp32; W4A16 requires bf16).  `in == NULL` chains the layer to the
  * previous layer's `out` (its N must equal this K).  mode W8A8: wq = int8 [N,K], w_scale = fp32
  * [N]; mode W4A16: wq = packed int4 [N,K/2], w_scale = fp16 bits [N,K/32].  bias has dtype `io`,
- * may be NULL.  Capturable: enqueue only.                                                   */
+ * may be NULL.  Capturable: enqueue only.  Mode W8A8: the S1 pass of a layer whose input the
+ * previous layer does not write is overlapped with that layer's GEMM (programmatic dependent
+ * launch, two alternating Xq / sx buffers in `ws`); results are those of array order.         */
 typedef struct {
     int K, N;
     int act; /* aria_act applied to this layer's output */
@@ -134,9 +137,11 @@ ARIA_API int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M
  * bf16 I/O, every K % 256 == 0 and no output buffer overlapping another output or an earlier
  * input, the step is ONE persistent weight-streaming kernel over all layers (HBM bound; layers
  * whose input is not an earlier layer's output may overlap, results are identical to array
- * order); there the dequantised weight is w^ = fp16_rn(q * sg) (fp16 operand x bf16 activations
- * in the same tcgen05 kind::f16 MMA; needs sg <= 127), or bf16_rne(q * sg) as in
- * aria_linear_w4a16 when the environment variable ARIA_W4_F16A=0 is set at plan creation.
+ * order); there the dequantised weight is w^ = fp16_rn((q + 8) * sg) - 8 * sg (offset-binary
+ * code scaled and rounded to fp16, zero point subtracted exactly by an extra tensor-core k-step;
+ * activations enter the same tcgen05 kind::f16 MMA as fp16, exact for 2^-14 <= |x| <= 65504;
+ * needs sg <= 63; reading R12c), or bf16_rne(q * sg) as in aria_linear_w4a16 when the
+ * environment variable ARIA_W4_F16A=0 is set at plan creation.
  * Any other list runs the per-layer path.  A plan's scratch serves ONE step at a time: do not
  * run the same plan concurrently on two streams.  aria_stack_plan_is_streaming: 1 if the plan
  * uses the stream kernel.                                                                   */

@@ -168,7 +168,14 @@ __device__ __forceinline__ void w4_store(void* Y, int out_t, int64_t idx, float 
         static_cast<__nv_bfloat16*>(Y)[idx] = __float2bfloat16_rn(y);
 }
 
-template <int TT, bool GELU, int CTAS>
+// MC (CTAS == 1 only): the two CTAs of a cluster work on the same token tile and adjacent weight-row
+// tiles in lockstep, and each loads HALF of every X tile with TMA multicast into both CTAs' shared
+// memory: the X operand is read from L2 once per pair.  At M >= 2048 the kernel is bound by L2 -> SM
+// traffic of X (every 128-row weight tile streams all of X: 226 MB per QKV layer against 3.5 MB of
+// weights), not by the tensor pipe.  All MMAs stay CTA-local (cta_group::1): the only cross-CTA
+// signals are the multicast TMA's complete_tx and the multicast tcgen05.commit that frees an X slot
+// in both CTAs -- no thread ever waits on a cluster-scope arrive.
+template <int TT, bool GELU, int CTAS, bool MC>
 __global__ void __launch_bounds__(W4Cfg<TT, CTAS>::THREADS, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmX,
                   const __grid_constant__ CUtensorMap tmY, const W4Params p) {
@@ -192,6 +199,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const uint32_t rank = CTAS == 2 ? cluster_ctarank() : 0u;   // position in the CTA pair
+    const uint32_t mc_rank = MC ? cluster_ctarank() : 0u;       // which half of the X tile this CTA loads
     constexpr int UN = W4_BN * CTAS;                            // output channels per work unit
     const int num_n = (p.N + UN - 1) / UN;
     const int num_t = (p.M + TT - 1) / TT;
@@ -206,7 +214,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         tma_prefetch_desc(&tmY);
         for (int s = 0; s < XS; ++s) {
             mbar_init(xfull0 + 8 * s, 1);
-            mbar_init(xempty0 + 8 * s, 1);      // MMA commit
+            mbar_init(xempty0 + 8 * s, MC ? 2 : 1);      // MMA commit (MC: of both CTAs)
         }
         for (int s = 0; s < PS; ++s) {
             mbar_init(pfull0 + 8 * s, 1);
@@ -234,7 +242,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         }
     }
     tc_fence_before();
-    if (CTAS == 2) cluster_sync(); else __syncthreads();
+    if (CTAS == 2 || MC) cluster_sync(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_g;
 
@@ -259,8 +267,12 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                         tma_load_2d_2sm(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0,
                                         (xfull0 + 8 * stage) & PEER_BIT_MASK);
                     } else {
-                        mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);
-                        tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
+                        mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);   // MC: both halves land here
+                        if (MC)
+                            tma_load_2d_mc(sX + stage * Cfg::X_BYTES + mc_rank * (Cfg::X_BYTES / 2), &tmX, kb * W4_BK,
+                                           t0 + mc_rank * (TT / 2), xfull0 + 8 * stage, 3);
+                        else
+                            tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
                     }
                 }
                 __syncwarp();
@@ -320,7 +332,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                             tc_commit_2sm(aempty0 + 8 * ab, 3);
                             if (kb == kb1 - 1) tc_commit_2sm(tfull0 + 8 * acc, 3);
                         } else {
-                            tc_commit(xempty0 + 8 * stage);
+                            if (MC) tc_commit_mc(xempty0 + 8 * stage, 3); else tc_commit(xempty0 + 8 * stage);
                             tc_commit(aempty0 + 8 * ab);
                             if (kb == kb1 - 1) tc_commit(tfull0 + 8 * acc);
                         }
@@ -529,7 +541,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
 
     if (warp >= W4_EPI_WARP0 && warp < W4_DEQ_WARP0 && lane == 0) tma_store_wait<0>();
     tc_fence_before();
-    if (CTAS == 2) cluster_sync(); else __syncthreads();
+    if (CTAS == 2 || MC) cluster_sync(); else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
         if (CTAS == 2) tmem_dealloc_2sm(tmem_base, Cfg::TMEM_COLS);
@@ -537,12 +549,12 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     }
 }
 
-template <int TT, bool GELU, int CTAS>
+template <int TT, bool GELU, int CTAS, bool MC = false>
 static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, const W4Params& p,
                      int grid, cudaStream_t st, bool pdl) {
     using Cfg = W4Cfg<TT, CTAS>;
     static bool attr_set = false;
-    auto kern = w4a16_gemm_kernel<TT, GELU, CTAS>;
+    auto kern = w4a16_gemm_kernel<TT, GELU, CTAS, MC>;
     if (!attr_set) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES) !=
             cudaSuccess)
@@ -552,7 +564,7 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
     CUtensorMap tmP, tmX, tmY;
     int rc = make_tmap_2d(&tmP, Wq4, 1, N, K / 2, W4_BN, Cfg::P_ROW, Cfg::P_ROW);
     if (rc != ARIA_OK) return rc;
-    rc = make_tmap_2d(&tmX, X, 2, M, K, Cfg::X_ROWS, 64, 128);
+    rc = make_tmap_2d(&tmX, X, 2, M, K, MC ? Cfg::X_ROWS / 2 : Cfg::X_ROWS, 64, 128);   // MC: each CTA loads half a tile
     if (rc != ARIA_OK) return rc;
     // output: box = 32 tokens x 32 channels (64 B bf16 rows / 128 B fp32 rows)
     rc = make_tmap_2d(&tmY, p.Y, p.out_t == ARIA_F32 ? 4 : 2, M, N, 32, 32, p.out_t == ARIA_F32 ? 128 : 64);
@@ -569,7 +581,7 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
         at[na].val.programmaticStreamSerializationAllowed = 1;
         ++na;
     }
-    if (CTAS == 2) {
+    if (CTAS == 2 || MC) {
         at[na].id = cudaLaunchAttributeClusterDimension;
         at[na].val.clusterDim.x = 2;
         at[na].val.clusterDim.y = 1;
@@ -647,13 +659,23 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
     const bool pair = want_pair && tt == 256 && s == 1 && N > W4_BN && sms >= 2;
     const int units = pair ? ((N + 2 * W4_BN - 1) / (2 * W4_BN)) * ((M + tt - 1) / tt) : static_cast<int>(tiles) * s;
     const int slots = pair ? sms / 2 : sms;
-    const int grid = (units < slots ? units : slots) * (pair ? 2 : 1);
+    int grid = (units < slots ? units : slots) * (pair ? 2 : 1);
+    // X multicast over CTA couples (see the kernel): big token tiles, no split-K, an even number of
+    // weight-row tiles so that a couple always shares its token tile
+    // Measured on C5 (M = 2048): 3.79 ms with multicast vs 3.81 ms without -- the L2 already serves
+    // the two CTAs' identical reads at no extra cost, so the mode is parity-tested but OFF by default.
+    static const bool want_mc = getenv("ARIA_W4_MC") != nullptr;
+    const bool mc = want_mc && !pair && tt == 256 && s == 1 && ((N + W4_BN - 1) / W4_BN) % 2 == 0 && grid >= 2;
+    if (mc) grid &= ~1;
     if (s > 1 && cudaMemsetAsync(p.counters, 0, tiles * 4 * sizeof(unsigned), st) != cudaSuccess)
         return ARIA_ERR_CUDA;
     const bool gelu = act == ARIA_ACT_GELU_ERF;
 #define ARIA_W4_LAUNCH(TTV)                                                        \
     return gelu ? launch_w4<TTV, true, 1>(X, M, K, Wq4, N, p, grid, st, pdl)       \
                 : launch_w4<TTV, false, 1>(X, M, K, Wq4, N, p, grid, st, pdl)
+    if (mc)
+        return gelu ? launch_w4<256, true, 1, true>(X, M, K, Wq4, N, p, grid, st, pdl)
+                    : launch_w4<256, false, 1, true>(X, M, K, Wq4, N, p, grid, st, pdl);
     if (pair)
         return gelu ? launch_w4<256, true, 2>(X, M, K, Wq4, N, p, grid, st, pdl)
                     : launch_w4<256, false, 2>(X, M, K, Wq4, N, p, grid, st, pdl);

@@ -11,30 +11,39 @@
 // split-K: a cross-CTA reduction costs a chain of ~6 global round trips per unit (partials, fence,
 // counter, re-read) -- measured 4k-25k cycles per unit against ~2.7k cycles of dequantisation, the
 // reason the per-layer kernel is latency bound at M = 32.  Instead the host deals the units of ALL
-// layers to the CTAs at plan time (in layer order, always to the least-loaded CTA), so every CTA
-// streams the same number of stages and a layer with few tiles simply overlaps its neighbours.
-// Roles (768 threads, 1 CTA / SM):
-//   warp 0      X producer: [32 tokens x 64 k] bf16 tiles by TMA (L2 resident), after the unit's
-//               dependency (a chained layer waits for its producer layer's completion counter).
-//   warp 2      weight producer: packed + scale tiles by TMA, evict-first (the HBM stream).
-//   warp 1      MMA issuer: tcgen05.mma kind::f16, A = dequantised weights IN TENSOR MEMORY
-//               (128 rows x 16 k per instruction), B = X tile in shared memory, D = fp32 in TMEM.
-//   warps 4-7   epilogue: tcgen05.ld -> + bias, GELU, cast -> coalesced stores; a layer that feeds a
-//               later layer also bumps its completion counter (release).
-//   warps 8-23  four dequantiser groups (thread = weight row; group g = 64-k sub-block g of every
+// layers to the CTAs at plan time (one global order, always to the CTA with the fewest stages so far),
+// so every CTA streams the same number of stages and a layer with few tiles simply overlaps its
+// neighbours; layers that read an earlier layer's output are moved behind the independent ones.
+// Roles (768 threads, 1 CTA / SM; the single latency-critical warps have the HIGH warp ids because the
+// SM's warp arbiter prefers them):
+//   warps 0-15  four dequantiser groups (thread = weight row; group g = 64-k sub-block g of every
 //               stage): LDS -> registers -> tcgen05.st into a ring of TMEM A slots.  The dequantised
 //               tile never touches shared memory: per weight shared memory sees 0.5 B (TMA write)
 //               + 0.5 B (LDS) instead of 4.5 B with an smem A tile, which would cap the stream at
 //               ~28 weights/clk/SM -- below the ~41 weights/clk/SM that HBM delivers.
-// Dequantisation (AF16): the offset-binary nibble u = q + 8 in a byte 0x0u IS the e4m3 number
-// u * 2^-9; cvt.rn.f16x2.e4m3x2 turns two of them into fp16 and one HFMA2
-// (u 2^-9)(512 sg) - 8 sg = fp16_rn(q sg) finishes: w^ is the correctly rounded fp16 value of the
-// dequantised weight, 13 instructions per 8 weights (the exact-bf16 path of gemm_w4a16.cu needs 18
-// and saturates the ALU pipe at 24.6 weights/clk/SM -- 60% of what HBM delivers).  kind::f16 takes
-// fp16 x fp16 or bf16 x bf16 but not a mix (illegal instruction on sm_100a), so the bf16 activations
-// are converted to fp16 too: external inputs once per launch by the otherwise idle warps, chained
-// outputs by the producing epilogue (exact for 2^-14 <= |x| <= 65504).  AF16 = false keeps
-// w^ = bf16_rne(q sg) and bf16 activations (slower).
+//   warps 16-19 epilogue: tcgen05.ld -> + bias, GELU, cast -> coalesced stores; a layer that feeds a
+//               later layer also writes that layer's fp16 operand copy and bumps its completion
+//               counter (release).
+//   warp 20     X producer: [32 tokens x 64 k] fp16 tiles by TMA (L2 resident), after the unit's
+//               dependency (a chained layer waits for its producer layer's completion counter).
+//   warp 21     MMA issuer: tcgen05.mma kind::f16, A = dequantised weights IN TENSOR MEMORY
+//               (128 rows x 16 k per instruction), B = X tile in shared memory, D = fp32 in TMEM;
+//               17 instructions per stage: 16 of weights + 1 of zero points (below).
+//   warp 22     weight producer: packed + scale tiles by TMA, evict-first (the HBM stream).
+// Dequantisation (AF16), 9 instructions per 8 weights (the loop is issue bound, so this count IS the
+// kernel's speed): the offset-binary nibble u = q + 8 is masked into the mantissa of an fp16 constant
+// (1024 + u or 64 + u, one LOP3 per pair of weights) and one HFMA2 (B + u) sg - B sg returns
+// fp16_rn(u sg), the correctly rounded UNSIGNED dequantised weight.  The zero point -8 sg x is linear
+// and exact, so the tensor core applies it: per stage 16 extra k-values with A = -8 sg of the stage's
+// 8 groups and B = the (hi, lo) fp16 split of the groups' activation sums.  The dequantised weight is
+// therefore w^ = fp16_rn((q + 8) sg) - 8 sg (reading R12c, oracle variant 3).  kind::f16
+// takes fp16 x fp16 or bf16 x bf16 but not a mix (illegal instruction on sm_100a), so the bf16
+// activations are converted to fp16 too: external inputs once per launch by the dequantiser and
+// epilogue warps, chained outputs by the producing epilogue (exact for 2^-14 <= |x| <= 65504), both
+// in the k order the dequantiser produces ([0,4,1,5,2,6,3,7] inside each 8-k word) and with the
+// group sums appended to every 256-k stage.  AF16 = false keeps w^ = bf16_rne(q sg) and bf16
+// activations (18 instructions per 8 weights; used when a chained layer's geometry rules the fp16
+// copy out).
 #include <cstdlib>
 #include <cstring>
 #include <new>
