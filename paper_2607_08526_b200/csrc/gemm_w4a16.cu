@@ -54,8 +54,8 @@ struct W4Cfg {
     static constexpr int X_BYTES = X_ROWS * 128;               // x 64 bf16
     static constexpr int A_BYTES = W4_BN * 128;                // 16 KB: 128 rows x 64 bf16
     static constexpr int STG_BYTES = 4096;                     // per epilogue warp: 32 tokens x 128 B
-    static constexpr int XS = X_ROWS == 256 ? 3 : X_ROWS == 128 ? 4 : X_ROWS == 64 ? 6 : 8;   // X ring depth
-    static constexpr int PS = TT == 256 ? 8 : TT == 128 ? 12 : 16;                // packed ring depth
+    static constexpr int XS = X_ROWS == 256 ? 3 : X_ROWS == 192 ? 4 : X_ROWS == 128 ? 4 : X_ROWS == 64 ? 6 : 8;   // X ring depth
+    static constexpr int PS = TT >= 192 ? 8 : TT == 128 ? 12 : 16;                // packed ring depth
     static constexpr int X_OFF = 0;
     static constexpr int A_OFF = X_OFF + XS * X_BYTES;
     static constexpr int P_OFF = A_OFF + NB * A_BYTES;
@@ -63,9 +63,11 @@ struct W4Cfg {
     static constexpr int BAR_OFF = STG_OFF + 4 * STG_BYTES;
     static constexpr int NBAR = 2 * XS + 2 * PS + 3 * NB + 4;
     static constexpr int SMEM_BYTES = BAR_OFF + NBAR * 8 + 16 + 1024;
-    static constexpr int ACC_STRIDE = TT;
-    static constexpr int TMEM_COLS = 2 * TT < 32 ? 32 : 2 * TT;
-    static_assert(TT == 32 || TT == 64 || TT == 128 || TT == 256, "TT");
+    // TT = 192 fills the SMs when N / 128 is small: 12 row tiles x 11 token tiles = 132 units on 148 SMs
+    // at M = 2048 (TT = 256: 96 units)
+    static constexpr int ACC_STRIDE = TT == 192 ? 256 : TT;
+    static constexpr int TMEM_COLS = 2 * ACC_STRIDE < 32 ? 32 : 2 * ACC_STRIDE;
+    static_assert(TT == 32 || TT == 64 || TT == 128 || TT == 192 || TT == 256, "TT");
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
@@ -364,21 +366,31 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             const bool row_ok = n0 + r < p.N;
             const uint32_t* srow = reinterpret_cast<const uint32_t*>(
                 p.g_scale + static_cast<int64_t>(row_ok ? n0 + r : 0) * gpr);
+            // the two fp16 group scales of this row and a k-block: one aligned 32-bit load.  The load for
+            // this group's NEXT k-block (kb + G) is issued before the current one is processed, which
+            // takes the L2 round trip (uncoalesced: one line per row) off the per-k-block chain.
+            auto load_scales = [&](int kb) -> uint32_t {
+                uint32_t v = 0;
+                if (row_ok && kb < kb1) {
+                    if ((gpr & 1) == 0) {
+                        v = __ldg(srow + kb);
+                    } else {  // odd group count: rows are only 2-byte aligned
+                        const uint16_t* s16 = reinterpret_cast<const uint16_t*>(srow);
+                        v = __ldg(s16 + 2 * kb);
+                        if (2 * kb + 1 < gpr) v |= static_cast<uint32_t>(__ldg(s16 + 2 * kb + 1)) << 16;
+                    }
+                }
+                return v;
+            };
+            // first k-block of this unit that belongs to this group
+            const int kfirst = kb0 + ((g - it % G) + G) % G;
+            uint32_t sc_next = load_scales(kfirst);
             for (int kb = kb0; kb < kb1; ++kb, ++it) {
                 if (it % G != g) continue;
                 const int stage = it % PS;
                 const uint32_t phase = (it / PS) & 1;
-                // the two fp16 group scales of this row and k-block: one aligned 32-bit load
-                uint32_t sc2 = 0;
-                if (row_ok) {
-                    if ((gpr & 1) == 0) {
-                        sc2 = __ldg(srow + kb);
-                    } else {  // odd group count: rows are only 2-byte aligned
-                        const uint16_t* s16 = reinterpret_cast<const uint16_t*>(srow);
-                        sc2 = __ldg(s16 + 2 * kb);
-                        if (2 * kb + 1 < gpr) sc2 |= static_cast<uint32_t>(__ldg(s16 + 2 * kb + 1)) << 16;
-                    }
-                }
+                const uint32_t sc2 = sc_next;
+                sc_next = load_scales(kb + G);
                 mbar_wait(pfull0 + 8 * stage, phase);
                 const uint32_t ps = sP + stage * Cfg::P_BYTES;
                 const uint4 pk0 = lds128(ps + poff0);
@@ -601,10 +613,10 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
 void w4_plan(int M, int N, int K, int sms, int* tt_out, int* splits_out) {
     const int num_kb = (K + W4_BK - 1) / W4_BK;
     const int num_n = (N + W4_BN - 1) / W4_BN;
-    const int tts[4] = {256, 128, 64, 32};
+    const int tts[5] = {256, 192, 128, 64, 32};
     long best = -1;
     int best_tt = 32, best_s = 1;
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < 5; ++i) {
         const int tt = tts[i];
         if (tt > 32 && tt >= 2 * M) continue;                 // mostly padding
         const int tiles = num_n * ((M + tt - 1) / tt);
@@ -682,6 +694,7 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
     if (tt == 32) { ARIA_W4_LAUNCH(32); }
     if (tt == 64) { ARIA_W4_LAUNCH(64); }
     if (tt == 128) { ARIA_W4_LAUNCH(128); }
+    if (tt == 192) { ARIA_W4_LAUNCH(192); }
     ARIA_W4_LAUNCH(256);
 #undef ARIA_W4_LAUNCH
 }

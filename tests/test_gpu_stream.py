@@ -149,3 +149,47 @@ def test_aliasing_outputs_disable_streaming(aria, oracle):
     b, _ = _layer(aria, oracle, M, K, N, 86, 10)
     b["out"] = a["out"]                       # two layers write the same buffer: order matters
     list(_run_plan(aria, [a, b], M, expect_stream=False))
+
+
+@pytest.mark.parametrize("M", [5, 32])
+def test_three_layer_chain_and_reordered_independents(aria, oracle, M):
+    # a -> b -> c chained (in == NULL twice) with two independent linears in between in array order:
+    # the plan moves dependents behind independents; results must equal array-order semantics
+    specs, hosts = [], []
+    # (K, N, chained): layer 1 reads layer 0, layer 2 reads layer 1 (in == NULL chains to the PREVIOUS
+    # layer), layers 3 and 4 are independent and may be scheduled ahead of the dependents
+    shapes = [(256, 512, None), (512, 256, True), (256, 256, True), (256, 384, None), (768, 128, None)]
+    for i, (K, N, chained) in enumerate(shapes):
+        sp, h = _layer(aria, oracle, M, K, N, 87, 30 * i, act=1 if i == 0 else 0, x=True if chained else None)
+        specs.append(sp)
+        hosts.append(h)
+    runs = list(_run_plan(aria, specs, M))
+    v = _variant()
+    for i, h in enumerate(hosts):
+        assert np.array_equal(runs[0][i], runs[1][i])
+        x = h["x"] if "x" in h else inputs.bf16_as_f32(runs[0][i - 1])[:M]
+        _check(oracle, h, x, runs[0][i], v)
+
+
+def test_graph_replay_of_a_plan_is_bit_stable(aria, oracle):
+    M = 32
+    pairs = [_layer(aria, oracle, M, 256, 256, 88, 10 * i, x=True if i == 1 else None) for i in range(3)]
+    specs = [p[0] for p in pairs]
+    layers = aria.make_layers(specs)
+    plan = aria.aria_stack_plan_create(layers, M, aria.W4A16, aria.BF16)
+    try:
+        aria.aria_stack_plan_run(plan)
+        torch.cuda.synchronize()
+        ref = [host_bits16(s["out"]).copy() for s in specs]
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            aria.aria_stack_plan_run(plan)
+        for _ in range(3):
+            for s in specs:
+                s["out"].zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            for r, s in zip(ref, specs):
+                assert np.array_equal(r, host_bits16(s["out"]))
+    finally:
+        aria.aria_stack_plan_destroy(plan)
