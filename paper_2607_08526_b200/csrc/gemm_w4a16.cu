@@ -120,34 +120,35 @@ __device__ __forceinline__ uint32_t fma2_to_bf16x2(uint64_t x, uint64_t s, uint6
     return cvt_bf16x2(lo, hi);
 }
 
-// Per-group constants, as the four (scale, offset) pairs the element pairs of a word need.
+// Per-group constants: (scale, offset) for a nibble sitting at mantissa bit 8, 12 or 16 of 1.0f.
+// Scalar FFMAs on purpose: the packed f32x2 form needs both operands in aligned register pairs and cost
+// 2.6 IMAD.MOV per weight pair in this loop (ncu: 84 of its 325 instructions), more than it saved.
 struct GroupConst {
-    uint64_t s_8_12, c_8_12, s_16_12, c_16_12, s_16_8, c_16_8, s_12_16, c_12_16;
+    float s8, c8, s12, c12, s16, c16;
 };
 __device__ __forceinline__ GroupConst group_const(float sg) {
-    const float s8 = sg * 32768.0f, c8 = -(sg * 32776.0f);   // 2^15, 2^15 + 8
-    const float s12 = sg * 2048.0f, c12 = -(sg * 2056.0f);   // 2^11, 2^11 + 8
-    const float s16 = sg * 128.0f, c16 = -(sg * 136.0f);     // 2^7,  2^7  + 8
     GroupConst g;
-    g.s_8_12 = pack2(s8, s12);   g.c_8_12 = pack2(c8, c12);
-    g.s_16_12 = pack2(s16, s12); g.c_16_12 = pack2(c16, c12);
-    g.s_16_8 = pack2(s16, s8);   g.c_16_8 = pack2(c16, c8);
-    g.s_12_16 = pack2(s12, s16); g.c_12_16 = pack2(c12, c16);
+    g.s8 = sg * 32768.0f;  g.c8 = -(sg * 32776.0f);    // 2^15, 2^15 + 8
+    g.s12 = sg * 2048.0f;  g.c12 = -(sg * 2056.0f);    // 2^11, 2^11 + 8
+    g.s16 = sg * 128.0f;   g.c16 = -(sg * 136.0f);     // 2^7,  2^7  + 8
     return g;
 }
 // 8 codes of one 32-bit word (nibble i = code of k = 8w + i) -> 4 packed bf16x2, k ascending.
+// x = 1.0f | (u << pos) with u = q + 8, so x * (2^(23-pos) sg) - (2^(23-pos) + 8) sg = q sg exactly
+// (both addends and the result are representable), and one cvt.rn.bf16x2 rounds it: w^ = bf16_rne(q sg).
 __device__ __forceinline__ uint4 dequant_word(uint32_t w, const GroupConst& g) {
     const uint32_t wa = w << 8, wb = w >> 12;
     const uint32_t M8 = 0x00000F00u, M12 = 0x0000F000u, M16 = 0x000F0000u;
     const uint32_t X8 = 0x3F800800u, X12 = 0x3F808000u, X16 = 0x3F880000u;  // 1.0f | (8 << pos)
-    const uint32_t e0 = lop_and_xor(wa, M8, X8), e1 = lop_and_xor(wa, M12, X12);
-    const uint32_t e2 = lop_and_xor(wa, M16, X16), e3 = lop_and_xor(w, M12, X12);
-    const uint32_t e4 = lop_and_xor(w, M16, X16), e5 = lop_and_xor(wb, M8, X8);
-    const uint32_t e6 = lop_and_xor(wb, M12, X12), e7 = lop_and_xor(wb, M16, X16);
-    return make_uint4(fma2_to_bf16x2(pack2u(e0, e1), g.s_8_12, g.c_8_12),
-                      fma2_to_bf16x2(pack2u(e2, e3), g.s_16_12, g.c_16_12),
-                      fma2_to_bf16x2(pack2u(e4, e5), g.s_16_8, g.c_16_8),
-                      fma2_to_bf16x2(pack2u(e6, e7), g.s_12_16, g.c_12_16));
+    const float f0 = fmaf(__uint_as_float(lop_and_xor(wa, M8, X8)), g.s8, g.c8);
+    const float f1 = fmaf(__uint_as_float(lop_and_xor(wa, M12, X12)), g.s12, g.c12);
+    const float f2 = fmaf(__uint_as_float(lop_and_xor(wa, M16, X16)), g.s16, g.c16);
+    const float f3 = fmaf(__uint_as_float(lop_and_xor(w, M12, X12)), g.s12, g.c12);
+    const float f4 = fmaf(__uint_as_float(lop_and_xor(w, M16, X16)), g.s16, g.c16);
+    const float f5 = fmaf(__uint_as_float(lop_and_xor(wb, M8, X8)), g.s8, g.c8);
+    const float f6 = fmaf(__uint_as_float(lop_and_xor(wb, M12, X12)), g.s12, g.c12);
+    const float f7 = fmaf(__uint_as_float(lop_and_xor(wb, M16, X16)), g.s16, g.c16);
+    return make_uint4(cvt_bf16x2(f0, f1), cvt_bf16x2(f2, f3), cvt_bf16x2(f4, f5), cvt_bf16x2(f6, f7));
 }
 
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
@@ -457,6 +458,40 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 // 64 B bf16 / 128 B fp32, swizzled as the output tensor map expects), then one TMA
                 // store writes the block -- coalesced, asynchronous, clipped at M and N.
                 const uint32_t stg = base + Cfg::STG_OFF + (warp - W4_EPI_WARP0) * Cfg::STG_BYTES;
+                if (p.out_t == ARIA_BF16) {
+                    // bf16 fast path (measured: the epilogue of the LAST tile of a CTA is fully exposed --
+                    // 8.6k of 28k cycles for a one-tile-per-CTA layer with the generic loop below).  One
+                    // tcgen05.ld of 32 columns per block, everything unrolled: the swizzled address of
+                    // token row j is one of 4 per-thread bases (chunk index ^ ((j >> 1) & 3)) plus the
+                    // immediate j * 64, so a value costs add + (GELU) + cvt + st.shared.u16.
+                    uint32_t sb[4];
+#pragma unroll
+                    for (int cj = 0; cj < 4; ++cj)
+                        sb[cj] = stg + ((static_cast<uint32_t>((lane >> 3) ^ cj)) << 4) + ((lane * 2) & 15);
+#pragma unroll 1
+                    for (int c = 0; c < TT / 32; ++c) {
+                        uint32_t v[32];
+                        tmem_ld_32x32b_x32(t_addr + c * 32, v);
+                        if (lane == 0) tma_store_wait_read<0>();   // previous block left the staging buffer
+                        tmem_wait_ld();
+                        __syncwarp();
+#pragma unroll
+                        for (int j = 0; j < 32; j += 2) {
+                            float y0 = __uint_as_float(v[j]) + bv, y1 = __uint_as_float(v[j + 1]) + bv;
+                            if (GELU) gelu_erf2(y0, y1);
+                            const uint16_t h0 = __bfloat16_as_ushort(__float2bfloat16_rn(y0));
+                            const uint16_t h1 = __bfloat16_as_ushort(__float2bfloat16_rn(y1));
+                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(sb[(j >> 1) & 3] + j * 64), "h"(h0) : "memory");
+                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(sb[(j >> 1) & 3] + (j + 1) * 64), "h"(h1) : "memory");
+                        }
+                        fence_proxy_async_smem();
+                        __syncwarp();
+                        if (lane == 0) {
+                            tma_store_2d(&tmY, stg, n0 + q * 32, t0 + c * 32);
+                            tma_store_commit();
+                        }
+                    }
+                } else {
 #pragma unroll 1
                 for (int c = 0; c < TT / 32; ++c) {
                     if (lane == 0) tma_store_wait_read<0>();   // previous block left the staging buffer
@@ -471,14 +506,8 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                             const int j = gq * 8 + jj;         // token row inside the block
                             float y = __uint_as_float(v[jj]) + bv;
                             if (GELU) y = gelu_erf(y);
-                            if (p.out_t == ARIA_BF16) {
-                                const uint32_t off = j * 64 + ((((lane * 2) >> 4) ^ ((j >> 1) & 3)) << 4) + ((lane * 2) & 15);
-                                const uint16_t h = __bfloat16_as_ushort(__float2bfloat16_rn(y));
-                                asm volatile("st.shared.u16 [%0], %1;" ::"r"(stg + off), "h"(h) : "memory");
-                            } else {
-                                const uint32_t off = j * 128 + ((((lane * 4) >> 4) ^ (j & 7)) << 4) + ((lane * 4) & 15);
-                                asm volatile("st.shared.f32 [%0], %1;" ::"r"(stg + off), "f"(y) : "memory");
-                            }
+                            const uint32_t off = j * 128 + ((((lane * 4) >> 4) ^ (j & 7)) << 4) + ((lane * 4) & 15);
+                            asm volatile("st.shared.f32 [%0], %1;" ::"r"(stg + off), "f"(y) : "memory");
                         }
                     }
                     fence_proxy_async_smem();
@@ -487,6 +516,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                         tma_store_2d(&tmY, stg, n0 + q * 32, t0 + c * 32);
                         tma_store_commit();
                     }
+                }
                 }
                 tc_fence_before();
                 __syncwarp();
