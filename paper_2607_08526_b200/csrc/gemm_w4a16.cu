@@ -249,13 +249,20 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_g;
 
-    pdl_wait_prior_grid();
+    // Programmatic dependent launch: only the roles that touch activations wait for the previous grid
+    // -- the X producer before its first load, the epilogue warps before anything they store (which
+    // also keeps "this grid complete => every earlier grid complete": no CTA exits before its epilogue
+    // warps have waited).  The weight stream and the dequantisers depend on nothing the previous grid
+    // writes, so the first k-blocks are fetched and dequantised during its tail.
+    constexpr bool EARLY_W = CTAS == 1;
+    if (!EARLY_W) pdl_wait_prior_grid();
     pdl_launch_dependents();   // the next kernel may become resident now; it blocks in its own wait
     const long long t_start = clock64();
 
     // Producer / MMA warps: warp-uniform loops, one elected lane issues (see gemm_w8a8.cu).
     if (warp == 0) {
         // ------------------------------------------------------------ TMA producer: X
+        if (EARLY_W) pdl_wait_prior_grid();
         int stage = 0;
         uint32_t phase = 0;
         for (int u = unit0; u < num_units; u += unit_step) {
@@ -438,6 +445,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         }
     } else if (warp >= W4_EPI_WARP0) {
         // ------------------------------------------------------------ epilogue (warps 4..7)
+        if (EARLY_W) pdl_wait_prior_grid();
         const int q = warp & 3;
         int acc = 0;
         uint32_t acc_phase = 0;

@@ -121,18 +121,24 @@ def test_c4_m4096_sampled_rows(aria, oracle, K, N):
     assert rel_err(host_f32(y)[rows], ref0) <= 2e-2 and rel_err(host_f32(y)[rows], ref1) <= 2e-2
 
 
+@pytest.mark.parametrize("mode_name", ["w8a8", "w4a16"])
 @pytest.mark.parametrize("M", [200, 1024])
-def test_w8a8_stack_eager_equals_per_layer_calls(aria, M):
+def test_stack_eager_equals_per_layer_calls(aria, M, mode_name):
     """Eager (no graph) aria_denoiser_linears under programmatic dependent launch: every layer's
     output must be bit-identical to the same linear called on its own, also right after the output
-    buffers were cleared (a chained layer's quantiser that reads its input before the producing GEMM
-    has finished would see the cleared buffer) and with the overlapped S1 pass switched on."""
+    buffers were cleared (a chained layer that reads its input before the producing GEMM has
+    finished would see the cleared buffer) -- with the overlapped S1 pass (W8A8) and the weight
+    stream that starts before griddepcontrol.wait (W4A16) switched on."""
     from paper_2607_08526_b200.stack import LinearStack
-    st = LinearStack(aria.W8A8, M=M, n_blocks=2, shared_inputs=False)
+    mode = aria.W8A8 if mode_name == "w8a8" else aria.W4A16
+    st = LinearStack(mode, M=M, n_blocks=2, shared_inputs=False)
     refs, prev = [], None
     for s in st.specs:
         x = s["in"] if s["in"] is not None else prev
-        prev = aria.aria_linear_w8a8(x, s["wq"], s["w_scale"], s["bias"], s["act"], aria.BF16)
+        if mode == aria.W8A8:
+            prev = aria.aria_linear_w8a8(x, s["wq"], s["w_scale"], s["bias"], s["act"], aria.BF16)
+        else:
+            prev = aria.aria_linear_w4a16(x, s["wq"], s["w_scale"], s["bias"], s["act"], aria.BF16)
         torch.cuda.synchronize()
         refs.append(host_bits16(prev).copy())
     for _ in range(3):
