@@ -65,6 +65,7 @@ struct W8Params {
     int bias_t, act;
     int M, N, K;
     long long* prof;   // debug: per-CTA role timestamps (clock64), or nullptr
+    int dbg;           // debug experiments (ARIA_W8_DBG): 1 = no TMA stores, 2 = no staging stores either, 4 = no math
 };
 
 static long long* g_w8_prof = nullptr;
@@ -89,7 +90,7 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, ui
 template <int BN, int OUT_T, bool GELU, int NBUF>
 __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const float* swb, int cb, float sxv,
                                                uint32_t stg0, int& sbuf, int lane, const CUtensorMap* tmY,
-                                               int n0, int row0) {
+                                               int n0, int row0, int dbg = 0) {
     const uint32_t rowb = stg0 + sbuf * W8_STG_BYTES + lane * 64;
     const uint32_t xr = (lane >> 1) & 3;
     const bool first = OUT_T != 1 || (cb & 16) == 0;   // first group of a 64-byte block
@@ -124,6 +125,7 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
             for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[j]);
         }
     }
+    if (dbg & 2) return;
     if (first) {   // the TMA store issued NBUF blocks ago must have finished reading this block
         if (elect_one()) tma_store_wait_read<NBUF - 1>();
         __syncwarp();
@@ -140,7 +142,7 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
     if (last) {
         fence_proxy_async_smem();
         __syncwarp();
-        if (elect_one()) {
+        if (!(dbg & 1) && elect_one()) {
             tma_store_2d(tmY, stg0 + sbuf * W8_STG_BYTES, n0 + (OUT_T == 1 ? (cb & ~31) : cb), row0);
             tma_store_commit();
         }
@@ -356,9 +358,9 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 #pragma unroll 1
             for (; c < c_end; ++c) {
                 const int cn = c + 1;
-                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(va, swb, c * 32, sxv, stg0, sbuf, lane, &tmY, n0, row0);
+                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(va, swb, c * 32, sxv, stg0, sbuf, lane, &tmY, n0, row0, p.dbg);
                 if (cn < c_end) tmem_ld_32x32b_x16(t_addr + cn * 32, va);
-                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(vb, swb, c * 32 + 16, sxv, stg0, sbuf, lane, &tmY, n0, row0);
+                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(vb, swb, c * 32 + 16, sxv, stg0, sbuf, lane, &tmY, n0, row0, p.dbg);
                 if (cn < c_end) {
                     tmem_ld_32x32b_x16(t_addr + cn * 32 + 16, vb);
                     tmem_wait_ld_x16(va);
@@ -500,6 +502,7 @@ int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, co
     p.bias_t = ep.bias_t; p.act = ep.act;
     p.M = M; p.N = N; p.K = K;
     p.prof = g_w8_prof;
+    p.dbg = getenv("ARIA_W8_DBG") ? atoi(getenv("ARIA_W8_DBG")) : 0;
     const int um = W8_BM * ctas;
     const int tiles = ((M + um - 1) / um) * ((N + bn - 1) / bn);
     const int slots = sms / ctas;

@@ -122,9 +122,12 @@ struct WsParams {
     const WsLayer* layers;    // [n_layers]
     const WsConv* conv;       // [n_conv] (AF16)
     int n_conv, conv_chunks;
-    const int* sched;         // units (layer << 16 | tile), CTA b owns sched[sched_off[b] .. sched_off[b+1])
-    const int* sched_off;     // [grid + 1]
-    const int* sched_total;   // [grid] stages of each CTA
+    // Dense schedule: CTA b owns units sched[b * max_units .. + sched_cnt[b].x), each {layer << 16 | tile,
+    // stages of the unit}; sched_cnt[b] = {units, total stages}.  One load per unit, and the first
+    // unit's address depends on nothing: it is fetched at kernel entry, before the prologue's barrier.
+    const int2* sched;
+    const int2* sched_cnt;
+    int max_units;
     unsigned* done;           // [n_layers] completion counters + [n_layers] = CTAs done converting (zeroed before each launch)
     int n_layers, M;
     long long* prof;          // debug: per-CTA role timestamps (16 per CTA), or nullptr
@@ -279,19 +282,20 @@ __device__ __forceinline__ void mbar_wait_lean(uint32_t bar, uint32_t parity) {
 
 // Walks this CTA's unit list; every role runs an identical copy.
 struct UnitIter {
-    const int* sched;
+    const int2* sched;
     int i, end;
     int l, tile, sb0, sb1;
+    int2 pre;                 // the CTA's first unit, loaded at kernel entry
     bool first;
-    __device__ __forceinline__ UnitIter(const WsParams& p)
-        : sched(p.sched), i(p.sched_off[blockIdx.x]), end(p.sched_off[blockIdx.x + 1]), first(true) {}
+    __device__ __forceinline__ UnitIter(const WsParams& p, int2 cnt, int2 u0)
+        : sched(p.sched + static_cast<size_t>(blockIdx.x) * p.max_units), i(0), end(cnt.x), pre(u0), first(true) {}
     __device__ __forceinline__ bool valid() const { return i < end; }
-    __device__ __forceinline__ void locate(const WsParams& p) {   // call when valid()
-        const int e = __ldg(sched + i);
-        l = e >> 16;
-        tile = e & 0xFFFF;
+    __device__ __forceinline__ void locate(const WsParams&) {   // call when valid()
+        const int2 e = i == 0 ? pre : __ldg(sched + i);
+        l = e.x >> 16;
+        tile = e.x & 0xFFFF;
         sb0 = 0;
-        sb1 = p.layers[l].num_sb;
+        sb1 = e.y;
     }
     __device__ __forceinline__ void next() { ++i; first = false; }
 };
@@ -314,6 +318,17 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
+
+    // Start-up chain: the CTA's unit count / stage total and its first unit come from two independent
+    // loads issued here, and the producers prefetch the first layer's tensor maps, all while the
+    // barriers are initialised and tensor memory is allocated.
+    const int2 sched_cnt = __ldg(p.sched_cnt + blockIdx.x);
+    const int2 unit0 = __ldg(p.sched + static_cast<size_t>(blockIdx.x) * p.max_units);
+    if (lane == 0 && sched_cnt.x > 0) {
+        const WsLayer& L0 = p.layers[unit0.x >> 16];
+        if (warp == WS_WPROD_WARP) { tma_prefetch_desc(&L0.tmP); tma_prefetch_desc(&L0.tmS); }
+        if (warp == WS_XPROD_WARP) tma_prefetch_desc(&L0.tmX);
+    }
 
     if (warp == WS_XPROD_WARP && lane == 0) {
         for (int s = 0; s < WS_PS; ++s) {
@@ -344,6 +359,8 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_g;
     const long long t_start = clock64();
+    unsigned long long gt_start = 0;
+    if (PROF) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_start));
 
     if (AF16 && p.n_conv > 0 && warp < WS_XPROD_WARP) {
         // bf16 -> fp16 of the external inputs (exact for 2^-14 <= |x| <= 65504, saturating above,
@@ -406,7 +423,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         }
         int stage = 0;
         uint32_t phase = 0;
-        for (UnitIter it(p); it.valid(); it.next()) {
+        for (UnitIter it(p, sched_cnt, unit0); it.valid(); it.next()) {
             it.locate(p);
             const WsLayer& L = p.layers[it.l];
             if (L.dep >= 0 && !(p.dbg & 128)) {       // chained layer: the producer layer must be complete
@@ -436,7 +453,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         const uint64_t pol_w = policy_evict_first();
         int stage = 0;
         uint32_t phase = 0;
-        for (UnitIter it(p); it.valid(); it.next()) {
+        for (UnitIter it(p, sched_cnt, unit0); it.valid(); it.next()) {
             it.locate(p);
             const WsLayer& L = p.layers[it.l];
             const int n0 = it.tile * WS_ROWS;
@@ -463,7 +480,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         int xs = 0, slot = 0, acc = 0;
         uint32_t xphase = 0, aphase = 0, acc_phase = 0;
         long long w_t = 0, w_x = 0, w_a = 0;
-        for (UnitIter it(p); it.valid(); it.next()) {
+        for (UnitIter it(p, sched_cnt, unit0); it.valid(); it.next()) {
             it.locate(p);
             WS_TIMED(w_t, mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1));
             tc_fence_after();
@@ -519,7 +536,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         const uint32_t sa = sS + r * 16 + g * 4;
         const uint32_t a_base = tmem_base + WS_A_COL0 + g * 32 + (static_cast<uint32_t>(q * 32) << 16);
         const uint32_t z_base = tmem_base + WS_A_COL0 + 128 + g * 2 + (static_cast<uint32_t>(q * 32) << 16);
-        const int total = __ldg(p.sched_total + blockIdx.x);      // stages of this CTA
+        const int total = sched_cnt.y;            // stages of this CTA
         uint4 pk0 = make_uint4(0, 0, 0, 0), pk1 = pk0;
         uint32_t sc2 = 0;
         if (total > 0) {
@@ -615,7 +632,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         const int q = warp & 3;
         int acc = 0;
         uint32_t acc_phase = 0;
-        for (UnitIter it(p); it.valid(); it.next()) {
+        for (UnitIter it(p, sched_cnt, unit0); it.valid(); it.next()) {
             it.locate(p);
             // layer fields into registers FIRST: the compiler must assume the output stores below may
             // alias the layer table and would otherwise re-load them from L2 after every store
@@ -732,7 +749,14 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             }
             if (q == 0 && lane == 0 && it.first) WS_STAMP(7);
         }
-        if (q == 0 && lane == 0) WS_STAMP(8);
+        if (q == 0 && lane == 0) {
+            WS_STAMP(8);
+            if (PROF && p.prof) {      // slot 15: the same interval in ns (globaltimer) -> SM clock of this run
+                unsigned long long gt;
+                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+                p.prof[blockIdx.x * 16 + 15] = static_cast<long long>(gt - gt_start);
+            }
+        }
     }
 
     tc_fence_before();
@@ -752,7 +776,7 @@ namespace aria {
 struct WsPlan {
     bool a_f16 = true;
     WsLayer* d_layers = nullptr;
-    int* d_sched = nullptr;         // unit lists + offsets
+    int2* d_sched = nullptr;        // dense unit lists + per-CTA counts
     unsigned* d_done = nullptr;
     size_t done_bytes = 0;
     WsConv* d_conv = nullptr;
@@ -939,22 +963,23 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
             load[best] += unit_cost(h[i]);
             totals[best] += h[i].num_sb;
         }
-    std::vector<int> sched;
-    std::vector<int> off(grid + 1, 0);
+    size_t max_units = 1;
+    for (int c = 0; c < grid; ++c) max_units = lists[c].size() > max_units ? lists[c].size() : max_units;
+    std::vector<int2> sched(static_cast<size_t>(grid) * max_units, make_int2(0, 0));
+    std::vector<int2> cnt(grid);
     for (int c = 0; c < grid; ++c) {
-        off[c] = static_cast<int>(sched.size());
-        sched.insert(sched.end(), lists[c].begin(), lists[c].end());
+        for (size_t i = 0; i < lists[c].size(); ++i)
+            sched[c * max_units + i] = make_int2(lists[c][i], h[lists[c][i] >> 16].num_sb);
+        cnt[c] = make_int2(static_cast<int>(lists[c].size()), totals[c]);
     }
-    off[grid] = static_cast<int>(sched.size());
     const size_t sched_n = sched.size();
-    sched.insert(sched.end(), off.begin(), off.end());
-    sched.insert(sched.end(), totals.begin(), totals.end());
+    sched.insert(sched.end(), cnt.begin(), cnt.end());
     plan->done_bytes = (static_cast<size_t>(n_layers) + 1) * sizeof(unsigned);
     if (cudaMalloc(&plan->d_layers, h.size() * sizeof(WsLayer)) != cudaSuccess ||
-        cudaMalloc(&plan->d_sched, sched.size() * sizeof(int)) != cudaSuccess ||
+        cudaMalloc(&plan->d_sched, sched.size() * sizeof(int2)) != cudaSuccess ||
         cudaMalloc(&plan->d_done, plan->done_bytes) != cudaSuccess ||
         cudaMemcpy(plan->d_layers, h.data(), h.size() * sizeof(WsLayer), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(plan->d_sched, sched.data(), sched.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(plan->d_sched, sched.data(), sched.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess ||
         (!conv.empty() && (cudaMalloc(&plan->d_conv, conv.size() * sizeof(WsConv)) != cudaSuccess ||
                            cudaMemcpy(plan->d_conv, conv.data(), conv.size() * sizeof(WsConv), cudaMemcpyHostToDevice) != cudaSuccess))) {
         ws_plan_destroy(plan);
@@ -962,8 +987,8 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     }
     plan->params.layers = plan->d_layers;
     plan->params.sched = plan->d_sched;
-    plan->params.sched_off = plan->d_sched + sched_n;
-    plan->params.sched_total = plan->d_sched + sched_n + grid + 1;
+    plan->params.sched_cnt = plan->d_sched + sched_n;
+    plan->params.max_units = static_cast<int>(max_units);
     plan->params.done = plan->d_done;
     plan->params.conv = plan->d_conv;
     plan->params.n_conv = static_cast<int>(conv.size());
