@@ -949,8 +949,13 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
             ++n_placed;
         }
     }
-    // cost of a unit in quarter stages: its stages + ~1/4 stage of accumulator hand-off
-    auto unit_cost = [&](const WsLayer& w) { return 4 * w.num_sb + 1; };
+    // cost of a unit in quarter stages: its stages, ~1/4 stage of accumulator hand-off, and the issue
+    // slots a GELU / fp16-copy epilogue takes from the dequantisers of its SM
+    const char* ec = getenv("ARIA_WS_EPI_COST");
+    const int epi_cost = ec ? atoi(ec) : 1;
+    auto unit_cost = [&](const WsLayer& w) {
+        return 4 * w.num_sb + 1 + ((w.act == ARIA_ACT_GELU_ERF ? 1 : 0) + (w.notify ? 1 : 0)) * epi_cost;
+    };
     std::vector<std::vector<int>> lists(grid);
     std::vector<long> load(grid, 0);
     std::vector<int> totals(grid, 0);
