@@ -534,52 +534,76 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 }
             } else {
                 float* part = p.partials + static_cast<int64_t>(sp) * p.M * p.N;
+                float* prow = part + static_cast<int64_t>(t0) * p.N + n;
+                const int tleft = p.M - t0;
 #pragma unroll 1
-                for (int c8 = 0; c8 < TT / 8; ++c8) {
-                    uint32_t v[8];
-                    tmem_ld_32x32b_x8(t_addr + c8 * 8, v);
+                for (int c = 0; c < TT / 32; ++c) {
+                    uint32_t v[32];
+                    tmem_ld_32x32b_x32(t_addr + c * 32, v);
                     tmem_wait_ld();
+                    if (n_ok) {
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const int tok = t0 + c8 * 8 + j;
-                        if (n_ok && tok < p.M)
-                            __stcg(part + static_cast<int64_t>(tok) * p.N + n, __uint_as_float(v[j]));
+                        for (int j = 0; j < 32; ++j)
+                            if (c * 32 + j < tleft) __stcg(prow + static_cast<int64_t>(c * 32 + j) * p.N, __uint_as_float(v[j]));
                     }
                 }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(tempty0 + 8 * acc);
-                // last arriver of this (tile, quarter) reduces in split order
+                // Reduction, spread over the splits: every split's warp publishes its partials, waits until
+                // all S splits of this (tile, quarter) have published, and then reduces ITS share of the
+                // tile's tokens (a contiguous 1/S) in fixed split order -- deterministic, and S times more
+                // warps than a last-arriver reduction (measured: that took 48 of 58 us at 512 x 6144 -> 1536
+                // with 6 splits).  No deadlock: the S units of a tile are consecutive unit indices, hence
+                // on S different CTAs, each of which has finished every smaller unit it owns before it
+                // gets here; a unit's mainloop and partial stores wait for nobody.
                 __threadfence();
                 __syncwarp();
-                unsigned old = 0;
-                if (lane == 0) old = atomicAdd(p.counters + tile * 4 + q, 1u);
-                old = __shfl_sync(0xffffffffu, old, 0);
-                if (old == static_cast<unsigned>(S - 1)) {
-                    __threadfence();
-                    const int tmax = min(TT, p.M - t0);
-                    const int64_t sstride = static_cast<int64_t>(p.M) * p.N;
-                    for (int j0 = 0; j0 < tmax; j0 += 16) {  // 16 tokens x 2 splits = 32 loads in flight
-                        float y[16];
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) y[j] = 0.0f;
-                        for (int s = 0; s < S; s += 2) {     // fixed split order: deterministic sum
-                            float a[16], b[16];
-                            const bool two = s + 1 < S;
-#pragma unroll
-                            for (int j = 0; j < 16; ++j) {
-                                const int64_t idx = static_cast<int64_t>(t0 + j0 + j) * p.N + n;
-                                const bool ok = n_ok && j0 + j < tmax;
-                                a[j] = ok ? __ldcg(p.partials + s * sstride + idx) : 0.0f;
-                                b[j] = ok && two ? __ldcg(p.partials + (s + 1) * sstride + idx) : 0.0f;
+                if (lane == 0) {
+                    unsigned* cnt = p.counters + tile * 4 + q;
+                    atomicAdd(cnt, 1u);
+                    const long long t_spin = clock64();
+                    unsigned seen;
+                    do {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
+                        if (seen < static_cast<unsigned>(S)) {
+                            __nanosleep(100);
+                            if (clock64() - t_spin > 4000000000LL) {
+                                printf("aria: split-K watchdog (block %d tile %d)\n", blockIdx.x, tile);
+                                __trap();
                             }
+                        }
+                    } while (seen < static_cast<unsigned>(S));
+                }
+                __syncwarp();
+                __threadfence();
+                {
+                    const int tmax = min(TT, p.M - t0);
+                    const int j_beg = (sp * tmax) / S, j_end = ((sp + 1) * tmax) / S;
+                    const int64_t sstride = static_cast<int64_t>(p.M) * p.N;
+                    for (int j0 = j_beg; j0 < j_end; j0 += 8) {   // 8 tokens x 4 splits = 32 loads in flight
+                        float y[8];
 #pragma unroll
-                            for (int j = 0; j < 16; ++j) y[j] = (y[j] + a[j]) + b[j];
+                        for (int j = 0; j < 8; ++j) y[j] = 0.0f;
+                        for (int s = 0; s < S; s += 4) {          // fixed split order: deterministic sum
+                            float a[4][8];
+#pragma unroll
+                            for (int ss = 0; ss < 4; ++ss)
+#pragma unroll
+                                for (int j = 0; j < 8; ++j) {
+                                    const int64_t idx = static_cast<int64_t>(t0 + j0 + j) * p.N + n;
+                                    const bool ok = n_ok && j0 + j < j_end && s + ss < S;
+                                    a[ss][j] = ok ? __ldcg(p.partials + (s + ss) * sstride + idx) : 0.0f;
+                                }
+#pragma unroll
+                            for (int ss = 0; ss < 4; ++ss)
+#pragma unroll
+                                for (int j = 0; j < 8; ++j) y[j] += a[ss][j];
                         }
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) {
+                        for (int j = 0; j < 8; ++j) {
                             const int64_t idx = static_cast<int64_t>(t0 + j0 + j) * p.N + n;
-                            if (n_ok && j0 + j < tmax) w4_store(p.Y, p.out_t, idx, GELU ? gelu_erf(y[j] + bv) : y[j] + bv);
+                            if (n_ok && j0 + j < j_end) w4_store(p.Y, p.out_t, idx, GELU ? gelu_erf(y[j] + bv) : y[j] + bv);
                         }
                     }
                 }
