@@ -193,3 +193,29 @@ def test_graph_replay_of_a_plan_is_bit_stable(aria, oracle):
                 assert np.array_equal(r, host_bits16(s["out"]))
     finally:
         aria.aria_stack_plan_destroy(plan)
+
+
+def test_c5_stack_m32_full_size_as_benched(aria, oracle):
+    """The workload bench.py's `small_m.c5_stack_m32` times: all 96 layers of config C5 at M = 32 as ONE
+    persistent launch (graph replay), every 5th layer plus the chained down-projections of the first
+    and last block checked against the oracle (variant 3; chained layers teacher-forced)."""
+    from paper_2607_08526_b200.stack import LinearStack
+    st = LinearStack(aria.W4A16, M=32, keep_host=True, shared_inputs=True, use_plan=True)
+    assert len(st.specs) == 96 and aria.aria_stack_plan_is_streaming(st.plan)
+    st.capture()
+    for s in st.specs:
+        s["out"].zero_()
+    st.replay()
+    torch.cuda.synchronize()
+    first = [host_bits16(s["out"]).copy() for s in st.specs]
+    picked = sorted(set(range(0, 96, 5)) | {3, 95})
+    for i in picked:
+        spec, h = st.specs[i], st.host[i]
+        x = inputs.bf16_as_f32(first[i - 1]) if spec["in"] is None else inputs.bf16_as_f32(h["X_bits"])
+        codes, sg, _ = oracle.quant_int4_groups(h["W"])
+        host = {"codes": codes, "sg": sg, "b": h["b"].astype(np.float64), "act": spec["act"]}
+        _check(oracle, host, x, first[i], 3)
+    st.replay()                                   # replays are bit-identical
+    torch.cuda.synchronize()
+    for a, s in zip(first, st.specs):
+        assert np.array_equal(a, host_bits16(s["out"]))
