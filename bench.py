@@ -371,8 +371,8 @@ def run_ours(args):
                 "frac_of_burst": ach / (pk["bf16_burst"] * NOMINAL_INT8_OVER_BF16),
                 "frac_of_nominal_4500": ach / 4500.0, "avg_launch_us": dur * 1e6, "launches": n_l,
                 # dram__bytes_read.sum + dram__bytes_write.sum per launch, mean of the 4 consecutive layers
-                # captured with `ncu --set full` in profiles/r1b_w8a8_full.md (10.28, 5.54, 12.66, 22.06 MB)
-                "traffic": 12.64e6, "traffic_unit": "bytes/launch (ncu, profiles/r1b_w8a8_full.md)"}
+                # captured with `ncu --set full` in profiles/r1c_w8a8_full.md (10.28, 5.54, 12.66, 22.06 MB)
+                "traffic": 12.64e6, "traffic_unit": "bytes/launch (ncu, profiles/r1c_w8a8_full.md)"}
 
     # ---- roofline of the DOMINANT kernel of the step: w4a16_gemm_kernel (0.63 of the step in the ncu
     # launch list profiles/r1c_launches.md, 0.65 by the live events below).  The W4A16 half of the step
