@@ -66,7 +66,7 @@ def test_c4_shapes(aria, oracle, M, K, N):
 
 
 @pytest.mark.parametrize("M,K,N", [(1, 32, 8), (17, 96, 40), (33, 160, 136), (64, 256, 128), (100, 1536, 264),
-                                   (129, 192, 128), (300, 416, 392)])
+                                   (129, 192, 128), (300, 416, 392), (2000, 256, 1536)])  # last: TT = 192 tiles, ragged token tail
 def test_ragged_shapes(aria, oracle, M, K, N):
     _case(aria, oracle, M, K, N, bias=(M % 2 == 1))
 
