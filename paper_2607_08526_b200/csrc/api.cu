@@ -78,6 +78,32 @@ int run_layer(const aria_layer& L, const void* in, void* out, int M, int mode, i
 
 }  // namespace
 
+// Copy streams and events of aria_denoiser_linears_host, created once per device.
+struct HostPipe {
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr},
+                ev_out[2] = {nullptr, nullptr};
+    bool ok = false;
+};
+static HostPipe* host_pipe() {
+    static HostPipe pipes[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    HostPipe& h = pipes[dev];
+    if (!h.ok) {
+        bool good = cudaStreamCreateWithFlags(&h.s_in, cudaStreamNonBlocking) == cudaSuccess &&
+                    cudaStreamCreateWithFlags(&h.s_out, cudaStreamNonBlocking) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&h.ev_start, cudaEventDisableTiming) == cudaSuccess;
+        for (int i = 0; good && i < 2; ++i)
+            good = cudaEventCreateWithFlags(&h.ev_in[i], cudaEventDisableTiming) == cudaSuccess &&
+                   cudaEventCreateWithFlags(&h.ev_comp[i], cudaEventDisableTiming) == cudaSuccess &&
+                   cudaEventCreateWithFlags(&h.ev_out[i], cudaEventDisableTiming) == cudaSuccess;
+        if (!good) return nullptr;
+        h.ok = true;
+    }
+    return &h;
+}
+
 struct aria_stack_plan {
     std::vector<aria_layer> layers;
     int M = 0, mode = 0, io = 0;
@@ -307,26 +333,46 @@ int aria_denoiser_linears_host(const aria_layer* layers, int n_layers, int M, in
     uint8_t* base = static_cast<uint8_t*>(ws);
     uint8_t* in_stage[2] = {base + dev, base + dev + in_b};
     uint8_t* out_stage[2] = {base + dev + 2 * in_b, base + dev + 2 * in_b + out_b};
-    // One stream, in order: H2D(in_i) -> layer_i -> D2H(out_i).  Staging buffers alternate so a
-    // chained layer (in == NULL) can read the previous layer's device output.
-    for (int i = 0; i < n_layers; ++i) {
+    // Three streams: H2D(in_i) on a copy-in stream, layer_i on the caller's stream, D2H(out_i) on a
+    // copy-out stream, chained by events, so the (full-duplex) PCIe copies of neighbouring layers overlap
+    // each other and the compute.  Two staging buffers per direction: in_stage[b] is rewritten by
+    // H2D(i+2) only after layer i has run, out_stage[b] by layer i+2 only after D2H(i) has read it; a
+    // chained layer (in == NULL) reads the previous layer's device output on the compute stream.
+    HostPipe* hp = host_pipe();
+    if (!hp) return ARIA_ERR_CUDA;
+    bool ok = cudaEventRecord(hp->ev_start, st) == cudaSuccess &&
+              cudaStreamWaitEvent(hp->s_in, hp->ev_start, 0) == cudaSuccess &&
+              cudaStreamWaitEvent(hp->s_out, hp->ev_start, 0) == cudaSuccess;
+    for (int i = 0; ok && i < n_layers; ++i) {
         const aria_layer& L = layers[i];
+        const int b = i & 1;
         const void* din;
         if (L.in) {
-            if (cudaMemcpyAsync(in_stage[i & 1], L.in, static_cast<size_t>(M) * L.K * dsize(io),
-                                cudaMemcpyHostToDevice, st) != cudaSuccess)
-                return ARIA_ERR_CUDA;
-            din = in_stage[i & 1];
+            if (i >= 2) ok = ok && cudaStreamWaitEvent(hp->s_in, hp->ev_comp[b], 0) == cudaSuccess;
+            ok = ok && cudaMemcpyAsync(in_stage[b], L.in, static_cast<size_t>(M) * L.K * dsize(io),
+                                       cudaMemcpyHostToDevice, hp->s_in) == cudaSuccess &&
+                 cudaEventRecord(hp->ev_in[b], hp->s_in) == cudaSuccess &&
+                 cudaStreamWaitEvent(st, hp->ev_in[b], 0) == cudaSuccess;
+            din = in_stage[b];
         } else {
             din = out_stage[(i - 1) & 1];
         }
-        rc = run_layer(L, din, out_stage[i & 1], M, mode, io, ws, dev, st);
-        if (rc != ARIA_OK) return rc;
-        if (cudaMemcpyAsync(L.out, out_stage[i & 1], static_cast<size_t>(M) * L.N * dsize(io),
-                            cudaMemcpyDeviceToHost, st) != cudaSuccess)
-            return ARIA_ERR_CUDA;
+        if (i >= 2) ok = ok && cudaStreamWaitEvent(st, hp->ev_out[b], 0) == cudaSuccess;
+        if (!ok) break;
+        rc = run_layer(L, din, out_stage[b], M, mode, io, ws, dev, st);
+        if (rc != ARIA_OK) break;
+        ok = cudaEventRecord(hp->ev_comp[b], st) == cudaSuccess &&
+             cudaStreamWaitEvent(hp->s_out, hp->ev_comp[b], 0) == cudaSuccess &&
+             cudaMemcpyAsync(L.out, out_stage[b], static_cast<size_t>(M) * L.N * dsize(io),
+                             cudaMemcpyDeviceToHost, hp->s_out) == cudaSuccess &&
+             cudaEventRecord(hp->ev_out[b], hp->s_out) == cudaSuccess;
     }
-    return cudaStreamSynchronize(st) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    // always drain all three streams, also on an error path: the staging buffers are the caller's
+    const bool s1 = cudaStreamSynchronize(hp->s_in) == cudaSuccess;
+    const bool s2 = cudaStreamSynchronize(st) == cudaSuccess;
+    const bool s3 = cudaStreamSynchronize(hp->s_out) == cudaSuccess;
+    if (rc != ARIA_OK) return rc;
+    return ok && s1 && s2 && s3 ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
 }  // extern "C"
