@@ -156,7 +156,8 @@ ARIA_API void aria_stack_plan_destroy(aria_stack_plan* plan);
  * each layer's input is copied host->device into `ws`, the layer runs, and its output is
  * copied device->host.  The copies run on two library-owned copy streams chained to `stream` by
  * events (double-buffered staging in `ws`), so the H2D / D2H transfers of neighbouring layers
- * overlap each other and the compute; the call returns after synchronising all three streams.  Weights, scales and
+ * overlap each other and the compute; the call returns after synchronising all three streams
+ * (the copy streams are per device and shared by all calls: one _host call at a time per device).  Weights, scales and
  * biases stay DEVICE pointers (the compressed copy is resident).  ws must hold
  * aria_workspace_bytes_host(...) bytes.  Not capturable.                                    */
 ARIA_API int aria_denoiser_linears_host(const aria_layer* layers, int n_layers, int M, int mode, int io,
