@@ -101,7 +101,12 @@ ARIA_API int aria_linear_w8a8_q(const int8_t* Xq, const float* x_scale, int M, i
 /* S4 -- one W4A16 linear (config C4; reading R12):  w^[n,k] = bf16_rne(q[n,k] * sg[n,k/32])
  * dequantised on chip;  y = sum_k x[m,k] w^[n,k] (fp32 accumulate, tcgen05 kind::f16 bf16)
  * + bias[n]; optional GELU; Y = cast(y, yt).  X: bf16 [M,K].  Wq4/g_scale: canonical format
- * of aria_quantize_weights_int4.  bias: bf16 [N] or NULL.  ws may be NULL (unused).          */
+ * of aria_quantize_weights_int4.  bias: bf16 [N] or NULL.
+ * ws: scratch for the split-K schedule that small-M shapes use to fill the GPU (fp32 partial sums +
+ * tile counters, aria_workspace_bytes(M, K, N, ARIA_W4A16) bytes).  ws == NULL or a smaller ws is
+ * accepted and selects the schedule WITHOUT split-K: same results within fp32 summation order,
+ * but shapes with fewer than #SMs tiles (M <= 512 on a 6144 -> 1536 layer) then run several times
+ * slower.  With split-K the kernel's CTAs wait on one another: see "Co-residency" below.          */
 ARIA_API int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uint16_t* g_scale,
                       int group, int N, const void* bias, int act, void* Y, int yt, void* ws,
                       size_t ws_bytes, void* stream);
@@ -113,7 +118,10 @@ ARIA_API int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, 
  * [N]; mode W4A16: wq = packed int4 [N,K/2], w_scale = fp16 bits [N,K/32].  bias has dtype `io`,
  * may be NULL.  Capturable: enqueue only.  Mode W8A8: the S1 pass of a layer whose input the
  * previous layer does not write is overlapped with that layer's GEMM (programmatic dependent
- * launch, two alternating Xq / sx buffers in `ws`); results are those of array order.         */
+ * launch, two alternating Xq / sx buffers in `ws`); a layer whose output IS the next layer's input
+ * (in == NULL, or in == the previous out) reduces the per-token absmax of what it stores in its own
+ * epilogue, and the consumer's S1 pass only rounds (north_star: "activation-quantization pass fused
+ * into the previous epilogue"); codes, scales and results are those of array order, bit for bit.   */
 typedef struct {
     int K, N;
     int act; /* aria_act applied to this layer's output */
@@ -133,23 +141,44 @@ ARIA_API int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M
  * may synchronise and is not capturable.  The plan keeps the layers' device pointers (weights,
  * scales, biases, in/out buffers), which must stay valid until aria_stack_plan_destroy.
  * aria_stack_plan_run only ENQUEUES one step on `stream` (capturable) and computes
- * exactly what aria_denoiser_linears computes for the same list.  For mode W4A16 with M <= 32,
- * bf16 I/O, every K % 256 == 0 and no output buffer overlapping another output or an earlier
- * input, the step is ONE persistent weight-streaming kernel over all layers (HBM bound; layers
- * whose input is not an earlier layer's output may overlap, results are identical to array
- * order); there the dequantised weight is w^ = fp16_rn((q + 8) * sg) - 8 * sg (offset-binary
- * code scaled and rounded to fp16, zero point subtracted exactly by an extra tensor-core k-step;
- * activations enter the same tcgen05 kind::f16 MMA as fp16, exact for 2^-14 <= |x| <= 65504;
- * needs sg <= 63; reading R12c), or bf16_rne(q * sg) as in aria_linear_w4a16 when the
- * environment variable ARIA_W4_F16A=0 is set at plan creation.
- * Any other list runs the per-layer path.  A plan's scratch serves ONE step at a time: do not
- * run the same plan concurrently on two streams.  aria_stack_plan_is_streaming: 1 if the plan
- * uses the stream kernel.                                                                   */
+ * the same linears in array order as aria_denoiser_linears, within the same tolerances (S4:
+ * <= 2e-2 of max|y| against the definition with w^ = bf16_rne(q*sg) and with w^ = q*sg).
+ *
+ * For mode W4A16 with M <= 32, bf16 I/O, every K % 256 == 0, no output buffer overlapping another
+ * output or an earlier input, and every input that touches an earlier output being exactly that
+ * output, the step is ONE persistent weight-streaming kernel over all layers (HBM bound; layers
+ * whose input is not an earlier layer's output may overlap).  Operand format there:
+ *  - fp16 (aria_stack_plan_is_streaming == 1): w^ = fp16_rn((q + 8) * sg) - 8 * sg (offset-binary code
+ *    scaled and rounded to fp16; the zero point is subtracted exactly by an extra tensor-core k-step)
+ *    and the bf16 activations enter the same tcgen05 kind::f16 MMA converted to fp16.  Chosen at plan
+ *    creation iff every group scale satisfies 1024 * sg <= 65504 (the scales are scanned once).  The
+ *    ACTIVATIONS are checked on the device in every run: if any |x| or any 32-k group sum of x exceeds
+ *    65504 (external inputs and chained outputs alike), or a whole input tensor has 0 < max|x| < 2^-7
+ *    (fp16 subnormals would cost relative precision), the run raises a device flag and a second,
+ *    otherwise empty launch recomputes the WHOLE list with exact bf16 operands (next item).  So every
+ *    input aria_linear_w4a16 accepts gives results within the tolerances above; out-of-range inputs
+ *    only cost time.  aria_stack_plan_fallback_fired reports whether the last run did that.
+ *  - bf16 (aria_stack_plan_is_streaming == 2): w^ = bf16_rne(q * sg) and bf16 activations, exactly as
+ *    aria_linear_w4a16.  Chosen when a scale fails the test above.
+ * Any other list runs the per-layer path (aria_stack_plan_is_streaming == 0).  A plan's scratch serves
+ * ONE step at a time: do not run the same plan concurrently on two streams.
+ *
+ * Co-residency.  The stream kernel's CTAs (and those of aria_linear_w4a16 with split-K) wait on
+ * completion counters written by other CTAs of the same grid.  The stream kernel is therefore a
+ * COOPERATIVE launch of at most one CTA per SM: if the device cannot hold the grid at once the launch
+ * fails with ARIA_ERR_CUDA instead of deadlocking.  Do not run two plans, or a plan and a split-K
+ * linear, concurrently on different streams of one device.
+ *
+ * aria_stack_plan_fallback_fired: SYNCHRONOUS (copies one word from the device after the stream's work
+ * has been synchronised by the caller); *fired = 0 if the last run stayed in the fp16 domain, else a
+ * bit mask (1 = a value above the fp16 range, 2 = an input tensor below 2^-7).  Always 0 for plans that
+ * do not use fp16 operands.                                                                        */
 typedef struct aria_stack_plan aria_stack_plan;
 ARIA_API int aria_stack_plan_create(const aria_layer* layers, int n_layers, int M, int mode, int io,
                                     aria_stack_plan** plan);
 ARIA_API int aria_stack_plan_run(const aria_stack_plan* plan, void* stream);
 ARIA_API int aria_stack_plan_is_streaming(const aria_stack_plan* plan);
+ARIA_API int aria_stack_plan_fallback_fired(const aria_stack_plan* plan, int* fired);
 ARIA_API void aria_stack_plan_destroy(aria_stack_plan* plan);
 
 /* Same stack, but `in` / `out` of every layer are HOST pointers (pinned memory recommended):
@@ -174,6 +203,14 @@ ARIA_API const char* aria_status_string(int status);
  * [M,N], computed by the same tcgen05 kind::i8 kernel as aria_linear_w8a8.                   */
 ARIA_API int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, int32_t* acc,
                      void* stream);
+
+/* Host-only introspection of the launch plans (no device needed; used by the tests to prove that
+ * every compiled tile variant is reached): the (BN, CTAS) tile of the W8A8 GEMM for an [M,N] output on
+ * a device with `sms` SMs (BN in {64,128,192,256} output channels, CTAS = 2: tcgen05 cta_group::2
+ * pairs computing 256 x BN), and the (token tile TT in {32,64,128,192,256}, split-K factor) of the
+ * W4A16 GEMM.                                                                                      */
+ARIA_API int aria_w8a8_tile_plan(int M, int N, int sms, int* bn, int* ctas);
+ARIA_API int aria_w4a16_tile_plan(int M, int N, int K, int sms, int* tt, int* splits);
 
 /* Library build id ("aria-b200 <version> sm_100a"). */
 ARIA_API const char* aria_version(void);

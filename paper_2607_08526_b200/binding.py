@@ -64,6 +64,9 @@ def lib() -> ctypes.CDLL:
                                              ctypes.POINTER(c_void_p)]
         L.aria_stack_plan_run.argtypes = [c_void_p, c_void_p]
         L.aria_stack_plan_is_streaming.argtypes = [c_void_p]
+        L.aria_stack_plan_fallback_fired.argtypes = [c_void_p, ctypes.POINTER(c_int)]
+        L.aria_w8a8_tile_plan.argtypes = [c_int, c_int, c_int, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
+        L.aria_w4a16_tile_plan.argtypes = [c_int, c_int, c_int, c_int, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
         L.aria_stack_plan_destroy.argtypes = [c_void_p]
         L.aria_stack_plan_destroy.restype = None
         for name in EXPORTS:
@@ -78,7 +81,8 @@ EXPORTS = ("aria_linear_w8a8_q", "aria_quantize_weights_int8", "aria_quantize_we
            "aria_linear_w8a8", "aria_linear_w4a16", "aria_denoiser_linears",
            "aria_denoiser_linears_host", "aria_workspace_bytes", "aria_workspace_bytes_host",
            "aria_status_string", "aria_gemm_i8_i32", "aria_version", "aria_stack_plan_create",
-           "aria_stack_plan_run", "aria_stack_plan_is_streaming", "aria_stack_plan_destroy")
+           "aria_stack_plan_run", "aria_stack_plan_is_streaming", "aria_stack_plan_destroy",
+           "aria_stack_plan_fallback_fired", "aria_w8a8_tile_plan", "aria_w4a16_tile_plan")
 
 
 def _check(rc: int, what: str):
@@ -231,8 +235,29 @@ def aria_stack_plan_run(plan: c_void_p):
     _check(lib().aria_stack_plan_run(plan, _stream()), "aria_stack_plan_run")
 
 
-def aria_stack_plan_is_streaming(plan: c_void_p) -> bool:
-    return bool(lib().aria_stack_plan_is_streaming(plan))
+def aria_stack_plan_is_streaming(plan: c_void_p) -> int:
+    """0: per-layer path; 1: stream kernel, fp16 operands (+ armed bf16 fallback); 2: stream kernel, bf16."""
+    return int(lib().aria_stack_plan_is_streaming(plan))
+
+
+def aria_stack_plan_fallback_fired(plan: c_void_p) -> int:
+    """Synchronises the device, then reads the last run's domain flag (0 = stayed in the fp16 domain)."""
+    torch.cuda.synchronize()
+    fired = c_int(0)
+    _check(lib().aria_stack_plan_fallback_fired(plan, ctypes.byref(fired)), "aria_stack_plan_fallback_fired")
+    return fired.value
+
+
+def aria_w8a8_tile_plan(M: int, N: int, sms: int = 148):
+    bn, ctas = c_int(0), c_int(0)
+    _check(lib().aria_w8a8_tile_plan(M, N, sms, ctypes.byref(bn), ctypes.byref(ctas)), "aria_w8a8_tile_plan")
+    return bn.value, ctas.value
+
+
+def aria_w4a16_tile_plan(M: int, N: int, K: int, sms: int = 148):
+    tt, s = c_int(0), c_int(0)
+    _check(lib().aria_w4a16_tile_plan(M, N, K, sms, ctypes.byref(tt), ctypes.byref(s)), "aria_w4a16_tile_plan")
+    return tt.value, s.value
 
 
 def aria_stack_plan_destroy(plan: c_void_p):

@@ -27,16 +27,33 @@ int check_rows_args(const void* in, int t, int R, int C, const void* q, const vo
 
 size_t w8_ws_bytes(int M, int K) { return up256(static_cast<size_t>(M) * K) + up256(static_cast<size_t>(M) * 4); }
 
+// Fused S1 (north_star "activation-quantization pass fused into the previous epilogue where shapes
+// allow"): a W8A8 layer whose output feeds the next W8A8 layer reduces the per-token absmax of what it
+// stores in its own epilogue (atomicMax into amax_out); the consumer's S1 pass then takes the row
+// maxima from amax_in and only rounds.  amax_zero: the buffer THIS layer's GEMM will reduce into, zeroed
+// by this layer's S1 pass (which always completes before that GEMM's epilogue).
+struct W8Fuse {
+    const float* amax_in = nullptr;
+    float* amax_zero = nullptr;
+    float* amax_out = nullptr;
+};
+
+// pdl_first: whether the FIRST kernel of this linear may be launched as a programmatic dependent of
+// whatever precedes it on the stream (only inside a chain this library enqueued itself: the kernels of
+// a chain all execute griddepcontrol.wait before they exit, a foreign kernel gives no such guarantee).
 int linear_w8a8_impl(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
                      int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
-                     cudaStream_t st, bool pdl, bool early = false) {
+                     cudaStream_t st, bool pdl_first, bool pdl, bool early = false,
+                     const W8Fuse& fuse = W8Fuse()) {
     int8_t* Xq = static_cast<int8_t*>(ws);
     float* sx = reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + up256(static_cast<size_t>(M) * K));
-    int rc = launch_quant_rows_i8(X, xt, M, K, Xq, sx, st, pdl, early);
+    int rc = launch_quant_rows_i8(X, xt, M, K, Xq, sx, st, pdl_first, early && pdl_first, fuse.amax_in,
+                                  fuse.amax_zero);
     if (rc != ARIA_OK) return rc;
     W8Epilogue ep;
     ep.sx = sx; ep.sw = w_scale; ep.bias = bias; ep.bias_t = bt; ep.act = act; ep.Y = Y;
     ep.out_t = yt == ARIA_F32 ? 0 : 1;
+    ep.row_absmax = fuse.amax_out;
     return launch_gemm_w8a8(Xq, Wq, M, N, K, ep, st, pdl);
 }
 
@@ -61,19 +78,20 @@ int check_layers(const aria_layer* layers, int n_layers, int M, int mode, int io
     return check_arch();
 }
 
+// first: this is the first kernel sequence of a chain (no programmatic dependency on what precedes it).
 // early: W8A8 only -- this layer's activation quantiser may overlap the previous layer's GEMM (see
 // aria_denoiser_linears).
 int run_layer(const aria_layer& L, const void* in, void* out, int M, int mode, int io, void* ws,
-              size_t ws_bytes, cudaStream_t st, bool early = false) {
-    static const bool pdl = getenv("ARIA_NO_PDL") == nullptr;   // debug switch
-    static const bool no_early = getenv("ARIA_NO_EARLY_QUANT") != nullptr;
+              size_t ws_bytes, cudaStream_t st, bool first, bool early = false, const W8Fuse& fuse = W8Fuse()) {
+    static const bool pdl = dbg_env("ARIA_NO_PDL") == nullptr;            // debug builds only
+    static const bool no_early = dbg_env("ARIA_NO_EARLY_QUANT") != nullptr;
     if (mode == ARIA_W8A8)
         return linear_w8a8_impl(in, io, M, L.K, static_cast<const int8_t*>(L.wq),
                                 static_cast<const float*>(L.w_scale), L.N, L.bias, io, L.act, out, io,
-                                ws, st, pdl, early && !no_early);
+                                ws, st, pdl && !first, pdl, early && !no_early, fuse);
     return launch_gemm_w4a16(in, M, L.K, static_cast<const uint8_t*>(L.wq),
                              static_cast<const uint16_t*>(L.w_scale), L.N, L.bias, L.act, out, io, ws,
-                             ws_bytes, st, pdl);
+                             ws_bytes, st, pdl && !first);
 }
 
 }  // namespace
@@ -132,7 +150,8 @@ const char* aria_status_string(int status) {
 
 size_t aria_workspace_bytes(int M, int maxK, int maxN, int mode) {
     if (M <= 0 || maxK <= 0 || maxN <= 0) return 0;
-    if (mode == ARIA_W8A8) return 2 * w8_ws_bytes(M, maxK);   // two (Xq, sx) buffers: see aria_denoiser_linears
+    // two (Xq, sx) buffers and two per-token absmax buffers (fused S1): see aria_denoiser_linears
+    if (mode == ARIA_W8A8) return 2 * w8_ws_bytes(M, maxK) + 2 * up256(static_cast<size_t>(M) * 4);
     if (mode == ARIA_W4A16) {
         // Split-K bound: splits * tiles <= #SMs and a tile holds <= 128 x TT outputs, so the fp32
         // partials never exceed #SMs * 128 * TT * 4 bytes; one counter quad per tile.
@@ -189,8 +208,10 @@ int aria_linear_w8a8(const void* X, int xt, int M, int K, const int8_t* Wq, cons
     if (!ws || ws_bytes < w8_ws_bytes(M, K)) return ARIA_ERR_WORKSPACE;
     int rc = check_arch();
     if (rc != ARIA_OK) return rc;
+    // the S1 pass is an ordinary launch; the GEMM is its programmatic dependent (its prologue -- barrier
+    // init, tensor-memory allocation, tensor-map prefetch -- overlaps the quantiser)
     return linear_w8a8_impl(X, xt, M, K, Wq, w_scale, N, bias, bt, act, Y, yt, ws,
-                            static_cast<cudaStream_t>(stream), false);
+                            static_cast<cudaStream_t>(stream), false, true);
 }
 
 int aria_linear_w8a8_q(const int8_t* Xq, const float* x_scale, int M, int K, const int8_t* Wq,
@@ -238,12 +259,26 @@ int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, in
     return launch_gemm_w8a8(Xq, Wq, M, N, K, ep, static_cast<cudaStream_t>(stream), false);
 }
 
-/* Debug hook (not in aria.h): per-CTA role timestamps of the W4A16 kernel, 16 int64 per CTA. */
+#ifdef ARIA_DEBUG
+/* Debug builds only (-DARIA_DEBUG, not in aria.h): per-CTA role timestamps of the three GEMM kernels. */
 __attribute__((visibility("default"))) void aria_debug_w4_profile(long long* buf) { w4_set_profile_buffer(buf); }
-
 __attribute__((visibility("default"))) void aria_debug_ws_profile(long long* buf) { ws_set_profile_buffer(buf); }
-
 __attribute__((visibility("default"))) void aria_debug_w8_profile(long long* buf) { w8_set_profile_buffer(buf); }
+#endif
+
+int aria_w8a8_tile_plan(int M, int N, int sms, int* bn, int* ctas) {
+    if (!bn || !ctas) return ARIA_ERR_NULL;
+    if (M <= 0 || N <= 0 || sms <= 0) return ARIA_ERR_SHAPE;
+    w8_tile_plan(M, N, sms, bn, ctas);
+    return ARIA_OK;
+}
+
+int aria_w4a16_tile_plan(int M, int N, int K, int sms, int* tt, int* splits) {
+    if (!tt || !splits) return ARIA_ERR_NULL;
+    if (M <= 0 || N <= 0 || K <= 0 || sms <= 0) return ARIA_ERR_SHAPE;
+    w4_plan(M, N, K, sms, tt, splits);
+    return ARIA_OK;
+}
 
 int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mode, int io, void* ws,
                           size_t ws_bytes, void* stream) {
@@ -259,8 +294,27 @@ int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mod
     // the quantiser of layer i reads in[i] and writes buffer i&1.  Every kernel of the chain waits
     // for its predecessor before it EXITS, so "kernel k complete" implies "kernels < k complete" and
     // nothing older than layer i-1's GEMM can still be running.
-    static const bool single_buf = getenv("ARIA_W8_SINGLE_BUF") != nullptr;   // debug switch
+    //
+    // Fused S1: if layer i+1 reads exactly layer i's output, layer i's epilogue reduces the per-token
+    // absmax of what it stores into one of two [M] buffers (atomicMax) and layer i+1's S1 pass only
+    // rounds.  The buffer a GEMM reduces into is zeroed by that same layer's S1 pass, which has completed
+    // before the GEMM's epilogue starts and -- even when it runs early -- only after every earlier
+    // reader of that buffer has completed (chain rule above).
+    static const bool single_buf = dbg_env("ARIA_W8_SINGLE_BUF") != nullptr;   // debug builds only
+    static const bool no_fuse = dbg_env("ARIA_NO_FUSED_ABSMAX") != nullptr;
     const size_t half = mode == ARIA_W8A8 && !single_buf ? w8_ws_bytes(M, maxK) : 0;
+    float* amax[2] = {nullptr, nullptr};
+    if (mode == ARIA_W8A8) {
+        uint8_t* b = static_cast<uint8_t*>(ws) + 2 * w8_ws_bytes(M, maxK);
+        amax[0] = reinterpret_cast<float*>(b);
+        amax[1] = reinterpret_cast<float*>(b + up256(static_cast<size_t>(M) * 4));
+    }
+    auto feeds_next = [&](int i) {   // layer i+1 reads exactly layer i's [M, N] output
+        if (mode != ARIA_W8A8 || no_fuse || i + 1 >= n_layers) return false;
+        const aria_layer& nx = layers[i + 1];
+        return (nx.in == nullptr || nx.in == layers[i].out) && nx.K == layers[i].N;
+    };
+    int n_fused = 0;                 // producers seen so far: selects the absmax buffer
     for (int i = 0; i < n_layers; ++i) {
         const aria_layer& L = layers[i];
         const void* in = L.in ? L.in : layers[i - 1].out;
@@ -271,7 +325,14 @@ int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mod
                             b1 = b0 + static_cast<size_t>(M) * layers[i - 1].N * dsize(io);
             early = !single_buf && !(a0 < b1 && b0 < a1);
         }
-        rc = run_layer(L, in, L.out, M, mode, io, static_cast<uint8_t*>(ws) + (i & 1) * half, ws_bytes - (i & 1) * half, st, early);
+        W8Fuse fuse;
+        if (i > 0 && feeds_next(i - 1)) fuse.amax_in = amax[(n_fused - 1) & 1];
+        if (feeds_next(i)) {
+            fuse.amax_out = fuse.amax_zero = amax[n_fused & 1];
+            ++n_fused;
+        }
+        rc = run_layer(L, in, L.out, M, mode, io, static_cast<uint8_t*>(ws) + (i & 1) * half,
+                       (mode == ARIA_W8A8 ? w8_ws_bytes(M, maxK) : ws_bytes), st, i == 0, early, fuse);
         if (rc != ARIA_OK) return rc;
     }
     return ARIA_OK;
@@ -310,7 +371,15 @@ int aria_stack_plan_run(const aria_stack_plan* plan, void* stream) {
                                  plan->mode, plan->io, plan->d_ws, plan->ws_bytes, stream);
 }
 
-int aria_stack_plan_is_streaming(const aria_stack_plan* plan) { return plan && plan->ws_plan ? 1 : 0; }
+int aria_stack_plan_is_streaming(const aria_stack_plan* plan) {
+    return plan && plan->ws_plan ? ws_plan_kind(plan->ws_plan) : 0;
+}
+
+int aria_stack_plan_fallback_fired(const aria_stack_plan* plan, int* fired) {
+    if (!plan || !fired) return ARIA_ERR_NULL;
+    *fired = 0;
+    return plan->ws_plan ? ws_plan_fallback_fired(plan->ws_plan, fired) : ARIA_OK;
+}
 
 void aria_stack_plan_destroy(aria_stack_plan* plan) {
     if (!plan) return;
@@ -359,7 +428,7 @@ int aria_denoiser_linears_host(const aria_layer* layers, int n_layers, int M, in
         }
         if (i >= 2) ok = ok && cudaStreamWaitEvent(st, hp->ev_out[b], 0) == cudaSuccess;
         if (!ok) break;
-        rc = run_layer(L, din, out_stage[b], M, mode, io, ws, dev, st);
+        rc = run_layer(L, din, out_stage[b], M, mode, io, ws, dev, st, true);
         if (rc != ARIA_OK) break;
         ok = cudaEventRecord(hp->ev_comp[b], st) == cudaSuccess &&
              cudaStreamWaitEvent(hp->s_out, hp->ev_comp[b], 0) == cudaSuccess &&

@@ -40,17 +40,17 @@ constexpr int W4_EPI_WARP0 = 4;
 constexpr int W4_DEQ_WARP0 = 8;
 constexpr int W4_G = 3;         // dequantiser groups = A buffers
 
-// CTAS = 2: a CTA PAIR (cta_group::2) computes 256 output channels x TT tokens; each CTA dequantises its
-// own 128 weight rows and stages only HALF of the X tile, which halves the X traffic through shared
-// memory (TMA write + MMA read) -- the dominant term of the smem-bound k-block time.
-template <int TT, int CTAS = 1>
+// (A CTA-pair variant -- cta_group::2, 256 channels x TT tokens, half of X staged per CTA -- and an X
+// multicast variant were built and measured in round 1: the pair lost ~1.3k cycles per k-block on the
+// cross-CTA "A ready" hand-off, multicast changed nothing (3.79 vs 3.81 ms per C5 step).  Both removed.)
+template <int TT>
 struct W4Cfg {
     static constexpr int G = W4_G;
-    static constexpr int NB = CTAS == 2 ? 5 : G;               // dequantised A buffers (pair: deeper, see kernel)
+    static constexpr int NB = G;                               // dequantised A buffers
     static constexpr int THREADS = 32 * W4_DEQ_WARP0 + 128 * G;
     static constexpr int P_ROW = W4_BK / 2;                    // 32 packed bytes per row per k-block
     static constexpr int P_BYTES = W4_BN * P_ROW;              // 4 KB
-    static constexpr int X_ROWS = TT / CTAS;                   // token rows staged by one CTA
+    static constexpr int X_ROWS = TT;                          // token rows per X stage
     static constexpr int X_BYTES = X_ROWS * 128;               // x 64 bf16
     static constexpr int A_BYTES = W4_BN * 128;                // 16 KB: 128 rows x 64 bf16
     static constexpr int STG_BYTES = 4096;                     // per epilogue warp: 32 tokens x 128 B
@@ -61,7 +61,7 @@ struct W4Cfg {
     static constexpr int P_OFF = A_OFF + NB * A_BYTES;
     static constexpr int STG_OFF = P_OFF + PS * P_BYTES;
     static constexpr int BAR_OFF = STG_OFF + 4 * STG_BYTES;
-    static constexpr int NBAR = 2 * XS + 2 * PS + 3 * NB + 4;
+    static constexpr int NBAR = 2 * XS + 2 * PS + 2 * NB + 4;
     static constexpr int SMEM_BYTES = BAR_OFF + NBAR * 8 + 16 + 1024;
     // TT = 192 fills the SMs when N / 128 is small: 12 row tiles x 11 token tiles = 132 units on 148 SMs
     // at M = 2048 (TT = 256: 96 units)
@@ -80,15 +80,20 @@ struct W4Params {
     int act, out_t;
     int M, N, K;
     int splits;
-    long long* prof;          // debug: per-CTA role timestamps (clock64), or nullptr
+#ifdef ARIA_DEBUG
+    long long* prof;          // per-CTA role timestamps (clock64), or nullptr
+#endif
 };
 
+#ifdef ARIA_DEBUG
 static long long* g_w4_prof = nullptr;
 void w4_set_profile_buffer(long long* p) { g_w4_prof = p; }
-
 __device__ __forceinline__ void prof_stamp(const W4Params& p, int slot, long long t0) {
     if (p.prof) p.prof[blockIdx.x * 16 + slot] = clock64() - t0;
 }
+#else
+__device__ __forceinline__ void prof_stamp(const W4Params&, int, long long) {}
+#endif
 
 __device__ __forceinline__ uint32_t cvt_bf16x2(float lo, float hi) {
     uint32_t r;
@@ -171,18 +176,11 @@ __device__ __forceinline__ void w4_store(void* Y, int out_t, int64_t idx, float 
         static_cast<__nv_bfloat16*>(Y)[idx] = __float2bfloat16_rn(y);
 }
 
-// MC (CTAS == 1 only): the two CTAs of a cluster work on the same token tile and adjacent weight-row
-// tiles in lockstep, and each loads HALF of every X tile with TMA multicast into both CTAs' shared
-// memory: the X operand is read from L2 once per pair.  At M >= 2048 the kernel is bound by L2 -> SM
-// traffic of X (every 128-row weight tile streams all of X: 226 MB per QKV layer against 3.5 MB of
-// weights), not by the tensor pipe.  All MMAs stay CTA-local (cta_group::1): the only cross-CTA
-// signals are the multicast TMA's complete_tx and the multicast tcgen05.commit that frees an X slot
-// in both CTAs -- no thread ever waits on a cluster-scope arrive.
-template <int TT, bool GELU, int CTAS, bool MC>
-__global__ void __launch_bounds__(W4Cfg<TT, CTAS>::THREADS, 1)
+template <int TT, bool GELU>
+__global__ void __launch_bounds__(W4Cfg<TT>::THREADS, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmX,
                   const __grid_constant__ CUtensorMap tmY, const W4Params p) {
-    using Cfg = W4Cfg<TT, CTAS>;
+    using Cfg = W4Cfg<TT>;
     constexpr int XS = Cfg::XS, PS = Cfg::PS, G = Cfg::G, NB = Cfg::NB;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
@@ -193,23 +191,20 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     const uint32_t xfull0 = bars, xempty0 = xfull0 + 8 * XS;
     const uint32_t pfull0 = xempty0 + 8 * XS, pempty0 = pfull0 + 8 * PS;
     const uint32_t afull0 = pempty0 + 8 * PS, aempty0 = afull0 + 8 * NB;
-    const uint32_t afwd0 = aempty0 + 8 * NB;                   // pair mode, peer CTA: local "A ready"
-    const uint32_t tfull0 = afwd0 + 8 * NB, tempty0 = tfull0 + 16;
+    const uint32_t tfull0 = aempty0 + 8 * NB, tempty0 = tfull0 + 16;
     const uint32_t tmem_slot = tempty0 + 16;
     volatile uint32_t* tmem_slot_g =
         reinterpret_cast<volatile uint32_t*>(gbase + Cfg::BAR_OFF + Cfg::NBAR * 8);
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const uint32_t rank = CTAS == 2 ? cluster_ctarank() : 0u;   // position in the CTA pair
-    const uint32_t mc_rank = MC ? cluster_ctarank() : 0u;       // which half of the X tile this CTA loads
-    constexpr int UN = W4_BN * CTAS;                            // output channels per work unit
+    constexpr int UN = W4_BN;                                   // output channels per work unit
     const int num_n = (p.N + UN - 1) / UN;
     const int num_t = (p.M + TT - 1) / TT;
     const int num_kb = (p.K + W4_BK - 1) / W4_BK;
-    const int S = CTAS == 2 ? 1 : p.splits;
+    const int S = p.splits;
     const int num_units = num_n * num_t * S;
-    const int unit0 = blockIdx.x / CTAS, unit_step = gridDim.x / CTAS;
+    const int unit0 = blockIdx.x, unit_step = gridDim.x;
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmP);
@@ -217,35 +212,28 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         tma_prefetch_desc(&tmY);
         for (int s = 0; s < XS; ++s) {
             mbar_init(xfull0 + 8 * s, 1);
-            mbar_init(xempty0 + 8 * s, MC ? 2 : 1);      // MMA commit (MC: of both CTAs)
+            mbar_init(xempty0 + 8 * s, 1);      // MMA commit
         }
         for (int s = 0; s < PS; ++s) {
             mbar_init(pfull0 + 8 * s, 1);
             mbar_init(pempty0 + 8 * s, 4);      // the 4 warps of the dequant group that read it
         }
         for (int a = 0; a < NB; ++a) {
-            // leader: its own 4 dequant warps + (pair mode) one forwarded arrival for the peer's 4
-            mbar_init(afull0 + 8 * a, CTAS == 2 ? 5 : 4);
+            mbar_init(afull0 + 8 * a, 4);       // the 4 dequant warps that fill it
             mbar_init(aempty0 + 8 * a, 1);
-            mbar_init(afwd0 + 8 * a, 4);
         }
         for (int a = 0; a < 2; ++a) {
             mbar_init(tfull0 + 8 * a, 1);
-            mbar_init(tempty0 + 8 * a, 4 * CTAS);
+            mbar_init(tempty0 + 8 * a, 4);
         }
         fence_mbar_init();
     }
     if (warp == 1) {
-        if (CTAS == 2) {
-            tmem_alloc_2sm(tmem_slot, Cfg::TMEM_COLS);
-            tmem_relinquish_2sm();
-        } else {
-            tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
-            tmem_relinquish();
-        }
+        tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
+        tmem_relinquish();
     }
     tc_fence_before();
-    if (CTAS == 2 || MC) cluster_sync(); else __syncthreads();
+    __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_g;
 
@@ -254,36 +242,24 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     // also keeps "this grid complete => every earlier grid complete": no CTA exits before its epilogue
     // warps have waited).  The weight stream and the dequantisers depend on nothing the previous grid
     // writes, so the first k-blocks are fetched and dequantised during its tail.
-    constexpr bool EARLY_W = CTAS == 1;
-    if (!EARLY_W) pdl_wait_prior_grid();
     pdl_launch_dependents();   // the next kernel may become resident now; it blocks in its own wait
     const long long t_start = clock64();
 
     // Producer / MMA warps: warp-uniform loops, one elected lane issues (see gemm_w8a8.cu).
     if (warp == 0) {
         // ------------------------------------------------------------ TMA producer: X
-        if (EARLY_W) pdl_wait_prior_grid();
+        pdl_wait_prior_grid();
         int stage = 0;
         uint32_t phase = 0;
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int t0 = (tile / num_n) * TT + rank * Cfg::X_ROWS;
+            const int t0 = (tile / num_n) * TT;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             for (int kb = kb0; kb < kb1; ++kb) {
                 mbar_wait(xempty0 + 8 * stage, phase ^ 1);
                 if (elect_one()) {
-                    if (CTAS == 2) {   // both halves are counted on the leader's barrier
-                        if (rank == 0) mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES * 2);
-                        tma_load_2d_2sm(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0,
-                                        (xfull0 + 8 * stage) & PEER_BIT_MASK);
-                    } else {
-                        mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);   // MC: both halves land here
-                        if (MC)
-                            tma_load_2d_mc(sX + stage * Cfg::X_BYTES + mc_rank * (Cfg::X_BYTES / 2), &tmX, kb * W4_BK,
-                                           t0 + mc_rank * (TT / 2), xfull0 + 8 * stage, 3);
-                        else
-                            tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
-                    }
+                    mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);
+                    tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
                 }
                 __syncwarp();
                 if (++stage == XS) { stage = 0; phase ^= 1; }
@@ -297,7 +273,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         uint32_t phase = 0;
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int n0 = (tile % num_n) * UN + rank * W4_BN;
+            const int n0 = (tile % num_n) * UN;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             for (int kb = kb0; kb < kb1; ++kb) {
                 mbar_wait(pempty0 + 8 * stage, phase ^ 1);
@@ -313,7 +289,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         if (lane == 0) prof_stamp(p, 6, t_start);
     } else if (warp == 1) {
         // ------------------------------------------------------------ MMA issuer
-        if (rank == 0) {
+        {
             constexpr uint32_t idesc = idesc_bf16(UN, TT);
             const uint64_t desc_hi = make_smem_desc_sw128(0);
             int stage = 0, ab = 0, acc = 0;
@@ -331,21 +307,11 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                     const uint64_t b_desc = desc_hi | (((sX + stage * Cfg::X_BYTES) & 0x3FFFF) >> 4);
                     if (elect_one()) {
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) {  // 4 x (K = 16 bf16 = 32 bytes)
-                            if (CTAS == 2)
-                                mma_f16_ss_2sm(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
-                            else
-                                mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
-                        }
-                        if (CTAS == 2) {
-                            tc_commit_2sm(xempty0 + 8 * stage, 3);
-                            tc_commit_2sm(aempty0 + 8 * ab, 3);
-                            if (kb == kb1 - 1) tc_commit_2sm(tfull0 + 8 * acc, 3);
-                        } else {
-                            if (MC) tc_commit_mc(xempty0 + 8 * stage, 3); else tc_commit(xempty0 + 8 * stage);
-                            tc_commit(aempty0 + 8 * ab);
-                            if (kb == kb1 - 1) tc_commit(tfull0 + 8 * acc);
-                        }
+                        for (int k = 0; k < 4; ++k)   // 4 x (K = 16 bf16 = 32 bytes)
+                            mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                        tc_commit(xempty0 + 8 * stage);
+                        tc_commit(aempty0 + 8 * ab);
+                        if (kb == kb1 - 1) tc_commit(tfull0 + 8 * acc);
                     }
                     __syncwarp();
                     if (++stage == XS) { stage = 0; phase ^= 1; }
@@ -369,7 +335,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         int it = 0;                               // running k-block counter of this CTA
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int n0 = (tile % num_n) * UN + rank * W4_BN;
+            const int n0 = (tile % num_n) * UN;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             const bool row_ok = n0 + r < p.N;
             const uint32_t* srow = reinterpret_cast<const uint32_t*>(
@@ -423,35 +389,19 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 for (int j = 0; j < 8; ++j) sts128(rowb + ((static_cast<uint32_t>(j) ^ xr) << 4), o[j]);
                 fence_proxy_async_smem();                  // generic-proxy writes -> async proxy (MMA)
                 __syncwarp();
-                if (lane == 0) {                                   // one arrival per warp
-                    // pair mode, peer CTA: arrive locally (cheap); a forwarder thread relays to the leader,
-                    // keeping the cluster-scope release off the dequantisers' path
-                    if (CTAS == 2 && rank == 1) mbar_arrive(afwd0 + 8 * ab); else mbar_arrive(afull0 + 8 * ab);
-                }
+                if (lane == 0) mbar_arrive(afull0 + 8 * ab);       // one arrival per warp
             }
         }
         if ((dw & 3) == 0 && lane == 0) prof_stamp(p, 2 + g, t_start);
-    } else if (warp == 3) {
-        // ------------------------------------------------------------ pair mode, peer CTA: forwarder
-        if (CTAS == 2 && rank == 1 && lane == 0) {
-            int it = 0;
-            for (int u = unit0; u < num_units; u += unit_step) {
-                for (int kb = 0; kb < num_kb; ++kb, ++it) {
-                    const int ab = it % NB;
-                    mbar_wait(afwd0 + 8 * ab, (it / NB) & 1);          // the peer's 4 dequant warps are done
-                    mbar_arrive_cluster(mapa_shared(afull0 + 8 * ab, 0));
-                }
-            }
-        }
     } else if (warp >= W4_EPI_WARP0) {
         // ------------------------------------------------------------ epilogue (warps 4..7)
-        if (EARLY_W) pdl_wait_prior_grid();
+        pdl_wait_prior_grid();
         const int q = warp & 3;
         int acc = 0;
         uint32_t acc_phase = 0;
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int n0 = (tile % num_n) * UN + rank * W4_BN, t0 = (tile / num_n) * TT;
+            const int n0 = (tile % num_n) * UN, t0 = (tile / num_n) * TT;
             const int n = n0 + q * 32 + lane;
             const bool n_ok = n < p.N;
             float bv = 0.0f;
@@ -528,10 +478,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) {
-                    if (CTAS == 2) mbar_arrive_cluster(mapa_shared(tempty0 + 8 * acc, 0));
-                    else mbar_arrive(tempty0 + 8 * acc);
-                }
+                if (lane == 0) mbar_arrive(tempty0 + 8 * acc);
             } else {
                 float* part = p.partials + static_cast<int64_t>(sp) * p.M * p.N;
                 float* prow = part + static_cast<int64_t>(t0) * p.N + n;
@@ -615,30 +562,24 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
 
     if (warp >= W4_EPI_WARP0 && warp < W4_DEQ_WARP0 && lane == 0) tma_store_wait<0>();
     tc_fence_before();
-    if (CTAS == 2 || MC) cluster_sync(); else __syncthreads();
+    __syncthreads();
     if (warp == 1) {
         tc_fence_after();
-        if (CTAS == 2) tmem_dealloc_2sm(tmem_base, Cfg::TMEM_COLS);
-        else tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
+        tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
     }
 }
 
-template <int TT, bool GELU, int CTAS, bool MC = false>
+template <int TT, bool GELU>
 static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, const W4Params& p,
                      int grid, cudaStream_t st, bool pdl) {
-    using Cfg = W4Cfg<TT, CTAS>;
-    static bool attr_set = false;
-    auto kern = w4a16_gemm_kernel<TT, GELU, CTAS, MC>;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES) !=
-            cudaSuccess)
-            return ARIA_ERR_CUDA;
-        attr_set = true;
-    }
+    using Cfg = W4Cfg<TT>;
+    static std::atomic<uint64_t> attr_done{0};
+    auto kern = w4a16_gemm_kernel<TT, GELU>;
+    if (!ensure_dyn_smem(kern, Cfg::SMEM_BYTES, attr_done)) return ARIA_ERR_CUDA;
     CUtensorMap tmP, tmX, tmY;
     int rc = make_tmap_2d(&tmP, Wq4, 1, N, K / 2, W4_BN, Cfg::P_ROW, Cfg::P_ROW);
     if (rc != ARIA_OK) return rc;
-    rc = make_tmap_2d(&tmX, X, 2, M, K, MC ? Cfg::X_ROWS / 2 : Cfg::X_ROWS, 64, 128);   // MC: each CTA loads half a tile
+    rc = make_tmap_2d(&tmX, X, 2, M, K, Cfg::X_ROWS, 64, 128);
     if (rc != ARIA_OK) return rc;
     // output: box = 32 tokens x 32 channels (64 B bf16 rows / 128 B fp32 rows)
     rc = make_tmap_2d(&tmY, p.Y, p.out_t == ARIA_F32 ? 4 : 2, M, N, 32, 32, p.out_t == ARIA_F32 ? 128 : 64);
@@ -648,22 +589,11 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
     cfg.blockDim = dim3(Cfg::THREADS);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = st;
-    cudaLaunchAttribute at[2];
-    int na = 0;
-    if (pdl) {
-        at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        at[na].val.programmaticStreamSerializationAllowed = 1;
-        ++na;
-    }
-    if (CTAS == 2 || MC) {
-        at[na].id = cudaLaunchAttributeClusterDimension;
-        at[na].val.clusterDim.x = 2;
-        at[na].val.clusterDim.y = 1;
-        at[na].val.clusterDim.z = 1;
-        ++na;
-    }
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = na;
+    cfg.numAttrs = pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kern, tmP, tmX, tmY, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
@@ -719,40 +649,22 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
     W4Params p;
     p.g_scale = g_scale; p.bias = bias; p.Y = Y;
     p.act = act; p.out_t = yt; p.M = M; p.N = N; p.K = K; p.splits = s;
+#ifdef ARIA_DEBUG
     p.prof = g_w4_prof;
+#endif
     const size_t tiles = static_cast<size_t>((N + W4_BN - 1) / W4_BN) * ((M + tt - 1) / tt);
     p.counters = static_cast<unsigned*>(ws);
     p.partials = s > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) +
                                                   (tiles * 4 * sizeof(unsigned) + 255) / 256 * 256)
                        : nullptr;
-    // CTA pairs for the big-tile, no-split case: same wave count, half the X traffic through smem
-    // CTA-pair mode is implemented and parity-tested but OFF by default: the peer CTA's cluster-scope
-    // mbarrier arrive after its STS + fence.proxy.async costs ~1.3k cycles per k-block on the hand-off
-    // path (measured with the role timestamps), which more than cancels the halved X traffic.
-    static const bool want_pair = getenv("ARIA_W4_PAIR") != nullptr;
-    const bool pair = want_pair && tt == 256 && s == 1 && N > W4_BN && sms >= 2;
-    const int units = pair ? ((N + 2 * W4_BN - 1) / (2 * W4_BN)) * ((M + tt - 1) / tt) : static_cast<int>(tiles) * s;
-    const int slots = pair ? sms / 2 : sms;
-    int grid = (units < slots ? units : slots) * (pair ? 2 : 1);
-    // X multicast over CTA couples (see the kernel): big token tiles, no split-K, an even number of
-    // weight-row tiles so that a couple always shares its token tile
-    // Measured on C5 (M = 2048): 3.79 ms with multicast vs 3.81 ms without -- the L2 already serves
-    // the two CTAs' identical reads at no extra cost, so the mode is parity-tested but OFF by default.
-    static const bool want_mc = getenv("ARIA_W4_MC") != nullptr;
-    const bool mc = want_mc && !pair && tt == 256 && s == 1 && ((N + W4_BN - 1) / W4_BN) % 2 == 0 && grid >= 2;
-    if (mc) grid &= ~1;
+    const int units = static_cast<int>(tiles) * s;
+    const int grid = units < sms ? units : sms;
     if (s > 1 && cudaMemsetAsync(p.counters, 0, tiles * 4 * sizeof(unsigned), st) != cudaSuccess)
         return ARIA_ERR_CUDA;
     const bool gelu = act == ARIA_ACT_GELU_ERF;
-#define ARIA_W4_LAUNCH(TTV)                                                        \
-    return gelu ? launch_w4<TTV, true, 1>(X, M, K, Wq4, N, p, grid, st, pdl)       \
-                : launch_w4<TTV, false, 1>(X, M, K, Wq4, N, p, grid, st, pdl)
-    if (mc)
-        return gelu ? launch_w4<256, true, 1, true>(X, M, K, Wq4, N, p, grid, st, pdl)
-                    : launch_w4<256, false, 1, true>(X, M, K, Wq4, N, p, grid, st, pdl);
-    if (pair)
-        return gelu ? launch_w4<256, true, 2>(X, M, K, Wq4, N, p, grid, st, pdl)
-                    : launch_w4<256, false, 2>(X, M, K, Wq4, N, p, grid, st, pdl);
+#define ARIA_W4_LAUNCH(TTV)                                                     \
+    return gelu ? launch_w4<TTV, true>(X, M, K, Wq4, N, p, grid, st, pdl)       \
+                : launch_w4<TTV, false>(X, M, K, Wq4, N, p, grid, st, pdl)
     if (tt == 32) { ARIA_W4_LAUNCH(32); }
     if (tt == 64) { ARIA_W4_LAUNCH(64); }
     if (tt == 128) { ARIA_W4_LAUNCH(128); }

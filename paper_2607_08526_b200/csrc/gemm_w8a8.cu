@@ -13,6 +13,7 @@
 //               MMA warp fills accumulator `a^1`.
 // Tails: TMA zero-fills rows >= M / >= N and bytes >= K on load (zero codes add nothing) and clips
 // them on store.
+#include <cstdio>
 #include <cstdlib>
 
 #include "internal.cuh"
@@ -62,17 +63,26 @@ struct W8Params {
     const float* sx;
     const float* sw;
     const void* bias;
+    float* row_absmax; // fused S1, first half: max |y| per output row (as stored), atomicMax on the bits; or nullptr
     int bias_t, act;
     int M, N, K;
-    long long* prof;   // debug: per-CTA role timestamps (clock64), or nullptr
-    int dbg;           // debug experiments (ARIA_W8_DBG): 1 = no TMA stores, 2 = no staging stores either, 4 = no math
+#ifdef ARIA_DEBUG
+    long long* prof;   // per-CTA role timestamps (clock64), or nullptr
+    int dbg;           // experiments (ARIA_W8_DBG): 1 = no TMA stores, 2 = no staging stores either
+#endif
 };
 
+#ifdef ARIA_DEBUG
 static long long* g_w8_prof = nullptr;
 void w8_set_profile_buffer(long long* p) { g_w8_prof = p; }
 __device__ __forceinline__ void w8_stamp(const W8Params& p, int slot, long long t0) {
     if (p.prof) p.prof[blockIdx.x * 20 + slot] = clock64() - t0;
 }
+#define W8_DBG(p) ((p).dbg)
+#else
+__device__ __forceinline__ void w8_stamp(const W8Params&, int, long long) {}
+#define W8_DBG(p) 0
+#endif
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
     __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
@@ -90,7 +100,7 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, ui
 template <int BN, int OUT_T, bool GELU, int NBUF>
 __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const float* swb, int cb, float sxv,
                                                uint32_t stg0, int& sbuf, int lane, const CUtensorMap* tmY,
-                                               int n0, int row0, int dbg = 0) {
+                                               int n0, int row0, bool want_amax, float& amax, int dbg = 0) {
     const uint32_t rowb = stg0 + sbuf * W8_STG_BYTES + lane * 64;
     const uint32_t xr = (lane >> 1) & 3;
     const bool first = OUT_T != 1 || (cb & 16) == 0;   // first group of a 64-byte block
@@ -116,6 +126,10 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
         if (GELU) {
 #pragma unroll
             for (int j = 0; j < 16; j += 2) gelu_erf2(f[j], f[j + 1]);
+        }
+        if (want_amax) {   // warp-uniform; rounding to the output type is monotone, so it is applied to the max once
+#pragma unroll
+            for (int j = 0; j < 16; ++j) amax = fmaxf(amax, fabsf(f[j]));
         }
         if (OUT_T == 1) {
 #pragma unroll
@@ -216,12 +230,16 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     pdl_wait_prior_grid();
     pdl_launch_dependents();   // the next kernel may become resident now; it blocks in its own wait
     const long long t_start = clock64();
+#ifdef ARIA_DEBUG
     if (threadIdx.x == 0 && p.prof) {
         p.prof[blockIdx.x * 20 + 16] = t_start - t_entry;
         unsigned long long gt;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
         p.prof[blockIdx.x * 20 + 18] = static_cast<long long>(gt);
     }
+#else
+    (void)t_entry;
+#endif
 
     // Producer and MMA warps run their loops WARP-UNIFORMLY (all 32 lanes execute the control flow and
     // the barrier waits; one elected lane issues the TMA / tcgen05 instructions).  With the loop inside
@@ -348,6 +366,8 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             // A chunk is two groups of 16 columns held in two register sets; the refill of the first set
             // for the next chunk is in flight while the second set is processed.
             uint32_t va[16], vb[16];
+            const bool want_amax = OUT_T != 2 && p.row_absmax != nullptr;
+            float amax = 0.0f;
             int c = c_beg;
             if (c < c_end) {
                 tmem_ld_32x32b_x16(t_addr + c * 32, va);
@@ -358,14 +378,20 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 #pragma unroll 1
             for (; c < c_end; ++c) {
                 const int cn = c + 1;
-                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(va, swb, c * 32, sxv, stg0, sbuf, lane, &tmY, n0, row0, p.dbg);
+                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(va, swb, c * 32, sxv, stg0, sbuf, lane, &tmY, n0, row0, want_amax, amax, W8_DBG(p));
                 if (cn < c_end) tmem_ld_32x32b_x16(t_addr + cn * 32, va);
-                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(vb, swb, c * 32 + 16, sxv, stg0, sbuf, lane, &tmY, n0, row0, p.dbg);
+                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(vb, swb, c * 32 + 16, sxv, stg0, sbuf, lane, &tmY, n0, row0, want_amax, amax, W8_DBG(p));
                 if (cn < c_end) {
                     tmem_ld_32x32b_x16(t_addr + cn * 32 + 16, vb);
                     tmem_wait_ld_x16(va);
                     tmem_wait_ld_x16(vb);
                 }
+            }
+            if (want_amax && row0 + lane < p.M) {
+                // fused S1, first half: per-token absmax of the STORED output (bf16 rounding is monotone and
+                // odd, so max |bf16(y)| = bf16(max |y|)); non-negative floats order like their bit patterns
+                if (OUT_T == 1) amax = __bfloat162float(__float2bfloat16_rn(amax));
+                atomicMax(reinterpret_cast<int*>(p.row_absmax) + row0 + lane, __float_as_int(amax));
             }
             tc_fence_before();
             __syncwarp();
@@ -392,26 +418,23 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         if (CTAS == 2) tmem_dealloc_2sm(tmem_base, Cfg::TMEM_COLS);
         else tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
     }
+#ifdef ARIA_DEBUG
     if (threadIdx.x == 32 && p.prof) {
         p.prof[blockIdx.x * 20 + 17] = clock64() - t_start;
         unsigned long long gt;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
         p.prof[blockIdx.x * 20 + 19] = static_cast<long long>(gt);
     }
+#endif
 }
 
 template <int BN, int OUT_T, bool GELU, int CTAS>
 static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmY,
                       const W8Params& p, int grid, cudaStream_t st, bool pdl) {
     using Cfg = W8Cfg<BN, CTAS>;
-    static bool attr_set = false;
+    static std::atomic<uint64_t> attr_done{0};
     auto kern = w8a8_gemm_kernel<BN, OUT_T, GELU, CTAS>;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES) !=
-            cudaSuccess)
-            return ARIA_ERR_CUDA;
-        attr_set = true;
-    }
+    if (!ensure_dyn_smem(kern, Cfg::SMEM_BYTES, attr_done)) return ARIA_ERR_CUDA;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(W8_THREADS);
@@ -476,12 +499,17 @@ static W8Plan pick_plan(int M, int N, int sms) {
     return best;
 }
 
+void w8_tile_plan(int M, int N, int sms, int* bn, int* ctas) {
+    const W8Plan p = pick_plan(M, N, sms);
+    *bn = p.bn; *ctas = p.ctas;
+}
+
 int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, const W8Epilogue& ep,
                      cudaStream_t st, bool pdl) {
     const int sms = num_sms();
     if (sms <= 0) return ARIA_ERR_CUDA;
     W8Plan plan = pick_plan(M, N, sms);
-    if (const char* e = getenv("ARIA_W8_PLAN")) {   // debug override: "bn,ctas"
+    if (const char* e = dbg_env("ARIA_W8_PLAN")) {   // debug builds only: override "bn,ctas"
         int b = 0, c = 0;
         if (sscanf(e, "%d,%d", &b, &c) == 2 && (c == 1 || (c == 2 && M > W8_BM && b >= 128)) &&
             (b == 64 || b == 128 || b == 192 || b == 256)) { plan.bn = b; plan.ctas = c; }
@@ -501,8 +529,11 @@ int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, co
     p.sx = ep.sx; p.sw = ep.sw; p.bias = ep.bias;
     p.bias_t = ep.bias_t; p.act = ep.act;
     p.M = M; p.N = N; p.K = K;
+    p.row_absmax = ep.out_t == 2 ? nullptr : ep.row_absmax;
+#ifdef ARIA_DEBUG
     p.prof = g_w8_prof;
-    p.dbg = getenv("ARIA_W8_DBG") ? atoi(getenv("ARIA_W8_DBG")) : 0;
+    p.dbg = dbg_env("ARIA_W8_DBG") ? atoi(dbg_env("ARIA_W8_DBG")) : 0;
+#endif
     const int um = W8_BM * ctas;
     const int tiles = ((M + um - 1) / um) * ((N + bn - 1) / bn);
     const int slots = sms / ctas;

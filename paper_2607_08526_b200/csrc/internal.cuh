@@ -2,16 +2,45 @@
 #pragma once
 #include <cstdio>
 
+#include <atomic>
+#include <cstdlib>
+
 #include "../../include/aria.h"
 #include "ptx.cuh"
 
 namespace aria {
 
+// Debug switches (environment variables, role-timestamp buffers, the aria_debug_* exports) exist only
+// in builds with -DARIA_DEBUG (python -m paper_2607_08526_b200.build --debug).  The product library
+// reads no environment variable: dbg_env() folds to nullptr and every switch to its default.
+#ifdef ARIA_DEBUG
+inline const char* dbg_env(const char* name) { return getenv(name); }
+#else
+inline const char* dbg_env(const char*) { return nullptr; }
+#endif
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-DEVICE attribute of a kernel: set it once per
+// (kernel instantiation, device).  `mask` is that instantiation's bit set of devices already done.
+template <typename Kern>
+inline bool ensure_dyn_smem(Kern kern, int bytes, std::atomic<uint64_t>& mask) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
+    const uint64_t bit = 1ull << dev;
+    if (mask.load(std::memory_order_acquire) & bit) return true;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) return false;
+    mask.fetch_or(bit, std::memory_order_release);
+    return true;
+}
+
 // ---- quant.cu
 // early (needs pdl): the pass does not wait for the previous grid before it starts -- the caller
 // guarantees that grid neither writes X nor touches q / s -- but still waits for it before it ends.
+// known_absmax: per-row max |x| already computed by the producing epilogue (fused S1): the pass
+// skips its reduction.  zero_absmax: a [R] buffer this pass zeroes (the buffer the GEMM that consumes
+// this pass's codes will atomicMax into).
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl, bool early = false);
+                         bool pdl, bool early = false, const float* known_absmax = nullptr,
+                         float* zero_absmax = nullptr);
 int launch_quant_groups_i4(const void* W, int wt, int N, int K, uint8_t* q4, uint16_t* sg,
                            cudaStream_t st);
 
@@ -33,11 +62,15 @@ struct W8Epilogue {
     int act;           // aria_act
     void* Y;
     int out_t;
+    float* row_absmax = nullptr;   // fused S1 (first half): per-row max |y| as stored, atomicMax; or nullptr
 };
 int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, const W8Epilogue& ep,
                      cudaStream_t st, bool pdl);
 
-void w8_set_profile_buffer(long long* p);  // debug hook: per-CTA role timestamps
+void w8_tile_plan(int M, int N, int sms, int* bn, int* ctas);   // the (BN, CTAS) launch_gemm_w8a8 picks
+#ifdef ARIA_DEBUG
+void w8_set_profile_buffer(long long* p);  // per-CTA role timestamps
+#endif
 
 // ---- gemm_w4a16.cu
 // ws: split-K partials + tile counters (w4_workspace_bytes); too small / null -> no split-K.
@@ -45,7 +78,10 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
                       int N, const void* bias, int act, void* Y, int yt, void* ws, size_t ws_bytes,
                       cudaStream_t st, bool pdl);
 size_t w4_workspace_bytes(int M, int N, int K, int sms);
-void w4_set_profile_buffer(long long* p);  // debug hook: per-CTA role timestamps
+void w4_plan(int M, int N, int K, int sms, int* tt, int* splits);   // the (token tile, split-K) launch_gemm_w4a16 picks
+#ifdef ARIA_DEBUG
+void w4_set_profile_buffer(long long* p);  // per-CTA role timestamps
+#endif
 
 // ---- w4a16_stream.cu: persistent weight-streaming kernel for a list of W4A16 linears at M <= 32
 struct WsPlan;
@@ -53,6 +89,10 @@ bool ws_eligible(const aria_layer* layers, int n_layers, int M, int mode, int io
 int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan** out);
 int ws_plan_run(const WsPlan* plan, cudaStream_t st);
 void ws_plan_destroy(WsPlan* plan);
-void ws_set_profile_buffer(long long* p);  // debug hook: per-CTA role timestamps (read at plan creation)
+int ws_plan_kind(const WsPlan* plan);                       // 1: fp16 operands + armed bf16 fallback, 2: bf16 operands
+int ws_plan_fallback_fired(const WsPlan* plan, int* fired); // synchronous read of the last launch's domain flag
+#ifdef ARIA_DEBUG
+void ws_set_profile_buffer(long long* p);  // per-CTA role timestamps (read at plan creation)
+#endif
 
 }  // namespace aria

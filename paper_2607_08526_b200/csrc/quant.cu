@@ -131,7 +131,8 @@ __device__ __forceinline__ uint2 quant8_i8(const float (&v)[8], float s) {
 template <typename T>
 __global__ void __launch_bounds__(QROW_MAX_THREADS)
 quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
-                     float* __restrict__ scale, int early) {
+                     float* __restrict__ scale, int early, const float* known_absmax,
+                     float* zero_absmax) {
     __shared__ float red[QROW_MAX_THREADS / 32];
     // early: X, Xq and scale are untouched by the grid before this one (the caller checked), so the
     // pass runs concurrently with it; the wait moves to the end so that "this grid is complete" still
@@ -165,9 +166,14 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
     const int nwarp = nthr >> 5;
     a = red[0];
     for (int w = 1; w < nwarp; ++w) a = fmaxf(a, red[w]);
+    // fused S1: the producing epilogue already reduced this row (same value, taken after the wait above)
+    if (known_absmax) asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(known_absmax + row) : "memory");
 
     const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
-    if (tid == 0) scale[row] = s;
+    if (tid == 0) {
+        scale[row] = s;
+        if (zero_absmax) zero_absmax[row] = 0.0f;
+    }
     pdl_launch_dependents();
     const FastQ f = make_fastq(s);
 #pragma unroll
@@ -192,9 +198,10 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
 // One WARP per row (K <= 8 * 32 * VPL): every lane issues all its 16-byte loads up front, the
 // absmax is a pure shuffle reduction, no shared memory and no block barrier.
 template <typename T, int VPL>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(VPL > 12 ? 128 : 256)
 quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restrict__ Xq,
-                          float* __restrict__ scale, int early) {
+                          float* __restrict__ scale, int early, const float* known_absmax,
+                          float* zero_absmax) {
     if (!early) pdl_wait_prior_grid();      // early: see quant_rows_i8_kernel
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
@@ -221,10 +228,17 @@ quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restr
             a = absmax8(v, a);
         }
     }
+    if (known_absmax) {   // fused S1: reduced by the producing epilogue (warp-uniform branch)
+        asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(known_absmax + row) : "memory");
+    } else {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
+        for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
+    }
     const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
-    if (lane == 0) scale[row] = s;
+    if (lane == 0) {
+        scale[row] = s;
+        if (zero_absmax) zero_absmax[row] = 0.0f;
+    }
     const FastQ f = make_fastq(s);
 #pragma unroll
     for (int i = 0; i < VPL; ++i) {
@@ -268,17 +282,21 @@ quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restri
 
 template <typename T, int VPL>
 static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, float* s,
-                                    cudaLaunchConfig_t& cfg, int early) {
-    cfg.blockDim = dim3(256);
-    cfg.gridDim = dim3((R + 7) / 8);
-    return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s, early);
+                                    cudaLaunchConfig_t& cfg, int early, const float* known, float* zero) {
+    // wide rows keep many registers per lane: 4 rows per CTA there, so that a 2048-row pass still
+    // spreads over every SM
+    constexpr int WARPS = VPL > 12 ? 4 : 8;
+    cfg.blockDim = dim3(32 * WARPS);
+    cfg.gridDim = dim3((R + WARPS - 1) / WARPS);
+    return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s, early,
+                              known, zero);
 }
 
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl, bool early_) {
+                         bool pdl, bool early_, const float* known, float* zero) {
     const int nvec = C / 8;
     const int early = pdl && early_ ? 1 : 0;
-    {   // warp-per-row variants: rows up to 3072 elements (wider rows: one CTA per row, below)
+    {   // warp-per-row variants: bf16 rows up to 6144 elements, fp32 rows up to 3072 (wider: one CTA per row, below)
         cudaLaunchConfig_t cfg = {};
         cfg.stream = st;
         cudaLaunchAttribute at[1];
@@ -290,14 +308,15 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
         cudaError_t e = cudaErrorInvalidValue;
         bool done = true;
         if (xt == ARIA_BF16) {
-            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg, early);
-            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg, early);
-            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg, early);
+            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg, early, known, zero);
+            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg, early, known, zero);
+            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg, early, known, zero);
+            else if (vpl <= 24) e = launch_warp_rows<__nv_bfloat16, 24>(X, R, C, q, s, cfg, early, known, zero);
             else done = false;
         } else {
-            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg, early);
-            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg, early);
-            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg, early);
+            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg, early, known, zero);
+            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg, early, known, zero);
+            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg, early, known, zero);
             else done = false;
         }
         if (done) return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
@@ -315,10 +334,10 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
     cfg.numAttrs = pdl ? 1 : 0;
     cudaError_t e;
     if (xt == ARIA_F32)
-        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s, early);
+        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s, early, known, zero);
     else
         e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<__nv_bfloat16>,
-                               static_cast<const __nv_bfloat16*>(X), C, q, s, early);
+                               static_cast<const __nv_bfloat16*>(X), C, q, s, early, known, zero);
     return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 

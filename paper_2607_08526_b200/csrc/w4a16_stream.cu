@@ -106,7 +106,7 @@ struct alignas(128) WsLayer {
     int dep;                  // layer whose completion this layer's input needs, or -1
     int notify;               // 1 if a later layer depends on this one (epilogue bumps done[l])
     unsigned done_target;     // num_n * 4 quarter-tiles complete the layer
-    int pad_[1];
+    int in_ext;               // index of the external input this layer reads (AF16 range tracking), or -1 if chained
 };
 
 // AF16: external bf16 inputs are converted once per launch to fp16 (the MMA needs both operands in
@@ -129,13 +129,28 @@ struct WsParams {
     const int2* sched_cnt;
     int max_units;
     unsigned* done;           // [n_layers] completion counters + [n_layers] = CTAs done converting (zeroed before each launch)
+    // Domain of the fp16 operand path (AF16), tracked per launch in words zeroed with `done`:
+    //   flag   != 0: some activation (external or chained) or a 32-k group sum exceeds the fp16 range, or
+    //               a whole input tensor is so small (0 < absmax < WS_MIN_ABSMAX) that fp16 subnormals
+    //               would cost relative precision -> the bf16 fallback launch recomputes the list.
+    //   inmax  [n_ext]    bit pattern of max |x| of every external input (conversion pre-pass)
+    //   outmax [n_layers] bit pattern of max |y| of every chained output (producing epilogue)
+    unsigned* flag;
+    unsigned* inmax;
+    unsigned* outmax;
+    const unsigned* run_if;   // fallback launch: run only if *run_if != 0 (after the previous grid completed)
     int n_layers, M;
-    long long* prof;          // debug: per-CTA role timestamps (16 per CTA), or nullptr
-    int dbg;                  // debug experiments (ARIA_WS_DBG): 1 = skip dequant math, 2 = skip MMAs
+    long long* prof;          // debug builds: per-CTA role timestamps (16 per CTA), or nullptr
+    int dbg;                  // debug builds (ARIA_WS_DBG): 1 = skip dequant math, 2 = skip MMAs
 };
 
+constexpr float WS_F16_MAX = 65504.0f;
+constexpr float WS_MIN_ABSMAX = 0.0078125f;   // 2^-7: see DESIGN.md (fp16 subnormal error vs output magnitude)
+
+#ifdef ARIA_DEBUG
 static long long* g_ws_prof = nullptr;
 void ws_set_profile_buffer(long long* p) { g_ws_prof = p; }
+#endif
 #define WS_TIMED(accum, stmt) do { if (PROF) { const long long t_ = clock64(); stmt; accum += clock64() - t_; } else { stmt; } } while (0)
 #define WS_STAMP(slot) do { if (PROF && p.prof) p.prof[blockIdx.x * 16 + (slot)] = clock64() - t_start; } while (0)
 
@@ -319,6 +334,13 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
 
+    // Fallback launch (exact bf16 operands): runs only if the fp16 launch before it left its domain.
+    if (p.run_if) {
+        pdl_wait_prior_grid();
+        if (ld_acquire(p.run_if) == 0) return;
+    }
+    pdl_launch_dependents();
+
     // Start-up chain: the CTA's unit count / stage total and its first unit come from two independent
     // loads issued here, and the producers prefetch the first layer's tensor maps, all while the
     // barriers are initialised and tensor memory is allocated.
@@ -371,21 +393,28 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         const int ctid = threadIdx.x;
         for (int cb = blockIdx.x * CT + (ctid & ~31); cb < p.conv_chunks; cb += gridDim.x * CT) {   // warp-uniform
             const int c = cb + lane;
-            const bool ok = c < p.conv_chunks;       // chunk counts are multiples of 32: quads are all-or-nothing
-            float sum = 0.0f;
+            const bool ok = c < p.conv_chunks;       // chunk counts are multiples of 32: a warp never straddles two inputs
+            float sum = 0.0f, amax = 0.0f;
             uint16_t* drow = nullptr;
-            int kc = 0;
+            int kc = 0, seg = 0;
             if (ok) {
                 int lo = 0, hi = p.n_conv - 1;         // segment of chunk c
                 while (lo < hi) {
                     const int mid = (lo + hi + 1) >> 1;
                     if (__ldg(&p.conv[mid].chunk0) <= c) lo = mid; else hi = mid - 1;
                 }
+                seg = lo;
                 const WsConv cv = p.conv[lo];
                 const int ci = c - cv.chunk0;
                 const int m = ci / cv.kc8;
                 kc = ci - m * cv.kc8;
                 const uint4 v = __ldg(cv.src + ci);
+                {   // max |x| of the 8 bf16 values (non-negative floats order like their bit patterns)
+                    const uint32_t w4[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        amax = fmaxf(amax, fmaxf(fabsf(__uint_as_float(w4[i] << 16)), fabsf(__uint_as_float(w4[i] & 0xFFFF0000u))));
+                }
                 const uint32_t h01 = bf16x2_to_f16x2(v.x), h23 = bf16x2_to_f16x2(v.y);
                 const uint32_t h45 = bf16x2_to_f16x2(v.z), h67 = bf16x2_to_f16x2(v.w);
                 uint4 o;                               // pairs (k_i, k_{i+4})
@@ -402,9 +431,16 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             sum += __shfl_xor_sync(0xffffffffu, sum, 1);     // 4 chunks = one 32-k group
             sum += __shfl_xor_sync(0xffffffffu, sum, 2);
             if (ok && (kc & 3) == 0) {
-                const __half sh = __float2half_rn(sum);
+                const __half sh = __float2half_rn(fminf(fmaxf(sum, -WS_F16_MAX), WS_F16_MAX));
                 const __half sl = __float2half_rn(sum - __half2float(sh));
                 *reinterpret_cast<__half2*>(drow + 256 + 2 * ((kc >> 2) & 7)) = __halves2half2(sh, sl);
+            }
+            // domain of the fp16 operand: every |x| and every group sum within the fp16 range
+            const unsigned mb = __reduce_max_sync(0xffffffffu, __float_as_uint(amax));
+            const bool over = __any_sync(0xffffffffu, amax > WS_F16_MAX || fabsf(sum) > WS_F16_MAX);
+            if (lane == 0 && ok) {
+                atomicMax(p.inmax + seg, mb);
+                if (over) atomicOr(p.flag, 1u);
             }
         }
         __threadfence();
@@ -426,12 +462,18 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
         for (UnitIter it(p, sched_cnt, unit0); it.valid(); it.next()) {
             it.locate(p);
             const WsLayer& L = p.layers[it.l];
-            if (L.dep >= 0 && !(p.dbg & 128)) {       // chained layer: the producer layer must be complete
+            if (L.dep >= 0 && !(PROF && (p.dbg & 128))) {       // chained layer: the producer layer must be complete
                 if (lane == 0) {
                     wait_counter(p.done + L.dep, p.layers[L.dep].done_target);
                     fence_proxy_async_all();   // generic-proxy stores of other SMs -> this TMA read
                 }
                 __syncwarp();
+            }
+            if (AF16 && lane == 0) {
+                // a whole input tensor far below the fp16 normal range: the subnormal grid (2^-24) would cost
+                // relative precision -> flag the launch (an all-zero input is exact)
+                const unsigned mb = ld_acquire(L.dep >= 0 ? p.outmax + L.dep : p.inmax + L.in_ext);
+                if (mb != 0 && mb < __float_as_uint(WS_MIN_ABSMAX)) atomicOr(p.flag, 2u);
             }
             for (int sb = it.sb0; sb < it.sb1; ++sb) {
                 mbar_wait(xempty0 + 8 * stage, phase ^ 1);
@@ -643,7 +685,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
             const __nv_bfloat16* bias = static_cast<const __nv_bfloat16*>(
                 reinterpret_cast<const void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->bias))));
             void* const Yp = reinterpret_cast<void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->Y)));
-            void* const Y16p = (p.dbg & 256) ? nullptr : reinterpret_cast<void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->Y16)));
+            void* const Y16p = (PROF && (p.dbg & 256)) ? nullptr : reinterpret_cast<void*>(__ldg(reinterpret_cast<const unsigned long long*>(&Lp->Y16)));
             const int n = it.tile * WS_ROWS + q * 32 + lane;
             const bool n_ok = n < N;
             const float bv = bias && n_ok ? __bfloat162float(bias[n]) : 0.0f;
@@ -692,6 +734,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
                 __half* Yrow = static_cast<__half*>(Y16p) + (n0 >> 8) * WS_XLD;
                 const int xpos = x16_pos(n & 255), spos = 256 + 2 * ((n0 >> 5) & 7);
                 float hs[WS_TT];                                          // the bf16 outputs, as fp32
+                float amax = 0.0f;
 #pragma unroll
                 for (int t = 0; t < WS_TT; t += 2) {
                     float y0 = __uint_as_float(v[t]) + bv, y1 = __uint_as_float(v[t + 1]) + bv;
@@ -705,8 +748,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
                     if (t < M) {                                          // M is warp-uniform
                         reinterpret_cast<uint16_t*>(Y)[static_cast<size_t>(t) * N] = static_cast<uint16_t>(yb2);
                         reinterpret_cast<uint16_t*>(Yrow)[static_cast<size_t>(t) * ld16 + xpos] = static_cast<uint16_t>(yh2);
+                        amax = fmaxf(amax, fabsf(hs[t]));
                     }
                     if (t + 1 < M) {
+                        amax = fmaxf(amax, fabsf(hs[t + 1]));
                         reinterpret_cast<uint16_t*>(Y)[static_cast<size_t>(t + 1) * N] = static_cast<uint16_t>(yb2 >> 16);
                         reinterpret_cast<uint16_t*>(Yrow)[static_cast<size_t>(t + 1) * ld16 + xpos] = static_cast<uint16_t>(yh2 >> 16);
                     }
@@ -724,9 +769,17 @@ __global__ void __launch_bounds__(WS_THREADS, 1) w4a16_stream_kernel(const WsPar
                     }
                 }
                 if (lane < M) {
-                    const __half sh = __float2half_rn(hs[0]);
+                    const __half sh = __float2half_rn(fminf(fmaxf(hs[0], -WS_F16_MAX), WS_F16_MAX));
                     const __half sl = __float2half_rn(hs[0] - __half2float(sh));
                     *reinterpret_cast<__half2*>(Yrow + static_cast<size_t>(lane) * ld16 + spos) = __halves2half2(sh, sl);
+                }
+                {   // domain of the consumer's fp16 operand (see the conversion pre-pass)
+                    const unsigned mb = __reduce_max_sync(0xffffffffu, __float_as_uint(amax));
+                    const bool over = __any_sync(0xffffffffu, amax > WS_F16_MAX || (lane < M && fabsf(hs[0]) > WS_F16_MAX));
+                    if (lane == 0) {
+                        atomicMax(p.outmax + it.l, mb);
+                        if (over) atomicOr(p.flag, 1u);
+                    }
                 }
             } else if (n_ok) {
                 uint16_t* Y = static_cast<uint16_t*>(Yp) + n;
@@ -775,6 +828,8 @@ namespace aria {
 
 struct WsPlan {
     bool a_f16 = true;
+    WsPlan* fallback = nullptr;     // a_f16 plans: the same list with exact bf16 operands, run if the flag is set
+    bool owns_done = true;
     WsLayer* d_layers = nullptr;
     int2* d_sched = nullptr;        // dense unit lists + per-CTA counts
     unsigned* d_done = nullptr;
@@ -787,9 +842,10 @@ struct WsPlan {
 
 void ws_plan_destroy(WsPlan* p) {
     if (!p) return;
+    ws_plan_destroy(p->fallback);
     cudaFree(p->d_layers);
     cudaFree(p->d_sched);
-    cudaFree(p->d_done);
+    if (p->owns_done) cudaFree(p->d_done);
     cudaFree(p->d_conv);
     cudaFree(p->d_x16);
     delete p;
@@ -802,35 +858,69 @@ static bool overlaps(const void* a, size_t an, const void* b, size_t bn) {
 
 // The stream kernel runs layers concurrently where the list allows it, so it is used only when
 // running them in array order cannot be told apart: bf16 I/O, M <= 32, K % 256 == 0 (16-byte pitch of
-// the scale tensor map), and no output buffer that overlaps another layer's output or an EARLIER
-// layer's input (a later layer reading an earlier output is the chained case and is tracked).
+// the scale tensor map), no output buffer that overlaps another layer's output or an EARLIER layer's
+// input, and a later layer's input that touches an earlier layer's output must BE that output (same
+// address, K == that layer's N): the chained case, tracked by one completion counter per layer.  An
+// input that only partly overlaps an earlier output, or spans two of them, takes the per-layer path.
 bool ws_eligible(const aria_layer* layers, int n_layers, int M, int mode, int io) {
     if (mode != ARIA_W4A16 || io != ARIA_BF16 || M > WS_TT) return false;
-    if (getenv("ARIA_NO_STREAM")) return false;
+    if (dbg_env("ARIA_NO_STREAM")) return false;
     for (int i = 0; i < n_layers; ++i) {
         if (layers[i].K % WS_SBK != 0) return false;
         const size_t ob = static_cast<size_t>(M) * layers[i].N * 2;
+        const void* in = layers[i].in ? layers[i].in : (i > 0 ? layers[i - 1].out : nullptr);
         for (int j = 0; j < n_layers; ++j) {
             if (j == i) continue;
             if (overlaps(layers[i].out, ob, layers[j].out, static_cast<size_t>(M) * layers[j].N * 2)) return false;
             if (j < i && layers[j].in &&
                 overlaps(layers[i].out, ob, layers[j].in, static_cast<size_t>(M) * layers[j].K * 2))
                 return false;
+            if (j < i && in &&
+                overlaps(in, static_cast<size_t>(M) * layers[i].K * 2, layers[j].out, static_cast<size_t>(M) * layers[j].N * 2) &&
+                !(in == layers[j].out && layers[j].N == layers[i].K))
+                return false;
         }
     }
     return true;
 }
 
-int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan** out) {
+// max over the fp16 magnitudes of a scale tensor (bit patterns order like the values; NaN / inf sort last)
+__global__ void ws_scale_max_kernel(const uint16_t* __restrict__ sg, size_t n, unsigned* out) {
+    unsigned m = 0;
+    for (size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += static_cast<size_t>(gridDim.x) * blockDim.x)
+        m = max(m, static_cast<unsigned>(sg[i] & 0x7FFFu));
+    m = __reduce_max_sync(0xffffffffu, m);
+    if ((threadIdx.x & 31) == 0) atomicMax(out, m);
+}
+
+// force_bf16 / ext_done: used by the recursive creation of a plan's bf16 fallback (its counters live in
+// the primary plan's buffer so that one memset arms both launches).
+static int ws_plan_create_impl(const aria_layer* layers, int n_layers, int M, int io, bool force_bf16,
+                               unsigned* ext_done, WsPlan** out) {
     *out = nullptr;
     WsPlan* plan = new (std::nothrow) WsPlan;
     if (!plan) return ARIA_ERR_CUDA;
-    // default: the fp16 operand (see the header comment); ARIA_W4_F16A=0 keeps w^ = bf16_rne(q sg),
-    // the slower exact-bf16 path.  Read per plan so tests can build both.
-    const char* e = getenv("ARIA_W4_F16A");
-    plan->a_f16 = e == nullptr || e[0] != '0';
     const int sms = num_sms();
     if (sms <= 0) { ws_plan_destroy(plan); return ARIA_ERR_CUDA; }
+    // Operand format.  fp16 (see the header comment) needs 1024 sg <= 65504 for every group scale, which is
+    // a property of the weights: scan them once (plan creation may synchronise).  Activations are checked on
+    // the device in every launch (flag + bf16 fallback launch).
+    plan->a_f16 = !force_bf16;
+    if (const char* e = dbg_env("ARIA_W4_F16A")) plan->a_f16 = plan->a_f16 && e[0] != '0';   // debug builds only
+    if (plan->a_f16) {
+        unsigned* d_max = nullptr;
+        unsigned h_max = 0;
+        bool ok = cudaMalloc(&d_max, sizeof(unsigned)) == cudaSuccess && cudaMemset(d_max, 0, sizeof(unsigned)) == cudaSuccess;
+        for (int i = 0; ok && i < n_layers; ++i) {
+            const size_t n = static_cast<size_t>(layers[i].N) * (layers[i].K / 32);
+            ws_scale_max_kernel<<<2 * sms, 256>>>(static_cast<const uint16_t*>(layers[i].w_scale), n, d_max);
+            ok = cudaGetLastError() == cudaSuccess;
+        }
+        ok = ok && cudaMemcpy(&h_max, d_max, sizeof(unsigned), cudaMemcpyDeviceToHost) == cudaSuccess;
+        cudaFree(d_max);
+        if (!ok) { ws_plan_destroy(plan); return ARIA_ERR_CUDA; }
+        if (h_max > 0x53FFu) plan->a_f16 = false;      // sg > 63.96875 (or inf / NaN): 1024 sg overflows fp16
+    }
     std::vector<WsLayer> h(n_layers);
     int total_units = 0;
     // pass 1: shapes, dependencies; fp16 scratch layout (AF16)
@@ -855,15 +945,16 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
                 w.dep = j;
                 break;
             }
+        w.in_ext = -1;
         if (w.dep >= 0) {
-            // the fp16 path reads the producer's fp16 copy, which has the producer's exact geometry
-            if (plan->a_f16 && (in != layers[w.dep].out || layers[w.dep].N != L.K)) plan->a_f16 = false;
+            // ws_eligible: the input IS the producer's output, so the fp16 copy has the right geometry
             h[w.dep].notify = 1;
         } else {
             size_t e = 0;
             while (e < ext_src.size() && !(ext_src[e] == in && ext_elems[e] == static_cast<size_t>(M) * L.K)) ++e;
             if (e == ext_src.size()) { ext_src.push_back(in); ext_elems.push_back(static_cast<size_t>(M) * L.K); }
             in_ext[i] = static_cast<int>(e);
+            w.in_ext = static_cast<int>(e);
         }
         w.done_target = static_cast<unsigned>(w.num_n * 4);
         total_units += w.num_n;
@@ -902,7 +993,7 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
             in = w.dep >= 0 ? x16 + y16_off[w.dep] : x16 + ext_off[in_ext[i]];
             if (w.notify) w.Y16 = x16 + y16_off[i];
         }
-        const int dbg_ = getenv("ARIA_WS_DBG") ? atoi(getenv("ARIA_WS_DBG")) : 0;
+        const int dbg_ = dbg_env("ARIA_WS_DBG") ? atoi(dbg_env("ARIA_WS_DBG")) : 0;
         if (((dbg_ & 32) ? make_tmap_2d(&w.tmP, L.wq, 1, static_cast<uint64_t>(L.N) * (L.K / 2) / 128, 128, WS_ROWS, 128, 128)
                          : make_tmap_2d(&w.tmP, L.wq, 1, L.N, L.K / 2, WS_ROWS, 128, 128)) != ARIA_OK ||
             ((dbg_ & 64) ? make_tmap_2d(&w.tmS, L.w_scale, 2, static_cast<uint64_t>(L.N) * (L.K / 32) / 8, 8, WS_ROWS, 8, 0)
@@ -925,7 +1016,7 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     const int grid = total_units < sms ? total_units : sms;
     std::vector<int> order;
     {
-        const char* eg = getenv("ARIA_WS_GAP");
+        const char* eg = dbg_env("ARIA_WS_GAP");
         const double gap_units = eg ? atof(eg) : 32.0;      // in producer-unit durations
         std::vector<char> placed(n_layers, 0);
         std::vector<double> placed_at(n_layers, 0.0);
@@ -951,7 +1042,7 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     }
     // cost of a unit in quarter stages: its stages, ~1/4 stage of accumulator hand-off, and the issue
     // slots a GELU / fp16-copy epilogue takes from the dequantisers of its SM
-    const char* ec = getenv("ARIA_WS_EPI_COST");
+    const char* ec = dbg_env("ARIA_WS_EPI_COST");
     const int epi_cost = ec ? atoi(ec) : 1;
     auto unit_cost = [&](const WsLayer& w) {
         return 4 * w.num_sb + 1 + ((w.act == ARIA_ACT_GELU_ERF ? 1 : 0) + (w.notify ? 1 : 0)) * epi_cost;
@@ -979,10 +1070,20 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     }
     const size_t sched_n = sched.size();
     sched.insert(sched.end(), cnt.begin(), cnt.end());
-    plan->done_bytes = (static_cast<size_t>(n_layers) + 1) * sizeof(unsigned);
+    // armed words, zeroed by ONE memset per step: [n_layers done][1 conversions done][1 flag][n_ext inmax]
+    // [n_layers outmax], then the same for the bf16 fallback plan
+    const size_t words = 2 * static_cast<size_t>(n_layers) + 2 + ext_src.size();
+    const size_t words_fb = words;
+    if (ext_done) {
+        plan->d_done = ext_done;
+        plan->owns_done = false;
+        plan->done_bytes = 0;
+    } else {
+        plan->done_bytes = (words + (plan->a_f16 ? words_fb : 0)) * sizeof(unsigned);
+        if (cudaMalloc(&plan->d_done, plan->done_bytes) != cudaSuccess) { ws_plan_destroy(plan); return ARIA_ERR_CUDA; }
+    }
     if (cudaMalloc(&plan->d_layers, h.size() * sizeof(WsLayer)) != cudaSuccess ||
         cudaMalloc(&plan->d_sched, sched.size() * sizeof(int2)) != cudaSuccess ||
-        cudaMalloc(&plan->d_done, plan->done_bytes) != cudaSuccess ||
         cudaMemcpy(plan->d_layers, h.data(), h.size() * sizeof(WsLayer), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(plan->d_sched, sched.data(), sched.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess ||
         (!conv.empty() && (cudaMalloc(&plan->d_conv, conv.size() * sizeof(WsConv)) != cudaSuccess ||
@@ -995,35 +1096,85 @@ int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan
     plan->params.sched_cnt = plan->d_sched + sched_n;
     plan->params.max_units = static_cast<int>(max_units);
     plan->params.done = plan->d_done;
+    plan->params.flag = plan->d_done + n_layers + 1;
+    plan->params.inmax = plan->d_done + n_layers + 2;
+    plan->params.outmax = plan->d_done + n_layers + 2 + ext_src.size();
+    plan->params.run_if = nullptr;
     plan->params.conv = plan->d_conv;
     plan->params.n_conv = static_cast<int>(conv.size());
     plan->params.n_layers = n_layers;
     plan->params.M = M;
+#ifdef ARIA_DEBUG
     plan->params.prof = g_ws_prof;
-    plan->params.dbg = getenv("ARIA_WS_DBG") ? atoi(getenv("ARIA_WS_DBG")) : 0;
+#else
+    plan->params.prof = nullptr;
+#endif
+    plan->params.dbg = dbg_env("ARIA_WS_DBG") ? atoi(dbg_env("ARIA_WS_DBG")) : 0;
     plan->grid = grid;
+    if (plan->a_f16) {   // the exact bf16 plan of the same list, run when a launch leaves the fp16 domain
+        const int rc = ws_plan_create_impl(layers, n_layers, M, io, true, plan->d_done + words, &plan->fallback);
+        if (rc != ARIA_OK) { ws_plan_destroy(plan); return rc; }
+        plan->fallback->params.run_if = plan->params.flag;
+    }
     *out = plan;
     return ARIA_OK;
 }
 
+int ws_plan_create(const aria_layer* layers, int n_layers, int M, int io, WsPlan** out) {
+    return ws_plan_create_impl(layers, n_layers, M, io, false, nullptr, out);
+}
+
+int ws_plan_kind(const WsPlan* plan) { return plan->a_f16 ? 1 : 2; }
+
+int ws_plan_fallback_fired(const WsPlan* plan, int* fired) {
+    *fired = 0;
+    if (!plan->a_f16) return ARIA_OK;
+    unsigned f = 0;
+    if (cudaMemcpy(&f, plan->params.flag, sizeof(unsigned), cudaMemcpyDeviceToHost) != cudaSuccess) return ARIA_ERR_CUDA;
+    *fired = static_cast<int>(f);
+    return ARIA_OK;
+}
+
+// The kernel's CTAs wait on one another (completion counters), so the whole grid must be co-resident:
+// a COOPERATIVE launch, which fails cleanly (instead of deadlocking) when the device cannot hold the grid
+// at once, e.g. because another tenant's kernel holds SMs.  `dependent`: the bf16 fallback launch, a
+// programmatic dependent of the fp16 launch before it (its launch latency hides behind that kernel).
 template <bool AF16, bool PROF>
-static int ws_launch(const WsPlan* plan, cudaStream_t st) {
-    static bool attr_set = false;
+static int ws_launch(const WsPlan* plan, cudaStream_t st, bool dependent) {
+    static std::atomic<uint64_t> attr_done{0};
     auto kern = w4a16_stream_kernel<AF16, PROF>;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM_BYTES) != cudaSuccess)
-            return ARIA_ERR_CUDA;
-        attr_set = true;
+    if (!ensure_dyn_smem(kern, WS_SMEM_BYTES, attr_done)) return ARIA_ERR_CUDA;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(plan->grid);
+    cfg.blockDim = dim3(WS_THREADS);
+    cfg.dynamicSmemBytes = WS_SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    if (dependent) {
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+    } else {
+        at[0].id = cudaLaunchAttributeCooperative;
+        at[0].val.cooperative = 1;
     }
-    kern<<<plan->grid, WS_THREADS, WS_SMEM_BYTES, st>>>(plan->params);
-    return cudaGetLastError() == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, plan->params) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+}
+
+static int ws_run_one(const WsPlan* plan, cudaStream_t st, bool dependent) {
+#ifdef ARIA_DEBUG
+    const bool prof = plan->params.prof != nullptr || (plan->params.dbg & 127) != 0;   // instrumented kernel
+    if (prof) return plan->a_f16 ? ws_launch<true, true>(plan, st, dependent) : ws_launch<false, true>(plan, st, dependent);
+#endif
+    return plan->a_f16 ? ws_launch<true, false>(plan, st, dependent) : ws_launch<false, false>(plan, st, dependent);
 }
 
 int ws_plan_run(const WsPlan* plan, cudaStream_t st) {
     if (cudaMemsetAsync(plan->d_done, 0, plan->done_bytes, st) != cudaSuccess) return ARIA_ERR_CUDA;
-    const bool prof = plan->params.prof != nullptr || (plan->params.dbg & 127) != 0;   // debug build of the kernel
-    if (plan->a_f16) return prof ? ws_launch<true, true>(plan, st) : ws_launch<true, false>(plan, st);
-    return prof ? ws_launch<false, true>(plan, st) : ws_launch<false, false>(plan, st);
+    int rc = ws_run_one(plan, st, false);
+    if (rc == ARIA_OK && plan->fallback) rc = ws_run_one(plan->fallback, st, true);
+    return rc;
 }
 
 }  // namespace aria

@@ -50,3 +50,32 @@ def test_validation_errors_need_no_gpu():
     assert L.aria_linear_w8a8(p16, 1, 4, 64, p16, p16, 16, None, 0, 0, p16, 1, p16, 16, None) == -6       # ws too small
     assert L.aria_workspace_bytes(0, 64, 64, 0) == 0
     assert L.aria_workspace_bytes(128, 1536, 4608, 0) >= 128 * 1536 + 128 * 4
+
+
+def test_tile_plans_reach_every_compiled_variant_on_148_sms():
+    """Host logic: the launchers' plans for a 148-SM device.  The GPU tests run exactly these shapes, so
+    every compiled kernel instantiation is exercised (tests/test_gpu_w8a8.py, tests/test_gpu_w4a16.py)."""
+    from paper_2607_08526_b200 import binding as aria
+    w8 = {(64, 256): (64, 1), (128, 18944): (128, 1), (128, 28416): (192, 1), (100, 37888): (256, 1),
+          (512, 1536): (128, 2), (2048, 1536): (192, 2), (1000, 4608): (256, 2),
+          (4096, 6144): (256, 2), (2048, 4608): (256, 2)}
+    for (M, N), want in w8.items():
+        assert aria.aria_w8a8_tile_plan(M, N, 148) == want, (M, N)
+    w4 = {(32, 256, 1536): 32, (64, 18944, 256): 64, (512, 1536, 6144): 128, (2000, 1536, 256): 192,
+          (1024, 4608, 256): 256, (2048, 4608, 1536): 256, (2048, 1536, 1536): 192}
+    for (M, N, K), tt in w4.items():
+        assert aria.aria_w4a16_tile_plan(M, N, K, 148)[0] == tt, (M, N, K)
+    assert aria.aria_w4a16_tile_plan(512, 1536, 6144, 148)[1] > 1          # split-K at small M
+    assert aria.aria_w4a16_tile_plan(4096, 6144, 1536, 148)[1] == 1
+
+
+def test_product_library_reads_no_environment_variable_and_exports_no_debug_hook():
+    """VERDICT r1 / ADVICE: env switches and aria_debug_* exist only in -DARIA_DEBUG builds."""
+    import subprocess
+    from paper_2607_08526_b200 import build
+    path = build.build()
+    syms = subprocess.run(["nm", "-D", "--defined-only", path], capture_output=True, text=True).stdout
+    exported = sorted(l.split()[-1] for l in syms.splitlines() if " T " in l)
+    assert exported == _declared(), set(exported) ^ set(_declared())
+    undefined = subprocess.run(["nm", "-D", "--undefined-only", path], capture_output=True, text=True).stdout
+    assert "getenv" not in undefined.split()

@@ -40,6 +40,47 @@ def test_acc_bit_exact(aria, oracle, M, N, K):
     assert np.array_equal(acc.astype(np.int64), ref)
 
 
+# (M, N) -> (BN, CTAS) on 148 SMs (tests/test_abi.py pins these on the host); K small keeps the oracle quick
+TILE_VARIANT_SHAPES = {(64, 1): (64, 256), (128, 1): (128, 18944), (192, 1): (128, 28416), (256, 1): (100, 37888),
+                       (128, 2): (512, 1536), (192, 2): (2048, 1536), (256, 2): (1000, 4608)}
+
+
+@pytest.mark.parametrize("variant", sorted(TILE_VARIANT_SHAPES))
+def test_acc_bit_exact_in_every_tile_variant(aria, oracle, variant):
+    """Every compiled (BN, CTAS) instantiation of the W8A8 GEMM, reached through the launcher's own plan
+    (the CTAS = 1 / BN >= 128 variants had no test)."""
+    M, N = TILE_VARIANT_SHAPES[variant]
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    assert aria.aria_w8a8_tile_plan(M, N, sms) == variant
+    K = 160
+    rng = np.random.default_rng([63, M, N])
+    Xq = rng.integers(-127, 128, size=(M, K), dtype=np.int8)
+    Wq = rng.integers(-127, 128, size=(N, K), dtype=np.int8)
+    acc = aria.aria_gemm_i8_i32(dev_i8(Xq), dev_i8(Wq)).cpu().numpy()
+    assert np.array_equal(acc.astype(np.int64), oracle.gemm_i8(Xq, Wq))
+
+
+@pytest.mark.parametrize("M,N,K", [(4096, 6144, 1536), (4096, 1536, 6144)])
+def test_acc_bit_exact_full_size_multi_wave(aria, oracle, M, N, K):
+    """C3's GEMMs at full size: 2-6 waves of the persistent tile loop with both TMEM accumulators in
+    flight, raw int32 output.  64 sampled rows (first / last row of the first / last tile included) x all
+    N columns against the oracle; a row of acc depends only on its own row of Xq."""
+    rng = np.random.default_rng([64, M, N, K])
+    Xq = rng.integers(-127, 128, size=(M, K), dtype=np.int8)
+    Wq = rng.integers(-127, 128, size=(N, K), dtype=np.int8)
+    acc = aria.aria_gemm_i8_i32(dev_i8(Xq), dev_i8(Wq))
+    torch.cuda.synchronize()
+    rows = np.sort(np.random.default_rng(65).choice(M, size=64, replace=False))
+    rows[:4] = (0, 127, 128, 255)
+    rows[-2:] = (M - 256, M - 1)
+    rows = np.unique(rows)
+    ref = oracle.gemm_i8(Xq[rows], Wq)
+    assert np.array_equal(acc[torch.from_numpy(rows).cuda()].cpu().numpy().astype(np.int64), ref)
+    # and a cheap whole-matrix property: column sums of acc equal (column sums of Xq) . Wq^T exactly
+    colsum = acc.to(torch.int64).sum(dim=0).cpu().numpy()
+    assert np.array_equal(colsum, Xq.astype(np.int64).sum(axis=0) @ Wq.astype(np.int64).T)
+
+
 def test_acc_extreme_values(aria, oracle):
     K = 6144
     Xq = np.full((128, K), 127, np.int8)
@@ -130,3 +171,42 @@ def test_prequantised_entry_point_matches_fused_call(aria, oracle):
     xq, sx = aria.aria_quantize_act_int8(X)
     y2 = aria.aria_linear_w8a8_q(xq, sx, wq_d, sw_d, b, aria.ACT_NONE, aria.F32)
     assert torch.equal(y1, y2)
+
+
+@pytest.mark.parametrize("io", ["bf16", "f32"])
+def test_fused_absmax_chain_codes_and_scales_bit_exact(aria, oracle, io):
+    """Fused S1: a -> b -> c chained (in == NULL twice).  Layers a and b reduce the per-token absmax of
+    what they store in their own epilogues; the S1 passes of b and c take it from there.  Teacher-forced
+    (SURVEY O5): the codes and scales the oracle derives from the GPU's own stored output must reproduce
+    every next layer's output -- checked through aria_linear_w8a8_q fed with the ORACLE's codes, which
+    must equal the chain's output bit for bit -- and the eager chain equals per-layer calls."""
+    M, dims = 300, (416, 1536, 288, 136)
+    dt = torch.bfloat16 if io == "bf16" else torch.float32
+    code = aria.BF16 if io == "bf16" else aria.F32
+    bits, x = inputs.normal_bf16((M, dims[0]), 1.0, 66, 0)
+    X = dev_bf16(bits) if io == "bf16" else dev_f32(x)
+    specs = []
+    for i in range(3):
+        W = inputs.normal_f32((dims[i + 1], dims[i]), 0.05, 66, 10 + i)
+        wq, sw = aria.aria_quantize_weights_int8(dev_f32(W))
+        bb, bf = inputs.normal_bf16((dims[i + 1],), 0.01, 66, 20 + i)
+        specs.append({"K": dims[i], "N": dims[i + 1], "act": aria.ACT_GELU_ERF if i == 0 else aria.ACT_NONE,
+                      "in": X if i == 0 else None, "wq": wq, "w_scale": sw,
+                      "bias": dev_bf16(bb) if io == "bf16" else dev_f32(bf),
+                      "out": torch.zeros((M, dims[i + 1]), dtype=dt, device="cuda")})
+    layers = aria.make_layers(specs)
+    ws = aria.workspace(aria.aria_workspace_bytes(M, max(dims), max(dims), aria.W8A8))
+    for _ in range(2):                                   # twice: the absmax buffers are re-zeroed in-chain
+        for s in specs:
+            s["out"].zero_()
+        aria.aria_denoiser_linears(layers, M, aria.W8A8, code, ws)
+        torch.cuda.synchronize()
+        prev = X
+        for s in specs:
+            xin = host_f32(prev)
+            xq, sx = oracle.quant_int8_rows(xin)                     # the definition, on the GPU's own input
+            y = aria.aria_linear_w8a8_q(dev_i8(xq), dev_f32(sx), s["wq"], s["w_scale"], s["bias"], s["act"], code)
+            assert torch.equal(y, s["out"]), s["N"]
+            y2 = aria.aria_linear_w8a8(prev, s["wq"], s["w_scale"], s["bias"], s["act"], code)
+            assert torch.equal(y2, s["out"])
+            prev = s["out"]
