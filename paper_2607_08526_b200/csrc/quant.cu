@@ -198,7 +198,7 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
 // One WARP per row (K <= 8 * 32 * VPL): every lane issues all its 16-byte loads up front, the
 // absmax is a pure shuffle reduction, no shared memory and no block barrier.
 template <typename T, int VPL>
-__global__ void __launch_bounds__(VPL > 12 ? 128 : 256)
+__global__ void __launch_bounds__(256)
 quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restrict__ Xq,
                           float* __restrict__ scale, int early, const float* known_absmax,
                           float* zero_absmax) {
@@ -283,9 +283,7 @@ quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restri
 template <typename T, int VPL>
 static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, float* s,
                                     cudaLaunchConfig_t& cfg, int early, const float* known, float* zero) {
-    // wide rows keep many registers per lane: 4 rows per CTA there, so that a 2048-row pass still
-    // spreads over every SM
-    constexpr int WARPS = VPL > 12 ? 4 : 8;
+    constexpr int WARPS = 8;
     cfg.blockDim = dim3(32 * WARPS);
     cfg.gridDim = dim3((R + WARPS - 1) / WARPS);
     return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s, early,
@@ -296,7 +294,8 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
                          bool pdl, bool early_, const float* known, float* zero) {
     const int nvec = C / 8;
     const int early = pdl && early_ ? 1 : 0;
-    {   // warp-per-row variants: bf16 rows up to 6144 elements, fp32 rows up to 3072 (wider: one CTA per row, below)
+    {   // warp-per-row variants: rows up to 3072 elements (wider rows: one CTA per row, below; a 24-vector
+        // warp-per-row variant for 6144-element bf16 rows was measured slower: 2.18 vs 2.08 ms per C5 step)
         cudaLaunchConfig_t cfg = {};
         cfg.stream = st;
         cudaLaunchAttribute at[1];
@@ -311,7 +310,6 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
             if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg, early, known, zero);
             else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg, early, known, zero);
             else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg, early, known, zero);
-            else if (vpl <= 24) e = launch_warp_rows<__nv_bfloat16, 24>(X, R, C, q, s, cfg, early, known, zero);
             else done = false;
         } else {
             if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg, early, known, zero);
