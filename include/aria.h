@@ -204,6 +204,17 @@ ARIA_API const char* aria_status_string(int status);
 ARIA_API int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, int32_t* acc,
                      void* stream);
 
+/* Measurement helper, NOT part of the hot path (SURVEY.md S7 hard part 2 / S8(d): "measure an int8
+ * peak on the box first: a plain back-to-back tcgen05.mma kind::i8 issue loop with no memory
+ * traffic"): every SM (ctas = 1) or SM pair (ctas = 2, cta_group::2) issues `iters` groups of four
+ * 128*ctas x 256 x K tcgen05.mma (K = 32 for kind 0 = kind::i8 s8 x s8 -> s32, K = 16 for kind 1 =
+ * kind::f16 bf16 x bf16 -> f32) on pseudo-random operands resident in shared memory, nothing loaded or
+ * stored meanwhile.  The launch is repeated back to back for `seconds` (0: once after a warm-up) and
+ * the LAST launch is reported: out[0] = operations per second (2 MNK per MMA, CUDA events), out[1] =
+ * SM clock in MHz inside the loop (clock64 / globaltimer), out[2] = SM cycles per tcgen05.mma, out[3] =
+ * launches made.  SYNCHRONOUS; allocates and frees a few hundred bytes of device memory.            */
+ARIA_API int aria_tensor_peak(int kind, int ctas, int iters, double seconds, double* out, void* stream);
+
 /* Host-only introspection of the launch plans (no device needed; used by the tests to prove that
  * every compiled tile variant is reached): the (BN, CTAS) tile of the W8A8 GEMM for an [M,N] output on
  * a device with `sms` SMs (BN in {64,128,192,256} output channels, CTAS = 2: tcgen05 cta_group::2

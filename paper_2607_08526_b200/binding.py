@@ -67,6 +67,7 @@ def lib() -> ctypes.CDLL:
         L.aria_stack_plan_fallback_fired.argtypes = [c_void_p, ctypes.POINTER(c_int)]
         L.aria_w8a8_tile_plan.argtypes = [c_int, c_int, c_int, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
         L.aria_w4a16_tile_plan.argtypes = [c_int, c_int, c_int, c_int, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
+        L.aria_tensor_peak.argtypes = [c_int, c_int, c_int, ctypes.c_double, ctypes.POINTER(ctypes.c_double), c_void_p]
         L.aria_stack_plan_destroy.argtypes = [c_void_p]
         L.aria_stack_plan_destroy.restype = None
         for name in EXPORTS:
@@ -82,7 +83,7 @@ EXPORTS = ("aria_linear_w8a8_q", "aria_quantize_weights_int8", "aria_quantize_we
            "aria_denoiser_linears_host", "aria_workspace_bytes", "aria_workspace_bytes_host",
            "aria_status_string", "aria_gemm_i8_i32", "aria_version", "aria_stack_plan_create",
            "aria_stack_plan_run", "aria_stack_plan_is_streaming", "aria_stack_plan_destroy",
-           "aria_stack_plan_fallback_fired", "aria_w8a8_tile_plan", "aria_w4a16_tile_plan")
+           "aria_stack_plan_fallback_fired", "aria_w8a8_tile_plan", "aria_w4a16_tile_plan", "aria_tensor_peak")
 
 
 def _check(rc: int, what: str):
@@ -262,3 +263,10 @@ def aria_w4a16_tile_plan(M: int, N: int, K: int, sms: int = 148):
 
 def aria_stack_plan_destroy(plan: c_void_p):
     lib().aria_stack_plan_destroy(plan)
+
+
+def aria_tensor_peak(kind: int, ctas: int = 1, iters: int = 4096, seconds: float = 0.0):
+    """Tensor-pipe issue-loop peak (measurement helper): kind 0 = int8, 1 = bf16.  Returns a dict."""
+    out = (ctypes.c_double * 4)()
+    _check(lib().aria_tensor_peak(kind, ctas, iters, float(seconds), out, _stream()), "aria_tensor_peak")
+    return {"ops_per_s": out[0], "sm_mhz": out[1], "cycles_per_mma": out[2], "launches": int(out[3])}

@@ -266,6 +266,16 @@ __attribute__((visibility("default"))) void aria_debug_ws_profile(long long* buf
 __attribute__((visibility("default"))) void aria_debug_w8_profile(long long* buf) { w8_set_profile_buffer(buf); }
 #endif
 
+int aria_tensor_peak(int kind, int ctas, int iters, double seconds, double* out, void* stream) {
+    if (!out) return ARIA_ERR_NULL;
+    if ((kind != 0 && kind != 1) || (ctas != 1 && ctas != 2) || iters <= 0 || iters > (1 << 24) || seconds < 0.0 ||
+        seconds > 30.0)
+        return ARIA_ERR_SHAPE;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    return tensor_peak(kind, ctas, iters, seconds, out, static_cast<cudaStream_t>(stream));
+}
+
 int aria_w8a8_tile_plan(int M, int N, int sms, int* bn, int* ctas) {
     if (!bn || !ctas) return ARIA_ERR_NULL;
     if (M <= 0 || N <= 0 || sms <= 0) return ARIA_ERR_SHAPE;

@@ -83,6 +83,9 @@ void w4_plan(int M, int N, int K, int sms, int* tt, int* splits);   // the (toke
 void w4_set_profile_buffer(long long* p);  // per-CTA role timestamps
 #endif
 
+// ---- peak.cu: measurement helper (tensor-pipe issue loop)
+int tensor_peak(int kind, int ctas, int iters, double seconds, double* out, cudaStream_t st);
+
 // ---- w4a16_stream.cu: persistent weight-streaming kernel for a list of W4A16 linears at M <= 32
 struct WsPlan;
 bool ws_eligible(const aria_layer* layers, int n_layers, int M, int mode, int io);
