@@ -22,7 +22,9 @@
  *
  * Parity pins: tests/test_oracle_*.py (hand-worked H1/H2 from SURVEY.md S8(c),
  * brute-force nearest-code search, invariants, closed forms, numpy fp64 matmul,
- * numpy/ml_dtypes conversions).  Parity unpinned: none.
+ * numpy/ml_dtypes conversions; O6 and O7: hand-worked H3 / H4 in tests/golden/,
+ * integer special cases, numpy, the alpha = 0 / beta = -1 invariants).
+ * Parity unpinned: none.
  */
 #include <math.h>
 #include <stdint.h>
@@ -331,6 +333,74 @@ void oracle_dequant_int4(const int8_t *codes, const uint16_t *sg_bits, int varia
                                   ? (double)oracle_fp16_bits_to_f32(oracle_f32_to_fp16_bits(prod))
                                   : (double)prod;
         }
+}
+
+/* -------------------------------------------------------------------- O6 */
+/* q8 weight-only linear, "W8A16" (weights
+ * "compressed to 8-bit ... integers (labelled q8)" with the arithmetic left in half
+ * precision; Table II col. q8, L129-131).  Weights: the S0 int8 format (per-output-
+ * channel scale sw[n], codes in [-127,127]); activations bf16; like O4 the
+ * dequantised weight is fed to a bf16 GEMM with fp32 accumulation (R18):
+ *   variant 0: w^ = bf16_rne(q * sw[n])   (ONE rounding of the exact product)
+ *   variant 1: w^ = q * sw[n] exactly
+ *   y = sum_k (double)x[m,k] * (double)w^[n,k] + (double)b[n]; act == 1: GELU. */
+void oracle_linear_w8a16(const float *X, const int8_t *Wq, const float *sw, const double *bias,
+                         int act, int variant, int64_t M, int64_t N, int64_t K, double *y)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < N; ++n) {
+        double wrow[K];
+        for (int64_t k = 0; k < K; ++k) {
+            double prod = (double)Wq[n * K + k] * (double)sw[n]; /* exact: 8-bit x 24-bit */
+            if (variant == 0)
+                wrow[k] = (double)oracle_bf16_bits_to_f32(oracle_f64_to_bf16_bits(prod));
+            else
+                wrow[k] = prod;
+        }
+        for (int64_t m = 0; m < M; ++m) {
+            double a = 0.0;
+            for (int64_t k = 0; k < K; ++k)
+                a += (double)X[m * K + k] * wrow[k];
+            if (bias)
+                a += bias[n];
+            if (act == 1)
+                a = oracle_gelu_erf(a);
+            y[m * N + n] = a;
+        }
+    }
+}
+
+/* -------------------------------------------------------------------- O7 */
+/* In-graph activation steering of the residual stream.
+ * op 0, additive injection -- PAPER.md eq. 2 (L94-98): for every token row t
+ *     h[t,:] <- h[t,:] + alpha * hbar_norm * d[:]
+ *   "where ||h-bar|| is the mean baseline residual norm at l" (a given scalar),
+ *   d the unit direction of eq. 1.
+ * op 1, projection -- PAPER.md L192 / L248: "amplifying (beta > 0) or removing
+ *   (beta < 0) the direction component already present per token":
+ *     c_t = sum_j h[t,j] * d[j];   h[t,:] <- h[t,:] + beta * c_t * d[:]
+ *   (beta = -1 removes the component when |d| = 1; R19).
+ * Strength 0 "leaves the pass unchanged" (L98) / "the output is bit-identical to
+ * the base model" (L77): the caller's array is returned untouched, -0.0 included.
+ * All arithmetic in fp64; H is fp32 (bf16 values widened by the caller). */
+void oracle_steer(const float *H, int64_t M, int64_t D, const float *d, double strength,
+                  double hbar_norm, int op, double *out)
+{
+    for (int64_t t = 0; t < M; ++t) {
+        double c = 0.0;
+        if (op == 1)
+            for (int64_t j = 0; j < D; ++j)
+                c += (double)H[t * D + j] * (double)d[j];
+        for (int64_t j = 0; j < D; ++j) {
+            double h = (double)H[t * D + j];
+            if (strength == 0.0)
+                out[t * D + j] = h;
+            else if (op == 0)
+                out[t * D + j] = h + strength * hbar_norm * (double)d[j];
+            else
+                out[t * D + j] = h + strength * c * (double)d[j];
+        }
+    }
 }
 
 /* ------------------------------------------------------------ output cast */

@@ -69,6 +69,12 @@ def _load():
         L.oracle_dequant_int4.restype = None
         L.oracle_dequant_int4.argtypes = [POINTER(c_int8), POINTER(c_uint16), c_int, c_int64,
                                           c_int64, c_int, POINTER(c_double)]
+        L.oracle_linear_w8a16.restype = None
+        L.oracle_linear_w8a16.argtypes = [POINTER(c_float), POINTER(c_int8), POINTER(c_float), POINTER(c_double),
+                                          c_int, c_int, c_int64, c_int64, c_int64, POINTER(c_double)]
+        L.oracle_steer.restype = None
+        L.oracle_steer.argtypes = [POINTER(c_float), c_int64, c_int64, POINTER(c_float), c_double, c_double, c_int,
+                                   POINTER(c_double)]
         L.oracle_round_out.restype = None
         L.oracle_round_out.argtypes = [POINTER(c_double), c_int64, c_int, POINTER(c_float)]
         L.oracle_num_threads.restype = c_int
@@ -212,6 +218,35 @@ def linear_w4a16(X, codes, sg_bits, bias=None, act: int = ACT_NONE, variant: int
                                 None if b is None else _p(b, c_double), act, variant, M, N, K,
                                 group, _p(y, c_double))
     return y
+
+
+# ------------------------------------------------------------------------ O6
+def linear_w8a16(X, Wq, sw, bias=None, act: int = ACT_NONE, variant: int = 0):
+    """O6 (q8 weight-only): y fp64 [M,N].  X fp32 holding bf16 values; Wq int8 [N,K]; sw fp32 [N]."""
+    X = _c(X, np.float32)
+    Wq = _c(Wq, np.int8)
+    sw = _c(sw, np.float32)
+    M, K = X.shape
+    N = Wq.shape[0]
+    y = np.empty((M, N), np.float64)
+    b = None if bias is None else _c(bias, np.float64)
+    _load().oracle_linear_w8a16(_p(X, c_float), _p(Wq, c_int8), _p(sw, c_float),
+                                None if b is None else _p(b, c_double), act, variant, M, N, K, _p(y, c_double))
+    return y
+
+
+# ------------------------------------------------------------------------ O7
+STEER_ADD, STEER_PROJECT = 0, 1
+
+
+def steer(H, d, strength: float, hbar_norm: float = 1.0, op: int = STEER_ADD):
+    """O7: eq. 2 additive injection (op 0) or per-token projection (op 1), fp64 out [M,D]."""
+    H = _c(H, np.float32)
+    d = _c(d, np.float32)
+    M, D = H.shape
+    out = np.empty((M, D), np.float64)
+    _load().oracle_steer(_p(H, c_float), M, D, _p(d, c_float), float(strength), float(hbar_norm), op, _p(out, c_double))
+    return out
 
 
 # ---------------------------------------------------------------- output cast
