@@ -263,6 +263,40 @@ def per_linear_table(torch, aria, inputs, pk):
     return out
 
 
+def next_rows(torch, aria, inputs, pk):
+    """SURVEY S8(f) rows built in round 2, each timed the same way as the main step (CUDA-graph replay, CUDA
+    events): NEXT-1 the C5 stack in q8 weight-only mode (W8A16), NEXT-3/4 the paper's per-clip unit -- 8
+    sampling steps of the small-music stack (d_model 1024 x 20 blocks, L47) in W8A8 with the
+    steering step inside the captured graph (L77), strength refreshed per step."""
+    from paper_2607_08526_b200.stack import LinearStack
+    out = {}
+    st = LinearStack(aria.W8A16, M=2048)
+    st.capture()
+    for _ in range(3):
+        st.replay()
+    ms = time_region(torch, st.replay, 10)
+    out["w8a16_c5_stack"] = {"ms": ms, "eff_tflops": st.ops / (ms * 1e-3) / 1e12,
+                             "frac_of_bf16_burst": st.ops / (ms * 1e-3) / 1e12 / pk["bf16_burst"],
+                             "launches": len(st.specs), "weight_mb": round(st.weight_bytes / 1e6, 1)}
+    del st
+    d_model, n_blocks = inputs.MODELS["small-music"]
+    sm = LinearStack(aria.W8A8, M=2048, n_blocks=n_blocks, d_model=d_model)
+    d, norm = inputs.steer_direction(d_model, 0)
+    sm.set_steering(n_blocks // 2, d, norm)
+    sm.capture()
+    span = [0.0, 0.0, 0.3, 0.3, 0.3, 0.3, 0.0, 0.0]
+    off = [0.0] * inputs.SAMPLING_STEPS
+    for _ in range(2):
+        sm.sample(span)
+    ms_on = time_region(torch, lambda: sm.sample(span), 5)
+    ms_off = time_region(torch, lambda: sm.sample(off), 5)
+    out["small_music_8_steps_w8a8_steered"] = {
+        "ms_per_clip": ms_on, "ms_per_clip_strength_0": ms_off, "steps": inputs.SAMPLING_STEPS,
+        "tops": inputs.SAMPLING_STEPS * sm.ops / (ms_on * 1e-3) / 1e12, "layers_per_step": len(sm.specs),
+        "steering": "additive (eq. 2) after block 10, strength 0.3 in steps 2-5, device scalar refreshed per replay"}
+    return out
+
+
 def small_m_stream(torch, aria, inputs, pk, iters=20):
     """SURVEY S8(d) 'C5-shaped stack at M=32, W4A16': the weight-bound regime.  One plan
     (aria_stack_plan_*) = ONE persistent weight-streaming kernel over all 96 layers, captured in a CUDA
@@ -471,10 +505,14 @@ def run_ours(args):
         cpu = {"value": ops / t / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"block 0's 4 linears at 1024 of the 2048 tokens, both modes, {t:.1f} s"}
     ops8, ops4 = st8.ops, st4.ops
-    table = small = None
+    table = small = nxt = None
     if world == 1 and not args.no_per_linear:
         table = per_linear_table(torch, aria, inputs, pk)
         small = small_m_stream(torch, aria, inputs, pk)
+        try:
+            nxt = next_rows(torch, aria, inputs, pk)
+        except Exception as ex:                  # noqa: BLE001
+            log(f"[bench] next_rows failed: {ex!r}")
     # last (they heat the part): the long replay of the same step, then the sustained tensor peaks
     sustained = None
     if world == 1 and not args.no_sustained:
@@ -501,7 +539,7 @@ def run_ours(args):
         "roofline": roofline, "roofline_w8a8_gemm": roofline_w8a8, "tensor_peaks": tp, "sustained": sustained,
         "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": args.steps * (2 * n_l + n_l), "clocks": clocks, "per_linear": table,
-        "small_m": small,
+        "small_m": small, "next_rows": nxt,
     }
     log("[bench] " + json.dumps({k: line[k] for k in ("value", "ms_per_step", "modes", "roofline", "roofline_w8a8_gemm",
                                                        "tensor_peaks", "sustained")}))

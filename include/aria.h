@@ -56,7 +56,8 @@ typedef enum {
 
 typedef enum { ARIA_F32 = 0, ARIA_BF16 = 1 } aria_dtype;
 typedef enum { ARIA_ACT_NONE = 0, ARIA_ACT_GELU_ERF = 1 } aria_act;
-typedef enum { ARIA_W8A8 = 0, ARIA_W4A16 = 1 } aria_mode;
+typedef enum { ARIA_W8A8 = 0, ARIA_W4A16 = 1, ARIA_W8A16 = 2 } aria_mode;
+typedef enum { ARIA_STEER_ADD = 0, ARIA_STEER_PROJECT = 1 } aria_steer_op;
 
 /* ---------------------------------------------------------------------------------------
  * S0 -- weight quantisation, once at load (configs C1-C3; readings R2-R4).
@@ -111,11 +112,24 @@ ARIA_API int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, 
                       int group, int N, const void* bias, int act, void* Y, int yt, void* ws,
                       size_t ws_bytes, void* stream);
 
+/* NEXT-1 -- one q8 weight-only ("W8A16") linear: PAPER.md L78, weights "compressed to 8-bit ...
+ * integers (labelled q8)" with the arithmetic left in half precision; Table II col. q8 (L129-131).
+ * Weights are the S0 int8 format of aria_quantize_weights_int8 (Wq int8 [N,K], w_scale fp32 [N]);
+ * w^[n,k] = bf16(q[n,k] * w_scale[n]) dequantised on chip (the fp32 product rounded to bf16: equals the
+ * definition's single rounding bf16_rne(q * sw) except when the fp32 rounding hits a bf16 tie, < 2^-16 of
+ * the weights, by one ulp); y = sum_k x[m,k] w^[n,k] (fp32 accumulate, tcgen05 kind::f16 bf16) + bias[n];
+ * optional GELU; Y = cast(y, yt).  X: bf16 [M,K].  bias: bf16 [N] or NULL.  ws: as aria_linear_w4a16
+ * (aria_workspace_bytes(M, K, N, ARIA_W8A16)).                                                       */
+ARIA_API int aria_linear_w8a16(const void* X, int M, int K, const int8_t* Wq, const float* w_scale, int N,
+                               const void* bias, int act, void* Y, int yt, void* ws, size_t ws_bytes,
+                               void* stream);
+
 /* S5 -- one denoising step's stack of linears (PAPER.md L73 graph replay; config C5).
  * Layers run in array order on `stream`, each reading `in` [M,K] and writing `out` [M,N], both
  * of dtype `io` (bf16 or fp32; W4A16 requires bf16).  `in == NULL` chains the layer to the
  * previous layer's `out` (its N must equal this K).  mode W8A8: wq = int8 [N,K], w_scale = fp32
- * [N]; mode W4A16: wq = packed int4 [N,K/2], w_scale = fp16 bits [N,K/32].  bias has dtype `io`,
+ * [N]; mode W4A16: wq = packed int4 [N,K/2], w_scale = fp16 bits [N,K/32]; mode W8A16: wq = int8 [N,K],
+ * w_scale = fp32 [N], bf16 I/O.  bias has dtype `io`,
  * may be NULL.  Capturable: enqueue only.  Mode W8A8: the S1 pass of a layer whose input the
  * previous layer does not write is overlapped with that layer's GEMM (programmatic dependent
  * launch, two alternating Xq / sx buffers in `ws`); a layer whose output IS the next layer's input
@@ -203,6 +217,19 @@ ARIA_API const char* aria_status_string(int status);
  * [M,N], computed by the same tcgen05 kind::i8 kernel as aria_linear_w8a8.                   */
 ARIA_API int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, int32_t* acc,
                      void* stream);
+
+/* NEXT-3 -- in-graph activation steering of the residual stream, in place (eq. 2,
+ * L94-98; projection variant L192 / L248).  H: [M,D] of dtype `ht` (a DiT block's output, row = token),
+ * d: fp32 [D] direction (unit norm by eq. 1; not checked), strength: DEVICE pointer to one fp32 read at
+ * run time -- a captured graph is replayed with a new strength without re-capture (L77).
+ *   op ARIA_STEER_ADD:      h[t,:] <- h[t,:] + alpha * hbar_norm * d[:]     (eq. 2; hbar_norm = "the mean
+ *                            baseline residual norm" of that block, a host scalar fixed at capture)
+ *   op ARIA_STEER_PROJECT:  c_t = h[t,:] . d;  h[t,:] <- h[t,:] + beta * c_t * d[:]   (beta < 0 removes,
+ *                            beta > 0 amplifies the component already present; hbar_norm ignored)
+ * *strength == 0 leaves H untouched, bit for bit ("at strength 0 the output is bit-identical to the base
+ * model", L77).  D % 8 == 0; fp32 arithmetic, one rounding to `ht`.  Enqueue only, capturable.        */
+ARIA_API int aria_steer(void* H, int ht, int M, int D, const float* d, const float* strength, float hbar_norm,
+                        int op, void* stream);
 
 /* Measurement helper, NOT part of the hot path (SURVEY.md S7 hard part 2 / S8(d): "measure an int8
  * peak on the box first: a plain back-to-back tcgen05.mma kind::i8 issue loop with no memory

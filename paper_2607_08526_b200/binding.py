@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libaria_b200.so")
 
 F32, BF16 = 0, 1
 ACT_NONE, ACT_GELU_ERF = 0, 1
-W8A8, W4A16 = 0, 1
+W8A8, W4A16, W8A16 = 0, 1, 2
+STEER_ADD, STEER_PROJECT = 0, 1
 
 _lib = None
 
@@ -56,6 +57,9 @@ def lib() -> ctypes.CDLL:
                                          c_int, c_int, c_void_p, c_int, c_void_p]
         L.aria_linear_w4a16.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p,
                                         c_int, c_void_p, c_int, c_void_p, c_size_t, c_void_p]
+        L.aria_linear_w8a16.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p,
+                                        c_int, c_void_p, c_int, c_void_p, c_size_t, c_void_p]
+        L.aria_steer.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, ctypes.c_float, c_int, c_void_p]
         L.aria_gemm_i8_i32.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
         L.aria_denoiser_linears.argtypes = [ctypes.POINTER(aria_layer), c_int, c_int, c_int, c_int,
                                             c_void_p, c_size_t, c_void_p]
@@ -83,7 +87,7 @@ EXPORTS = ("aria_linear_w8a8_q", "aria_quantize_weights_int8", "aria_quantize_we
            "aria_denoiser_linears_host", "aria_workspace_bytes", "aria_workspace_bytes_host",
            "aria_status_string", "aria_gemm_i8_i32", "aria_version", "aria_stack_plan_create",
            "aria_stack_plan_run", "aria_stack_plan_is_streaming", "aria_stack_plan_destroy",
-           "aria_stack_plan_fallback_fired", "aria_w8a8_tile_plan", "aria_w4a16_tile_plan", "aria_tensor_peak")
+           "aria_stack_plan_fallback_fired", "aria_w8a8_tile_plan", "aria_w4a16_tile_plan", "aria_tensor_peak", "aria_linear_w8a16", "aria_steer")
 
 
 def _check(rc: int, what: str):
@@ -189,6 +193,26 @@ def aria_linear_w4a16(X, Wq4, g_scale, bias=None, act: int = ACT_NONE, yt: int =
     _check(lib().aria_linear_w4a16(_ptr(X), M, K, _ptr(Wq4), _ptr(g_scale), group, N, _ptr(bias), act,
                                    _ptr(Y), yt, _ptr(ws), ws.numel(), _stream()), "aria_linear_w4a16")
     return Y
+
+
+def aria_linear_w8a16(X, Wq, w_scale, bias=None, act: int = ACT_NONE, yt: int = BF16, ws=None, out=None):
+    M, K = X.shape
+    N = Wq.shape[0]
+    if ws is None:
+        ws = workspace(aria_workspace_bytes(M, K, N, W8A16), X.device)
+    Y = out if out is not None else torch.empty((M, N), dtype=_out_dtype(yt), device=X.device)
+    _check(lib().aria_linear_w8a16(_ptr(X), M, K, _ptr(Wq), _ptr(w_scale), N, _ptr(bias), act, _ptr(Y), yt,
+                                   _ptr(ws), ws.numel(), _stream()), "aria_linear_w8a16")
+    return Y
+
+
+def aria_steer(H: torch.Tensor, d: torch.Tensor, strength: torch.Tensor, hbar_norm: float = 1.0, op: int = STEER_ADD):
+    """In place on H [M,D]; `strength` is a 1-element fp32 DEVICE tensor read by the kernel at run time."""
+    M, D = H.shape
+    assert d.dtype == torch.float32 and strength.dtype == torch.float32 and strength.is_cuda
+    _check(lib().aria_steer(_ptr(H), _dt(H), M, D, _ptr(d), _ptr(strength), float(hbar_norm), op, _stream()),
+           "aria_steer")
+    return H
 
 
 def aria_gemm_i8_i32(Xq, Wq):

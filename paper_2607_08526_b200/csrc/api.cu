@@ -61,8 +61,8 @@ int check_layers(const aria_layer* layers, int n_layers, int M, int mode, int io
                  int* maxN, bool host_io) {
     if (!layers) return ARIA_ERR_NULL;
     if (n_layers <= 0 || M <= 0) return ARIA_ERR_SHAPE;
-    if (mode != ARIA_W8A8 && mode != ARIA_W4A16) return ARIA_ERR_DTYPE;
-    if (bad_dtype(io) || (mode == ARIA_W4A16 && io != ARIA_BF16)) return ARIA_ERR_DTYPE;
+    if (mode != ARIA_W8A8 && mode != ARIA_W4A16 && mode != ARIA_W8A16) return ARIA_ERR_DTYPE;
+    if (bad_dtype(io) || (mode != ARIA_W8A8 && io != ARIA_BF16)) return ARIA_ERR_DTYPE;
     *maxK = 0; *maxN = 0;
     for (int i = 0; i < n_layers; ++i) {
         const aria_layer& L = layers[i];
@@ -89,9 +89,8 @@ int run_layer(const aria_layer& L, const void* in, void* out, int M, int mode, i
         return linear_w8a8_impl(in, io, M, L.K, static_cast<const int8_t*>(L.wq),
                                 static_cast<const float*>(L.w_scale), L.N, L.bias, io, L.act, out, io,
                                 ws, st, pdl && !first, pdl, early && !no_early, fuse);
-    return launch_gemm_w4a16(in, M, L.K, static_cast<const uint8_t*>(L.wq),
-                             static_cast<const uint16_t*>(L.w_scale), L.N, L.bias, L.act, out, io, ws,
-                             ws_bytes, st, pdl && !first);
+    return launch_gemm_w4a16(in, M, L.K, static_cast<const uint8_t*>(L.wq), L.w_scale, L.N, L.bias, L.act,
+                             out, io, ws, ws_bytes, st, pdl && !first, mode == ARIA_W8A16 ? 8 : 4);
 }
 
 }  // namespace
@@ -152,7 +151,7 @@ size_t aria_workspace_bytes(int M, int maxK, int maxN, int mode) {
     if (M <= 0 || maxK <= 0 || maxN <= 0) return 0;
     // two (Xq, sx) buffers and two per-token absmax buffers (fused S1): see aria_denoiser_linears
     if (mode == ARIA_W8A8) return 2 * w8_ws_bytes(M, maxK) + 2 * up256(static_cast<size_t>(M) * 4);
-    if (mode == ARIA_W4A16) {
+    if (mode == ARIA_W4A16 || mode == ARIA_W8A16) {
         // Split-K bound: splits * tiles <= #SMs and a tile holds <= 128 x TT outputs, so the fp32
         // partials never exceed #SMs * 128 * TT * 4 bytes; one counter quad per tile.
         int sms = num_sms();
@@ -246,6 +245,20 @@ int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
                              static_cast<cudaStream_t>(stream), false);
 }
 
+int aria_linear_w8a16(const void* X, int M, int K, const int8_t* Wq, const float* w_scale, int N,
+                      const void* bias, int act, void* Y, int yt, void* ws, size_t ws_bytes, void* stream) {
+    if (!X || !Wq || !w_scale || !Y) return ARIA_ERR_NULL;
+    if (M <= 0 || N <= 0 || K <= 0 || K % 32 != 0 || N % 8 != 0) return ARIA_ERR_SHAPE;
+    if (bad_dtype(yt) || bad_act(act)) return ARIA_ERR_DTYPE;
+    if (misaligned(X) || misaligned(Wq) || misaligned(w_scale) || misaligned(bias) || misaligned(Y) ||
+        misaligned(ws))
+        return ARIA_ERR_ALIGN;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    return launch_gemm_w4a16(X, M, K, reinterpret_cast<const uint8_t*>(Wq), w_scale, N, bias, act, Y, yt, ws,
+                             ws ? ws_bytes : 0, static_cast<cudaStream_t>(stream), false, 8);
+}
+
 int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, int32_t* acc,
                      void* stream) {
     if (!Xq || !Wq || !acc) return ARIA_ERR_NULL;
@@ -265,6 +278,17 @@ __attribute__((visibility("default"))) void aria_debug_w4_profile(long long* buf
 __attribute__((visibility("default"))) void aria_debug_ws_profile(long long* buf) { ws_set_profile_buffer(buf); }
 __attribute__((visibility("default"))) void aria_debug_w8_profile(long long* buf) { w8_set_profile_buffer(buf); }
 #endif
+
+int aria_steer(void* H, int ht, int M, int D, const float* d, const float* strength, float hbar_norm, int op,
+               void* stream) {
+    if (!H || !d || !strength) return ARIA_ERR_NULL;
+    if (M <= 0 || D <= 0 || D % 8 != 0) return ARIA_ERR_SHAPE;
+    if (bad_dtype(ht) || (op != ARIA_STEER_ADD && op != ARIA_STEER_PROJECT)) return ARIA_ERR_DTYPE;
+    if (misaligned(H) || misaligned(d) || (reinterpret_cast<uintptr_t>(strength) & 3u)) return ARIA_ERR_ALIGN;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    return launch_steer(H, ht, M, D, d, strength, hbar_norm, op, static_cast<cudaStream_t>(stream));
+}
 
 int aria_tensor_peak(int kind, int ctas, int iters, double seconds, double* out, void* stream) {
     if (!out) return ARIA_ERR_NULL;

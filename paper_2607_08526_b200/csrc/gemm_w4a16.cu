@@ -43,19 +43,22 @@ constexpr int W4_G = 3;         // dequantiser groups = A buffers
 // (A CTA-pair variant -- cta_group::2, 256 channels x TT tokens, half of X staged per CTA -- and an X
 // multicast variant were built and measured in round 1: the pair lost ~1.3k cycles per k-block on the
 // cross-CTA "A ready" hand-off, multicast changed nothing (3.79 vs 3.81 ms per C5 step).  Both removed.)
-template <int TT>
+// WB = weight bits: 4 (S4, int4 group-32 + fp16 group scales) or 8 (NEXT-1 "q8", int8 per-channel + fp32
+// scales).  The two formats share everything but the packed-tile geometry and the dequantiser arithmetic.
+template <int TT, int WB = 4>
 struct W4Cfg {
     static constexpr int G = W4_G;
     static constexpr int NB = G;                               // dequantised A buffers
     static constexpr int THREADS = 32 * W4_DEQ_WARP0 + 128 * G;
-    static constexpr int P_ROW = W4_BK / 2;                    // 32 packed bytes per row per k-block
-    static constexpr int P_BYTES = W4_BN * P_ROW;              // 4 KB
+    static constexpr int P_ROW = W4_BK * WB / 8;               // 32 (int4) / 64 (int8) packed bytes per row per k-block
+    static constexpr int P_BYTES = W4_BN * P_ROW;              // 4 KB / 8 KB
     static constexpr int X_ROWS = TT;                          // token rows per X stage
     static constexpr int X_BYTES = X_ROWS * 128;               // x 64 bf16
     static constexpr int A_BYTES = W4_BN * 128;                // 16 KB: 128 rows x 64 bf16
     static constexpr int STG_BYTES = 4096;                     // per epilogue warp: 32 tokens x 128 B
     static constexpr int XS = X_ROWS == 256 ? 3 : X_ROWS == 192 ? 4 : X_ROWS == 128 ? 4 : X_ROWS == 64 ? 6 : 8;   // X ring depth
-    static constexpr int PS = TT >= 192 ? 8 : TT == 128 ? 12 : 16;                // packed ring depth
+    static constexpr int PS = WB == 8 ? (TT >= 192 ? 8 : TT == 32 ? 16 : 12)      // packed ring depth
+                                      : (TT >= 192 ? 8 : TT == 128 ? 12 : 16);
     static constexpr int X_OFF = 0;
     static constexpr int A_OFF = X_OFF + XS * X_BYTES;
     static constexpr int P_OFF = A_OFF + NB * A_BYTES;
@@ -68,11 +71,12 @@ struct W4Cfg {
     static constexpr int ACC_STRIDE = TT == 192 ? 256 : TT;
     static constexpr int TMEM_COLS = 2 * ACC_STRIDE < 32 ? 32 : 2 * ACC_STRIDE;
     static_assert(TT == 32 || TT == 64 || TT == 128 || TT == 192 || TT == 256, "TT");
+    static_assert(WB == 4 || WB == 8, "weight bits");
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
 struct W4Params {
-    const uint16_t* g_scale;  // fp16 bits [N, K/32]
+    const void* g_scale;      // WB = 4: fp16 bits [N, K/32];  WB = 8: fp32 [N]
     const void* bias;         // bf16 [N] or nullptr
     void* Y;
     float* partials;          // [splits, M, N] fp32 (split-K only)
@@ -176,11 +180,30 @@ __device__ __forceinline__ void w4_store(void* Y, int out_t, int64_t idx, float 
         static_cast<__nv_bfloat16*>(Y)[idx] = __float2bfloat16_rn(y);
 }
 
-template <int TT, bool GELU>
-__global__ void __launch_bounds__(W4Cfg<TT>::THREADS, 1)
+// 16 int8 codes (4 words) x one per-channel scale -> 16 bf16, k ascending: w^ = bf16_rne(fl32(q * sw)).
+// (The definition rounds the exact product once; rounding it to fp32 first changes the bf16 result only
+// when the fp32 rounding lands exactly on a bf16 tie: < 2^-16 of the weights, by one bf16 ulp.)
+__device__ __forceinline__ void dequant_i8x16(const uint4& v, float sw, uint4& lo, uint4& hi) {
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    uint32_t o[8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float f0 = static_cast<float>(static_cast<int8_t>(w[i] & 0xFF)) * sw;
+        const float f1 = static_cast<float>(static_cast<int8_t>((w[i] >> 8) & 0xFF)) * sw;
+        const float f2 = static_cast<float>(static_cast<int8_t>((w[i] >> 16) & 0xFF)) * sw;
+        const float f3 = static_cast<float>(static_cast<int8_t>(w[i] >> 24)) * sw;
+        o[2 * i] = cvt_bf16x2(f0, f1);
+        o[2 * i + 1] = cvt_bf16x2(f2, f3);
+    }
+    lo = make_uint4(o[0], o[1], o[2], o[3]);
+    hi = make_uint4(o[4], o[5], o[6], o[7]);
+}
+
+template <int TT, bool GELU, int WB>
+__global__ void __launch_bounds__(W4Cfg<TT, WB>::THREADS, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmX,
                   const __grid_constant__ CUtensorMap tmY, const W4Params p) {
-    using Cfg = W4Cfg<TT>;
+    using Cfg = W4Cfg<TT, WB>;
     constexpr int XS = Cfg::XS, PS = Cfg::PS, G = Cfg::G, NB = Cfg::NB;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
@@ -330,16 +353,44 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         const uint32_t rowoff = (r >> 3) * 1024 + (r & 7) * 128;
         const uint32_t xr = r & 7;
         const uint32_t off0 = r * Cfg::P_ROW;
-        const uint32_t poff0 = off0 ^ (((off0 >> 7) & 1u) << 4);          // 32-byte swizzle
+        const uint32_t poff0 = off0 ^ (((off0 >> 7) & 1u) << 4);          // WB = 4: 32-byte swizzle
         const uint32_t poff1 = (off0 + 16) ^ (((off0 >> 7) & 1u) << 4);
+        const uint32_t px8 = (r >> 1) & 3;                                 // WB = 8: 64-byte swizzle (chunk ^ bits 7-8)
         int it = 0;                               // running k-block counter of this CTA
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
             const int n0 = (tile % num_n) * UN;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             const bool row_ok = n0 + r < p.N;
+            if (WB == 8) {
+                // ---- int8 codes, one fp32 scale per output channel (this thread's row)
+                const float sw = row_ok ? __ldg(static_cast<const float*>(p.g_scale) + n0 + r) : 0.0f;
+                for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    if (it % G != g) continue;
+                    const int stage = it % PS;
+                    mbar_wait(pfull0 + 8 * stage, (it / PS) & 1);
+                    const uint32_t ps = sP + stage * Cfg::P_BYTES + off0;
+                    uint4 pk[4];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) pk[c] = lds128(ps + ((static_cast<uint32_t>(c) ^ px8) << 4));
+                    uint4 o[8];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) dequant_i8x16(pk[c], sw, o[2 * c], o[2 * c + 1]);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(pempty0 + 8 * stage);   // packed bytes are in registers
+                    const int ab = it % NB;
+                    const uint32_t rowb = sA + ab * Cfg::A_BYTES + rowoff;
+                    mbar_wait(aempty0 + 8 * ab, ((it / NB) & 1) ^ 1);  // MMAs reading this A buffer retired
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) sts128(rowb + ((static_cast<uint32_t>(j) ^ xr) << 4), o[j]);
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(afull0 + 8 * ab);
+                }
+                continue;
+            }
             const uint32_t* srow = reinterpret_cast<const uint32_t*>(
-                p.g_scale + static_cast<int64_t>(row_ok ? n0 + r : 0) * gpr);
+                static_cast<const uint16_t*>(p.g_scale) + static_cast<int64_t>(row_ok ? n0 + r : 0) * gpr);
             // the two fp16 group scales of this row and a k-block: one aligned 32-bit load.  The load for
             // this group's NEXT k-block (kb + G) is issued before the current one is processed, which
             // takes the L2 round trip (uncoalesced: one line per row) off the per-k-block chain.
@@ -569,15 +620,15 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     }
 }
 
-template <int TT, bool GELU>
+template <int TT, bool GELU, int WB>
 static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, const W4Params& p,
                      int grid, cudaStream_t st, bool pdl) {
-    using Cfg = W4Cfg<TT>;
+    using Cfg = W4Cfg<TT, WB>;
     static std::atomic<uint64_t> attr_done{0};
-    auto kern = w4a16_gemm_kernel<TT, GELU>;
+    auto kern = w4a16_gemm_kernel<TT, GELU, WB>;
     if (!ensure_dyn_smem(kern, Cfg::SMEM_BYTES, attr_done)) return ARIA_ERR_CUDA;
     CUtensorMap tmP, tmX, tmY;
-    int rc = make_tmap_2d(&tmP, Wq4, 1, N, K / 2, W4_BN, Cfg::P_ROW, Cfg::P_ROW);
+    int rc = make_tmap_2d(&tmP, Wq4, 1, N, K * WB / 8, W4_BN, Cfg::P_ROW, Cfg::P_ROW);
     if (rc != ARIA_OK) return rc;
     rc = make_tmap_2d(&tmX, X, 2, M, K, Cfg::X_ROWS, 64, 128);
     if (rc != ARIA_OK) return rc;
@@ -638,9 +689,9 @@ size_t w4_workspace_bytes(int M, int N, int K, int sms) {
     return counters + (partials + 255) / 256 * 256;
 }
 
-int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uint16_t* g_scale,
+int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const void* g_scale,
                       int N, const void* bias, int act, void* Y, int yt, void* ws, size_t ws_bytes,
-                      cudaStream_t st, bool pdl) {
+                      cudaStream_t st, bool pdl, int wbits) {
     const int sms = num_sms();
     if (sms <= 0) return ARIA_ERR_CUDA;
     int tt, s;
@@ -662,9 +713,12 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uin
     if (s > 1 && cudaMemsetAsync(p.counters, 0, tiles * 4 * sizeof(unsigned), st) != cudaSuccess)
         return ARIA_ERR_CUDA;
     const bool gelu = act == ARIA_ACT_GELU_ERF;
-#define ARIA_W4_LAUNCH(TTV)                                                     \
-    return gelu ? launch_w4<TTV, true>(X, M, K, Wq4, N, p, grid, st, pdl)       \
-                : launch_w4<TTV, false>(X, M, K, Wq4, N, p, grid, st, pdl)
+#define ARIA_W4_LAUNCH(TTV)                                                                           \
+    if (wbits == 8)                                                                                   \
+        return gelu ? launch_w4<TTV, true, 8>(X, M, K, Wq4, N, p, grid, st, pdl)                      \
+                    : launch_w4<TTV, false, 8>(X, M, K, Wq4, N, p, grid, st, pdl);                    \
+    return gelu ? launch_w4<TTV, true, 4>(X, M, K, Wq4, N, p, grid, st, pdl)                          \
+                : launch_w4<TTV, false, 4>(X, M, K, Wq4, N, p, grid, st, pdl)
     if (tt == 32) { ARIA_W4_LAUNCH(32); }
     if (tt == 64) { ARIA_W4_LAUNCH(64); }
     if (tt == 128) { ARIA_W4_LAUNCH(128); }

@@ -74,14 +74,20 @@ void w8_set_profile_buffer(long long* p);  // per-CTA role timestamps
 
 // ---- gemm_w4a16.cu
 // ws: split-K partials + tile counters (w4_workspace_bytes); too small / null -> no split-K.
-int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uint16_t* g_scale,
+// wbits = 4: Wq = packed int4 [N, K/2], scale = fp16 bits [N, K/32];  wbits = 8 (W8A16): Wq = int8 [N, K],
+// scale = fp32 [N].
+int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq, const void* scale,
                       int N, const void* bias, int act, void* Y, int yt, void* ws, size_t ws_bytes,
-                      cudaStream_t st, bool pdl);
+                      cudaStream_t st, bool pdl, int wbits = 4);
 size_t w4_workspace_bytes(int M, int N, int K, int sms);
 void w4_plan(int M, int N, int K, int sms, int* tt, int* splits);   // the (token tile, split-K) launch_gemm_w4a16 picks
 #ifdef ARIA_DEBUG
 void w4_set_profile_buffer(long long* p);  // per-CTA role timestamps
 #endif
+
+// ---- steer.cu: in-graph activation steering (eq. 2 / projection), strength read from device memory
+int launch_steer(void* H, int ht, int M, int D, const float* d, const float* strength, float hbar_norm, int op,
+                 cudaStream_t st);
 
 // ---- peak.cu: measurement helper (tensor-pipe issue loop)
 int tensor_peak(int kind, int ctas, int iters, double seconds, double* out, cudaStream_t st);

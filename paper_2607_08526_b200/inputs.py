@@ -24,9 +24,18 @@ B_STD = 0.01              # config C1
 OUTLIER_FRAC = 0.01       # config C3: "1% of K channels scaled x20"
 OUTLIER_GAIN = 20.0
 
-# (name, K, N, activation-after) of one DiT block's linears, config C5 order.
-BLOCK_LINEARS = (("qkv", D_MODEL, D_QKV, "none"), ("out", D_MODEL, D_MODEL, "none"),
-                 ("up", D_MODEL, D_MLP, "gelu"), ("down", D_MLP, D_MODEL, "none"))
+# The paper's two released DiT sizes: (d_model, blocks).
+MODELS = {"medium": (1536, 24), "small-music": (1024, 20)}
+SAMPLING_STEPS = 8        # 8 denoising steps per clip ("fast preset" 6, L222)
+
+
+def block_linears(d_model: int = D_MODEL):
+    """(name, K, N, activation-after) of one DiT block's linears, config C5 order (fused QKV, MLP ratio 4)."""
+    return (("qkv", d_model, 3 * d_model, "none"), ("out", d_model, d_model, "none"),
+            ("up", d_model, 4 * d_model, "gelu"), ("down", 4 * d_model, d_model, "none"))
+
+
+BLOCK_LINEARS = block_linears(D_MODEL)
 
 
 def normal_f32(shape, std: float, config_id: int, tensor_id: int) -> np.ndarray:
@@ -97,11 +106,22 @@ def c4(M: int, K: int, N: int):
             "b": normal_bf16((N,), B_STD, 4, tid + 200000)}
 
 
-def c5_layer(block: int, which: int, M: int = 2048):
-    """C5: linear `which` (index into BLOCK_LINEARS) of block `block`: own N(0,1)
-    bf16 input (reading R14), W ~N(0,0.02), bf16 bias."""
-    name, K, N, act = BLOCK_LINEARS[which]
+def c5_layer(block: int, which: int, M: int = 2048, d_model: int = D_MODEL):
+    """C5: linear `which` (index into block_linears) of block `block`: own N(0,1)
+    bf16 input (reading R14), W ~N(0,0.02), bf16 bias.  d_model = 1024 gives the small-music
+    shapes (NEXT-4), drawn from config id 6 so that the medium tensors keep their seeds."""
+    name, K, N, act = block_linears(d_model)[which]
+    cid = 5 if d_model == D_MODEL else 6
     tid = block * 16 + which * 4
-    Xb, X = normal_bf16((M, K), 1.0, 5, tid)
+    Xb, X = normal_bf16((M, K), 1.0, cid, tid)
     return {"name": name, "K": K, "N": N, "act": act, "X_bits": Xb, "X": X,
-            "W": normal_f32((N, K), W_STD, 5, tid + 1), "b": normal_bf16((N,), B_STD, 5, tid + 2)}
+            "W": normal_f32((N, K), W_STD, cid, tid + 1), "b": normal_bf16((N,), B_STD, cid, tid + 2)}
+
+
+def steer_direction(d_model: int, tensor_id: int = 0):
+    """A seeded unit direction d (fp32, eq. 1's normalisation applied in fp64) standing in for a
+    difference-in-means direction, and a baseline residual norm ||h-bar|| of the magnitude a N(0,1)
+    residual row has (sqrt(d_model))."""
+    rng = np.random.default_rng([0, 7, int(tensor_id)])
+    v = rng.standard_normal(d_model)
+    return (v / np.linalg.norm(v)).astype(np.float32), float(np.sqrt(d_model))

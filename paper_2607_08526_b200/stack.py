@@ -24,8 +24,8 @@ class LinearStack:
     """`n_blocks` DiT blocks x (QKV, out-proj, MLP up [GELU], MLP down) at M tokens."""
 
     def __init__(self, mode: int, M: int = 2048, n_blocks: int = inputs.N_BLOCKS, keep_host: bool = False,
-                 shared_inputs: bool = True, use_plan: bool = False):
-        self.mode, self.M, self.n_blocks = mode, M, n_blocks
+                 shared_inputs: bool = True, use_plan: bool = False, d_model: int = inputs.D_MODEL):
+        self.mode, self.M, self.n_blocks, self.d_model = mode, M, n_blocks, d_model
         self.plan = None
         self.specs = []          # per layer: dict with device tensors
         self.host = []           # per layer: host arrays (tests only, keep_host=True)
@@ -33,8 +33,8 @@ class LinearStack:
         # its own weights); shared_inputs=False draws one per layer (reading R14, used by tests).
         in_cache = {}
         for blk in range(n_blocks):
-            for which, (name, K, N, act) in enumerate(inputs.BLOCK_LINEARS):
-                L = inputs.c5_layer(blk, which, M=M if not shared_inputs else 1)
+            for which, (name, K, N, act) in enumerate(inputs.block_linears(d_model)):
+                L = inputs.c5_layer(blk, which, M=M if not shared_inputs else 1, d_model=d_model)
                 if shared_inputs:
                     if K not in in_cache:
                         bits, _ = inputs.normal_bf16((M, K), 1.0, 5, 900000 + K)
@@ -43,7 +43,7 @@ class LinearStack:
                 else:
                     xbits, xdev = L["X_bits"], _dev_bf16(L["X_bits"])
                 Wd = torch.from_numpy(L["W"]).cuda()
-                if mode == aria.W8A8:
+                if mode in (aria.W8A8, aria.W8A16):
                     wq, ws = aria.aria_quantize_weights_int8(Wd)
                 else:
                     wq, ws = aria.aria_quantize_weights_int4(Wd)
@@ -69,12 +69,38 @@ class LinearStack:
         self.weight_bytes = sum(s["wq"].numel() * s["wq"].element_size() +
                                 s["w_scale"].numel() * s["w_scale"].element_size() for s in self.specs)
 
+    def set_steering(self, block: int, d: np.ndarray, hbar_norm: float, op: int = aria.STEER_ADD):
+        """In-graph activation steering (eq. 2): after block `block`'s last linear, its output
+        (the stand-in for the residual stream at that block) is steered in place; the strength is a device
+        scalar (`self.strength`) the kernel reads on every replay."""
+        self.steer_after = 4 * block + 3
+        self.steer_d = torch.from_numpy(np.ascontiguousarray(d, dtype=np.float32)).cuda()
+        self.steer_norm, self.steer_op = float(hbar_norm), op
+        self.strength = torch.zeros(1, dtype=torch.float32, device="cuda")
+        n = self.steer_after + 1
+        self._head = aria.make_layers(self.specs[:n])
+        self._tail = aria.make_layers(self.specs[n:]) if n < len(self.specs) else None
+
     def run(self):
         """Enqueue the whole stack on the current stream (no graph)."""
         if self.plan is not None:
             aria.aria_stack_plan_run(self.plan)
+        elif getattr(self, "steer_after", None) is not None:
+            aria.aria_denoiser_linears(self._head, self.M, self.mode, aria.BF16, self.ws)
+            aria.aria_steer(self.specs[self.steer_after]["out"], self.steer_d, self.strength, self.steer_norm,
+                            self.steer_op)
+            if self._tail is not None:
+                aria.aria_denoiser_linears(self._tail, self.M, self.mode, aria.BF16, self.ws)
         else:
             aria.aria_denoiser_linears(self.layers, self.M, self.mode, aria.BF16, self.ws)
+
+    def sample(self, strengths):
+        """The paper's per-clip unit: one graph replay per sampling step, the steering strength
+        refreshed between replays by a device-side copy (no re-capture, L77).  `strengths`: one value per
+        step (zero outside the chosen span of steps)."""
+        for a in strengths:
+            self.strength.fill_(float(a))
+            self.graph.replay()
 
     def __del__(self):
         if getattr(self, "plan", None) is not None:
