@@ -25,6 +25,9 @@ int check_rows_args(const void* in, int t, int R, int C, const void* q, const vo
     return check_arch();
 }
 
+// per-token absmax [M] + per-M-tile completion counters [ceil(M / 128)] of one fused-S1 producer
+size_t w8_fuse_bytes(int M) { return up256(static_cast<size_t>(M) * 4) + up256(static_cast<size_t>((M + 127) / 128) * 4); }
+
 size_t w8_ws_bytes(int M, int K) { return up256(static_cast<size_t>(M) * K) + up256(static_cast<size_t>(M) * 4); }
 
 // Fused S1 (north_star "activation-quantization pass fused into the previous epilogue where shapes
@@ -149,8 +152,9 @@ const char* aria_status_string(int status) {
 
 size_t aria_workspace_bytes(int M, int maxK, int maxN, int mode) {
     if (M <= 0 || maxK <= 0 || maxN <= 0) return 0;
-    // two (Xq, sx) buffers and two per-token absmax buffers (fused S1): see aria_denoiser_linears
-    if (mode == ARIA_W8A8) return 2 * w8_ws_bytes(M, maxK) + 2 * up256(static_cast<size_t>(M) * 4);
+    // two (Xq, sx) buffers, two per-token absmax buffers and two sets of M-tile counters (fused S1): see
+    // aria_denoiser_linears
+    if (mode == ARIA_W8A8) return 2 * w8_ws_bytes(M, maxK) + 2 * w8_fuse_bytes(M);
     if (mode == ARIA_W4A16 || mode == ARIA_W8A16) {
         // Split-K bound: splits * tiles <= #SMs and a tile holds <= 128 x TT outputs, so the fp32
         // partials never exceed #SMs * 128 * TT * 4 bytes; one counter quad per tile.
@@ -322,51 +326,91 @@ int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mod
     if (misaligned(ws)) return ARIA_ERR_ALIGN;
     if (!ws || ws_bytes < aria_workspace_bytes(M, maxK, maxN, mode)) return ARIA_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    // W8A8: the (Xq, sx) scratch alternates between two buffers, and the S1 pass of a layer whose
-    // input the previous layer does not write starts while that layer's GEMM is still running
-    // (programmatic dependent launch): the GEMM of layer i-1 reads buffer (i-1)&1 and writes out[i-1],
-    // the quantiser of layer i reads in[i] and writes buffer i&1.  Every kernel of the chain waits
-    // for its predecessor before it EXITS, so "kernel k complete" implies "kernels < k complete" and
-    // nothing older than layer i-1's GEMM can still be running.
-    //
-    // Fused S1: if layer i+1 reads exactly layer i's output, layer i's epilogue reduces the per-token
-    // absmax of what it stores into one of two [M] buffers (atomicMax) and layer i+1's S1 pass only
-    // rounds.  The buffer a GEMM reduces into is zeroed by that same layer's S1 pass, which has completed
-    // before the GEMM's epilogue starts and -- even when it runs early -- only after every earlier
-    // reader of that buffer has completed (chain rule above).
-    static const bool single_buf = dbg_env("ARIA_W8_SINGLE_BUF") != nullptr;   // debug builds only
-    static const bool no_fuse = dbg_env("ARIA_NO_FUSED_ABSMAX") != nullptr;
-    const size_t half = mode == ARIA_W8A8 && !single_buf ? w8_ws_bytes(M, maxK) : 0;
-    float* amax[2] = {nullptr, nullptr};
-    if (mode == ARIA_W8A8) {
-        uint8_t* b = static_cast<uint8_t*>(ws) + 2 * w8_ws_bytes(M, maxK);
-        amax[0] = reinterpret_cast<float*>(b);
-        amax[1] = reinterpret_cast<float*>(b + up256(static_cast<size_t>(M) * 4));
+    if (mode != ARIA_W8A8) {
+        for (int i = 0; i < n_layers; ++i) {
+            const aria_layer& L = layers[i];
+            rc = run_layer(L, L.in ? L.in : layers[i - 1].out, L.out, M, mode, io, ws, ws_bytes, st, i == 0);
+            if (rc != ARIA_OK) return rc;
+        }
+        return ARIA_OK;
     }
+    // W8A8.  The (Xq, sx) scratch alternates between two buffers.  The S1 pass of layer i+1 runs INSIDE
+    // the GEMM kernel of layer i, on spare warps (gemm_w8a8.cu: w8_side_quant), whenever layer i+1's
+    // input is either untouched by layer i (it is quantised during layer i's mainloop) or exactly layer
+    // i's output (fused S1: layer i's epilogue reduces the per-token absmax of what it stores and counts
+    // finished M-tiles; the side warps round each row as soon as its M-tile is complete).  Layer i+1's
+    // GEMM is then the direct programmatic dependent of layer i's GEMM.  Any other layer (and layer 0)
+    // gets a stand-alone S1 kernel.  Every kernel waits for its predecessor before it touches global
+    // memory, so "kernel k complete" implies "kernels < k complete"; the side job of GEMM i writes the
+    // Xq buffer last read by GEMM i-1.  The absmax / counter set a GEMM reduces into is zeroed by the S1
+    // pass of that same layer (side job of the previous GEMM, or the stand-alone kernel).
+    static const bool no_fuse = dbg_env("ARIA_NO_FUSED_ABSMAX") != nullptr;   // debug builds only
+    static const bool no_side = dbg_env("ARIA_NO_SIDE_QUANT") != nullptr;
+    static const bool pdl = dbg_env("ARIA_NO_PDL") == nullptr;
+    const size_t half = w8_ws_bytes(M, maxK);
+    uint8_t* wsb = static_cast<uint8_t*>(ws);
+    float* amax[2];
+    unsigned* cnt[2];
+    for (int b = 0; b < 2; ++b) {
+        uint8_t* f = wsb + 2 * half + b * w8_fuse_bytes(M);
+        amax[b] = reinterpret_cast<float*>(f);
+        cnt[b] = reinterpret_cast<unsigned*>(f + up256(static_cast<size_t>(M) * 4));
+    }
+    const int n_cnt = (M + 127) / 128;
+    auto xq_of = [&](int i) { return reinterpret_cast<int8_t*>(wsb + (i & 1) * half); };
+    auto sx_of = [&](int i) { return reinterpret_cast<float*>(wsb + (i & 1) * half + up256(static_cast<size_t>(M) * maxK)); };
+    auto in_of = [&](int i) { return layers[i].in ? layers[i].in : layers[i - 1].out; };
     auto feeds_next = [&](int i) {   // layer i+1 reads exactly layer i's [M, N] output
-        if (mode != ARIA_W8A8 || no_fuse || i + 1 >= n_layers) return false;
-        const aria_layer& nx = layers[i + 1];
-        return (nx.in == nullptr || nx.in == layers[i].out) && nx.K == layers[i].N;
+        if (no_fuse || i + 1 >= n_layers) return false;
+        return in_of(i + 1) == layers[i].out && layers[i + 1].K == layers[i].N;
     };
-    int n_fused = 0;                 // producers seen so far: selects the absmax buffer
+    auto independent_of_prev = [&](int i) {   // layer i's input is not written by layer i-1
+        const uintptr_t a0 = reinterpret_cast<uintptr_t>(in_of(i)), a1 = a0 + static_cast<size_t>(M) * layers[i].K * dsize(io);
+        const uintptr_t b0 = reinterpret_cast<uintptr_t>(layers[i - 1].out),
+                        b1 = b0 + static_cast<size_t>(M) * layers[i - 1].N * dsize(io);
+        return !(a0 < b1 && b0 < a1);
+    };
+    std::vector<int> prod(n_layers, -1);       // producer index (selects the absmax / counter set), or -1
+    for (int i = 0, k = 0; i < n_layers; ++i)
+        if (feeds_next(i)) prod[i] = k++;
+    bool s1_done = false;                      // layer i's S1 was done by the side job of GEMM i-1
     for (int i = 0; i < n_layers; ++i) {
         const aria_layer& L = layers[i];
-        const void* in = L.in ? L.in : layers[i - 1].out;
-        bool early = false;
-        if (mode == ARIA_W8A8 && i > 0) {
-            const uintptr_t a0 = reinterpret_cast<uintptr_t>(in), a1 = a0 + static_cast<size_t>(M) * L.K * dsize(io);
-            const uintptr_t b0 = reinterpret_cast<uintptr_t>(layers[i - 1].out),
-                            b1 = b0 + static_cast<size_t>(M) * layers[i - 1].N * dsize(io);
-            early = !single_buf && !(a0 < b1 && b0 < a1);
+        const bool first = i == 0;
+        if (!s1_done) {
+            const bool fused_in = i > 0 && prod[i - 1] >= 0;
+            rc = launch_quant_rows_i8(in_of(i), io, M, L.K, xq_of(i), sx_of(i), st, pdl && !first, false,
+                                      fused_in ? amax[prod[i - 1] & 1] : nullptr,
+                                      prod[i] >= 0 ? amax[prod[i] & 1] : nullptr,
+                                      prod[i] >= 0 ? cnt[prod[i] & 1] : nullptr, n_cnt);
+            if (rc != ARIA_OK) return rc;
         }
-        W8Fuse fuse;
-        if (i > 0 && feeds_next(i - 1)) fuse.amax_in = amax[(n_fused - 1) & 1];
-        if (feeds_next(i)) {
-            fuse.amax_out = fuse.amax_zero = amax[n_fused & 1];
-            ++n_fused;
+        W8Side side;
+        s1_done = false;
+        // (rows of up to 16 KB fit the side warps' staging buffers: K <= 8192 bf16 / 4096 fp32)
+        if (!no_side && i + 1 < n_layers && static_cast<size_t>(layers[i + 1].K) * dsize(io) <= 16384 &&
+            (prod[i] >= 0 || independent_of_prev(i + 1))) {
+            side.X = in_of(i + 1);
+            side.xt = io;
+            side.K2 = layers[i + 1].K;
+            side.q = xq_of(i + 1);
+            side.s = sx_of(i + 1);
+            if (prod[i] >= 0) {
+                side.known_absmax = amax[prod[i] & 1];
+                side.mtile_counters = cnt[prod[i] & 1];
+            }
+            if (prod[i + 1] >= 0) {
+                side.zero_absmax = amax[prod[i + 1] & 1];
+                side.zero_counters = cnt[prod[i + 1] & 1];
+                side.n_zero_counters = n_cnt;
+            }
+            s1_done = true;
         }
-        rc = run_layer(L, in, L.out, M, mode, io, static_cast<uint8_t*>(ws) + (i & 1) * half,
-                       (mode == ARIA_W8A8 ? w8_ws_bytes(M, maxK) : ws_bytes), st, i == 0, early, fuse);
+        W8Epilogue ep;
+        ep.sx = sx_of(i); ep.sw = static_cast<const float*>(L.w_scale); ep.bias = L.bias; ep.bias_t = io;
+        ep.act = L.act; ep.Y = L.out; ep.out_t = io == ARIA_F32 ? 0 : 1;
+        ep.row_absmax = prod[i] >= 0 ? amax[prod[i] & 1] : nullptr;
+        rc = launch_gemm_w8a8(xq_of(i), static_cast<const int8_t*>(L.wq), M, L.N, L.K, ep, st, pdl, &side);
         if (rc != ARIA_OK) return rc;
     }
     return ARIA_OK;

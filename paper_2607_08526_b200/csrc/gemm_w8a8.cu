@@ -17,6 +17,7 @@
 #include <cstdlib>
 
 #include "internal.cuh"
+#include "quant_dev.cuh"
 
 namespace aria {
 
@@ -24,8 +25,9 @@ constexpr int W8_BM = 128;        // MMA M (TMEM lanes)
 constexpr int W8_BK = 128;        // bytes (= int8 elements) per k-block: one 128-byte swizzle row
 constexpr int W8_UMMA_K = 32;     // K per tcgen05.mma for 8-bit operands
 constexpr int W8_EPI_WARPS = 8;   // two warps per TMEM lane quarter, each takes a contiguous run of column chunks (12 warps measured: no gain)
-constexpr int W8_THREADS = 64 + 32 * W8_EPI_WARPS;
-constexpr int W8_STG_BYTES = 2048;  // per-warp output staging: 32 rows x 64 bytes (64-byte swizzle)
+constexpr int W8_SIDE_WARPS = 4;  // spare warps: the S1 pass of the NEXT layer runs inside this kernel (see W8Side)
+constexpr int W8_THREADS = 64 + 32 * W8_EPI_WARPS + 32 * W8_SIDE_WARPS;
+constexpr int W8_SIDE_BYTES = 16384; // per side warp: row staging buffer of the S1 side job (one bulk copy per row)
 
 // CTAS = 1: one CTA computes a 128 x BN tile.  CTAS = 2: a CTA PAIR (cluster of 2, tcgen05 cta_group::2)
 // computes a 256 x BN tile; each CTA stages its own 128 rows of A and only HALF of the B tile, which
@@ -38,20 +40,16 @@ struct W8Cfg {
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int SWB_BYTES = 2 * 2 * BN * 4;           // double-buffered float sw[BN], bias[BN]
     static constexpr int FIXED = 1024 + 256 + SWB_BYTES;       // alignment slack + barriers + scales
-    // Output staging: every epilogue warp rotates through NBUF blocks of [32 rows x 64 B]; a block is
-    // only rewritten after the TMA store issued NBUF stores earlier has read it, so the stores of a
-    // whole tile stay in flight.  4 blocks if the operand ring keeps >= 4 stages, else 2.
-    static constexpr int BUDGET4 = 227 * 1024 - FIXED - W8_EPI_WARPS * 4 * W8_STG_BYTES;
-    static constexpr int NBUF = BUDGET4 / STAGE_BYTES >= 4 ? 4 : 2;
-    static constexpr int RING_BUDGET = 227 * 1024 - FIXED - W8_EPI_WARPS * NBUF * W8_STG_BYTES;
+    static constexpr int SIDE_TOTAL = W8_SIDE_WARPS * W8_SIDE_BYTES;   // 64 KB
+    static constexpr int RING_BUDGET = 227 * 1024 - FIXED - SIDE_TOTAL;
     static constexpr int STAGES = RING_BUDGET / STAGE_BYTES > 8 ? 8 : RING_BUDGET / STAGE_BYTES;
     static constexpr int ACC_STRIDE = BN <= 32 ? 32 : BN <= 64 ? 64 : BN <= 128 ? 128 : 256;
     static constexpr int TMEM_COLS = 2 * ACC_STRIDE < 32 ? 32 : 2 * ACC_STRIDE;
     static constexpr int RING_BYTES = STAGES * STAGE_BYTES;
-    static constexpr int STG_OFF = RING_BYTES;                                      // [8][NBUF][2 KB]
-    static constexpr int SWB_OFF = STG_OFF + W8_EPI_WARPS * NBUF * W8_STG_BYTES;
+    static constexpr int SIDE_OFF = RING_BYTES;                                     // [4][16 KB]
+    static constexpr int SWB_OFF = SIDE_OFF + SIDE_TOTAL;
     static constexpr int BAR_OFF = SWB_OFF + SWB_BYTES;
-    static constexpr int BAR_BYTES = (2 * STAGES + 4) * 8 + 16;
+    static constexpr int BAR_BYTES = (2 * STAGES + 4 + W8_SIDE_WARPS) * 8 + 16;
     static constexpr int SMEM_BYTES = BAR_OFF + BAR_BYTES + 1024;            // + alignment slack
     static_assert(BN % 32 == 0 && BN >= 32 && BN <= 256, "BN");
     static_assert(B_BYTES % 1024 == 0, "B tile must keep 1024-byte alignment");
@@ -60,21 +58,25 @@ struct W8Cfg {
 };
 
 struct W8Params {
+    W8Side side;       // S1 of the next layer, done by the side warps (side.X == nullptr: none)
+    unsigned* mtile_done;   // per-M-tile completion counters bumped by the epilogue warps (chained side job), or nullptr
     const float* sx;
     const float* sw;
     const void* bias;
     float* row_absmax; // fused S1, first half: max |y| per output row (as stored), atomicMax on the bits; or nullptr
+    void* Y;           // [M, N] output (direct-store epilogue)
     int bias_t, act;
     int M, N, K;
 #ifdef ARIA_DEBUG
     long long* prof;   // per-CTA role timestamps (clock64), or nullptr
-    int dbg;           // experiments (ARIA_W8_DBG): 1 = no TMA stores, 2 = no staging stores either
+    int dbg;           // experiments (ARIA_W8_DBG), unused at present
 #endif
 };
 
 #ifdef ARIA_DEBUG
 static long long* g_w8_prof = nullptr;
-void w8_set_profile_buffer(long long* p) { g_w8_prof = p; }
+static int g_w8_prof_launch = 0;          // every launch (graph node) gets its own 148 x 20 slot, 256 slots
+void w8_set_profile_buffer(long long* p) { g_w8_prof = p; g_w8_prof_launch = 0; }
 __device__ __forceinline__ void w8_stamp(const W8Params& p, int slot, long long t0) {
     if (p.prof) p.prof[blockIdx.x * 20 + slot] = clock64() - t0;
 }
@@ -88,23 +90,27 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
     __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
     return *reinterpret_cast<uint32_t*>(&t);
 }
+__device__ __forceinline__ void stg256(void* p, const uint32_t* w) {
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(w[0]), "r"(w[1]), "r"(w[2]),
+                 "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7])
+                 : "memory");
+}
+__device__ __forceinline__ void stg128(void* p, const uint32_t* w) {
+    asm volatile("st.global.v4.b32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
+}
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d)
                  : "memory");
 }
 
-// Epilogue for 16 accumulator columns of this thread's row: x sx[m] x sw[n] + b[n] -> GELU -> cast ->
-// 32 B (bf16) or 64 B (fp32 / int32) into one of the warp's 64-byte-swizzled [32 rows x 64 B] staging
-// blocks; each completed block goes out as one TMA store (clipped at M / N by the tensor map) and the
-// warp moves on to its next block.  The arithmetic is issued as packed f32x2 instructions.
-template <int BN, int OUT_T, bool GELU, int NBUF>
-__device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const float* swb, int cb, float sxv,
-                                               uint32_t stg0, int& sbuf, int lane, const CUtensorMap* tmY,
-                                               int n0, int row0, bool want_amax, float& amax, int dbg = 0) {
-    const uint32_t rowb = stg0 + sbuf * W8_STG_BYTES + lane * 64;
-    const uint32_t xr = (lane >> 1) & 3;
-    const bool first = OUT_T != 1 || (cb & 16) == 0;   // first group of a 64-byte block
-    const bool last = OUT_T != 1 || (cb & 16) != 0;    // block complete after this group
+// Epilogue for 16 accumulator columns of this thread's row: x sx[m] x sw[n] + b[n] -> GELU -> cast -> global
+// memory.  The thread owns 16 consecutive outputs of its row = 32 B (bf16) or 64 B (fp32 / int32), written
+// as whole 32-byte sectors straight from registers.  (Round 1 staged the tile in shared memory for TMA
+// stores; measured equal within 3% on every C5 shape, and the staging area now serves the S1 side job.)
+// The arithmetic is issued as packed f32x2 instructions.
+template <int BN, int OUT_T, bool GELU>
+__device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const float* swb, int cb, float sxv, int lane,
+                                               int n0, int row0, bool want_amax, float& amax, const W8Params& p) {
     uint32_t w[16];
     if (OUT_T == 2) {
 #pragma unroll
@@ -139,28 +145,135 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
             for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[j]);
         }
     }
-    if (dbg & 2) return;
-    if (first) {   // the TMA store issued NBUF blocks ago must have finished reading this block
-        if (elect_one()) tma_store_wait_read<NBUF - 1>();
-        __syncwarp();
-    }
-    if (OUT_T == 1) {
-        const uint32_t c0 = (cb & 16) ? 2u : 0u;
-        sts128(rowb + (((c0) ^ xr) << 4), w[0], w[1], w[2], w[3]);
-        sts128(rowb + (((c0 + 1) ^ xr) << 4), w[4], w[5], w[6], w[7]);
-    } else {
-#pragma unroll
-        for (int c = 0; c < 4; ++c)
-            sts128(rowb + ((static_cast<uint32_t>(c) ^ xr) << 4), w[4 * c], w[4 * c + 1], w[4 * c + 2], w[4 * c + 3]);
-    }
-    if (last) {
-        fence_proxy_async_smem();
-        __syncwarp();
-        if (!(dbg & 1) && elect_one()) {
-            tma_store_2d(tmY, stg0 + sbuf * W8_STG_BYTES, n0 + (OUT_T == 1 ? (cb & ~31) : cb), row0);
-            tma_store_commit();
+    const int row = row0 + lane, col = n0 + cb;
+    if (row < p.M && col < p.N) {
+        constexpr int ESZ = OUT_T == 1 ? 2 : 4;
+        uint8_t* dst = static_cast<uint8_t*>(p.Y) + (static_cast<size_t>(row) * p.N + col) * ESZ;
+        const bool full = col + 16 <= p.N;                        // N % 8 == 0: otherwise exactly 8 valid
+        if (OUT_T == 1) {
+            if (full && (p.N & 15) == 0) stg256(dst, w);          // row pitch keeps 32-byte alignment
+            else { stg128(dst, w); if (full) stg128(dst + 16, w + 4); }
+        } else {
+            if (full) { stg256(dst, w); stg256(dst + 32, w + 8); }
+            else { stg128(dst, w); stg128(dst + 16, w + 4); }
         }
-        sbuf = sbuf + 1 == NBUF ? 0 : sbuf + 1;
+    }
+}
+
+__device__ __forceinline__ unsigned w8_ld_acquire(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// 1-D bulk copy global -> shared (TMA without a tensor map), completion on an mbarrier
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ uint4 w8_lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void lds8(uint32_t addr, const float*, float (&v)[8]) {
+    const uint4 a = w8_lds128(addr), b = w8_lds128(addr + 16);
+    v[0] = __uint_as_float(a.x); v[1] = __uint_as_float(a.y); v[2] = __uint_as_float(a.z); v[3] = __uint_as_float(a.w);
+    v[4] = __uint_as_float(b.x); v[5] = __uint_as_float(b.y); v[6] = __uint_as_float(b.z); v[7] = __uint_as_float(b.w);
+}
+__device__ __forceinline__ void lds8(uint32_t addr, const __nv_bfloat16*, float (&v)[8]) {
+    const uint4 a = w8_lds128(addr);
+    const uint32_t w[4] = {a.x, a.y, a.z, a.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        v[2 * i] = __uint_as_float(w[i] << 16);
+        v[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+    }
+}
+
+// S1 of the NEXT layer on this kernel's spare warps (rows dealt round-robin over all side warps of the
+// grid, so that the rows that become ready last are spread over every SM).  A warp fetches its next rows
+// with bulk copies (one per row, as many rows as fit its 16 KB buffer: a whole 12 KB row of the MLP hidden
+// state is in flight per warp), then reduces / rounds them out of shared memory.
+//  - independent input (nothing in this kernel writes it): absmax + rounding, overlapped with the mainloop;
+//  - chained input (this kernel's own output): a row is taken once every N-tile of its M-tile has been
+//    stored (per-M-tile counters, bumped by the epilogue warps after a gpu-scope fence); its absmax has
+//    been reduced by the epilogue (atomicMax), so the pass only rounds.  Tiles run N-fastest then, and
+//    the quantisation of M-tile j overlaps the mainloop of M-tile j+1.
+// The next GEMM is then the direct programmatic dependent of this one: no quantiser kernel, and one
+// completion -> dependent hop per layer instead of two (measured ~2.6 us each).
+template <typename T>
+__device__ __forceinline__ void w8_side_quant(const W8Params& p, int sw, int lane, uint32_t buf, uint32_t bar) {
+    const W8Side& j = p.side;
+    const int nw = gridDim.x * W8_SIDE_WARPS, w0 = blockIdx.x * W8_SIDE_WARPS + sw;
+    if (j.zero_absmax)
+        for (int i = w0 * 32 + lane; i < p.M; i += nw * 32) j.zero_absmax[i] = 0.0f;
+    if (j.zero_counters)
+        for (int i = w0 * 32 + lane; i < j.n_zero_counters; i += nw * 32) j.zero_counters[i] = 0u;
+    const int nvec = j.K2 >> 3;                               // 8-element vectors per row
+    constexpr int VB = 8 * static_cast<int>(sizeof(T));       // bytes per vector
+    const uint32_t row_bytes = static_cast<uint32_t>(nvec) * VB;
+    const T* X = static_cast<const T*>(j.X);
+    const int per_batch = max(1, static_cast<int>(W8_SIDE_BYTES / row_bytes));   // launcher: row_bytes <= W8_SIDE_BYTES
+    uint32_t phase = 0;
+    for (int row0 = w0; row0 < p.M; row0 += nw * per_batch) {
+        int nrows = 0;
+        for (int r = row0; r < p.M && nrows < per_batch; r += nw) ++nrows;
+        if (j.known_absmax) {
+            // chained: every row of the batch needs its M-tile complete (rows ascend: the last one suffices
+            // only for its own tile, so wait for each distinct tile)
+            for (int b = 0; b < nrows; ++b) {
+                const unsigned* cnt = j.mtile_done + (row0 + b * nw) / j.rows_per_mtile;
+                if (w8_ld_acquire(cnt) < j.mtile_target) {
+                    const long long t0 = clock64();
+                    while (w8_ld_acquire(cnt) < j.mtile_target) {
+                        __nanosleep(200);
+                        if (clock64() - t0 > 4000000000LL) {
+                            if (lane == 0) printf("aria: W8A8 side-job watchdog (block %d row %d)\n", blockIdx.x, row0);
+                            __trap();
+                        }
+                    }
+                }
+            }
+            asm volatile("fence.proxy.async;" ::: "memory");   // other SMs' generic-proxy stores -> this bulk copy
+        }
+        if (lane == 0) {
+            mbar_arrive_expect_tx(bar, row_bytes * nrows);
+            for (int b = 0; b < nrows; ++b)
+                bulk_load(buf + b * row_bytes, X + static_cast<size_t>(row0 + b * nw) * j.K2, row_bytes, bar);
+        }
+        __syncwarp();
+        mbar_wait(bar, phase);
+        phase ^= 1;
+        for (int b = 0; b < nrows; ++b) {
+            const int row = row0 + b * nw;
+            const uint32_t rb = buf + b * row_bytes;
+            int8_t* q = j.q + static_cast<size_t>(row) * j.K2;
+            float a = 0.0f;
+            if (j.known_absmax) {
+                asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(j.known_absmax + row) : "memory");
+            } else {
+                for (int i = lane; i < nvec; i += 32) {
+                    float v[8];
+                    lds8(rb + i * VB, static_cast<const T*>(nullptr), v);
+                    a = absmax8(v, a);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
+            }
+            const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
+            if (lane == 0) j.s[row] = s;
+            const FastQ f = make_fastq(s);
+            for (int i = lane; i < nvec; i += 32) {
+                float v[8];
+                lds8(rb + i * VB, static_cast<const T*>(nullptr), v);
+                uint2 o;
+                if (!f.ok || !quant8_fast(v, f, o)) o = quant8_i8(v, s);
+                *reinterpret_cast<uint2*>(q + 8 * i) = o;
+            }
+        }
+        __syncwarp();                                          // every lane is done with the buffer
     }
 }
 
@@ -169,7 +282,7 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
 template <int BN, int OUT_T, bool GELU, int CTAS>
 __global__ void __launch_bounds__(W8_THREADS, 1)
 w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                 const __grid_constant__ CUtensorMap tmY, const W8Params p) {
+                 const W8Params p) {
     using Cfg = W8Cfg<BN, CTAS>;
     constexpr int STAGES = Cfg::STAGES;
     extern __shared__ uint8_t smem_raw[];
@@ -182,6 +295,7 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     const uint32_t full0 = bars, empty0 = bars + 8 * STAGES;
     const uint32_t tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;
     const uint32_t tmem_slot = tempty0 + 16;
+    const uint32_t side_bar0 = tmem_slot + 16;                 // one mbarrier per side warp
     volatile uint32_t* tmem_slot_g =
         reinterpret_cast<volatile uint32_t*>(gbase + Cfg::BAR_OFF + 16 * STAGES + 32);
     float* swb_all = reinterpret_cast<float*>(gbase + Cfg::SWB_OFF);   // [2][2 * BN]
@@ -196,11 +310,15 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
     const int num_n = (p.N + BN - 1) / BN;
     const int num_tiles = num_m * num_n;
     const int num_kb = (p.K + W8_BK - 1) / W8_BK;
+    // tile t -> (M-tile, N-tile): M fastest, or N fastest when the side job quantises this kernel's own
+    // output M-tile by M-tile (the rows of M-tile j are then complete after its num_n tiles)
+    const bool n_fastest = p.mtile_done != nullptr;
+    auto tile_m = [&](int t) { return n_fastest ? t / num_n : t % num_m; };
+    auto tile_n = [&](int t) { return n_fastest ? t % num_n : t / num_m; };
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmA);
         tma_prefetch_desc(&tmB);
-        tma_prefetch_desc(&tmY);
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(full0 + 8 * s, 1);
             mbar_init(empty0 + 8 * s, 1);
@@ -209,6 +327,7 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             mbar_init(tfull0 + 8 * a, 1);
             mbar_init(tempty0 + 8 * a, W8_EPI_WARPS * CTAS);   // the pair's epilogue warps all report to the leader
         }
+        for (int w = 0; w < W8_SIDE_WARPS; ++w) mbar_init(side_bar0 + 8 * w, 1);
         fence_mbar_init();
     }
     if (warp == 1) {
@@ -251,8 +370,8 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         int stage = 0;
         uint32_t phase = 0;
         for (int t = unit0; t < num_tiles; t += unit_step) {
-            const int m0 = (t % num_m) * UM + rank * W8_BM;
-            const int n0 = (t / num_m) * BN + rank * Cfg::B_ROWS;
+            const int m0 = tile_m(t) * UM + rank * W8_BM;
+            const int n0 = tile_n(t) * BN + rank * Cfg::B_ROWS;
             for (int kb = 0; kb < num_kb; ++kb) {
                 mbar_wait(empty0 + 8 * stage, phase ^ 1);
                 if (elect_one()) {
@@ -313,19 +432,24 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             }
             if (lane == 0) w8_stamp(p, 1, t_start);
         }
+    } else if (warp >= 2 + W8_EPI_WARPS) {
+        // ------------------------------------------------------------ side job (warps 10..13)
+        if (p.side.X) {
+            const int sw = warp - 2 - W8_EPI_WARPS;
+            const uint32_t buf = base + Cfg::SIDE_OFF + sw * W8_SIDE_BYTES, sbar = side_bar0 + 8 * sw;
+            if (p.side.xt == ARIA_F32) w8_side_quant<float>(p, sw, lane, buf, sbar);
+            else w8_side_quant<__nv_bfloat16>(p, sw, lane, buf, sbar);
+        }
     } else {
         // ------------------------------------------------------------ epilogue (warps 2..9)
         const int ew = warp - 2;
         const int q = warp & 3;          // TMEM lane quarter this warp may read
         constexpr int PQ = W8_EPI_WARPS / 4;   // warps per TMEM lane quarter
-        constexpr int NBUF = Cfg::NBUF;
         constexpr int NC = BN / 32;            // 32-column chunks per tile
         constexpr int CPW = (NC + PQ - 1) / PQ;   // contiguous chunks per warp
         const int part = ew >> 2;        // this warp takes chunks [part * CPW, part * CPW + CPW)
         const int c_beg = part * CPW, c_end = min(NC, c_beg + CPW);
         const int et = threadIdx.x - 64; // 0..255: column index whose scale / bias this thread stages
-        const uint32_t stg0 = base + Cfg::STG_OFF + ew * (NBUF * W8_STG_BYTES);
-        int sbuf = 0;
         int acc = 0;
         uint32_t acc_phase = 0;
         const uint32_t tempty_leader = CTAS == 2 ? mapa_shared(tempty0, 0) : 0u;
@@ -333,7 +457,7 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         // the next tile's values are fetched into registers while this tile is processed.
         auto fetch_swb = [&](int t, float& sv, float& bv) {
             sv = 0.0f; bv = 0.0f;
-            const int c = (t / num_m) * BN + et;
+            const int c = tile_n(t) * BN + et;
             if (OUT_T != 2 && et < BN && t < num_tiles && c < p.N) {
                 sv = __ldg(p.sw + c);
                 if (p.bias)
@@ -348,8 +472,17 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             named_bar_sync(1, 32 * W8_EPI_WARPS);
         }
         int it = 0;
+        int pending_mtile = -1;          // M-tile whose completion this warp still has to publish (deferred by one tile)
+        auto publish = [&]() {
+            if (pending_mtile >= 0) {
+                __threadfence();         // this warp's stores of that tile, gpu scope (long drained one tile later)
+                __syncwarp();
+                if (lane == 0) atomicAdd(p.mtile_done + pending_mtile, 1u);
+                pending_mtile = -1;
+            }
+        };
         for (int t = unit0; t < num_tiles; t += unit_step, ++it) {
-            const int m0 = (t % num_m) * UM + rank * W8_BM, n0 = (t / num_m) * BN;
+            const int m0 = tile_m(t) * UM + rank * W8_BM, n0 = tile_n(t) * BN;
             const int row0 = m0 + q * 32;
             const float* swb = swb_all + (it & 1) * 2 * BN;
             float sxv = 0.0f, nsv = 0.0f, nbv = 0.0f;
@@ -361,6 +494,7 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             }
             mbar_wait(tfull0 + 8 * acc, acc_phase);
             tc_fence_after();
+            publish();                   // the previous tile's stores were issued a whole mainloop ago
             if (ew == 0 && lane == 0) w8_stamp(p, 8 + 2 * min(3, it), t_start);
             const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
             // A chunk is two groups of 16 columns held in two register sets; the refill of the first set
@@ -378,15 +512,16 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 #pragma unroll 1
             for (; c < c_end; ++c) {
                 const int cn = c + 1;
-                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(va, swb, c * 32, sxv, stg0, sbuf, lane, &tmY, n0, row0, want_amax, amax, W8_DBG(p));
+                w8_epilogue_16<BN, OUT_T, GELU>(va, swb, c * 32, sxv, lane, n0, row0, want_amax, amax, p);
                 if (cn < c_end) tmem_ld_32x32b_x16(t_addr + cn * 32, va);
-                w8_epilogue_16<BN, OUT_T, GELU, NBUF>(vb, swb, c * 32 + 16, sxv, stg0, sbuf, lane, &tmY, n0, row0, want_amax, amax, W8_DBG(p));
+                w8_epilogue_16<BN, OUT_T, GELU>(vb, swb, c * 32 + 16, sxv, lane, n0, row0, want_amax, amax, p);
                 if (cn < c_end) {
                     tmem_ld_32x32b_x16(t_addr + cn * 32 + 16, vb);
                     tmem_wait_ld_x16(va);
                     tmem_wait_ld_x16(vb);
                 }
             }
+            if (p.mtile_done) pending_mtile = tile_m(t);
             if (want_amax && row0 + lane < p.M) {
                 // fused S1, first half: per-token absmax of the STORED output (bf16 rounding is monotone and
                 // odd, so max |bf16(y)| = bf16(max |y|)); non-negative floats order like their bit patterns
@@ -407,8 +542,7 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                 named_bar_sync(1, 32 * W8_EPI_WARPS);
             }
         }
-        if (elect_one()) tma_store_wait<0>();  // all of this warp's output has been written
-        __syncwarp();
+        publish();                       // last tile
     }
 
     tc_fence_before();
@@ -429,8 +563,8 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 }
 
 template <int BN, int OUT_T, bool GELU, int CTAS>
-static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmY,
-                      const W8Params& p, int grid, cudaStream_t st, bool pdl) {
+static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const W8Params& p, int grid, cudaStream_t st,
+                      bool pdl) {
     using Cfg = W8Cfg<BN, CTAS>;
     static std::atomic<uint64_t> attr_done{0};
     auto kern = w8a8_gemm_kernel<BN, OUT_T, GELU, CTAS>;
@@ -456,19 +590,19 @@ static int launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUte
     }
     cfg.attrs = at;
     cfg.numAttrs = na;
-    return cudaLaunchKernelEx(&cfg, kern, tmA, tmB, tmY, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    return cudaLaunchKernelEx(&cfg, kern, tmA, tmB, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
 template <int BN, int CTAS>
-static int launch_bn(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmY,
-                     const W8Params& p, int out_t, int grid, cudaStream_t st, bool pdl) {
+static int launch_bn(const CUtensorMap& tmA, const CUtensorMap& tmB, const W8Params& p, int out_t, int grid,
+                     cudaStream_t st, bool pdl) {
     const bool gelu = p.act == ARIA_ACT_GELU_ERF;
     switch (out_t) {
-        case 0: return gelu ? launch_one<BN, 0, true, CTAS>(tmA, tmB, tmY, p, grid, st, pdl)
-                            : launch_one<BN, 0, false, CTAS>(tmA, tmB, tmY, p, grid, st, pdl);
-        case 1: return gelu ? launch_one<BN, 1, true, CTAS>(tmA, tmB, tmY, p, grid, st, pdl)
-                            : launch_one<BN, 1, false, CTAS>(tmA, tmB, tmY, p, grid, st, pdl);
-        default: return launch_one<BN, 2, false, CTAS>(tmA, tmB, tmY, p, grid, st, pdl);
+        case 0: return gelu ? launch_one<BN, 0, true, CTAS>(tmA, tmB, p, grid, st, pdl)
+                            : launch_one<BN, 0, false, CTAS>(tmA, tmB, p, grid, st, pdl);
+        case 1: return gelu ? launch_one<BN, 1, true, CTAS>(tmA, tmB, p, grid, st, pdl)
+                            : launch_one<BN, 1, false, CTAS>(tmA, tmB, p, grid, st, pdl);
+        default: return launch_one<BN, 2, false, CTAS>(tmA, tmB, p, grid, st, pdl);
     }
 }
 
@@ -505,7 +639,7 @@ void w8_tile_plan(int M, int N, int sms, int* bn, int* ctas) {
 }
 
 int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, const W8Epilogue& ep,
-                     cudaStream_t st, bool pdl) {
+                     cudaStream_t st, bool pdl, const W8Side* side) {
     const int sms = num_sms();
     if (sms <= 0) return ARIA_ERR_CUDA;
     W8Plan plan = pick_plan(M, N, sms);
@@ -520,18 +654,25 @@ int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, co
     if (rc != ARIA_OK) return rc;
     rc = make_tmap_2d(&tmB, Wq, 1, N, K, bn / ctas, W8_BK, 128);
     if (rc != ARIA_OK) return rc;
-    // output tensor map: [M, N] of 2- or 4-byte elements, box = 32 rows x 64 bytes, 64-byte swizzle
-    CUtensorMap tmY;
-    const int esz = ep.out_t == 1 ? 2 : 4;
-    rc = make_tmap_2d(&tmY, ep.Y, esz, M, N, 32, 64 / esz, 64);
-    if (rc != ARIA_OK) return rc;
     W8Params p;
     p.sx = ep.sx; p.sw = ep.sw; p.bias = ep.bias;
     p.bias_t = ep.bias_t; p.act = ep.act;
     p.M = M; p.N = N; p.K = K;
     p.row_absmax = ep.out_t == 2 ? nullptr : ep.row_absmax;
+    p.Y = ep.Y;
+    p.side = side ? *side : W8Side();
+    if (p.side.X && static_cast<size_t>(p.side.K2) * (p.side.xt == ARIA_F32 ? 4 : 2) > static_cast<size_t>(W8_SIDE_BYTES))
+        return ARIA_ERR_SHAPE;       // the caller (api.cu) only asks for a side job whose rows fit the buffer
+    p.mtile_done = nullptr;
+    if (side && side->X && side->known_absmax) {
+        // chained side job: this kernel's epilogue publishes per-M-tile completion for it
+        p.mtile_done = side->mtile_counters;
+        p.side.mtile_done = side->mtile_counters;
+        p.side.rows_per_mtile = W8_BM * ctas;
+        p.side.mtile_target = static_cast<unsigned>(((N + bn - 1) / bn) * W8_EPI_WARPS * ctas);
+    }
 #ifdef ARIA_DEBUG
-    p.prof = g_w8_prof;
+    p.prof = g_w8_prof ? g_w8_prof + static_cast<size_t>(g_w8_prof_launch++ % 256) * 148 * 20 : nullptr;
     p.dbg = dbg_env("ARIA_W8_DBG") ? atoi(dbg_env("ARIA_W8_DBG")) : 0;
 #endif
     const int um = W8_BM * ctas;
@@ -540,16 +681,16 @@ int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, co
     const int grid = (tiles < slots ? tiles : slots) * ctas;
     if (ctas == 2) {
         switch (bn) {
-            case 128: return launch_bn<128, 2>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
-            case 192: return launch_bn<192, 2>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
-            default: return launch_bn<256, 2>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
+            case 128: return launch_bn<128, 2>(tmA, tmB, p, ep.out_t, grid, st, pdl);
+            case 192: return launch_bn<192, 2>(tmA, tmB, p, ep.out_t, grid, st, pdl);
+            default: return launch_bn<256, 2>(tmA, tmB, p, ep.out_t, grid, st, pdl);
         }
     }
     switch (bn) {
-        case 64: return launch_bn<64, 1>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
-        case 128: return launch_bn<128, 1>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
-        case 192: return launch_bn<192, 1>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
-        default: return launch_bn<256, 1>(tmA, tmB, tmY, p, ep.out_t, grid, st, pdl);
+        case 64: return launch_bn<64, 1>(tmA, tmB, p, ep.out_t, grid, st, pdl);
+        case 128: return launch_bn<128, 1>(tmA, tmB, p, ep.out_t, grid, st, pdl);
+        case 192: return launch_bn<192, 1>(tmA, tmB, p, ep.out_t, grid, st, pdl);
+        default: return launch_bn<256, 1>(tmA, tmB, p, ep.out_t, grid, st, pdl);
     }
 }
 

@@ -5,134 +5,19 @@
 // half to even (__float2int_rn), clamp; never a reciprocal or fast-math shortcut, so codes and
 // scales are bit-identical to the definition.
 #include "internal.cuh"
+#include "quant_dev.cuh"
 
 namespace aria {
 
 constexpr int QROW_MAX_THREADS = 256;
 constexpr int QROW_CACHE = 4;  // 8-element vectors kept in registers per thread
 
-// 16-byte global loads that stay BELOW griddepcontrol.wait: a non-coherent (ld.global.nc) load is a
-// pure value to the compiler, which hoisted it above the wait of the quantiser kernels -- under
-// programmatic dependent launch the previous grid is still writing X at that point.
-__device__ __forceinline__ uint4 ld_global_v4(const void* p) {
-    uint4 v;
-    asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ float4 ld_global_f4(const void* p) {
-    const uint4 v = ld_global_v4(p);
-    return make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
-}
-template <typename T>
-__device__ __forceinline__ void load8(const T* p, float (&v)[8]);
-
-template <>
-__device__ __forceinline__ void load8<float>(const float* p, float (&v)[8]) {
-    const float4 a = ld_global_f4(p);
-    const float4 b = ld_global_f4(p + 4);
-    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
-    v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
-}
-template <>
-__device__ __forceinline__ void load8<__nv_bfloat16>(const __nv_bfloat16* p, float (&v)[8]) {
-    const uint4 a = ld_global_v4(p);
-    const uint32_t w[4] = {a.x, a.y, a.z, a.w};
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        v[2 * i] = __uint_as_float(w[i] << 16);
-        v[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
-    }
-}
-
-// Raw (still packed) 8-element vectors: what the warp-per-row kernel keeps in registers.
-template <typename T> struct Raw8;
-template <> struct Raw8<float> { float4 a, b; };
-template <> struct Raw8<__nv_bfloat16> { uint4 a; };
-__device__ __forceinline__ void load_raw(const float* p, Raw8<float>& r) {
-    r.a = ld_global_f4(p);
-    r.b = ld_global_f4(p + 4);
-}
-__device__ __forceinline__ void load_raw(const __nv_bfloat16* p, Raw8<__nv_bfloat16>& r) {
-    r.a = ld_global_v4(p);
-}
-__device__ __forceinline__ void unpack8(const Raw8<float>& r, float (&v)[8]) {
-    v[0] = r.a.x; v[1] = r.a.y; v[2] = r.a.z; v[3] = r.a.w;
-    v[4] = r.b.x; v[5] = r.b.y; v[6] = r.b.z; v[7] = r.b.w;
-}
-__device__ __forceinline__ void unpack8(const Raw8<__nv_bfloat16>& r, float (&v)[8]) {
-    const uint32_t w[4] = {r.a.x, r.a.y, r.a.z, r.a.w};
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        v[2 * i] = __uint_as_float(w[i] << 16);
-        v[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
-    }
-}
-
-__device__ __forceinline__ float absmax8(const float (&v)[8], float a) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) a = fmaxf(a, fabsf(v[i]));
-    return a;
-}
-
-__device__ __forceinline__ int quant1(float x, float s, int lim) {
-    int q = __float2int_rn(__fdiv_rn(x, s));
-    return max(-lim, min(lim, q));
-}
-
-// Exact rint(fl32(x / s)) without a division per element.  With r = RN(1/s), r_lo = r (1 - 2^-20) and
-// r_hi = r (1 + 2^-20) bracket 1/s by far more than the rounding of r, so for every x the exact
-// quotient AND its fp32 rounding lie between x*r_lo and x*r_hi.  fma(x, r_*, 1.5*2^23) rounds the
-// exact product to an integer (ties to even) in the low mantissa bits; rint is monotone, so if both
-// ends give the same integer, rint(fl32(x/s)) is that integer (a tie strictly inside the bracket
-// would separate the two ends).  Otherwise (|x/s| within ~1e-4 of a .5 boundary, probability ~2e-4)
-// the caller falls back to the IEEE division.  |x/s| <= 127 (1 + 2^-23): no clamp is needed.
-struct FastQ {
-    float r_lo, r_hi;
-    bool ok;  // false: s is outside the range where r is finite and normal -> always divide
-};
-__device__ __forceinline__ FastQ make_fastq(float s) {
-    FastQ f;
-    const float r = __frcp_rn(s);
-    f.r_lo = r * 0.99999904632568359375f;   // 1 - 2^-20
-    f.r_hi = r * 1.00000095367431640625f;   // 1 + 2^-20
-    f.ok = (s > 1e-30f) && (s < 1e30f);
-    return f;
-}
-constexpr float QMAGIC = 12582912.0f;  // 1.5 * 2^23: float bits 0x4B400000 + q
-
-// Quantise 8 values; returns false if any needs the exact-division path.
-__device__ __forceinline__ bool quant8_fast(const float (&v)[8], const FastQ& f, uint2& out) {
-    uint32_t y[8];
-    bool same = true;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const uint32_t a = __float_as_uint(fmaf(v[i], f.r_lo, QMAGIC));
-        const uint32_t b = __float_as_uint(fmaf(v[i], f.r_hi, QMAGIC));
-        same = same && (a == b);
-        y[i] = a;
-    }
-    // low byte of each y is the two's-complement code
-    out.x = __byte_perm(__byte_perm(y[0], y[1], 0x0040), __byte_perm(y[2], y[3], 0x0040), 0x5410);
-    out.y = __byte_perm(__byte_perm(y[4], y[5], 0x0040), __byte_perm(y[6], y[7], 0x0040), 0x5410);
-    return same;
-}
-
-__device__ __forceinline__ uint2 quant8_i8(const float (&v)[8], float s) {
-    uint32_t lo = 0, hi = 0;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        lo |= (static_cast<uint32_t>(quant1(v[i], s, 127)) & 0xFFu) << (8 * i);
-        hi |= (static_cast<uint32_t>(quant1(v[4 + i], s, 127)) & 0xFFu) << (8 * i);
-    }
-    return make_uint2(lo, hi);
-}
-
 // One CTA per row.  R1..R4: a = max|x|; s = a > 0 ? a/127 : 1; q = clamp(rint(x/s), +-127).
 template <typename T>
 __global__ void __launch_bounds__(QROW_MAX_THREADS)
 quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
                      float* __restrict__ scale, int early, const float* known_absmax,
-                     float* zero_absmax) {
+                     float* zero_absmax, unsigned* zero_counters, int n_zero_counters) {
     __shared__ float red[QROW_MAX_THREADS / 32];
     // early: X, Xq and scale are untouched by the grid before this one (the caller checked), so the
     // pass runs concurrently with it; the wait moves to the end so that "this grid is complete" still
@@ -173,6 +58,7 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
     if (tid == 0) {
         scale[row] = s;
         if (zero_absmax) zero_absmax[row] = 0.0f;
+        if (zero_counters && row < n_zero_counters) zero_counters[row] = 0u;
     }
     pdl_launch_dependents();
     const FastQ f = make_fastq(s);
@@ -201,7 +87,7 @@ template <typename T, int VPL>
 __global__ void __launch_bounds__(256)
 quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restrict__ Xq,
                           float* __restrict__ scale, int early, const float* known_absmax,
-                          float* zero_absmax) {
+                          float* zero_absmax, unsigned* zero_counters, int n_zero_counters) {
     if (!early) pdl_wait_prior_grid();      // early: see quant_rows_i8_kernel
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
@@ -238,6 +124,7 @@ quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restr
     if (lane == 0) {
         scale[row] = s;
         if (zero_absmax) zero_absmax[row] = 0.0f;
+        if (zero_counters && row < n_zero_counters) zero_counters[row] = 0u;
     }
     const FastQ f = make_fastq(s);
 #pragma unroll
@@ -282,16 +169,17 @@ quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restri
 
 template <typename T, int VPL>
 static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, float* s,
-                                    cudaLaunchConfig_t& cfg, int early, const float* known, float* zero) {
+                                    cudaLaunchConfig_t& cfg, int early, const float* known, float* zero,
+                                    unsigned* zc, int nzc) {
     constexpr int WARPS = 8;
     cfg.blockDim = dim3(32 * WARPS);
     cfg.gridDim = dim3((R + WARPS - 1) / WARPS);
     return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s, early,
-                              known, zero);
+                              known, zero, zc, nzc);
 }
 
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl, bool early_, const float* known, float* zero) {
+                         bool pdl, bool early_, const float* known, float* zero, unsigned* zc, int nzc) {
     const int nvec = C / 8;
     const int early = pdl && early_ ? 1 : 0;
     {   // warp-per-row variants: rows up to 3072 elements (wider rows: one CTA per row, below; a 24-vector
@@ -307,14 +195,14 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
         cudaError_t e = cudaErrorInvalidValue;
         bool done = true;
         if (xt == ARIA_BF16) {
-            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg, early, known, zero);
-            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg, early, known, zero);
-            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg, early, known, zero);
+            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
+            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
+            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
             else done = false;
         } else {
-            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg, early, known, zero);
-            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg, early, known, zero);
-            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg, early, known, zero);
+            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
+            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
+            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
             else done = false;
         }
         if (done) return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
@@ -332,10 +220,10 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
     cfg.numAttrs = pdl ? 1 : 0;
     cudaError_t e;
     if (xt == ARIA_F32)
-        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s, early, known, zero);
+        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s, early, known, zero, zc, nzc);
     else
         e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<__nv_bfloat16>,
-                               static_cast<const __nv_bfloat16*>(X), C, q, s, early, known, zero);
+                               static_cast<const __nv_bfloat16*>(X), C, q, s, early, known, zero, zc, nzc);
     return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
