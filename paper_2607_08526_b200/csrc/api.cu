@@ -25,38 +25,26 @@ int check_rows_args(const void* in, int t, int R, int C, const void* q, const vo
     return check_arch();
 }
 
-// per-token absmax [M] + per-M-tile completion counters [ceil(M / 128)] of one fused-S1 producer
-size_t w8_fuse_bytes(int M) { return up256(static_cast<size_t>(M) * 4) + up256(static_cast<size_t>((M + 127) / 128) * 4); }
+// per-token absmax [M] of one fused-S1 producer
+size_t w8_fuse_bytes(int M) { return up256(static_cast<size_t>(M) * 4); }
 
 size_t w8_ws_bytes(int M, int K) { return up256(static_cast<size_t>(M) * K) + up256(static_cast<size_t>(M) * 4); }
 
-// Fused S1 (north_star "activation-quantization pass fused into the previous epilogue where shapes
-// allow"): a W8A8 layer whose output feeds the next W8A8 layer reduces the per-token absmax of what it
-// stores in its own epilogue (atomicMax into amax_out); the consumer's S1 pass then takes the row
-// maxima from amax_in and only rounds.  amax_zero: the buffer THIS layer's GEMM will reduce into, zeroed
-// by this layer's S1 pass (which always completes before that GEMM's epilogue).
-struct W8Fuse {
-    const float* amax_in = nullptr;
-    float* amax_zero = nullptr;
-    float* amax_out = nullptr;
-};
-
-// pdl_first: whether the FIRST kernel of this linear may be launched as a programmatic dependent of
-// whatever precedes it on the stream (only inside a chain this library enqueued itself: the kernels of
-// a chain all execute griddepcontrol.wait before they exit, a foreign kernel gives no such guarantee).
+// One W8A8 linear as two launches: the S1 kernel, then the GEMM as its programmatic dependent (the GEMM's
+// prologue -- barrier init, tensor-memory allocation, tensor-map prefetch -- overlaps the quantiser).
+// pdl_first: whether the S1 kernel itself may be a programmatic dependent of what precedes it on the stream
+// (only inside a chain this library enqueued: its kernels all execute griddepcontrol.wait before they touch
+// global memory, a foreign kernel gives no such guarantee).
 int linear_w8a8_impl(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
                      int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
-                     cudaStream_t st, bool pdl_first, bool pdl, bool early = false,
-                     const W8Fuse& fuse = W8Fuse()) {
+                     cudaStream_t st, bool pdl_first, bool pdl) {
     int8_t* Xq = static_cast<int8_t*>(ws);
     float* sx = reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + up256(static_cast<size_t>(M) * K));
-    int rc = launch_quant_rows_i8(X, xt, M, K, Xq, sx, st, pdl_first, early && pdl_first, fuse.amax_in,
-                                  fuse.amax_zero);
+    int rc = launch_quant_rows_i8(X, xt, M, K, Xq, sx, st, pdl_first);
     if (rc != ARIA_OK) return rc;
     W8Epilogue ep;
     ep.sx = sx; ep.sw = w_scale; ep.bias = bias; ep.bias_t = bt; ep.act = act; ep.Y = Y;
     ep.out_t = yt == ARIA_F32 ? 0 : 1;
-    ep.row_absmax = fuse.amax_out;
     return launch_gemm_w8a8(Xq, Wq, M, N, K, ep, st, pdl);
 }
 
@@ -82,16 +70,13 @@ int check_layers(const aria_layer* layers, int n_layers, int M, int mode, int io
 }
 
 // first: this is the first kernel sequence of a chain (no programmatic dependency on what precedes it).
-// early: W8A8 only -- this layer's activation quantiser may overlap the previous layer's GEMM (see
-// aria_denoiser_linears).
 int run_layer(const aria_layer& L, const void* in, void* out, int M, int mode, int io, void* ws,
-              size_t ws_bytes, cudaStream_t st, bool first, bool early = false, const W8Fuse& fuse = W8Fuse()) {
+              size_t ws_bytes, cudaStream_t st, bool first) {
     static const bool pdl = dbg_env("ARIA_NO_PDL") == nullptr;            // debug builds only
-    static const bool no_early = dbg_env("ARIA_NO_EARLY_QUANT") != nullptr;
     if (mode == ARIA_W8A8)
         return linear_w8a8_impl(in, io, M, L.K, static_cast<const int8_t*>(L.wq),
                                 static_cast<const float*>(L.w_scale), L.N, L.bias, io, L.act, out, io,
-                                ws, st, pdl && !first, pdl, early && !no_early, fuse);
+                                ws, st, pdl && !first, pdl);
     return launch_gemm_w4a16(in, M, L.K, static_cast<const uint8_t*>(L.wq), L.w_scale, L.N, L.bias, L.act,
                              out, io, ws, ws_bytes, st, pdl && !first, mode == ARIA_W8A16 ? 8 : 4);
 }
@@ -152,8 +137,7 @@ const char* aria_status_string(int status) {
 
 size_t aria_workspace_bytes(int M, int maxK, int maxN, int mode) {
     if (M <= 0 || maxK <= 0 || maxN <= 0) return 0;
-    // two (Xq, sx) buffers, two per-token absmax buffers and two sets of M-tile counters (fused S1): see
-    // aria_denoiser_linears
+    // two (Xq, sx) buffers and two per-token absmax buffers (fused S1): see aria_denoiser_linears
     if (mode == ARIA_W8A8) return 2 * w8_ws_bytes(M, maxK) + 2 * w8_fuse_bytes(M);
     if (mode == ARIA_W4A16 || mode == ARIA_W8A16) {
         // Split-K bound: splits * tiles <= #SMs and a tile holds <= 128 x TT outputs, so the fp32
@@ -334,29 +318,27 @@ int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mod
         }
         return ARIA_OK;
     }
-    // W8A8.  The (Xq, sx) scratch alternates between two buffers.  The S1 pass of layer i+1 runs INSIDE
-    // the GEMM kernel of layer i, on spare warps (gemm_w8a8.cu: w8_side_quant), whenever layer i+1's
-    // input is either untouched by layer i (it is quantised during layer i's mainloop) or exactly layer
-    // i's output (fused S1: layer i's epilogue reduces the per-token absmax of what it stores and counts
-    // finished M-tiles; the side warps round each row as soon as its M-tile is complete).  Layer i+1's
-    // GEMM is then the direct programmatic dependent of layer i's GEMM.  Any other layer (and layer 0)
-    // gets a stand-alone S1 kernel.  Every kernel waits for its predecessor before it touches global
-    // memory, so "kernel k complete" implies "kernels < k complete"; the side job of GEMM i writes the
-    // Xq buffer last read by GEMM i-1.  The absmax / counter set a GEMM reduces into is zeroed by the S1
-    // pass of that same layer (side job of the previous GEMM, or the stand-alone kernel).
+    // W8A8.  The (Xq, sx) scratch alternates between two buffers.
+    //  - A layer whose input is NOT written by the previous layer gets its S1 pass from the previous layer's
+    //    GEMM kernel: the epilogue warps quantise it while they wait for their first accumulator
+    //    (gemm_w8a8.cu: w8_side_quant).  The GEMM of layer i+1 is then the direct programmatic dependent
+    //    of the GEMM of layer i: one completion -> launch hop between GEMMs instead of two.
+    //  - A layer whose input IS the previous layer's output (in == NULL, or in == that out) takes the fused
+    //    S1 (north_star "activation-quantization pass fused into the previous epilogue"): the producing
+    //    epilogue reduces the per-token absmax of what it stores (atomicMax into one of two [M] buffers) and
+    //    a stand-alone S1 kernel only rounds.  The buffer a GEMM reduces into is zeroed by the S1 pass of
+    //    that same layer (side job of the previous GEMM, or the stand-alone kernel).
+    //  - Layer 0, and a layer whose input only partly overlaps the previous output or whose rows exceed the
+    //    side job's 8 KB staging buffer, get a plain stand-alone S1 kernel.
+    // Every kernel waits for its predecessor (griddepcontrol.wait) before it touches global memory, so
+    // "kernel k complete" implies "kernels < k complete"; the side job of GEMM i writes the Xq buffer last
+    // read by GEMM i-1, and results equal array order bit for bit.
     static const bool no_fuse = dbg_env("ARIA_NO_FUSED_ABSMAX") != nullptr;   // debug builds only
     static const bool no_side = dbg_env("ARIA_NO_SIDE_QUANT") != nullptr;
     static const bool pdl = dbg_env("ARIA_NO_PDL") == nullptr;
     const size_t half = w8_ws_bytes(M, maxK);
     uint8_t* wsb = static_cast<uint8_t*>(ws);
-    float* amax[2];
-    unsigned* cnt[2];
-    for (int b = 0; b < 2; ++b) {
-        uint8_t* f = wsb + 2 * half + b * w8_fuse_bytes(M);
-        amax[b] = reinterpret_cast<float*>(f);
-        cnt[b] = reinterpret_cast<unsigned*>(f + up256(static_cast<size_t>(M) * 4));
-    }
-    const int n_cnt = (M + 127) / 128;
+    float* amax[2] = {reinterpret_cast<float*>(wsb + 2 * half), reinterpret_cast<float*>(wsb + 2 * half + w8_fuse_bytes(M))};
     auto xq_of = [&](int i) { return reinterpret_cast<int8_t*>(wsb + (i & 1) * half); };
     auto sx_of = [&](int i) { return reinterpret_cast<float*>(wsb + (i & 1) * half + up256(static_cast<size_t>(M) * maxK)); };
     auto in_of = [&](int i) { return layers[i].in ? layers[i].in : layers[i - 1].out; };
@@ -370,40 +352,28 @@ int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M, int mod
                         b1 = b0 + static_cast<size_t>(M) * layers[i - 1].N * dsize(io);
         return !(a0 < b1 && b0 < a1);
     };
-    std::vector<int> prod(n_layers, -1);       // producer index (selects the absmax / counter set), or -1
+    std::vector<int> prod(n_layers, -1);       // producer index (selects the absmax buffer), or -1
     for (int i = 0, k = 0; i < n_layers; ++i)
         if (feeds_next(i)) prod[i] = k++;
     bool s1_done = false;                      // layer i's S1 was done by the side job of GEMM i-1
     for (int i = 0; i < n_layers; ++i) {
         const aria_layer& L = layers[i];
-        const bool first = i == 0;
         if (!s1_done) {
-            const bool fused_in = i > 0 && prod[i - 1] >= 0;
-            rc = launch_quant_rows_i8(in_of(i), io, M, L.K, xq_of(i), sx_of(i), st, pdl && !first, false,
-                                      fused_in ? amax[prod[i - 1] & 1] : nullptr,
-                                      prod[i] >= 0 ? amax[prod[i] & 1] : nullptr,
-                                      prod[i] >= 0 ? cnt[prod[i] & 1] : nullptr, n_cnt);
+            rc = launch_quant_rows_i8(in_of(i), io, M, L.K, xq_of(i), sx_of(i), st, pdl && i > 0,
+                                      i > 0 && prod[i - 1] >= 0 ? amax[prod[i - 1] & 1] : nullptr,
+                                      prod[i] >= 0 ? amax[prod[i] & 1] : nullptr);
             if (rc != ARIA_OK) return rc;
         }
         W8Side side;
         s1_done = false;
-        // (rows of up to 16 KB fit the side warps' staging buffers: K <= 8192 bf16 / 4096 fp32)
-        if (!no_side && i + 1 < n_layers && static_cast<size_t>(layers[i + 1].K) * dsize(io) <= 16384 &&
-            (prod[i] >= 0 || independent_of_prev(i + 1))) {
+        if (!no_side && i + 1 < n_layers && prod[i] < 0 && independent_of_prev(i + 1) &&
+            static_cast<size_t>(layers[i + 1].K) * dsize(io) <= 8192) {
             side.X = in_of(i + 1);
             side.xt = io;
             side.K2 = layers[i + 1].K;
             side.q = xq_of(i + 1);
             side.s = sx_of(i + 1);
-            if (prod[i] >= 0) {
-                side.known_absmax = amax[prod[i] & 1];
-                side.mtile_counters = cnt[prod[i] & 1];
-            }
-            if (prod[i + 1] >= 0) {
-                side.zero_absmax = amax[prod[i + 1] & 1];
-                side.zero_counters = cnt[prod[i + 1] & 1];
-                side.n_zero_counters = n_cnt;
-            }
+            if (prod[i + 1] >= 0) side.zero_absmax = amax[prod[i + 1] & 1];
             s1_done = true;
         }
         W8Epilogue ep;

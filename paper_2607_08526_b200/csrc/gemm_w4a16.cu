@@ -48,7 +48,13 @@ constexpr int W4_G = 3;         // dequantiser groups = A buffers
 template <int TT, int WB = 4>
 struct W4Cfg {
     static constexpr int G = W4_G;
-    static constexpr int NB = G;                               // dequantised A buffers
+    // ATM: the dequantised A tile goes registers -> TENSOR MEMORY (tcgen05.st) and the MMA reads it from there.
+    // At M >= 512 the k-block time was set by shared-memory traffic (measured 800-860 cycles per 64-k block
+    // against 384-512 of tensor time: X tile written by TMA and read by the MMA, plus 16 KB of A written by
+    // the dequantisers and 16 KB read back by the MMA); A in TMEM removes those 32 KB per k-block.  Needs
+    // 2 TT accumulator columns + 4 x 32 A columns <= 512: every token tile but TT = 256.
+    static constexpr bool ATM = TT <= 192;
+    static constexpr int NB = ATM ? 4 : G;                     // dequantised A buffers (TMEM slots / smem tiles)
     static constexpr int THREADS = 32 * W4_DEQ_WARP0 + 128 * G;
     static constexpr int P_ROW = W4_BK * WB / 8;               // 32 (int4) / 64 (int8) packed bytes per row per k-block
     static constexpr int P_BYTES = W4_BN * P_ROW;              // 4 KB / 8 KB
@@ -56,20 +62,22 @@ struct W4Cfg {
     static constexpr int X_BYTES = X_ROWS * 128;               // x 64 bf16
     static constexpr int A_BYTES = W4_BN * 128;                // 16 KB: 128 rows x 64 bf16
     static constexpr int STG_BYTES = 4096;                     // per epilogue warp: 32 tokens x 128 B
-    static constexpr int XS = X_ROWS == 256 ? 3 : X_ROWS == 192 ? 4 : X_ROWS == 128 ? 4 : X_ROWS == 64 ? 6 : 8;   // X ring depth
+    static constexpr int XS = X_ROWS == 256 ? 3 : X_ROWS == 192 ? (WB == 8 ? 5 : 6) : X_ROWS == 128 ? 6 : 8;   // X ring depth
     static constexpr int PS = WB == 8 ? (TT >= 192 ? 8 : TT == 32 ? 16 : 12)      // packed ring depth
                                       : (TT >= 192 ? 8 : TT == 128 ? 12 : 16);
     static constexpr int X_OFF = 0;
     static constexpr int A_OFF = X_OFF + XS * X_BYTES;
-    static constexpr int P_OFF = A_OFF + NB * A_BYTES;
+    static constexpr int P_OFF = A_OFF + (ATM ? 0 : NB * A_BYTES);
     static constexpr int STG_OFF = P_OFF + PS * P_BYTES;
     static constexpr int BAR_OFF = STG_OFF + 4 * STG_BYTES;
     static constexpr int NBAR = 2 * XS + 2 * PS + 2 * NB + 4;
     static constexpr int SMEM_BYTES = BAR_OFF + NBAR * 8 + 16 + 1024;
     // TT = 192 fills the SMs when N / 128 is small: 12 row tiles x 11 token tiles = 132 units on 148 SMs
     // at M = 2048 (TT = 256: 96 units)
-    static constexpr int ACC_STRIDE = TT == 192 ? 256 : TT;
-    static constexpr int TMEM_COLS = 2 * ACC_STRIDE < 32 ? 32 : 2 * ACC_STRIDE;
+    static constexpr int ACC_STRIDE = TT;
+    static constexpr int A_COL0 = 2 * ACC_STRIDE;             // ATM: 4 slots of 32 columns (128 rows x 64 k bf16)
+    static constexpr int TMEM_COLS = ATM ? (A_COL0 + 4 * 32 <= 256 ? 256 : 512) : 512;
+    static_assert(!ATM || A_COL0 + NB * 32 <= TMEM_COLS, "tensor memory");
     static_assert(TT == 32 || TT == 64 || TT == 128 || TT == 192 || TT == 256, "TT");
     static_assert(WB == 4 || WB == 8, "weight bits");
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
@@ -86,17 +94,21 @@ struct W4Params {
     int splits;
 #ifdef ARIA_DEBUG
     long long* prof;          // per-CTA role timestamps (clock64), or nullptr
+    int dbg;                  // timing experiments (ARIA_W4_DBG; results are WRONG): 1 = X loaded for every other k-block only, 2 = no X loads
 #endif
 };
 
 #ifdef ARIA_DEBUG
 static long long* g_w4_prof = nullptr;
-void w4_set_profile_buffer(long long* p) { g_w4_prof = p; }
+static int g_w4_prof_launch = 0;          // every launch (graph node) gets its own 148 x 16 slot, 256 slots
+void w4_set_profile_buffer(long long* p) { g_w4_prof = p; g_w4_prof_launch = 0; }
 __device__ __forceinline__ void prof_stamp(const W4Params& p, int slot, long long t0) {
     if (p.prof) p.prof[blockIdx.x * 16 + slot] = clock64() - t0;
 }
+#define W4_TIMED(acc, stmt) do { const long long t_ = clock64(); stmt; acc += clock64() - t_; } while (0)
 #else
 __device__ __forceinline__ void prof_stamp(const W4Params&, int, long long) {}
+#define W4_TIMED(acc, stmt) do { stmt; } while (0)
 #endif
 
 __device__ __forceinline__ uint32_t cvt_bf16x2(float lo, float hi) {
@@ -199,6 +211,9 @@ __device__ __forceinline__ void dequant_i8x16(const uint4& v, float sw, uint4& l
     hi = make_uint4(o[4], o[5], o[6], o[7]);
 }
 
+// (X multicast over CTA couples -- both CTAs of a cluster on the same token tile, each loading half of every X
+// tile into both -- was built twice: with A in shared memory (round 1: 3.79 vs 3.81 ms per C5 step) and with A
+// in tensor memory (round 2: 3.29 vs 3.32 ms).  The k-block time is not set by L2 reads of X; removed.)
 template <int TT, bool GELU, int WB>
 __global__ void __launch_bounds__(W4Cfg<TT, WB>::THREADS, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmX,
@@ -267,6 +282,13 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     // writes, so the first k-blocks are fetched and dequantised during its tail.
     pdl_launch_dependents();   // the next kernel may become resident now; it blocks in its own wait
     const long long t_start = clock64();
+#ifdef ARIA_DEBUG
+    if (threadIdx.x == 0 && p.prof) {
+        unsigned long long gt;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+        p.prof[blockIdx.x * 16 + 14] = static_cast<long long>(gt);
+    }
+#endif
 
     // Producer / MMA warps: warp-uniform loops, one elected lane issues (see gemm_w8a8.cu).
     if (warp == 0) {
@@ -280,6 +302,14 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             for (int kb = kb0; kb < kb1; ++kb) {
                 mbar_wait(xempty0 + 8 * stage, phase ^ 1);
+#ifdef ARIA_DEBUG
+                if ((p.dbg == 1 && (kb & 1)) || p.dbg == 2) {
+                    if (elect_one()) mbar_arrive(xfull0 + 8 * stage);
+                    __syncwarp();
+                    if (++stage == XS) { stage = 0; phase ^= 1; }
+                    continue;
+                }
+#endif
                 if (elect_one()) {
                     mbar_arrive_expect_tx(xfull0 + 8 * stage, Cfg::X_BYTES);
                     tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xfull0 + 8 * stage);
@@ -317,21 +347,25 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             const uint64_t desc_hi = make_smem_desc_sw128(0);
             int stage = 0, ab = 0, acc = 0;
             uint32_t phase = 0, aphase = 0, acc_phase = 0;
+            long long w_x = 0, w_a = 0, w_t = 0;
             for (int u = unit0; u < num_units; u += unit_step) {
                 const int sp = u % S;
                 const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
-                mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1);
+                W4_TIMED(w_t, mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1));
                 const uint32_t d_tmem = tmem_base + acc * Cfg::ACC_STRIDE;
                 for (int kb = kb0; kb < kb1; ++kb) {
-                    mbar_wait(xfull0 + 8 * stage, phase);   // X landed
-                    mbar_wait(afull0 + 8 * ab, aphase);     // weights dequantised
+                    W4_TIMED(w_x, mbar_wait(xfull0 + 8 * stage, phase));   // X landed
+                    W4_TIMED(w_a, mbar_wait(afull0 + 8 * ab, aphase));     // weights dequantised
                     tc_fence_after();
                     const uint64_t a_desc = desc_hi | (((sA + ab * Cfg::A_BYTES) & 0x3FFFF) >> 4);
+                    const uint32_t a_tmem = tmem_base + Cfg::A_COL0 + ab * 32;
                     const uint64_t b_desc = desc_hi | (((sX + stage * Cfg::X_BYTES) & 0x3FFFF) >> 4);
                     if (elect_one()) {
 #pragma unroll
-                        for (int k = 0; k < 4; ++k)   // 4 x (K = 16 bf16 = 32 bytes)
-                            mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                        for (int k = 0; k < 4; ++k) {  // 4 x (K = 16 bf16 = 32 bytes of X / 8 TMEM columns of A)
+                            if (Cfg::ATM) mma_f16_ts(d_tmem, a_tmem + 8 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                            else mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                        }
                         tc_commit(xempty0 + 8 * stage);
                         tc_commit(aempty0 + 8 * ab);
                         if (kb == kb1 - 1) tc_commit(tfull0 + 8 * acc);
@@ -343,9 +377,34 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 if (++acc == 2) { acc = 0; acc_phase ^= 1; }
             }
             if (lane == 0) prof_stamp(p, 1, t_start);
+#ifdef ARIA_DEBUG
+            if (lane == 0 && p.prof) { p.prof[blockIdx.x * 16 + 5] = w_x; p.prof[blockIdx.x * 16 + 7] = w_a; p.prof[blockIdx.x * 16 + 12] = w_t; }
+#endif
         }
     } else if (warp >= W4_DEQ_WARP0) {
         // ------------------------------------------------------------ dequantiser groups
+        // hand-off of one dequantised row (64 bf16 = 8 x 16 B, k ascending) to the MMA: tensor memory
+        // (this thread's lane, 32 columns of the slot) or the 128-byte-swizzled shared-memory A tile
+        auto publish_a = [&](const uint4 (&o)[8], int it_, uint32_t rowoff_, uint32_t xr_, int q_) {
+            const int ab = it_ % NB;
+            mbar_wait(aempty0 + 8 * ab, ((it_ / NB) & 1) ^ 1);     // MMAs reading this A buffer retired
+            if (Cfg::ATM) {
+                tc_fence_after();
+                uint32_t w[32];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) { w[4 * j] = o[j].x; w[4 * j + 1] = o[j].y; w[4 * j + 2] = o[j].z; w[4 * j + 3] = o[j].w; }
+                tmem_st_32x32b_x32(tmem_base + Cfg::A_COL0 + ab * 32 + (static_cast<uint32_t>(q_ * 32) << 16), w);
+                tmem_wait_st();
+                tc_fence_before();
+            } else {
+                const uint32_t rowb = sA + ab * Cfg::A_BYTES + rowoff_;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) sts128(rowb + ((static_cast<uint32_t>(j) ^ xr_) << 4), o[j]);
+                fence_proxy_async_smem();                  // generic-proxy writes -> async proxy (MMA)
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(afull0 + 8 * ab);           // one arrival per warp
+        };
         const int dw = warp - W4_DEQ_WARP0;
         const int g = dw >> 2;                    // group = A buffer index
         const int r = (dw & 3) * 32 + lane;       // weight row inside the tile
@@ -378,14 +437,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                     for (int c = 0; c < 4; ++c) dequant_i8x16(pk[c], sw, o[2 * c], o[2 * c + 1]);
                     __syncwarp();
                     if (lane == 0) mbar_arrive(pempty0 + 8 * stage);   // packed bytes are in registers
-                    const int ab = it % NB;
-                    const uint32_t rowb = sA + ab * Cfg::A_BYTES + rowoff;
-                    mbar_wait(aempty0 + 8 * ab, ((it / NB) & 1) ^ 1);  // MMAs reading this A buffer retired
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) sts128(rowb + ((static_cast<uint32_t>(j) ^ xr) << 4), o[j]);
-                    fence_proxy_async_smem();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(afull0 + 8 * ab);
+                    publish_a(o, it, rowoff, xr, dw & 3);
                 }
                 continue;
             }
@@ -433,14 +485,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(pempty0 + 8 * stage);   // packed bytes are in registers
-                const int ab = it % NB;                            // A buffer of this k-block
-                const uint32_t rowb = sA + ab * Cfg::A_BYTES + rowoff;
-                mbar_wait(aempty0 + 8 * ab, ((it / NB) & 1) ^ 1);  // MMAs reading this A buffer retired
-#pragma unroll
-                for (int j = 0; j < 8; ++j) sts128(rowb + ((static_cast<uint32_t>(j) ^ xr) << 4), o[j]);
-                fence_proxy_async_smem();                  // generic-proxy writes -> async proxy (MMA)
-                __syncwarp();
-                if (lane == 0) mbar_arrive(afull0 + 8 * ab);       // one arrival per warp
+                publish_a(o, it, rowoff, xr, dw & 3);
             }
         }
         if ((dw & 3) == 0 && lane == 0) prof_stamp(p, 2 + g, t_start);
@@ -614,6 +659,14 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     if (warp >= W4_EPI_WARP0 && warp < W4_DEQ_WARP0 && lane == 0) tma_store_wait<0>();
     tc_fence_before();
     __syncthreads();
+#ifdef ARIA_DEBUG
+    if (threadIdx.x == 0 && p.prof) {
+        unsigned long long gt;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+        p.prof[blockIdx.x * 16 + 15] = static_cast<long long>(gt);
+        p.prof[blockIdx.x * 16 + 13] = clock64() - t_start;
+    }
+#endif
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
@@ -671,7 +724,10 @@ void w4_plan(int M, int N, int K, int sms, int* tt_out, int* splits_out) {
             const long units = static_cast<long>(tiles) * s;
             const long waves = (units + sms - 1) / sms;
             const long kb = (num_kb + s - 1) / s;
-            long unit = kb * (2 * tt + 320) + 40L * tt + 3000;
+            // measured steady-state cycles per 64-k block (role timestamps, C5 layers at M = 2048): tt = 256, A in
+            // shared memory: ~800; tt = 192, A in tensor memory: ~560; smaller tiles: dequantiser bound, ~450
+            const long kcost = tt == 256 ? 800 : tt == 192 ? 560 : 450;
+            long unit = kb * kcost + 40L * tt + 3000;
             if (s > 1) unit += 100L * tt + 4000;
             const long cost = waves * unit;
             if (best < 0 || cost < best) { best = cost; best_tt = tt; best_s = s; }
@@ -701,7 +757,8 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const voi
     p.g_scale = g_scale; p.bias = bias; p.Y = Y;
     p.act = act; p.out_t = yt; p.M = M; p.N = N; p.K = K; p.splits = s;
 #ifdef ARIA_DEBUG
-    p.prof = g_w4_prof;
+    p.dbg = dbg_env("ARIA_W4_DBG") ? atoi(dbg_env("ARIA_W4_DBG")) : 0;
+    p.prof = g_w4_prof ? g_w4_prof + static_cast<size_t>(g_w4_prof_launch++ % 256) * 148 * 16 : nullptr;
 #endif
     const size_t tiles = static_cast<size_t>((N + W4_BN - 1) / W4_BN) * ((M + tt - 1) / tt);
     p.counters = static_cast<unsigned*>(ws);

@@ -33,14 +33,11 @@ inline bool ensure_dyn_smem(Kern kern, int bytes, std::atomic<uint64_t>& mask) {
 }
 
 // ---- quant.cu
-// early (needs pdl): the pass does not wait for the previous grid before it starts -- the caller
-// guarantees that grid neither writes X nor touches q / s -- but still waits for it before it ends.
 // known_absmax: per-row max |x| already computed by the producing epilogue (fused S1): the pass
 // skips its reduction.  zero_absmax: a [R] buffer this pass zeroes (the buffer the GEMM that consumes
 // this pass's codes will atomicMax into).
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl, bool early = false, const float* known_absmax = nullptr,
-                         float* zero_absmax = nullptr, unsigned* zero_counters = nullptr, int n_zero_counters = 0);
+                         bool pdl, const float* known_absmax = nullptr, float* zero_absmax = nullptr);
 int launch_quant_groups_i4(const void* W, int wt, int N, int K, uint8_t* q4, uint16_t* sg,
                            cudaStream_t st);
 
@@ -64,21 +61,14 @@ struct W8Epilogue {
     int out_t;
     float* row_absmax = nullptr;   // fused S1 (first half): per-row max |y| as stored, atomicMax; or nullptr
 };
-// S1 of the NEXT layer, run by spare warps of the GEMM kernel (gemm_w8a8.cu: w8_side_quant).
+// S1 of the NEXT layer, run by the GEMM kernel's epilogue warps while they wait for their first accumulator
+// (gemm_w8a8.cu: w8_side_quant).  Only for an input that the GEMM does not write.
 struct W8Side {
-    const void* X = nullptr;             // [M, K2] activations of the next layer (a row <= 16 KB); nullptr: no side job
+    const void* X = nullptr;             // [M, K2] activations of the next layer, a row <= 8 KB; nullptr: no side job
     int xt = 0, K2 = 0;
     int8_t* q = nullptr;                 // [M, K2] codes
     float* s = nullptr;                  // [M] scales
-    const float* known_absmax = nullptr; // chained (X is THIS GEMM's output): per-row absmax from its epilogue
-    unsigned* mtile_counters = nullptr;  // chained: [ceil(M / 128)] counters, zero before this GEMM's epilogue
-    float* zero_absmax = nullptr;        // the [M] buffer / counters the NEXT GEMM will reduce into: zeroed here
-    unsigned* zero_counters = nullptr;
-    int n_zero_counters = 0;
-    // filled by the launcher:
-    const unsigned* mtile_done = nullptr;
-    unsigned mtile_target = 0;
-    int rows_per_mtile = 0;
+    float* zero_absmax = nullptr;        // the [M] absmax buffer the NEXT GEMM's epilogue will reduce into: zeroed here
 };
 int launch_gemm_w8a8(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, const W8Epilogue& ep,
                      cudaStream_t st, bool pdl, const W8Side* side = nullptr);

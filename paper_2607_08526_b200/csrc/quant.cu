@@ -16,13 +16,9 @@ constexpr int QROW_CACHE = 4;  // 8-element vectors kept in registers per thread
 template <typename T>
 __global__ void __launch_bounds__(QROW_MAX_THREADS)
 quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
-                     float* __restrict__ scale, int early, const float* known_absmax,
-                     float* zero_absmax, unsigned* zero_counters, int n_zero_counters) {
+                     float* __restrict__ scale, const float* known_absmax, float* zero_absmax) {
     __shared__ float red[QROW_MAX_THREADS / 32];
-    // early: X, Xq and scale are untouched by the grid before this one (the caller checked), so the
-    // pass runs concurrently with it; the wait moves to the end so that "this grid is complete" still
-    // implies "every earlier grid is complete" for whoever waits on this one.
-    if (!early) pdl_wait_prior_grid();
+    pdl_wait_prior_grid();
     const int64_t row = blockIdx.x;
     const T* x = X + row * K;
     int8_t* q = Xq + row * K;
@@ -58,7 +54,6 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
     if (tid == 0) {
         scale[row] = s;
         if (zero_absmax) zero_absmax[row] = 0.0f;
-        if (zero_counters && row < n_zero_counters) zero_counters[row] = 0u;
     }
     pdl_launch_dependents();
     const FastQ f = make_fastq(s);
@@ -78,7 +73,6 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
         if (!f.ok || !quant8_fast(t, f, o)) o = quant8_i8(t, s);
         *reinterpret_cast<uint2*>(q + 8 * idx) = o;
     }
-    if (early) pdl_wait_prior_grid();
 }
 
 // One WARP per row (K <= 8 * 32 * VPL): every lane issues all its 16-byte loads up front, the
@@ -86,16 +80,12 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
 template <typename T, int VPL>
 __global__ void __launch_bounds__(256)
 quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restrict__ Xq,
-                          float* __restrict__ scale, int early, const float* known_absmax,
-                          float* zero_absmax, unsigned* zero_counters, int n_zero_counters) {
-    if (!early) pdl_wait_prior_grid();      // early: see quant_rows_i8_kernel
+                          float* __restrict__ scale, const float* known_absmax, float* zero_absmax) {
+    pdl_wait_prior_grid();
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
     const int64_t row = static_cast<int64_t>(blockIdx.x) * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (row >= R) {
-        if (early) pdl_wait_prior_grid();
-        return;
-    }
+    if (row >= R) return;
     const T* x = X + row * K;
     int8_t* q = Xq + row * K;
     const int nvec = K >> 3;
@@ -124,7 +114,6 @@ quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restr
     if (lane == 0) {
         scale[row] = s;
         if (zero_absmax) zero_absmax[row] = 0.0f;
-        if (zero_counters && row < n_zero_counters) zero_counters[row] = 0u;
     }
     const FastQ f = make_fastq(s);
 #pragma unroll
@@ -138,7 +127,6 @@ quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restr
             *reinterpret_cast<uint2*>(q + 8 * idx) = o;
         }
     }
-    if (early) pdl_wait_prior_grid();
 }
 
 // int4, group 32 along K: 4 threads per group, 8 elements each (R3, R4, R7, R8).
@@ -169,19 +157,16 @@ quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restri
 
 template <typename T, int VPL>
 static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, float* s,
-                                    cudaLaunchConfig_t& cfg, int early, const float* known, float* zero,
-                                    unsigned* zc, int nzc) {
+                                    cudaLaunchConfig_t& cfg, const float* known, float* zero) {
     constexpr int WARPS = 8;
     cfg.blockDim = dim3(32 * WARPS);
     cfg.gridDim = dim3((R + WARPS - 1) / WARPS);
-    return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s, early,
-                              known, zero, zc, nzc);
+    return cudaLaunchKernelEx(&cfg, quant_rows_i8_warp_kernel<T, VPL>, static_cast<const T*>(X), R, C, q, s, known, zero);
 }
 
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl, bool early_, const float* known, float* zero, unsigned* zc, int nzc) {
+                         bool pdl, const float* known, float* zero) {
     const int nvec = C / 8;
-    const int early = pdl && early_ ? 1 : 0;
     {   // warp-per-row variants: rows up to 3072 elements (wider rows: one CTA per row, below; a 24-vector
         // warp-per-row variant for 6144-element bf16 rows was measured slower: 2.18 vs 2.08 ms per C5 step)
         cudaLaunchConfig_t cfg = {};
@@ -195,14 +180,14 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
         cudaError_t e = cudaErrorInvalidValue;
         bool done = true;
         if (xt == ARIA_BF16) {
-            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
-            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
-            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
+            if (vpl <= 2) e = launch_warp_rows<__nv_bfloat16, 2>(X, R, C, q, s, cfg, known, zero);
+            else if (vpl <= 6) e = launch_warp_rows<__nv_bfloat16, 6>(X, R, C, q, s, cfg, known, zero);
+            else if (vpl <= 12) e = launch_warp_rows<__nv_bfloat16, 12>(X, R, C, q, s, cfg, known, zero);
             else done = false;
         } else {
-            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
-            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
-            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg, early, known, zero, zc, nzc);
+            if (vpl <= 2) e = launch_warp_rows<float, 2>(X, R, C, q, s, cfg, known, zero);
+            else if (vpl <= 6) e = launch_warp_rows<float, 6>(X, R, C, q, s, cfg, known, zero);
+            else if (vpl <= 12) e = launch_warp_rows<float, 12>(X, R, C, q, s, cfg, known, zero);
             else done = false;
         }
         if (done) return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
@@ -220,10 +205,10 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
     cfg.numAttrs = pdl ? 1 : 0;
     cudaError_t e;
     if (xt == ARIA_F32)
-        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s, early, known, zero, zc, nzc);
+        e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<float>, static_cast<const float*>(X), C, q, s, known, zero);
     else
         e = cudaLaunchKernelEx(&cfg, quant_rows_i8_kernel<__nv_bfloat16>,
-                               static_cast<const __nv_bfloat16*>(X), C, q, s, early, known, zero, zc, nzc);
+                               static_cast<const __nv_bfloat16*>(X), C, q, s, known, zero);
     return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
