@@ -23,7 +23,11 @@
  * Parity pins: tests/test_oracle_*.py (hand-worked H1/H2 from SURVEY.md S8(c),
  * brute-force nearest-code search, invariants, closed forms, numpy fp64 matmul,
  * numpy/ml_dtypes conversions; O6 and O7: hand-worked H3 / H4 in tests/golden/,
- * integer special cases, numpy, the alpha = 0 / beta = -1 invariants).
+ * integer special cases, numpy, the alpha = 0 / beta = -1 invariants; O8 and O9:
+ * hand-worked H5 / H6 in tests/golden/, zero-mean / unit-variance and shift / scale
+ * invariances, uniform and one-hot attention, key-permutation and key-shift
+ * invariance, torch fp64 layer_norm / scaled_dot_product_attention as the library
+ * routine).
  * Parity unpinned: none.
  */
 #include <math.h>
@@ -401,6 +405,85 @@ void oracle_steer(const float *H, int64_t M, int64_t D, const float *d, double s
                 out[t * D + j] = h + strength * c * (double)d[j];
         }
     }
+}
+
+/* -------------------------------------------------------------------- O8 */
+/* Normalisation that precedes QKV / MLP-up inside a DiT block, the producer whose
+ * output S1 quantises (SURVEY S8(f) NEXT-2 "norm -> act-quant fusion"
+ * names only "the diffusion transformer (DiT)" [10] and L224 / L278 the blocks'
+ * self-attention; it gives no formula, so the textbook definitions are taken,
+ * DESIGN.md R20):
+ *   kind 0, LayerNorm:  mu = mean_k x;  var = mean_k (x - mu)^2  (biased);
+ *                       n[k] = (x[k] - mu) / sqrt(var + eps) * gamma[k] + beta[k]
+ *   kind 1, RMSNorm:    n[k] = x[k] / sqrt(mean_k x^2 + eps) * gamma[k] + beta[k]
+ * beta may be NULL (0).  All arithmetic in fp64; the caller rounds n once to the
+ * activation dtype (oracle_round_out) -- the tensor an unfused norm kernel would
+ * store -- and feeds that to O1. */
+void oracle_norm_rows(const float *X, int64_t M, int64_t K, const float *gamma, const float *beta,
+                      int kind, double eps, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < M; ++m) {
+        const float *x = X + m * K;
+        double mu = 0.0;
+        if (kind == 0) {
+            for (int64_t k = 0; k < K; ++k)
+                mu += (double)x[k];
+            mu /= (double)K;
+        }
+        double var = 0.0;
+        for (int64_t k = 0; k < K; ++k)
+            var += ((double)x[k] - mu) * ((double)x[k] - mu);
+        var /= (double)K;
+        double rstd = 1.0 / sqrt(var + eps);
+        for (int64_t k = 0; k < K; ++k)
+            out[m * K + k] = ((double)x[k] - mu) * rstd * (double)gamma[k] + (beta ? (double)beta[k] : 0.0);
+    }
+}
+
+/* -------------------------------------------------------------------- O9 */
+/* Full (unmasked, non-causal) multi-head self-attention between the fused QKV
+ * projection and the out-projection ("the
+ * transformer's full self-attention ... a fused attention kernel (FlashAttention-
+ * class)", L224).  The definition, per sequence b, head h, query i:
+ *     s_j = scale * sum_d q_i[d] k_j[d];   p_j = exp(s_j - max_j s) / sum_j exp(s_j - max_j s);
+ *     o_i[d] = sum_j p_j v_j[d]
+ * Layout (R21): QKV [B*S, 3*H*Dh], row = token b*S + i, columns
+ * [ q (H*Dh) | k (H*Dh) | v (H*Dh) ], head h at columns h*Dh .. h*Dh+Dh-1 of its
+ * third; O [B*S, H*Dh].  fp64 throughout (subtracting the row maximum changes
+ * nothing mathematically; it only keeps exp() in range). */
+void oracle_attention(const float *QKV, int64_t B, int64_t S, int64_t H, int64_t Dh, double scale, double *O)
+{
+    const int64_t ld = 3 * H * Dh;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int64_t b = 0; b < B; ++b)
+        for (int64_t h = 0; h < H; ++h) {
+            double s[S];
+            for (int64_t i = 0; i < S; ++i) {
+                const float *q = QKV + (b * S + i) * ld + h * Dh;
+                double mx = -INFINITY;
+                for (int64_t j = 0; j < S; ++j) {
+                    const float *k = QKV + (b * S + j) * ld + H * Dh + h * Dh;
+                    double a = 0.0;
+                    for (int64_t d = 0; d < Dh; ++d)
+                        a += (double)q[d] * (double)k[d];
+                    s[j] = scale * a;
+                    if (s[j] > mx)
+                        mx = s[j];
+                }
+                double l = 0.0;
+                for (int64_t j = 0; j < S; ++j) {
+                    s[j] = exp(s[j] - mx);
+                    l += s[j];
+                }
+                for (int64_t d = 0; d < Dh; ++d) {
+                    double a = 0.0;
+                    for (int64_t j = 0; j < S; ++j)
+                        a += s[j] * (double)QKV[(b * S + j) * ld + 2 * H * Dh + h * Dh + d];
+                    O[(b * S + i) * H * Dh + h * Dh + d] = a / l;
+                }
+            }
+        }
 }
 
 /* ------------------------------------------------------------ output cast */

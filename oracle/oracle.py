@@ -75,6 +75,11 @@ def _load():
         L.oracle_steer.restype = None
         L.oracle_steer.argtypes = [POINTER(c_float), c_int64, c_int64, POINTER(c_float), c_double, c_double, c_int,
                                    POINTER(c_double)]
+        L.oracle_norm_rows.restype = None
+        L.oracle_norm_rows.argtypes = [POINTER(c_float), c_int64, c_int64, POINTER(c_float), POINTER(c_float), c_int,
+                                       c_double, POINTER(c_double)]
+        L.oracle_attention.restype = None
+        L.oracle_attention.argtypes = [POINTER(c_float), c_int64, c_int64, c_int64, c_int64, c_double, POINTER(c_double)]
         L.oracle_round_out.restype = None
         L.oracle_round_out.argtypes = [POINTER(c_double), c_int64, c_int, POINTER(c_float)]
         L.oracle_num_threads.restype = c_int
@@ -247,6 +252,41 @@ def steer(H, d, strength: float, hbar_norm: float = 1.0, op: int = STEER_ADD):
     out = np.empty((M, D), np.float64)
     _load().oracle_steer(_p(H, c_float), M, D, _p(d, c_float), float(strength), float(hbar_norm), op, _p(out, c_double))
     return out
+
+
+# ------------------------------------------------------------------------ O8
+NORM_LAYER, NORM_RMS = 0, 1
+
+
+def norm_rows(X, gamma, beta=None, kind: int = NORM_LAYER, eps: float = 1e-5):
+    """O8: LayerNorm (kind 0) / RMSNorm (kind 1) over the last axis, fp64 out [M,K]."""
+    X = _c(X, np.float32)
+    gamma = _c(gamma, np.float32)
+    b = None if beta is None else _c(beta, np.float32)
+    M, K = X.shape
+    out = np.empty((M, K), np.float64)
+    _load().oracle_norm_rows(_p(X, c_float), M, K, _p(gamma, c_float), None if b is None else _p(b, c_float), kind,
+                             float(eps), _p(out, c_double))
+    return out
+
+
+def norm_quant_int8(X, gamma, beta=None, kind: int = NORM_LAYER, eps: float = 1e-5, dtype: int = 1):
+    """O8 then O1: n = round_dtype(norm(X)) (the tensor an unfused norm kernel stores), (q, s) = O1(n)."""
+    n = round_out(norm_rows(X, gamma, beta, kind, eps), dtype)
+    q, s = quant_int8_rows(n)
+    return n, q, s
+
+
+# ------------------------------------------------------------------------ O9
+def attention(QKV, B: int, S: int, H: int, Dh: int, scale: float | None = None):
+    """O9: full softmax(q k^T * scale) v per (sequence, head), fp64 out [B*S, H*Dh]."""
+    QKV = _c(QKV, np.float32)
+    assert QKV.shape == (B * S, 3 * H * Dh)
+    if scale is None:
+        scale = 1.0 / np.sqrt(Dh)
+    O = np.empty((B * S, H * Dh), np.float64)
+    _load().oracle_attention(_p(QKV, c_float), B, S, H, Dh, float(scale), _p(O, c_double))
+    return O
 
 
 # ---------------------------------------------------------------- output cast
