@@ -58,6 +58,7 @@ typedef enum { ARIA_F32 = 0, ARIA_BF16 = 1 } aria_dtype;
 typedef enum { ARIA_ACT_NONE = 0, ARIA_ACT_GELU_ERF = 1 } aria_act;
 typedef enum { ARIA_W8A8 = 0, ARIA_W4A16 = 1, ARIA_W8A16 = 2 } aria_mode;
 typedef enum { ARIA_STEER_ADD = 0, ARIA_STEER_PROJECT = 1 } aria_steer_op;
+typedef enum { ARIA_NORM_LAYER = 0, ARIA_NORM_RMS = 1 } aria_norm;
 
 /* ---------------------------------------------------------------------------------------
  * S0 -- weight quantisation, once at load (configs C1-C3; readings R2-R4).
@@ -230,6 +231,42 @@ ARIA_API int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, 
  * model", L77).  D % 8 == 0; fp32 arithmetic, one rounding to `ht`.  Enqueue only, capturable.        */
 ARIA_API int aria_steer(void* H, int ht, int M, int D, const float* d, const float* strength, float hbar_norm,
                         int op, void* stream);
+
+/* NEXT-2 ("producers/consumers around the linears") -- the two pieces of a DiT block that
+ * sit between the quantized linears ("the diffusion transformer (DiT)"; L278 "the transformer's full
+ * self-attention ... a fused attention kernel (FlashAttention-class) ... is the open lever"; L224).  The paper
+ * gives neither formula; the textbook definitions are taken (R20-R22).
+ *
+ * aria_norm_quantize_act_int8 -- normalisation fused with S1: per token row,
+ *   norm ARIA_NORM_LAYER:  mu = mean_k x;  var = mean_k (x - mu)^2;  n = (x - mu) / sqrt(var + eps) * gamma + beta
+ *   norm ARIA_NORM_RMS:    n = x / sqrt(mean_k x^2 + eps) * gamma + beta
+ *   n is rounded once to dtype `xt` (the tensor an unfused norm kernel would store), then S1 exactly as
+ *   aria_quantize_act_int8:  x_scale = max|n| / 127 (1 for a zero row), Xq = clamp(rint(n / x_scale), +-127).
+ * X: [M,K] of dtype `xt`; gamma: fp32 [K]; beta: fp32 [K] or NULL; eps >= 0.  Xq int8 [M,K], x_scale fp32 [M]
+ * feed aria_linear_w8a8_q.  Xn: [M,K] of dtype `xt`, or NULL -- the normalised tensor is written only on request
+ * (the fused path reads X once and writes one byte per element).  fp32 arithmetic (two-pass variance); codes and
+ * scales are bit-identical to aria_quantize_act_int8 applied to Xn.  K % 32 == 0, K <= 24576.  Enqueue only.   */
+ARIA_API int aria_norm_quantize_act_int8(const void* X, int xt, int M, int K, const float* gamma, const float* beta,
+                                         int norm, float eps, void* Xn, int8_t* Xq, float* x_scale, void* stream);
+
+/* aria_attention -- full (unmasked, non-causal) multi-head self-attention on the fused QKV projection's output:
+ *   per sequence b, head h, query i:  s_j = scale * q_i . k_j;  p = softmax_j(s);  o_i = sum_j p_j v_j.
+ * QKV: bf16 [B*S, 3*H*Dh], row = token b*S + i, columns [ q (H*Dh) | k (H*Dh) | v (H*Dh) ], head h at columns
+ * h*Dh .. h*Dh+Dh-1 of its third.  O: bf16 [B*S, H*Dh] (the out-projection's input).  Dh must be 64; scale > 0
+ * (1/sqrt(Dh) = 0.125 for the usual choice).  Scores and the output accumulate in fp32 on the tensor cores
+ * (tcgen05 kind::f16, bf16 operands); the probabilities enter the second product rounded to bf16
+ * (FlashAttention-class; R22 derives the tolerance).  row_absmax: NULL, or fp32 [B*S] that the caller
+ * has ZEROED: the kernel reduces max_d |O[t, :]| over all heads into it (atomicMax on the stored bf16 values) --
+ * the first half of a fused S1 for a W8A8 out-projection, finished by aria_round_act_int8.  Enqueue only.   */
+ARIA_API int aria_attention(const void* QKV, int B, int S, int H, int Dh, float scale, void* O, float* row_absmax,
+                            void* stream);
+
+/* Second half of a fused S1 (north_star "activation-quantization pass fused into the previous epilogue"): the
+ * per-token max|x| is already known (reduced by the kernel that produced X, e.g. aria_attention), so the pass
+ * only rounds:  x_scale = absmax / 127 (1 if 0), Xq = clamp(rint(x / x_scale), +-127).  Bit-identical to
+ * aria_quantize_act_int8 when absmax[m] == max_k |X[m,k]|.  absmax: fp32 [M], left untouched.              */
+ARIA_API int aria_round_act_int8(const void* X, int xt, int M, int K, const float* absmax, int8_t* Xq, float* x_scale,
+                                 void* stream);
 
 /* Measurement helper, NOT part of the hot path (SURVEY.md S7 hard part 2 / S8(d): "measure an int8
  * peak on the box first: a plain back-to-back tcgen05.mma kind::i8 issue loop with no memory

@@ -20,6 +20,7 @@ F32, BF16 = 0, 1
 ACT_NONE, ACT_GELU_ERF = 0, 1
 W8A8, W4A16, W8A16 = 0, 1, 2
 STEER_ADD, STEER_PROJECT = 0, 1
+NORM_LAYER, NORM_RMS = 0, 1
 
 _lib = None
 
@@ -60,6 +61,10 @@ def lib() -> ctypes.CDLL:
         L.aria_linear_w8a16.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p,
                                         c_int, c_void_p, c_int, c_void_p, c_size_t, c_void_p]
         L.aria_steer.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, ctypes.c_float, c_int, c_void_p]
+        L.aria_norm_quantize_act_int8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int, ctypes.c_float,
+                                                  c_void_p, c_void_p, c_void_p, c_void_p]
+        L.aria_attention.argtypes = [c_void_p, c_int, c_int, c_int, c_int, ctypes.c_float, c_void_p, c_void_p, c_void_p]
+        L.aria_round_act_int8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p, c_void_p]
         L.aria_gemm_i8_i32.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
         L.aria_denoiser_linears.argtypes = [ctypes.POINTER(aria_layer), c_int, c_int, c_int, c_int,
                                             c_void_p, c_size_t, c_void_p]
@@ -87,7 +92,8 @@ EXPORTS = ("aria_linear_w8a8_q", "aria_quantize_weights_int8", "aria_quantize_we
            "aria_denoiser_linears_host", "aria_workspace_bytes", "aria_workspace_bytes_host",
            "aria_status_string", "aria_gemm_i8_i32", "aria_version", "aria_stack_plan_create",
            "aria_stack_plan_run", "aria_stack_plan_is_streaming", "aria_stack_plan_destroy",
-           "aria_stack_plan_fallback_fired", "aria_w8a8_tile_plan", "aria_w4a16_tile_plan", "aria_tensor_peak", "aria_linear_w8a16", "aria_steer")
+           "aria_stack_plan_fallback_fired", "aria_w8a8_tile_plan", "aria_w4a16_tile_plan", "aria_tensor_peak", "aria_linear_w8a16", "aria_steer",
+           "aria_norm_quantize_act_int8", "aria_attention", "aria_round_act_int8")
 
 
 def _check(rc: int, what: str):
@@ -213,6 +219,39 @@ def aria_steer(H: torch.Tensor, d: torch.Tensor, strength: torch.Tensor, hbar_no
     _check(lib().aria_steer(_ptr(H), _dt(H), M, D, _ptr(d), _ptr(strength), float(hbar_norm), op, _stream()),
            "aria_steer")
     return H
+
+
+def aria_norm_quantize_act_int8(X, gamma, beta=None, norm: int = NORM_LAYER, eps: float = 1e-5, want_xn: bool = False,
+                                out=None):
+    """Norm fused with S1.  Returns (Xq, x_scale) or (Xq, x_scale, Xn) with want_xn; `out` = (Xq, x_scale) to reuse."""
+    M, K = X.shape
+    assert gamma.dtype == torch.float32 and (beta is None or beta.dtype == torch.float32)
+    Xq, sx = out if out is not None else (torch.empty((M, K), dtype=torch.int8, device=X.device),
+                                          torch.empty((M,), dtype=torch.float32, device=X.device))
+    Xn = torch.empty_like(X) if want_xn else None
+    _check(lib().aria_norm_quantize_act_int8(_ptr(X), _dt(X), M, K, _ptr(gamma), _ptr(beta), norm, float(eps), _ptr(Xn),
+                                             _ptr(Xq), _ptr(sx), _stream()), "aria_norm_quantize_act_int8")
+    return (Xq, sx, Xn) if want_xn else (Xq, sx)
+
+
+def aria_attention(QKV, B: int, S: int, H: int, Dh: int = 64, scale: float | None = None, out=None, row_absmax=None):
+    """QKV bf16 [B*S, 3*H*Dh] -> O bf16 [B*S, H*Dh].  row_absmax: zeroed fp32 [B*S] tensor or None."""
+    assert QKV.dtype == torch.bfloat16 and tuple(QKV.shape) == (B * S, 3 * H * Dh)
+    O = out if out is not None else torch.empty((B * S, H * Dh), dtype=torch.bfloat16, device=QKV.device)
+    if scale is None:
+        scale = Dh ** -0.5
+    _check(lib().aria_attention(_ptr(QKV), B, S, H, Dh, float(scale), _ptr(O), _ptr(row_absmax), _stream()),
+           "aria_attention")
+    return O
+
+
+def aria_round_act_int8(X, absmax, out=None):
+    M, K = X.shape
+    Xq, sx = out if out is not None else (torch.empty((M, K), dtype=torch.int8, device=X.device),
+                                          torch.empty((M,), dtype=torch.float32, device=X.device))
+    _check(lib().aria_round_act_int8(_ptr(X), _dt(X), M, K, _ptr(absmax), _ptr(Xq), _ptr(sx), _stream()),
+           "aria_round_act_int8")
+    return Xq, sx
 
 
 def aria_gemm_i8_i32(Xq, Wq):

@@ -278,6 +278,35 @@ int aria_steer(void* H, int ht, int M, int D, const float* d, const float* stren
     return launch_steer(H, ht, M, D, d, strength, hbar_norm, op, static_cast<cudaStream_t>(stream));
 }
 
+int aria_norm_quantize_act_int8(const void* X, int xt, int M, int K, const float* gamma, const float* beta, int norm,
+                                float eps, void* Xn, int8_t* Xq, float* x_scale, void* stream) {
+    int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
+    if (rc != ARIA_OK) return rc;
+    if (!gamma) return ARIA_ERR_NULL;
+    if (norm != ARIA_NORM_LAYER && norm != ARIA_NORM_RMS) return ARIA_ERR_DTYPE;
+    if (!(eps >= 0.0f) || K > 24576) return ARIA_ERR_SHAPE;
+    if (misaligned(gamma) || misaligned(beta) || misaligned(Xn)) return ARIA_ERR_ALIGN;
+    return launch_norm_quant(X, xt, M, K, gamma, beta, norm, eps, Xn, Xq, x_scale, static_cast<cudaStream_t>(stream), false);
+}
+
+int aria_attention(const void* QKV, int B, int S, int H, int Dh, float scale, void* O, float* row_absmax, void* stream) {
+    if (!QKV || !O) return ARIA_ERR_NULL;
+    if (B <= 0 || S <= 0 || H <= 0 || Dh != 64 || !(scale > 0.0f) || B > 65535 || H > 65535) return ARIA_ERR_SHAPE;
+    if (misaligned(QKV) || misaligned(O) || (reinterpret_cast<uintptr_t>(row_absmax) & 3u)) return ARIA_ERR_ALIGN;
+    int rc = check_arch();
+    if (rc != ARIA_OK) return rc;
+    return launch_attention(QKV, B, S, H, scale, O, row_absmax, static_cast<cudaStream_t>(stream), false);
+}
+
+int aria_round_act_int8(const void* X, int xt, int M, int K, const float* absmax, int8_t* Xq, float* x_scale,
+                        void* stream) {
+    int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
+    if (rc != ARIA_OK) return rc;
+    if (!absmax) return ARIA_ERR_NULL;
+    if (reinterpret_cast<uintptr_t>(absmax) & 3u) return ARIA_ERR_ALIGN;
+    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), false, absmax, nullptr);
+}
+
 int aria_tensor_peak(int kind, int ctas, int iters, double seconds, double* out, void* stream) {
     if (!out) return ARIA_ERR_NULL;
     if ((kind != 0 && kind != 1) || (ctas != 1 && ctas != 2) || iters <= 0 || iters > (1 << 24) || seconds < 0.0 ||

@@ -46,6 +46,10 @@ int launch_quant_groups_i4(const void* W, int wt, int N, int K, uint8_t* q4, uin
 // swizzle_bytes in {0, 32, 64, 128}.  Returns ARIA_OK or ARIA_ERR_CUDA.
 int make_tmap_2d(CUtensorMap* out, const void* base, int elem_bytes, uint64_t rows, uint64_t cols,
                  uint32_t box_rows, uint32_t box_cols, int swizzle_bytes);
+// 3-D tensor, dims (d0 innermost, d1, d2) with byte strides of d1 and d2; box = (box0, box1, box2).
+int make_tmap_3d(CUtensorMap* out, const void* base, int elem_bytes, uint64_t d0, uint64_t d1, uint64_t d2,
+                 uint64_t stride1_bytes, uint64_t stride2_bytes, uint32_t box0, uint32_t box1, uint32_t box2,
+                 int swizzle_bytes);
 int num_sms();
 int check_arch();  // ARIA_OK on compute capability 10.x, else ARIA_ERR_ARCH / ARIA_ERR_CUDA
 
@@ -94,6 +98,14 @@ void w4_set_profile_buffer(long long* p);  // per-CTA role timestamps
 // ---- steer.cu: in-graph activation steering (eq. 2 / projection), strength read from device memory
 int launch_steer(void* H, int ht, int M, int D, const float* d, const float* strength, float hbar_norm, int op,
                  cudaStream_t st);
+
+// ---- norm.cu: LayerNorm / RMSNorm fused with the S1 quantiser (NEXT-2).  Xn (normalised tensor, dtype xt) may be nullptr.
+int launch_norm_quant(const void* X, int xt, int M, int K, const float* gamma, const float* beta, int kind, float eps,
+                      void* Xn, int8_t* q, float* s, cudaStream_t st, bool pdl);
+
+// ---- attention.cu: fused full self-attention on the [B*S, 3*H*64] bf16 output of the QKV projection (NEXT-2)
+int launch_attention(const void* QKV, int B, int S, int H, float scale, void* O, float* row_absmax, cudaStream_t st,
+                     bool pdl);
 
 // ---- peak.cu: measurement helper (tensor-pipe issue loop)
 int tensor_peak(int kind, int ctas, int iters, double seconds, double* out, cudaStream_t st);

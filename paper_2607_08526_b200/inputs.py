@@ -125,3 +125,32 @@ def steer_direction(d_model: int, tensor_id: int = 0):
     rng = np.random.default_rng([0, 7, int(tensor_id)])
     v = rng.standard_normal(d_model)
     return (v / np.linalg.norm(v)).astype(np.float32), float(np.sqrt(d_model))
+
+
+HEAD_DIM = 64             # reading R21: d_model / 64 heads (24 for medium, 16 for small-music)
+
+
+def norm_params(K: int, tensor_id: int = 0):
+    """Seeded LayerNorm / RMSNorm parameters (fp32): gain ~ 1 + 0.1 N(0,1), shift ~ 0.05 N(0,1)."""
+    g = (1.0 + normal_f32((K,), 0.1, 8, 2 * tensor_id)).astype(np.float32)
+    b = normal_f32((K,), 0.05, 8, 2 * tensor_id + 1)
+    return g, b
+
+
+def residual_stream(M: int, K: int, tensor_id: int = 0, outliers: bool = True, mean: float = 0.25):
+    """A bf16 residual-stream tensor [M,K] ~ N(mean, 1) with C3-style outlier channels (1% of K, x20): what the
+    block's normalisation sees.  Returns (bits, fp32 values)."""
+    x = normal_f32((M, K), 1.0, 8, 100 + tensor_id) + np.float32(mean)
+    if outliers:
+        x[:, outlier_channels(K, 8, 200 + tensor_id)] *= np.float32(OUTLIER_GAIN)
+    b = bf16_bits(x)
+    return b, bf16_as_f32(b)
+
+
+def qkv_activations(B: int, S: int, H: int, Dh: int = HEAD_DIM, tensor_id: int = 0, q_gain: float = 1.0):
+    """bf16 [B*S, 3*H*Dh] ~ N(0,1) standing in for the fused QKV projection's output (columns [q | k | v]);
+    q_gain > 1 sharpens the softmax.  Returns (bits, fp32 values)."""
+    x = normal_f32((B * S, 3 * H * Dh), 1.0, 8, 300 + tensor_id)
+    x[:, : H * Dh] *= np.float32(q_gain)
+    b = bf16_bits(x)
+    return b, bf16_as_f32(b)
