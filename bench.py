@@ -279,6 +279,69 @@ def next_rows(torch, aria, inputs, pk):
                              "frac_of_bf16_burst": st.ops / (ms * 1e-3) / 1e12 / pk["bf16_burst"],
                              "launches": len(st.specs), "weight_mb": round(st.weight_bytes / 1e6, 1)}
     del st
+    # NEXT-2: the producers around the linears.  (a) aria_attention alone at the step's shape (2 CFG branches x
+    # 1024 tokens, 24 heads of 64): the kernel is bound by the exponential unit (16 MUFU lanes per SM: 16384 ex2
+    # per 128 x 128 tile = 1024 cycles against 512 cycles of tensor work), so its roofline is exps / s.
+    # (b) aria_norm_quantize_act_int8 alone (HBM bound: 2 bytes in, 1 byte out per element).  (c) the whole
+    # truly chained W8A8 step with both inside the captured graph (BlockStack).
+    from paper_2607_08526_b200.stack import BlockStack
+    B, S, H = 2, 1024, inputs.D_MODEL // inputs.HEAD_DIM
+    bits, _ = inputs.qkv_activations(B, S, H, inputs.HEAD_DIM, 0)
+    qkvs = [torch.from_numpy(bits.view(np.int16).copy()).cuda().view(torch.bfloat16) for _ in range(8)]   # 8 x 18.9 MB > L2
+    O = torch.empty((B * S, H * inputs.HEAD_DIM), dtype=torch.bfloat16, device="cuda")
+
+    def att_all():
+        for q in qkvs:
+            aria.aria_attention(q, B, S, H, inputs.HEAD_DIM, None, out=O)
+    att_all()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        att_all()
+    g.replay()
+    ms = time_region(torch, g.replay, 10) / len(qkvs)
+    flops = 4.0 * B * H * S * S * inputs.HEAD_DIM
+    exps = float(B * H * S * S)
+    sm_hz = (pk.get("sm_mhz") or 1900.0) * 1e6
+    out["attention_2x1024x24x64"] = {
+        "us": ms * 1e3, "tflops": flops / (ms * 1e-3) / 1e12, "gexp_per_s": exps / (ms * 1e-3) / 1e9,
+        "bound": "alu (MUFU ex2)", "peak_gexp_per_s": 148 * 16 * sm_hz / 1e9,
+        "frac_of_mufu_peak": exps / (ms * 1e-3) / (148 * 16 * sm_hz),
+        "peak_note": "148 SMs x 16 ex2 / clk x 1.90 GHz (B300_MICROARCH.md unit counts; clock = typical under this kernel)",
+        "frac_of_bf16_burst": flops / (ms * 1e-3) / 1e12 / pk["bf16_burst"]}
+    del qkvs
+    xs = [torch.from_numpy(inputs.residual_stream(2048, inputs.D_MODEL, i)[0].view(np.int16).copy()).cuda().view(torch.bfloat16)
+          for i in range(24)]                                                                              # 24 x 6.3 MB > L2
+    gm, bt = inputs.norm_params(inputs.D_MODEL, 0)
+    gm, bt = torch.from_numpy(gm).cuda(), torch.from_numpy(bt).cuda()
+    xq = torch.empty((2048, inputs.D_MODEL), dtype=torch.int8, device="cuda")
+    sx = torch.empty((2048,), dtype=torch.float32, device="cuda")
+
+    def nq_all():
+        for x in xs:
+            aria.aria_norm_quantize_act_int8(x, gm, bt, aria.NORM_LAYER, 1e-5, out=(xq, sx))
+    nq_all()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        nq_all()
+    g.replay()
+    ms = time_region(torch, g.replay, 10) / len(xs)
+    nbytes = 2048 * inputs.D_MODEL * 3 + 2048 * 4 + 2 * 4 * inputs.D_MODEL
+    out["norm_quant_2048x1536"] = {"us": ms * 1e3, "gbs": nbytes / (ms * 1e-3) / 1e9,
+                                   "hbm_frac_measured": nbytes / (ms * 1e-3) / 1e9 / pk["hbm_gbs"], "bytes": nbytes}
+    del xs
+    bs = BlockStack(B=2, S=1024)
+    bs.capture()
+    for _ in range(3):
+        bs.replay()
+    ms = time_region(torch, bs.replay, 10)
+    out["dit_blocks_w8a8_chained"] = {
+        "ms": ms, "launches": bs.launches_per_block * bs.n_blocks,
+        "linear_tops": bs.lin_ops / (ms * 1e-3) / 1e12, "all_tops": bs.ops / (ms * 1e-3) / 1e12,
+        "what": "24 blocks x (LayerNorm+S1, QKV, attention+absmax, S1 rounding, out-proj, LayerNorm+S1, up+GELU, S1, down), "
+                "every tensor chained, one CUDA graph"}
+    del bs
     d_model, n_blocks = inputs.MODELS["small-music"]
     sm = LinearStack(aria.W8A8, M=2048, n_blocks=n_blocks, d_model=d_model)
     d, norm = inputs.steer_direction(d_model, 0)
@@ -605,7 +668,16 @@ def main():
                     help="only the per-linear table C2/C3/C4 (used for ncu captures)")
     ap.add_argument("--small-m-only", action="store_true",
                     help="only the M=32 W4A16 stream-kernel section (used for ncu captures)")
+    ap.add_argument("--next-rows-only", action="store_true",
+                    help="only the SURVEY S8(f) rows: W8A16 stack, attention, norm+S1, chained blocks, 8-step clip")
     args = ap.parse_args()
+    if args.next_rows_only:
+        import torch
+        from paper_2607_08526_b200 import binding as aria
+        from paper_2607_08526_b200 import inputs
+        aria.lib()
+        print(json.dumps({"next_rows": next_rows(torch, aria, inputs, peaks())}))
+        return
     if args.per_linear_only:
         import torch
         from paper_2607_08526_b200 import binding as aria

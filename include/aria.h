@@ -264,9 +264,10 @@ ARIA_API int aria_attention(const void* QKV, int B, int S, int H, int Dh, float 
 /* Second half of a fused S1 (north_star "activation-quantization pass fused into the previous epilogue"): the
  * per-token max|x| is already known (reduced by the kernel that produced X, e.g. aria_attention), so the pass
  * only rounds:  x_scale = absmax / 127 (1 if 0), Xq = clamp(rint(x / x_scale), +-127).  Bit-identical to
- * aria_quantize_act_int8 when absmax[m] == max_k |X[m,k]|.  absmax: fp32 [M], left untouched.              */
-ARIA_API int aria_round_act_int8(const void* X, int xt, int M, int K, const float* absmax, int8_t* Xq, float* x_scale,
-                                 void* stream);
+ * aria_quantize_act_int8 when absmax[m] == max_k |X[m,k]|.  absmax: fp32 [M]; clear != 0 resets absmax[m] to 0
+ * once it has been read, so the buffer is ready for the next producer without a memset in the captured step.  */
+ARIA_API int aria_round_act_int8(const void* X, int xt, int M, int K, float* absmax, int clear, int8_t* Xq,
+                                 float* x_scale, void* stream);
 
 /* Measurement helper, NOT part of the hot path (SURVEY.md S7 hard part 2 / S8(d): "measure an int8
  * peak on the box first: a plain back-to-back tcgen05.mma kind::i8 issue loop with no memory

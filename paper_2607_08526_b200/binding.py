@@ -64,7 +64,7 @@ def lib() -> ctypes.CDLL:
         L.aria_norm_quantize_act_int8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int, ctypes.c_float,
                                                   c_void_p, c_void_p, c_void_p, c_void_p]
         L.aria_attention.argtypes = [c_void_p, c_int, c_int, c_int, c_int, ctypes.c_float, c_void_p, c_void_p, c_void_p]
-        L.aria_round_act_int8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p, c_void_p]
+        L.aria_round_act_int8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_int, c_void_p, c_void_p, c_void_p]
         L.aria_gemm_i8_i32.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p]
         L.aria_denoiser_linears.argtypes = [ctypes.POINTER(aria_layer), c_int, c_int, c_int, c_int,
                                             c_void_p, c_size_t, c_void_p]
@@ -245,11 +245,11 @@ def aria_attention(QKV, B: int, S: int, H: int, Dh: int = 64, scale: float | Non
     return O
 
 
-def aria_round_act_int8(X, absmax, out=None):
+def aria_round_act_int8(X, absmax, clear: bool = False, out=None):
     M, K = X.shape
     Xq, sx = out if out is not None else (torch.empty((M, K), dtype=torch.int8, device=X.device),
                                           torch.empty((M,), dtype=torch.float32, device=X.device))
-    _check(lib().aria_round_act_int8(_ptr(X), _dt(X), M, K, _ptr(absmax), _ptr(Xq), _ptr(sx), _stream()),
+    _check(lib().aria_round_act_int8(_ptr(X), _dt(X), M, K, _ptr(absmax), int(clear), _ptr(Xq), _ptr(sx), _stream()),
            "aria_round_act_int8")
     return Xq, sx
 

@@ -298,13 +298,13 @@ int aria_attention(const void* QKV, int B, int S, int H, int Dh, float scale, vo
     return launch_attention(QKV, B, S, H, scale, O, row_absmax, static_cast<cudaStream_t>(stream), false);
 }
 
-int aria_round_act_int8(const void* X, int xt, int M, int K, const float* absmax, int8_t* Xq, float* x_scale,
+int aria_round_act_int8(const void* X, int xt, int M, int K, float* absmax, int clear, int8_t* Xq, float* x_scale,
                         void* stream) {
     int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
     if (rc != ARIA_OK) return rc;
     if (!absmax) return ARIA_ERR_NULL;
     if (reinterpret_cast<uintptr_t>(absmax) & 3u) return ARIA_ERR_ALIGN;
-    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), false, absmax, nullptr);
+    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), false, absmax, clear ? absmax : nullptr);
 }
 
 int aria_tensor_peak(int kind, int ctas, int iters, double seconds, double* out, void* stream) {

@@ -51,6 +51,7 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
     if (known_absmax) asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(known_absmax + row) : "memory");
 
     const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
+    if (known_absmax && zero_absmax == known_absmax) __syncthreads();   // every thread has read it before it is cleared
     if (tid == 0) {
         scale[row] = s;
         if (zero_absmax) zero_absmax[row] = 0.0f;

@@ -119,3 +119,107 @@ class LinearStack:
 
     def replay(self):
         self.graph.replay()
+
+
+class BlockStack:
+    """NEXT-2 wiring: `n_blocks` DiT blocks in W8A8 with the producers around the linears in
+    the captured step, every tensor truly chained (no stand-in inputs):
+
+        h -> LayerNorm+S1 -> QKV -> self-attention (+ per-token absmax) -> rounding-only S1 -> out-proj -> h'
+        h' -> LayerNorm+S1 -> MLP up + GELU -> S1 -> MLP down -> h (next block)
+
+    9 launches per block, all enqueue-only C-ABI calls, captured once and replayed.  There is no
+    residual add (out of scope: DESIGN.md 0); the LayerNorm at the head of each half keeps the activations O(1).
+    B sequences (CFG branches) of S tokens, d_model / 64 heads."""
+
+    def __init__(self, B: int = 2, S: int = 1024, n_blocks: int = inputs.N_BLOCKS, d_model: int = inputs.D_MODEL,
+                 keep_host: bool = False):
+        self.B, self.S, self.M, self.d_model, self.n_blocks = B, S, B * S, d_model, n_blocks
+        self.H = d_model // inputs.HEAD_DIM
+        M = self.M
+        self.blocks, self.host = [], []
+        for blk in range(n_blocks):
+            d = {}
+            hst = {}
+            for which, (name, K, N, act) in enumerate(inputs.block_linears(d_model)):
+                L = inputs.c5_layer(blk, which, M=1, d_model=d_model)
+                Wd = torch.from_numpy(L["W"]).cuda()
+                wq, sw = aria.aria_quantize_weights_int8(Wd)
+                torch.cuda.synchronize()
+                del Wd
+                d[name] = {"wq": wq, "sw": sw, "bias": _dev_bf16(L["b"][0]), "K": K, "N": N,
+                           "act": aria.ACT_GELU_ERF if act == "gelu" else aria.ACT_NONE}
+                if keep_host:
+                    hst[name] = {"W": L["W"], "b": L["b"][1]}
+            for i in (1, 2):
+                g, b = inputs.norm_params(d_model, 10 * blk + i)
+                d[f"g{i}"], d[f"b{i}"] = torch.from_numpy(g).cuda(), torch.from_numpy(b).cuda()
+                if keep_host:
+                    hst[f"g{i}"], hst[f"b{i}"] = g, b
+            self.blocks.append(d)
+            self.host.append(hst)
+        bits, _ = inputs.residual_stream(M, d_model, 0)
+        self.h_bits = bits
+        self.h0 = _dev_bf16(bits)
+        bf = dict(dtype=torch.bfloat16, device="cuda")
+        self.h = torch.empty((M, d_model), **bf)           # residual-stream stand-in, rewritten every block
+        self.h2 = torch.empty((M, d_model), **bf)
+        self.qkv = torch.empty((M, 3 * d_model), **bf)
+        self.att = torch.empty((M, d_model), **bf)
+        self.mid = torch.empty((M, 4 * d_model), **bf)
+        self.xq = torch.empty((M, 4 * d_model), dtype=torch.int8, device="cuda")
+        self.sx = torch.empty((M,), dtype=torch.float32, device="cuda")
+        self.amax = torch.zeros((M,), dtype=torch.float32, device="cuda")
+        self.ws = aria.workspace(aria.aria_workspace_bytes(M, 4 * d_model, 4 * d_model, aria.W8A8))
+        self.lin_ops = n_blocks * sum(2 * M * K * N for (_, K, N, _) in inputs.block_linears(d_model))
+        self.att_flops = n_blocks * 4 * B * self.H * S * S * inputs.HEAD_DIM
+        self.ops = self.lin_ops + self.att_flops
+        self.launches_per_block = 9
+        self.graph = None
+        self.taps = None          # tests: per-block copies of every intermediate
+
+    def _lin_q(self, p, xq, sx, out):
+        aria.aria_linear_w8a8_q(xq, sx, p["wq"], p["sw"], p["bias"], p["act"], aria.BF16, out=out)
+
+    def run(self, tap: bool = False):
+        M, d = self.M, self.d_model
+        if tap:
+            self.taps = []
+        src = self.h0
+        for blk in self.blocks:
+            xq_d = self.xq.view(-1)[: M * d].view(M, d)
+            out1 = aria.aria_norm_quantize_act_int8(src, blk["g1"], blk["b1"], aria.NORM_LAYER, 1e-5, want_xn=tap,
+                                                    out=(xq_d, self.sx))
+            self._lin_q(blk["qkv"], xq_d, self.sx, self.qkv)
+            aria.aria_attention(self.qkv, self.B, self.S, self.H, inputs.HEAD_DIM, None, out=self.att, row_absmax=self.amax)
+            t = {}
+            if tap:
+                t.update(src=src.clone(), xn1=out1[2], xq1=xq_d.clone(), sx1=self.sx.clone(), qkv=self.qkv.clone(),
+                         att=self.att.clone())
+            aria.aria_round_act_int8(self.att, self.amax, clear=True, out=(xq_d, self.sx))
+            if tap:
+                t.update(xq2=xq_d.clone(), sx2=self.sx.clone())
+            self._lin_q(blk["out"], xq_d, self.sx, self.h2)
+            out3 = aria.aria_norm_quantize_act_int8(self.h2, blk["g2"], blk["b2"], aria.NORM_LAYER, 1e-5, want_xn=tap,
+                                                    out=(xq_d, self.sx))
+            if tap:
+                t.update(h2=self.h2.clone(), xn3=out3[2], xq3=xq_d.clone(), sx3=self.sx.clone())
+            self._lin_q(blk["up"], xq_d, self.sx, self.mid)
+            p = blk["down"]
+            aria.aria_linear_w8a8(self.mid, p["wq"], p["sw"], p["bias"], p["act"], aria.BF16, ws=self.ws, out=self.h)
+            if tap:
+                t.update(mid=self.mid.clone(), h=self.h.clone())
+                self.taps.append(t)
+            src = self.h
+
+    def capture(self):
+        self.run()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            self.run()
+        self.graph = g
+        return g
+
+    def replay(self):
+        self.graph.replay()

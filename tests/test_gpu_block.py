@@ -198,6 +198,7 @@ def test_block_attention_half_chained_and_teacher_forced(aria, oracle):
     amax = torch.zeros((M,), dtype=torch.float32, device="cuda")
     o = aria.aria_attention(qkv, B, S, H, 64, None, row_absmax=amax)
     oq, so = aria.aria_round_act_int8(o, amax)
+    assert float(amax.min()) > 0.0                                # clear = False leaves the buffer alone
     y = aria.aria_linear_w8a8_q(oq, so, wq2, sw2, dev_bf16(bo_bits), aria.ACT_NONE, aria.F32)
     torch.cuda.synchronize()
     # stage by stage, each oracle stage fed the GPU's actual input of that stage
@@ -214,3 +215,53 @@ def test_block_attention_half_chained_and_teacher_forced(aria, oracle):
     w2_o, s2_o = oracle.quant_int8_rows(Wout)
     r2 = oracle.linear_w8a8(host_f32(o), w2_o, s2_o, bo.astype(np.float64))
     assert rel_err(host_f32(y), r2["y"]) <= 1e-3
+
+
+def test_block_stack_every_stage_teacher_forced_and_graph_replay(aria, oracle):
+    """BlockStack (stack.py): 2 whole DiT blocks, 9 launches each; every stage's output against the oracle fed the
+    GPU's actual input of that stage; the captured graph reproduces the eager run bit for bit."""
+    from paper_2607_08526_b200.stack import BlockStack
+    st = BlockStack(B=2, S=160, n_blocks=2, d_model=256, keep_host=True)
+    st.run(tap=True)
+    torch.cuda.synchronize()
+    taps = st.taps
+    for blk, (t, hst) in enumerate(zip(taps, st.host)):
+        f = lambda k: host_f32(t[k])
+        # LayerNorm 1 + S1
+        ref = oracle.norm_rows(f("src"), hst["g1"], hst["b1"], 0, 1e-5)
+        check_bf16_out(host_bits16(t["xn1"]), ref, inputs.bf16_bits(oracle.round_out(ref, 1)), 2e-6, 0.01)
+        q, s = oracle.quant_int8_rows(f("xn1"))
+        assert np.array_equal(t["xq1"].cpu().numpy(), q) and np.array_equal(t["sx1"].cpu().numpy(), s)
+        # QKV
+        wq, sw = oracle.quant_int8_rows(hst["qkv"]["W"])
+        y = oracle.epilogue_w8a8(oracle.gemm_i8(q, wq), s, sw, hst["qkv"]["b"].astype(np.float64))
+        assert rel_err(f("qkv"), y) <= 2.0 ** -8
+        # attention, fused absmax + rounding-only S1
+        assert rel_err(f("att"), oracle.attention(f("qkv"), st.B, st.S, st.H, 64)) <= ATT_TOL
+        q, s = oracle.quant_int8_rows(f("att"))
+        assert np.array_equal(t["xq2"].cpu().numpy(), q) and np.array_equal(t["sx2"].cpu().numpy(), s)
+        # out-projection
+        wq, sw = oracle.quant_int8_rows(hst["out"]["W"])
+        y = oracle.epilogue_w8a8(oracle.gemm_i8(q, wq), s, sw, hst["out"]["b"].astype(np.float64))
+        assert rel_err(f("h2"), y) <= 2.0 ** -8
+        # LayerNorm 2 + S1, MLP up + GELU, S1 + MLP down
+        ref = oracle.norm_rows(f("h2"), hst["g2"], hst["b2"], 0, 1e-5)
+        check_bf16_out(host_bits16(t["xn3"]), ref, inputs.bf16_bits(oracle.round_out(ref, 1)), 2e-6, 0.01)
+        q, s = oracle.quant_int8_rows(f("xn3"))
+        assert np.array_equal(t["xq3"].cpu().numpy(), q) and np.array_equal(t["sx3"].cpu().numpy(), s)
+        wq, sw = oracle.quant_int8_rows(hst["up"]["W"])
+        y = oracle.epilogue_w8a8(oracle.gemm_i8(q, wq), s, sw, hst["up"]["b"].astype(np.float64), oracle.ACT_GELU_ERF)
+        assert rel_err(f("mid"), y) <= 2.0 ** -8
+        wq, sw = oracle.quant_int8_rows(hst["down"]["W"])
+        r = oracle.linear_w8a8(f("mid"), wq, sw, hst["down"]["b"].astype(np.float64))
+        assert rel_err(f("h"), r["y"]) <= 2.0 ** -8
+        if blk + 1 < len(taps):
+            assert torch.equal(taps[blk + 1]["src"], t["h"])          # truly chained
+    eager = st.h.clone()
+    assert float(st.amax.abs().max()) == 0.0                          # the rounding pass left the buffer cleared
+    st.capture()
+    st.h.zero_()
+    st.replay()
+    st.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(st.h, eager)
