@@ -169,7 +169,7 @@ int aria_quantize_act_int8(const void* X, int xt, int M, int K, int8_t* Xq, floa
                            void* stream) {
     int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
     if (rc != ARIA_OK) return rc;
-    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), false);
+    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), true);
 }
 
 int aria_quantize_weights_int4(const void* W, int wt, int N, int K, int group, uint8_t* Wq4,
@@ -195,10 +195,11 @@ int aria_linear_w8a8(const void* X, int xt, int M, int K, const int8_t* Wq, cons
     if (!ws || ws_bytes < w8_ws_bytes(M, K)) return ARIA_ERR_WORKSPACE;
     int rc = check_arch();
     if (rc != ARIA_OK) return rc;
-    // the S1 pass is an ordinary launch; the GEMM is its programmatic dependent (its prologue -- barrier
-    // init, tensor-memory allocation, tensor-map prefetch -- overlaps the quantiser)
+    // both kernels are programmatic dependents of what precedes them (each waits before it touches global
+    // memory): the S1 pass overlaps the previous kernel's tail, the GEMM's prologue -- barrier init,
+    // tensor-memory allocation, tensor-map prefetch -- overlaps the quantiser
     return linear_w8a8_impl(X, xt, M, K, Wq, w_scale, N, bias, bt, act, Y, yt, ws,
-                            static_cast<cudaStream_t>(stream), false, true);
+                            static_cast<cudaStream_t>(stream), true, true);
 }
 
 int aria_linear_w8a8_q(const int8_t* Xq, const float* x_scale, int M, int K, const int8_t* Wq,
@@ -215,7 +216,9 @@ int aria_linear_w8a8_q(const int8_t* Xq, const float* x_scale, int M, int K, con
     W8Epilogue ep;
     ep.sx = x_scale; ep.sw = w_scale; ep.bias = bias; ep.bias_t = bt; ep.act = act; ep.Y = Y;
     ep.out_t = yt == ARIA_F32 ? 0 : 1;
-    return launch_gemm_w8a8(Xq, Wq, M, N, K, ep, static_cast<cudaStream_t>(stream), false);
+    // every kernel of this library touches global memory only after griddepcontrol.wait, so it may be launched as
+    // a programmatic dependent of WHATEVER precedes it on the stream: its prologue overlaps that kernel's tail
+    return launch_gemm_w8a8(Xq, Wq, M, N, K, ep, static_cast<cudaStream_t>(stream), true);
 }
 
 int aria_linear_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const uint16_t* g_scale,
@@ -286,7 +289,7 @@ int aria_norm_quantize_act_int8(const void* X, int xt, int M, int K, const float
     if (norm != ARIA_NORM_LAYER && norm != ARIA_NORM_RMS) return ARIA_ERR_DTYPE;
     if (!(eps >= 0.0f) || K > 24576) return ARIA_ERR_SHAPE;
     if (misaligned(gamma) || misaligned(beta) || misaligned(Xn)) return ARIA_ERR_ALIGN;
-    return launch_norm_quant(X, xt, M, K, gamma, beta, norm, eps, Xn, Xq, x_scale, static_cast<cudaStream_t>(stream), false);
+    return launch_norm_quant(X, xt, M, K, gamma, beta, norm, eps, Xn, Xq, x_scale, static_cast<cudaStream_t>(stream), true);
 }
 
 int aria_attention(const void* QKV, int B, int S, int H, int Dh, float scale, void* O, float* row_absmax, void* stream) {
@@ -295,7 +298,7 @@ int aria_attention(const void* QKV, int B, int S, int H, int Dh, float scale, vo
     if (misaligned(QKV) || misaligned(O) || (reinterpret_cast<uintptr_t>(row_absmax) & 3u)) return ARIA_ERR_ALIGN;
     int rc = check_arch();
     if (rc != ARIA_OK) return rc;
-    return launch_attention(QKV, B, S, H, scale, O, row_absmax, static_cast<cudaStream_t>(stream), false);
+    return launch_attention(QKV, B, S, H, scale, O, row_absmax, static_cast<cudaStream_t>(stream), true);
 }
 
 int aria_round_act_int8(const void* X, int xt, int M, int K, float* absmax, int clear, int8_t* Xq, float* x_scale,
@@ -304,7 +307,7 @@ int aria_round_act_int8(const void* X, int xt, int M, int K, float* absmax, int 
     if (rc != ARIA_OK) return rc;
     if (!absmax) return ARIA_ERR_NULL;
     if (reinterpret_cast<uintptr_t>(absmax) & 3u) return ARIA_ERR_ALIGN;
-    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), false, absmax, clear ? absmax : nullptr);
+    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), true, absmax, clear ? absmax : nullptr);
 }
 
 int aria_tensor_peak(int kind, int ctas, int iters, double seconds, double* out, void* stream) {

@@ -204,25 +204,29 @@ attention_kernel(const __grid_constant__ CUtensorMap tmQKV, const AttParams p) {
                     for (int k = 0; k < 32; ++k)
                         if (32 * i + k >= valid) v[i][k] = 0xFF800000u;   // -inf
             }
-            float mx = __uint_as_float(v[0][0]);
+            float mx4[4];                                        // four independent chains (latency, not count)
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
+            for (int i = 0; i < 4; ++i) {
+                mx4[i] = __uint_as_float(v[i][0]);
 #pragma unroll
-                for (int k = 0; k < 32; ++k) mx = fmaxf(mx, __uint_as_float(v[i][k]));
+                for (int k = 1; k < 32; ++k) mx4[i] = fmaxf(mx4[i], __uint_as_float(v[i][k]));
+            }
+            const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
             const float ms = mx * c;
             const bool move = (j == 0) || (ms > m + AT_LAZY);
             const float m_new = move ? ms : m;
             const float alpha = ex2(m - m_new);                  // 1 when the maximum stays
-            float sum = 0.0f;
+            float sum4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 #pragma unroll
             for (int i = 0; i < 4; ++i)
 #pragma unroll
                 for (int k = 0; k < 32; k += 2) {
                     const float p0 = ex2(fmaf(__uint_as_float(v[i][k]), c, -m_new));
                     const float p1 = ex2(fmaf(__uint_as_float(v[i][k + 1]), c, -m_new));
-                    sum += p0 + p1;
+                    sum4[(k >> 1) & 3] += p0 + p1;
                     v[i >> 1][(i & 1) * 16 + (k >> 1)] = bf16x2(p0, p1);   // in place: slot index <= source index
                 }
+            const float sum = (sum4[0] + sum4[1]) + (sum4[2] + sum4[3]);
             if (j > 0) {
                 mbar_wait(pvdone, (j - 1) & 1);                  // P_{j-1} consumed, O up to date
                 tc_fence_after();

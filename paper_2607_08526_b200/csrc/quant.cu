@@ -156,6 +156,73 @@ quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restri
     }
 }
 
+// bf16 rows up to 8192 elements: `tpr` threads per row (32..256, a power of two; 256 / tpr rows per CTA), each
+// holding VPT 16-byte vectors, everything packed: the absmax runs on bf16x2 (HMNMX2), the rounding on fp32
+// pairs (FFMA2), ~5 instructions per element instead of ~20 -- these passes were bound by instruction issue
+// at one warp per row (ncu r1c / r2a: 17 % of HBM bandwidth, 18-20 % warps active), not by memory.
+template <int VPT>
+__global__ void __launch_bounds__(256)
+quant_rows_bf16_kernel(const __nv_bfloat16* __restrict__ X, int R, int K, int tpr, int8_t* __restrict__ Xq,
+                       float* __restrict__ scale, const float* known_absmax, float* zero_absmax) {
+    __shared__ float red[8];
+    pdl_wait_prior_grid();
+    pdl_launch_dependents();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int t = threadIdx.x & (tpr - 1);
+    const int64_t row = static_cast<int64_t>(blockIdx.x) * (256 / tpr) + threadIdx.x / tpr;
+    const bool live = row < R;
+    const int nvec = K >> 3;
+    const __nv_bfloat16* x = X + (live ? row : 0) * K;
+    uint4 raw[VPT];
+#pragma unroll
+    for (int i = 0; i < VPT; ++i) {
+        const int idx = t + tpr * i;
+        raw[i] = (live && idx < nvec) ? ld_global_v4(x + 8 * idx) : make_uint4(0, 0, 0, 0);
+    }
+    float a;
+    if (known_absmax) {            // fused S1: reduced by the producing epilogue
+        a = 0.0f;
+        if (live) asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(known_absmax + row) : "memory");
+        if (zero_absmax == known_absmax && tpr > 32) __syncthreads();   // all of the row's threads have read it
+    } else {
+        uint32_t acc = 0;
+#pragma unroll
+        for (int i = 0; i < VPT; ++i) acc = absmax8_bf16(raw[i], acc);
+        a = absmax_bf16x2_to_f32(acc);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
+        if (tpr > 32) {
+            if (lane == 0) red[warp] = a;
+            __syncthreads();
+            const int wpr = tpr >> 5, w0 = (warp / wpr) * wpr;
+            a = red[w0];
+            for (int w = 1; w < wpr; ++w) a = fmaxf(a, red[w0 + w]);
+        }
+    }
+    const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
+    if (t == 0 && live) {
+        scale[row] = s;
+        if (zero_absmax) zero_absmax[row] = 0.0f;
+    }
+    const FastQ2 f = make_fastq2(s);
+    int8_t* q = Xq + (live ? row : 0) * K;
+#pragma unroll
+    for (int i = 0; i < VPT; ++i) {
+        const int idx = t + tpr * i;
+        if (live && idx < nvec) {
+            uint2 o;
+            if (!f.ok || !quant8_fast_bf16(raw[i], f, o)) {
+                float v[8];
+                Raw8<__nv_bfloat16> r8;
+                r8.a = raw[i];
+                unpack8(r8, v);
+                o = quant8_i8(v, s);
+            }
+            *reinterpret_cast<uint2*>(q + 8 * idx) = o;
+        }
+    }
+}
+
 template <typename T, int VPL>
 static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, float* s,
                                     cudaLaunchConfig_t& cfg, const float* known, float* zero) {
@@ -168,7 +235,29 @@ static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, floa
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
                          bool pdl, const float* known, float* zero) {
     const int nvec = C / 8;
-    {   // warp-per-row variants: rows up to 3072 elements (wider rows: one CTA per row, below; a 24-vector
+    if (xt == ARIA_BF16 && nvec <= 1024) {
+        int tpr = 32;
+        while (tpr < 256 && tpr * 3 < nvec) tpr *= 2;
+        const int vpt = (nvec + tpr - 1) / tpr;
+        cudaLaunchConfig_t cfg = {};
+        cfg.stream = st;
+        cfg.blockDim = dim3(256);
+        const int rpc = 256 / tpr;
+        cfg.gridDim = dim3((R + rpc - 1) / rpc);
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = pdl ? 1 : 0;
+        const __nv_bfloat16* x = static_cast<const __nv_bfloat16*>(X);
+        cudaError_t e;
+        if (vpt == 1) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<1>, x, R, C, tpr, q, s, known, zero);
+        else if (vpt == 2) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<2>, x, R, C, tpr, q, s, known, zero);
+        else if (vpt == 3) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<3>, x, R, C, tpr, q, s, known, zero);
+        else e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<4>, x, R, C, tpr, q, s, known, zero);
+        return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    }
+    {   // warp-per-row variants (fp32 rows, and bf16 rows wider than 8192 elements): rows up to 3072 elements (wider rows: one CTA per row, below; a 24-vector
         // warp-per-row variant for 6144-element bf16 rows was measured slower: 2.18 vs 2.08 ms per C5 step)
         cudaLaunchConfig_t cfg = {};
         cfg.stream = st;
