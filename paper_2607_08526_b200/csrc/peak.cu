@@ -18,7 +18,7 @@ constexpr int PK_A_BYTES = 128 * 128;
 constexpr int PK_THREADS = 128;
 
 template <int KIND, int CTAS>   // KIND 0: kind::i8 (s8 x s8 -> s32), 1: kind::f16 (bf16 x bf16 -> f32)
-__global__ void __launch_bounds__(PK_THREADS, 1) tensor_peak_kernel(int iters, long long* stamps) {
+__global__ void __launch_bounds__(PK_THREADS, 1) tensor_peak_kernel(int iters, long long* stamps, int ncols) {
     constexpr int B_ROWS = 256 / CTAS;
     constexpr int B_BYTES = B_ROWS * 128;
     extern __shared__ uint8_t smem_raw[];
@@ -54,7 +54,8 @@ __global__ void __launch_bounds__(PK_THREADS, 1) tensor_peak_kernel(int iters, l
     const uint32_t tmem_base = *tmem_slot_g;
 
     if (warp == 0 && rank == 0) {
-        constexpr uint32_t idesc = KIND == 0 ? idesc_i8(128 * CTAS, 256) : idesc_bf16(128 * CTAS, 256);
+        // ncols = 256 in the product; debug builds may time narrower instructions (ARIA_PEAK_N)
+        const uint32_t idesc = KIND == 0 ? idesc_i8(128 * CTAS, ncols) : idesc_bf16(128 * CTAS, ncols);
         const uint64_t desc_hi = make_smem_desc_sw128(0);
         const uint64_t a_desc = desc_hi | ((sA & 0x3FFFF) >> 4);
         const uint64_t b_desc = desc_hi | ((sB & 0x3FFFF) >> 4);
@@ -115,7 +116,9 @@ static int run_peak(int iters, int sms, long long* d_stamps, cudaStream_t st) {
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kern, iters, d_stamps) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    static const char* n_env = dbg_env("ARIA_PEAK_N");
+    const int ncols = n_env ? atoi(n_env) : 256;
+    return cudaLaunchKernelEx(&cfg, kern, iters, d_stamps, ncols) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
 int tensor_peak(int kind, int ctas, int iters, double seconds, double* out, cudaStream_t st) {
