@@ -283,10 +283,10 @@ ARIA_API int aria_tensor_peak(int kind, int ctas, int iters, double seconds, dou
 /* Host-only introspection of the launch plans (no device needed; used by the tests to prove that
  * every compiled tile variant is reached): the (BN, CTAS) tile of the W8A8 GEMM for an [M,N] output on
  * a device with `sms` SMs (BN in {64,128,192,256} output channels, CTAS = 2: tcgen05 cta_group::2
- * pairs computing 256 x BN), and the (token tile TT in {32,64,128,192,256}, split-K factor, CTAS = 2: a CTA
- * pair computing 256 channels x 192 tokens) of the W4A16 / W8A16 GEMM.                              */
+ * pairs computing 256 x BN), and the (token tile TT in {32,64,128,192,256}, split-K factor) of the
+ * W4A16 / W8A16 GEMM.                                                                              */
 ARIA_API int aria_w8a8_tile_plan(int M, int N, int sms, int* bn, int* ctas);
-ARIA_API int aria_w4a16_tile_plan(int M, int N, int K, int sms, int* tt, int* splits, int* ctas);
+ARIA_API int aria_w4a16_tile_plan(int M, int N, int K, int sms, int* tt, int* splits);
 
 /* Library build id ("aria-b200 <version> sm_100a"). */
 ARIA_API const char* aria_version(void);

@@ -75,8 +75,7 @@ def lib() -> ctypes.CDLL:
         L.aria_stack_plan_is_streaming.argtypes = [c_void_p]
         L.aria_stack_plan_fallback_fired.argtypes = [c_void_p, ctypes.POINTER(c_int)]
         L.aria_w8a8_tile_plan.argtypes = [c_int, c_int, c_int, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
-        L.aria_w4a16_tile_plan.argtypes = [c_int, c_int, c_int, c_int, ctypes.POINTER(c_int), ctypes.POINTER(c_int),
-                                           ctypes.POINTER(c_int)]
+        L.aria_w4a16_tile_plan.argtypes = [c_int, c_int, c_int, c_int, ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
         L.aria_tensor_peak.argtypes = [c_int, c_int, c_int, ctypes.c_double, ctypes.POINTER(ctypes.c_double), c_void_p]
         L.aria_stack_plan_destroy.argtypes = [c_void_p]
         L.aria_stack_plan_destroy.restype = None
@@ -320,11 +319,9 @@ def aria_w8a8_tile_plan(M: int, N: int, sms: int = 148):
 
 
 def aria_w4a16_tile_plan(M: int, N: int, K: int, sms: int = 148):
-    """(token tile, split-K factor, CTAs per unit) of the W4A16 / W8A16 GEMM."""
-    tt, s, ct = c_int(0), c_int(0), c_int(0)
-    _check(lib().aria_w4a16_tile_plan(M, N, K, sms, ctypes.byref(tt), ctypes.byref(s), ctypes.byref(ct)),
-           "aria_w4a16_tile_plan")
-    return tt.value, s.value, ct.value
+    tt, s = c_int(0), c_int(0)
+    _check(lib().aria_w4a16_tile_plan(M, N, K, sms, ctypes.byref(tt), ctypes.byref(s)), "aria_w4a16_tile_plan")
+    return tt.value, s.value
 
 
 def aria_stack_plan_destroy(plan: c_void_p):

@@ -327,10 +327,10 @@ int aria_w8a8_tile_plan(int M, int N, int sms, int* bn, int* ctas) {
     return ARIA_OK;
 }
 
-int aria_w4a16_tile_plan(int M, int N, int K, int sms, int* tt, int* splits, int* ctas) {
-    if (!tt || !splits || !ctas) return ARIA_ERR_NULL;
+int aria_w4a16_tile_plan(int M, int N, int K, int sms, int* tt, int* splits) {
+    if (!tt || !splits) return ARIA_ERR_NULL;
     if (M <= 0 || N <= 0 || K <= 0 || sms <= 0) return ARIA_ERR_SHAPE;
-    w4_plan(M, N, K, sms, tt, splits, ctas);
+    w4_plan(M, N, K, sms, tt, splits);
     return ARIA_OK;
 }
 

@@ -45,14 +45,15 @@ constexpr int W4_G = 3;         // dequantiser groups = A buffers
 // cross-CTA "A ready" hand-off, multicast changed nothing (3.79 vs 3.81 ms per C5 step).  Both removed.)
 // WB = weight bits: 4 (S4, int4 group-32 + fp16 group scales) or 8 (NEXT-1 "q8", int8 per-channel + fp32
 // scales).  The two formats share everything but the packed-tile geometry and the dequantiser arithmetic.
-// CT = 2: a CTA PAIR (cluster of 2, tcgen05 cta_group::2) computes 256 channels x TT tokens: each CTA dequantises its
-// own 128 weight rows into its own tensor memory and stages only HALF of the X tile (TT / 2 tokens); the MMA reads
-// both halves.  With one CTA the X tile crosses shared memory twice per k-block (TMA write + MMA read: 2 x TT x 128 B,
-// 48 KB at TT = 192 = 384 cycles of the 128 B/clk port -- as long as the MMAs themselves), which capped the k-block at
-// ~560 cycles against 384 of tensor time; the pair halves it.  Round 1's pair kept A in shared memory with as many
-// buffers as dequantiser groups, so the cross-CTA "A ready" latency sat on the critical path; here a group never
-// waits for the slot it has just published (4 tensor-memory slots, 3 groups).
-template <int TT, int WB = 4, int CT = 1>
+// (CTA pairs -- tcgen05 cta_group::2, 256 channels x 192 tokens per pair, each CTA dequantising its own 128 rows into
+// its own tensor memory and staging half of X -- were built and measured TWICE.  Round 1, A in shared memory: the
+// cross-CTA "A ready" hand-off cost ~1.3k cycles per k-block.  Round 2, A in tensor memory (4 slots, 3 groups, 8 X
+// stages, merged barriers as below): correct -- every parity test passed -- and, once the peer's arrivals used
+// mbarrier.arrive.RELAXED.cluster (the releasing form blocks the issuing warp ~1400 cycles), exactly as fast as one
+// CTA per unit: 127.9 vs 120.6 us per C5 block at M = 2048.  Halving the X traffic buys nothing because neither shared
+// memory, nor the L2, nor the tensor pipe sets the k-block time: issuing a quarter of the MMAs, or loading no X at
+// all, left it unchanged, while skipping the dequantiser arithmetic cut it by 27 %.  Pairs removed.)
+template <int TT, int WB = 4>
 struct W4Cfg {
     static constexpr int G = W4_G;
     // ATM: the dequantised A tile goes registers -> TENSOR MEMORY (tcgen05.st) and the MMA reads it from there.
@@ -61,22 +62,25 @@ struct W4Cfg {
     // the dequantisers and 16 KB read back by the MMA); A in TMEM removes those 32 KB per k-block.  Needs
     // 2 TT accumulator columns + 4 x 32 A columns <= 512: every token tile but TT = 256.
     static constexpr bool ATM = TT <= 192;
-    static_assert(CT == 1 || (CT == 2 && ATM && (TT / 2) % 8 == 0), "pairs need A in tensor memory");
     static constexpr int NB = ATM ? 4 : G;                     // dequantised A buffers (TMEM slots / smem tiles)
     static constexpr int THREADS = 32 * W4_DEQ_WARP0 + 128 * G;
     static constexpr int P_ROW = W4_BK * WB / 8;               // 32 (int4) / 64 (int8) packed bytes per row per k-block
     static constexpr int P_BYTES = W4_BN * P_ROW;              // 4 KB / 8 KB
-    static constexpr int X_ROWS = TT / CT;                     // token rows per X stage (per CTA)
+    static constexpr int X_ROWS = TT;                          // token rows per X stage
     static constexpr int X_BYTES = X_ROWS * 128;               // x 64 bf16
     static constexpr int A_BYTES = W4_BN * 128;                // 16 KB: 128 rows x 64 bf16
     static constexpr int STG_BYTES = 4096;                     // per epilogue warp: 32 tokens x 128 B
-    // LOCK (with A in tensor memory): the X ring and the A slots advance in LOCKSTEP (stage == slot == k-block mod 4)
-    // and share their barriers: full[i] collects the dequantiser warps' arrivals AND the X tile's bytes, empty[i] is
-    // ONE tcgen05.commit that frees both.  The MMA warp's loop is a serial chain (measured, role timestamps: ~100
-    // cycles per barrier wait, ~27 per tcgen05.mma, ~57 per tcgen05.commit): with two waits and two commits per
-    // 64-k block it took ~530 cycles, more than the 384 of tensor time it feeds.
+    // LOCK (with A in tensor memory): ONE full and ONE empty barrier per k-block, indexed by the X stage (k-block
+    // mod XS): full[i] collects the dequantiser warps' arrivals AND the X tile's bytes, empty[i] is the single
+    // tcgen05.commit of that k-block; the X producer waits on it before refilling stage i (k-block + XS) and the
+    // dequantisers before reusing the A slot (k-block + NB: they wait on the empty barrier of k-block - NB).  The MMA
+    // warp's loop is a serial chain (role timestamps: ~100 cycles per barrier wait, ~27 per tcgen05.mma, ~55 per
+    // tcgen05.commit): two waits and two commits per 64-k block made it ~530 cycles, more than the 384 of tensor
+    // time it feeds.  XS stays deep: an X tile takes ~2000 cycles to arrive when every SM pulls 24 KB per k-block
+    // through the L2 (role timestamps; with XS = NB = 4 the k-block period was (2000 + 700) / 4).
     static constexpr bool LOCK = ATM;
-    static constexpr int XS = LOCK ? NB : X_ROWS == 256 ? 3 : 8;   // X ring depth
+    static constexpr int XS = !LOCK ? (X_ROWS == 256 ? 3 : 8)
+                              : TT == 192 ? (WB == 8 ? 5 : 6) : TT == 128 ? 6 : 8;   // X ring depth
     static constexpr int PS = WB == 8 ? (TT >= 192 ? 8 : TT == 32 ? 16 : 12)      // packed ring depth
                                       : (TT >= 192 ? 8 : TT == 128 ? 12 : 16);
     static constexpr int X_OFF = 0;
@@ -117,7 +121,7 @@ static long long* g_w4_prof = nullptr;
 static int g_w4_prof_launch = 0;          // every launch (graph node) gets its own 148 x 32 slot, 256 slots
 void w4_set_profile_buffer(long long* p) { g_w4_prof = p; g_w4_prof_launch = 0; }
 __device__ __forceinline__ void prof_stamp(const W4Params& p, int slot, long long t0) {
-    if (p.prof) p.prof[blockIdx.x * 32 + slot] = clock64() - t0;
+    if (p.prof) p.prof[blockIdx.x * 64 + slot] = clock64() - t0;
 }
 #define W4_TIMED(acc, stmt) do { const long long t_ = clock64(); stmt; acc += clock64() - t_; } while (0)
 #define W4_CLK() clock64()
@@ -230,11 +234,11 @@ __device__ __forceinline__ void dequant_i8x16(const uint4& v, float sw, uint4& l
 // (X multicast over CTA couples -- both CTAs of a cluster on the same token tile, each loading half of every X
 // tile into both -- was built twice: with A in shared memory (round 1: 3.79 vs 3.81 ms per C5 step) and with A
 // in tensor memory (round 2: 3.29 vs 3.32 ms).  The k-block time is not set by L2 reads of X; removed.)
-template <int TT, bool GELU, int WB, int CT>
-__global__ void __launch_bounds__(W4Cfg<TT, WB, CT>::THREADS, 1)
+template <int TT, bool GELU, int WB>
+__global__ void __launch_bounds__(W4Cfg<TT, WB>::THREADS, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmX,
                   const __grid_constant__ CUtensorMap tmY, const W4Params p) {
-    using Cfg = W4Cfg<TT, WB, CT>;
+    using Cfg = W4Cfg<TT, WB>;
     constexpr int XS = Cfg::XS, PS = Cfg::PS, G = Cfg::G, NB = Cfg::NB;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
@@ -252,21 +256,20 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    constexpr int UN = W4_BN * CT;                              // output channels per work unit
-    const uint32_t rank = CT == 2 ? cluster_ctarank() : 0u;     // position in the CTA pair
+    constexpr int UN = W4_BN;                                   // output channels per work unit
     const int num_n = (p.N + UN - 1) / UN;
     const int num_t = (p.M + TT - 1) / TT;
     const int num_kb = (p.K + W4_BK - 1) / W4_BK;
     const int S = p.splits;
     const int num_units = num_n * num_t * S;
-    const int unit0 = blockIdx.x / CT, unit_step = gridDim.x / CT;
+    const int unit0 = blockIdx.x, unit_step = gridDim.x;
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmP);
         tma_prefetch_desc(&tmX);
         tma_prefetch_desc(&tmY);
         for (int s = 0; s < XS; ++s) {
-            mbar_init(xfull0 + 8 * s, 1);
+            mbar_init(xfull0 + 8 * s, Cfg::LOCK ? 1 + 4 : 1);   // LOCK: the X producer's expect_tx + the 4 dequant warps
             mbar_init(xempty0 + 8 * s, 1);      // MMA commit
         }
         for (int s = 0; s < PS; ++s) {
@@ -274,27 +277,21 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             mbar_init(pempty0 + 8 * s, 4);      // the 4 warps of the dequant group that read it
         }
         for (int a = 0; a < NB; ++a) {
-            // the 4 dequant warps that fill it (pair: both CTAs report to the leader); LOCK: + the X producer's expect_tx
-            mbar_init(afull0 + 8 * a, 4 * CT + (Cfg::LOCK ? 1 : 0));
+            mbar_init(afull0 + 8 * a, 4);       // the 4 dequant warps that fill it (unused with LOCK)
             mbar_init(aempty0 + 8 * a, 1);
         }
         for (int a = 0; a < 2; ++a) {
             mbar_init(tfull0 + 8 * a, 1);
-            mbar_init(tempty0 + 8 * a, 4 * CT);
+            mbar_init(tempty0 + 8 * a, 4);
         }
         fence_mbar_init();
     }
     if (warp == 1) {
-        if (CT == 2) {
-            tmem_alloc_2sm(tmem_slot, Cfg::TMEM_COLS);
-            tmem_relinquish_2sm();
-        } else {
-            tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
-            tmem_relinquish();
-        }
+        tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
+        tmem_relinquish();
     }
     tc_fence_before();
-    if (CT == 2) cluster_sync(); else __syncthreads();         // barriers visible to the peer CTA too
+    __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_g;
 
@@ -309,7 +306,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
     if (threadIdx.x == 0 && p.prof) {
         unsigned long long gt;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
-        p.prof[blockIdx.x * 32 + 14] = static_cast<long long>(gt);
+        p.prof[blockIdx.x * 64 + 14] = static_cast<long long>(gt);
     }
 #endif
 
@@ -321,29 +318,22 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         uint32_t phase = 0;
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int t0 = (tile / num_n) * TT + static_cast<int>(rank) * Cfg::X_ROWS;
+            const int t0 = (tile / num_n) * TT;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             for (int kb = kb0; kb < kb1; ++kb) {
-                const uint32_t xe = Cfg::LOCK ? aempty0 + 8 * stage : xempty0 + 8 * stage;   // LOCK: stage == A slot
-                const uint32_t xf = Cfg::LOCK ? afull0 + 8 * stage : xfull0 + 8 * stage;
+                const uint32_t xe = xempty0 + 8 * stage, xf = xfull0 + 8 * stage;
                 mbar_wait(xe, phase ^ 1);
 #ifdef ARIA_DEBUG
                 if ((p.dbg == 1 && (kb & 1)) || p.dbg == 2) {
-                    if (elect_one() && (CT == 1 || rank == 0)) mbar_arrive(xf);
+                    if (elect_one()) mbar_arrive(xf);
                     __syncwarp();
                     if (++stage == XS) { stage = 0; phase ^= 1; }
                     continue;
                 }
 #endif
                 if (elect_one()) {
-                    if (CT == 2) {
-                        // both halves are counted on the LEADER's barrier, where the MMA warp waits
-                        if (rank == 0) mbar_arrive_expect_tx(xf, Cfg::X_BYTES * 2);
-                        tma_load_2d_2sm(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xf & PEER_BIT_MASK);
-                    } else {
-                        mbar_arrive_expect_tx(xf, Cfg::X_BYTES);
-                        tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xf);
-                    }
+                    mbar_arrive_expect_tx(xf, Cfg::X_BYTES);
+                    tma_load_2d(sX + stage * Cfg::X_BYTES, &tmX, kb * W4_BK, t0, xf);
                 }
                 __syncwarp();
                 if (++stage == XS) { stage = 0; phase ^= 1; }
@@ -357,7 +347,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         uint32_t phase = 0;
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int n0 = (tile % num_n) * UN + static_cast<int>(rank) * W4_BN;
+            const int n0 = (tile % num_n) * UN;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             for (int kb = kb0; kb < kb1; ++kb) {
                 mbar_wait(pempty0 + 8 * stage, phase ^ 1);
@@ -373,7 +363,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         if (lane == 0) prof_stamp(p, 6, t_start);
     } else if (warp == 1) {
         // ------------------------------------------------------------ MMA issuer
-        if (rank == 0) {                                       // the pair's leader issues for both CTAs
+        {
             constexpr uint32_t idesc = idesc_bf16(UN, TT);
             const uint64_t desc_hi = make_smem_desc_sw128(0);
             int stage = 0, ab = 0, acc = 0;
@@ -385,34 +375,31 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 W4_TIMED(w_t, mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1));
                 const uint32_t d_tmem = tmem_base + acc * Cfg::ACC_STRIDE;
                 for (int kb = kb0; kb < kb1; ++kb) {
-                    if (!Cfg::LOCK) W4_TIMED(w_x, mbar_wait(xfull0 + 8 * stage, phase));   // X landed
-                    W4_TIMED(w_a, mbar_wait(afull0 + 8 * ab, aphase));     // weights dequantised
+                    W4_TIMED(w_x, mbar_wait(xfull0 + 8 * stage, phase));   // X landed (LOCK: and weights dequantised)
+                    if (!Cfg::LOCK) W4_TIMED(w_a, mbar_wait(afull0 + 8 * ab, aphase));     // weights dequantised
                     W4_TIMED(w_f, tc_fence_after());
                     const uint64_t a_desc = desc_hi | (((sA + ab * Cfg::A_BYTES) & 0x3FFFF) >> 4);
                     const uint32_t a_tmem = tmem_base + Cfg::A_COL0 + ab * 32;
                     const uint64_t b_desc = desc_hi | (((sX + stage * Cfg::X_BYTES) & 0x3FFFF) >> 4);
                     if (elect_one()) {
                         const long long t_m_ = W4_CLK();
+#ifdef ARIA_DEBUG
+                        if (p.prof && kb - kb0 >= 40 && kb - kb0 < 44 && u == unit0) p.prof[blockIdx.x * 64 + 24 + (kb - kb0 - 40)] = t_m_ - t_start;
+#endif
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {  // 4 x (K = 16 bf16 = 32 bytes of X / 8 TMEM columns of A)
 #ifdef ARIA_DEBUG
                             if (p.dbg == 4 && k != 0) continue;     // timing experiment: a quarter of the MMAs
 #endif
-                            if (CT == 2) mma_f16_ts_2sm(d_tmem, a_tmem + 8 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
-                            else if (Cfg::ATM) mma_f16_ts(d_tmem, a_tmem + 8 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
+                            if (Cfg::ATM) mma_f16_ts(d_tmem, a_tmem + 8 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
                             else mma_f16_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb != kb0 || k != 0) ? 1u : 0u);
                         }
                         const long long t_c_ = W4_CLK();
                         w_m += t_c_ - t_m_;
-                        if (CT == 2) {     // ring slot / A slot reusable, accumulator complete: in BOTH CTAs
-                            if (!Cfg::LOCK) tc_commit_2sm(xempty0 + 8 * stage, 3);
+                        {
+                            tc_commit(xempty0 + 8 * stage);
                             w_c1 += W4_CLK() - t_c_;
-                            tc_commit_2sm(aempty0 + 8 * ab, 3);
-                            w_c2 += W4_CLK() - t_c_;
-                            if (kb == kb1 - 1) tc_commit_2sm(tfull0 + 8 * acc, 3);
-                        } else {
-                            if (!Cfg::LOCK) tc_commit(xempty0 + 8 * stage);
-                            tc_commit(aempty0 + 8 * ab);
+                            if (!Cfg::LOCK) tc_commit(aempty0 + 8 * ab);
                             if (kb == kb1 - 1) tc_commit(tfull0 + 8 * acc);
                         }
                     }
@@ -424,10 +411,10 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             }
             if (lane == 0) prof_stamp(p, 1, t_start);
 #ifdef ARIA_DEBUG
-            if (lane == 0 && p.prof) { p.prof[blockIdx.x * 32 + 5] = w_x; p.prof[blockIdx.x * 32 + 7] = w_a; p.prof[blockIdx.x * 32 + 12] = w_t; }
+            if (lane == 0 && p.prof) { p.prof[blockIdx.x * 64 + 5] = w_x; p.prof[blockIdx.x * 64 + 7] = w_a; p.prof[blockIdx.x * 64 + 12] = w_t; }
             if (p.prof && w_m != 0) {   // the elected lane
-                p.prof[blockIdx.x * 32 + 20] = w_f; p.prof[blockIdx.x * 32 + 21] = w_m;
-                p.prof[blockIdx.x * 32 + 22] = w_c1; p.prof[blockIdx.x * 32 + 23] = w_c2;
+                p.prof[blockIdx.x * 64 + 20] = w_f; p.prof[blockIdx.x * 64 + 21] = w_m;
+                p.prof[blockIdx.x * 64 + 22] = w_c1; p.prof[blockIdx.x * 64 + 23] = w_c2;
             }
 #endif
         }
@@ -435,11 +422,14 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         // ------------------------------------------------------------ dequantiser groups
         // hand-off of one dequantised row (64 bf16 = 8 x 16 B, k ascending) to the MMA: tensor memory
         // (this thread's lane, 32 columns of the slot) or the 128-byte-swizzled shared-memory A tile
-        const uint32_t afull_leader = CT == 2 ? mapa_shared(afull0, 0) : 0u;
         long long d_pf = 0, d_ae = 0, d_st = 0, d_ar = 0;         // debug builds: cycles in each wait of this warp
         auto publish_a = [&](const uint4 (&o)[8], int it_, uint32_t rowoff_, uint32_t xr_, int q_) {
             const int ab = it_ % NB;
-            W4_TIMED(d_ae, mbar_wait(aempty0 + 8 * ab, ((it_ / NB) & 1) ^ 1));     // MMAs reading this A buffer retired
+            if (Cfg::LOCK) {       // the MMAs of k-block it_ - NB (this slot's previous tenant) have retired
+                if (it_ >= NB) W4_TIMED(d_ae, mbar_wait(xempty0 + 8 * ((it_ - NB) % XS), ((it_ - NB) / XS) & 1));
+            } else {
+                W4_TIMED(d_ae, mbar_wait(aempty0 + 8 * ab, ((it_ / NB) & 1) ^ 1));     // MMAs reading this A buffer retired
+            }
             const long long t_st_ = W4_CLK();
             if (Cfg::ATM) {
                 tc_fence_after();
@@ -459,11 +449,16 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
             const long long t_ar_ = W4_CLK();
             d_st += t_ar_ - t_st_;
             if (lane == 0) {                                       // one arrival per warp, on the leader's barrier
-                if (CT == 2 && rank != 0) mbar_arrive_cluster_relaxed(afull_leader + 8 * ab);   // payload is in tensor memory
-                else mbar_arrive(afull0 + 8 * ab);
+                mbar_arrive(Cfg::LOCK ? xfull0 + 8 * (it_ % XS) : afull0 + 8 * ab);
             }
             __syncwarp();
             d_ar += W4_CLK() - t_ar_;
+#ifdef ARIA_DEBUG
+            if (p.prof && lane == 0 && it_ >= 40 && it_ < 44) {
+                p.prof[blockIdx.x * 64 + 32 + (it_ - 40) * 4 + q_] = clock64() - t_start;     // published, per warp
+                p.prof[blockIdx.x * 64 + 48 + (it_ - 40) * 4 + q_] = t_st_ - t_start;         // slot was free
+            }
+#endif
         };
         const int dw = warp - W4_DEQ_WARP0;
         const int g = dw >> 2;                    // group = A buffer index
@@ -478,7 +473,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         int it = 0;                               // running k-block counter of this CTA
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int n0 = (tile % num_n) * UN + static_cast<int>(rank) * W4_BN;
+            const int n0 = (tile % num_n) * UN;
             const int kb0 = (sp * num_kb) / S, kb1 = ((sp + 1) * num_kb) / S;
             const bool row_ok = n0 + r < p.N;
             if (WB == 8) {
@@ -560,8 +555,8 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         if ((dw & 3) == 0 && lane == 0) prof_stamp(p, 2 + g, t_start);
 #ifdef ARIA_DEBUG
         if (dw == 0 && lane == 0 && p.prof) {
-            p.prof[blockIdx.x * 32 + 16] = d_pf; p.prof[blockIdx.x * 32 + 17] = d_ae;
-            p.prof[blockIdx.x * 32 + 18] = d_st; p.prof[blockIdx.x * 32 + 19] = d_ar;
+            p.prof[blockIdx.x * 64 + 16] = d_pf; p.prof[blockIdx.x * 64 + 17] = d_ae;
+            p.prof[blockIdx.x * 64 + 18] = d_st; p.prof[blockIdx.x * 64 + 19] = d_ar;
         }
 #else
         (void)d_pf; (void)d_ae; (void)d_st; (void)d_ar;
@@ -574,7 +569,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
         uint32_t acc_phase = 0;
         for (int u = unit0; u < num_units; u += unit_step) {
             const int tile = u / S, sp = u % S;
-            const int n0 = (tile % num_n) * UN + static_cast<int>(rank) * W4_BN, t0 = (tile / num_n) * TT;
+            const int n0 = (tile % num_n) * UN, t0 = (tile / num_n) * TT;
             const int n = n0 + q * 32 + lane;
             const bool n_ok = n < p.N;
             float bv = 0.0f;
@@ -651,10 +646,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) {
-                    if (CT == 2 && rank != 0) mbar_arrive_cluster(mapa_shared(tempty0 + 8 * acc, 0));
-                    else mbar_arrive(tempty0 + 8 * acc);
-                }
+                if (lane == 0) mbar_arrive(tempty0 + 8 * acc);
             } else {
                 float* part = p.partials + static_cast<int64_t>(sp) * p.M * p.N;
                 float* prow = part + static_cast<int64_t>(t0) * p.N + n;
@@ -738,27 +730,27 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
 
     if (warp >= W4_EPI_WARP0 && warp < W4_DEQ_WARP0 && lane == 0) tma_store_wait<0>();
     tc_fence_before();
-    if (CT == 2) cluster_sync(); else __syncthreads();   // pair: the peer's last remote arrivals have landed
+    __syncthreads();
 #ifdef ARIA_DEBUG
     if (threadIdx.x == 0 && p.prof) {
         unsigned long long gt;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
-        p.prof[blockIdx.x * 32 + 15] = static_cast<long long>(gt);
-        p.prof[blockIdx.x * 32 + 13] = clock64() - t_start;
+        p.prof[blockIdx.x * 64 + 15] = static_cast<long long>(gt);
+        p.prof[blockIdx.x * 64 + 13] = clock64() - t_start;
     }
 #endif
     if (warp == 1) {
         tc_fence_after();
-        if (CT == 2) tmem_dealloc_2sm(tmem_base, Cfg::TMEM_COLS); else tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
+        tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
     }
 }
 
-template <int TT, bool GELU, int WB, int CT = 1>
+template <int TT, bool GELU, int WB>
 static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, const W4Params& p,
                      int grid, cudaStream_t st, bool pdl) {
-    using Cfg = W4Cfg<TT, WB, CT>;
+    using Cfg = W4Cfg<TT, WB>;
     static std::atomic<uint64_t> attr_done{0};
-    auto kern = w4a16_gemm_kernel<TT, GELU, WB, CT>;
+    auto kern = w4a16_gemm_kernel<TT, GELU, WB>;
     if (!ensure_dyn_smem(kern, Cfg::SMEM_BYTES, attr_done)) return ARIA_ERR_CUDA;
     CUtensorMap tmP, tmX, tmY;
     int rc = make_tmap_2d(&tmP, Wq4, 1, N, K * WB / 8, W4_BN, Cfg::P_ROW, Cfg::P_ROW);
@@ -773,22 +765,11 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
     cfg.blockDim = dim3(Cfg::THREADS);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = st;
-    cudaLaunchAttribute at[2];
-    int na = 0;
-    if (CT == 2) {
-        at[na].id = cudaLaunchAttributeClusterDimension;
-        at[na].val.clusterDim.x = 2;
-        at[na].val.clusterDim.y = 1;
-        at[na].val.clusterDim.z = 1;
-        ++na;
-    }
-    if (pdl) {
-        at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        at[na].val.programmaticStreamSerializationAllowed = 1;
-        ++na;
-    }
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = na;
+    cfg.numAttrs = pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kern, tmP, tmX, tmY, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
@@ -797,7 +778,7 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
 // is written by TMA and read by the MMA; packed weights, dequantised A tile and its MMA read are the
 // constant), plus an epilogue ~ 40 TT, a fixed ~3000, and for split-K the fp32 partial round trip
 // ~ 100 TT + 4000.  Pick the (TT, splits) with the fewest wave-quantised cycles.
-void w4_plan(int M, int N, int K, int sms, int* tt_out, int* splits_out, int* ct_out) {
+void w4_plan(int M, int N, int K, int sms, int* tt_out, int* splits_out) {
     const int num_kb = (K + W4_BK - 1) / W4_BK;
     const int num_n = (N + W4_BN - 1) / W4_BN;
     const int tts[5] = {256, 192, 128, 64, 32};
@@ -824,22 +805,12 @@ void w4_plan(int M, int N, int K, int sms, int* tt_out, int* splits_out, int* ct
             if (best < 0 || cost < best) { best = cost; best_tt = tt; best_s = s; }
         }
     }
-    int best_ct = 1;
-    static const bool no_pair = dbg_env("ARIA_W4_NO_PAIR") != nullptr;   // debug builds only
-    if (ct_out && !no_pair && M > 96 && sms >= 2) {
-        // CTA pairs: 256 channels x 192 tokens per unit on sms / 2 pairs, ~430 cycles per k-block (tensor time 384)
-        const long units = static_cast<long>((N + 2 * W4_BN - 1) / (2 * W4_BN)) * ((M + 191) / 192);
-        const long waves = (units + sms / 2 - 1) / (sms / 2);
-        const long cost = waves * (static_cast<long>(num_kb) * 430 + 40L * 192 + 3500);
-        if (cost < best) { best = cost; best_tt = 192; best_s = 1; best_ct = 2; }
-    }
     *tt_out = best_tt; *splits_out = best_s;
-    if (ct_out) *ct_out = best_ct;
 }
 
 size_t w4_workspace_bytes(int M, int N, int K, int sms) {
     int tt, s;
-    w4_plan(M, N, K, sms, &tt, &s, nullptr);    // the single-CTA plan: an upper bound (a pair plan never splits K)
+    w4_plan(M, N, K, sms, &tt, &s);
     const size_t tiles = static_cast<size_t>((N + W4_BN - 1) / W4_BN) * ((M + tt - 1) / tt);
     size_t counters = (tiles * 4 * sizeof(unsigned) + 255) / 256 * 256;
     size_t partials = s > 1 ? static_cast<size_t>(s) * M * N * sizeof(float) : 0;
@@ -851,15 +822,15 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const voi
                       cudaStream_t st, bool pdl, int wbits) {
     const int sms = num_sms();
     if (sms <= 0) return ARIA_ERR_CUDA;
-    int tt, s, ct;
-    w4_plan(M, N, K, sms, &tt, &s, &ct);
+    int tt, s;
+    w4_plan(M, N, K, sms, &tt, &s);
     if (s > 1 && (ws == nullptr || ws_bytes < w4_workspace_bytes(M, N, K, sms))) s = 1;
     W4Params p;
     p.g_scale = g_scale; p.bias = bias; p.Y = Y;
     p.act = act; p.out_t = yt; p.M = M; p.N = N; p.K = K; p.splits = s;
 #ifdef ARIA_DEBUG
     p.dbg = dbg_env("ARIA_W4_DBG") ? atoi(dbg_env("ARIA_W4_DBG")) : 0;
-    p.prof = g_w4_prof ? g_w4_prof + static_cast<size_t>(g_w4_prof_launch++ % 256) * 148 * 32 : nullptr;
+    p.prof = g_w4_prof ? g_w4_prof + static_cast<size_t>(g_w4_prof_launch++ % 256) * 148 * 64 : nullptr;
 #endif
     const size_t tiles = static_cast<size_t>((N + W4_BN - 1) / W4_BN) * ((M + tt - 1) / tt);
     p.counters = static_cast<unsigned*>(ws);
@@ -867,11 +838,7 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const voi
                                                   (tiles * 4 * sizeof(unsigned) + 255) / 256 * 256)
                        : nullptr;
     const int units = static_cast<int>(tiles) * s;
-    int grid = units < sms ? units : sms;
-    if (ct == 2) {
-        const int pair_units = ((N + 2 * W4_BN - 1) / (2 * W4_BN)) * ((M + tt - 1) / tt);
-        grid = 2 * (pair_units < sms / 2 ? pair_units : sms / 2);
-    }
+    const int grid = units < sms ? units : sms;
     if (s > 1 && cudaMemsetAsync(p.counters, 0, tiles * 4 * sizeof(unsigned), st) != cudaSuccess)
         return ARIA_ERR_CUDA;
     const bool gelu = act == ARIA_ACT_GELU_ERF;
@@ -881,13 +848,6 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq4, const voi
                     : launch_w4<TTV, false, 8>(X, M, K, Wq4, N, p, grid, st, pdl);                    \
     return gelu ? launch_w4<TTV, true, 4>(X, M, K, Wq4, N, p, grid, st, pdl)                          \
                 : launch_w4<TTV, false, 4>(X, M, K, Wq4, N, p, grid, st, pdl)
-    if (ct == 2) {
-        if (wbits == 8)
-            return gelu ? launch_w4<192, true, 8, 2>(X, M, K, Wq4, N, p, grid, st, pdl)
-                        : launch_w4<192, false, 8, 2>(X, M, K, Wq4, N, p, grid, st, pdl);
-        return gelu ? launch_w4<192, true, 4, 2>(X, M, K, Wq4, N, p, grid, st, pdl)
-                    : launch_w4<192, false, 4, 2>(X, M, K, Wq4, N, p, grid, st, pdl);
-    }
     if (tt == 32) { ARIA_W4_LAUNCH(32); }
     if (tt == 64) { ARIA_W4_LAUNCH(64); }
     if (tt == 128) { ARIA_W4_LAUNCH(128); }

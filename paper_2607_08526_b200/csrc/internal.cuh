@@ -90,8 +90,7 @@ int launch_gemm_w4a16(const void* X, int M, int K, const uint8_t* Wq, const void
                       int N, const void* bias, int act, void* Y, int yt, void* ws, size_t ws_bytes,
                       cudaStream_t st, bool pdl, int wbits = 4);
 size_t w4_workspace_bytes(int M, int N, int K, int sms);
-// the (token tile, split-K, CTAs per unit) launch_gemm_w4a16 picks; ct == nullptr: the best single-CTA plan
-void w4_plan(int M, int N, int K, int sms, int* tt, int* splits, int* ct);
+void w4_plan(int M, int N, int K, int sms, int* tt, int* splits);   // the (token tile, split-K) launch_gemm_w4a16 picks
 #ifdef ARIA_DEBUG
 void w4_set_profile_buffer(long long* p);  // per-CTA role timestamps
 #endif

@@ -18,7 +18,7 @@ constexpr int PK_A_BYTES = 128 * 128;
 constexpr int PK_THREADS = 128;
 
 template <int KIND, int CTAS>   // KIND 0: kind::i8 (s8 x s8 -> s32), 1: kind::f16 (bf16 x bf16 -> f32)
-__global__ void __launch_bounds__(PK_THREADS, 1) tensor_peak_kernel(int iters, long long* stamps, int ncols) {
+__global__ void __launch_bounds__(PK_THREADS, 1) tensor_peak_kernel(int iters, long long* stamps, int ncols, int commit_every) {
     constexpr int B_ROWS = 256 / CTAS;
     constexpr int B_BYTES = B_ROWS * 128;
     extern __shared__ uint8_t smem_raw[];
@@ -27,7 +27,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1) tensor_peak_kernel(int iters, l
     uint8_t* gbase = smem_raw + (base - raw);
     const uint32_t sA = base, sB = base + PK_A_BYTES;
     const uint32_t bar = base + PK_A_BYTES + B_BYTES;
-    const uint32_t tmem_slot = bar + 8;
+    const uint32_t tmem_slot = bar + 8;   // bar + 16: spare barrier
     volatile uint32_t* tmem_slot_g = reinterpret_cast<volatile uint32_t*>(gbase + PK_A_BYTES + B_BYTES + 8);
     const int warp = threadIdx.x >> 5;
     const uint32_t rank = CTAS == 2 ? cluster_ctarank() : 0u;
@@ -42,6 +42,7 @@ __global__ void __launch_bounds__(PK_THREADS, 1) tensor_peak_kernel(int iters, l
     fence_proxy_async_smem();
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
+        mbar_init(bar + 16, 1 << 20);      // debug experiments: a barrier that absorbs extra commits
         fence_mbar_init();
     }
     if (warp == 1) {
@@ -77,6 +78,11 @@ __global__ void __launch_bounds__(PK_THREADS, 1) tensor_peak_kernel(int iters, l
                         else mma_f16_ss(d, a_desc + 2 * k, b_desc + 2 * k, idesc, accum);
                     }
                 }
+#ifdef ARIA_DEBUG
+                if (commit_every > 0 && (it % commit_every) == commit_every - 1) {     // timing experiment: commits in the stream
+                    if (CTAS == 2) tc_commit_2sm(bar + 16, 1); else tc_commit(bar + 16);
+                }
+#endif
             }
             if (CTAS == 2) tc_commit_2sm(bar, 1); else tc_commit(bar);
         }
@@ -118,7 +124,9 @@ static int run_peak(int iters, int sms, long long* d_stamps, cudaStream_t st) {
     cfg.numAttrs = 1;
     static const char* n_env = dbg_env("ARIA_PEAK_N");
     const int ncols = n_env ? atoi(n_env) : 256;
-    return cudaLaunchKernelEx(&cfg, kern, iters, d_stamps, ncols) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
+    static const char* c_env = dbg_env("ARIA_PEAK_COMMIT");
+    const int commit_every = c_env ? atoi(c_env) : 0;
+    return cudaLaunchKernelEx(&cfg, kern, iters, d_stamps, ncols, commit_every) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
 int tensor_peak(int kind, int ctas, int iters, double seconds, double* out, cudaStream_t st) {
