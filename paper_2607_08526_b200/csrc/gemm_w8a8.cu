@@ -116,9 +116,15 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, ui
 // stores; measured equal within 3% on every C5 shape, and the staging area now serves the S1 side job.)
 // The arithmetic is issued as packed f32x2 instructions.
 template <int BN, int OUT_T, bool GELU>
-__device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const float* swb, int cb, float sxv, int lane,
+__device__ __forceinline__ void w8_epilogue_16(const uint32_t* v, const float* swb, int cb, float sxv, int lane,
                                                int n0, int row0, bool want_amax, float& amax, const W8Params& p) {
     uint32_t w[16];
+#ifdef ARIA_DEBUG
+    if (W8_DBG(p) == 2) {                  // timing experiment: no arithmetic (results are WRONG)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) w[j] = v[2 * j] ^ (v[2 * j + 1] << 16);
+    } else
+#endif
     if (OUT_T == 2) {
 #pragma unroll
         for (int j = 0; j < 16; ++j) w[j] = v[j];
@@ -153,6 +159,12 @@ __device__ __forceinline__ void w8_epilogue_16(const uint32_t (&v)[16], const fl
         }
     }
     const int row = row0 + lane, col = n0 + cb;
+#ifdef ARIA_DEBUG
+    if (W8_DBG(p) == 1) {                  // timing experiment: no stores
+        if (w[0] == 0x12345678u && w[7] == 0x9abcdef0u) static_cast<uint32_t*>(p.Y)[0] = w[3];
+        return;
+    }
+#endif
     if (row < p.M && col < p.N) {
         constexpr int ESZ = OUT_T == 1 ? 2 : 4;
         uint8_t* dst = static_cast<uint8_t*>(p.Y) + (static_cast<size_t>(row) * p.N + col) * ESZ;
@@ -462,28 +474,30 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             tc_fence_after();
             if (ew == 0 && lane == 0) w8_stamp(p, 8 + 2 * min(3, it), t_start);
             const uint32_t t_addr = tmem_base + acc * Cfg::ACC_STRIDE + (static_cast<uint32_t>(q * 32) << 16);
-            // A chunk is two groups of 16 columns held in two register sets; the refill of the first set
-            // for the next chunk is in flight while the second set is processed.
-            uint32_t va[16], vb[16];
+            // Two 32-column register sets: the tcgen05.ld of chunk c + 1 is in flight while chunk c is processed, and
+            // the wait that follows the processing finds it complete.  (Round 1 / 2a used 16-column sets and waited
+            // right after issuing the second refill: role timestamps showed ~230 cycles of exposed tcgen05.ld latency
+            // per 32 columns, 3.6k of the 6.3k cycles a 128 x 256 tile's epilogue took.)
+            uint32_t va[32], vb[32];
             const bool want_amax = OUT_T != 2 && p.row_absmax != nullptr;
             float amax = 0.0f;
             int c = c_beg;
             if (c < c_end) {
-                tmem_ld_32x32b_x16(t_addr + c * 32, va);
-                tmem_ld_32x32b_x16(t_addr + c * 32 + 16, vb);
-                tmem_wait_ld_x16(va);
-                tmem_wait_ld_x16(vb);
+                tmem_ld_32x32b_x32(t_addr + c * 32, va);
+                tmem_wait_ld_x32(va);
             }
 #pragma unroll 1
-            for (; c < c_end; ++c) {
-                const int cn = c + 1;
+            for (; c < c_end; c += 2) {
+                const bool has_b = c + 1 < c_end, has_a2 = c + 2 < c_end;
+                if (has_b) tmem_ld_32x32b_x32(t_addr + (c + 1) * 32, vb);
                 w8_epilogue_16<BN, OUT_T, GELU>(va, swb, c * 32, sxv, lane, n0, row0, want_amax, amax, p);
-                if (cn < c_end) tmem_ld_32x32b_x16(t_addr + cn * 32, va);
-                w8_epilogue_16<BN, OUT_T, GELU>(vb, swb, c * 32 + 16, sxv, lane, n0, row0, want_amax, amax, p);
-                if (cn < c_end) {
-                    tmem_ld_32x32b_x16(t_addr + cn * 32 + 16, vb);
-                    tmem_wait_ld_x16(va);
-                    tmem_wait_ld_x16(vb);
+                w8_epilogue_16<BN, OUT_T, GELU>(va + 16, swb, c * 32 + 16, sxv, lane, n0, row0, want_amax, amax, p);
+                if (has_b) {
+                    tmem_wait_ld_x32(vb);
+                    if (has_a2) tmem_ld_32x32b_x32(t_addr + (c + 2) * 32, va);
+                    w8_epilogue_16<BN, OUT_T, GELU>(vb, swb, (c + 1) * 32, sxv, lane, n0, row0, want_amax, amax, p);
+                    w8_epilogue_16<BN, OUT_T, GELU>(vb + 16, swb, (c + 1) * 32 + 16, sxv, lane, n0, row0, want_amax, amax, p);
+                    if (has_a2) tmem_wait_ld_x32(va);
                 }
             }
             if (want_amax && row0 + lane < p.M) {
@@ -495,7 +509,8 @@ w8a8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             tc_fence_before();
             __syncwarp();
             if (lane == 0) {
-                if (CTAS == 2) mbar_arrive_cluster(tempty_leader + 8 * acc);   // leader's barrier
+                if (CTAS == 2) mbar_arrive_cluster_relaxed(tempty_leader + 8 * acc);   // leader's barrier; what it guards (our
+                                                                               // reads of the accumulator) is tensor memory
                 else mbar_arrive(tempty0 + 8 * acc);
             }
             if (ew == 0 && lane == 0) w8_stamp(p, 9 + 2 * min(3, it), t_start);
