@@ -205,6 +205,10 @@ def per_linear_table(torch, aria, inputs, pk):
     a CUDA graph that cycles through enough distinct weight copies to exceed 2 x L2 (HBM-cold)."""
     out = []
     L2 = 126e6
+    try:
+        peak8 = tensor_peaks(aria)["int8"]["burst"]
+    except Exception:                            # noqa: BLE001
+        peak8 = pk["bf16_burst"] * NOMINAL_INT8_OVER_BF16
 
     def dev_bf16(bits):
         return torch.from_numpy(bits.view(np.int16).copy()).cuda().view(torch.bfloat16)
@@ -214,7 +218,7 @@ def per_linear_table(torch, aria, inputs, pk):
         X = dev_bf16(bits)
         W = torch.from_numpy(inputs.normal_f32((N, K), inputs.W_STD, 9, M + K + N + 1)).cuda()
         b = dev_bf16(inputs.normal_bf16((N,), inputs.B_STD, 9, M + K + N + 2)[0])
-        if mode == "w8a8":
+        if mode in ("w8a8", "w8a8_gemm"):
             wq, sc = aria.aria_quantize_weights_int8(W)
             wbytes = N * K + 4 * N
         else:
@@ -226,12 +230,16 @@ def per_linear_table(torch, aria, inputs, pk):
         wqs = [wq.clone() for _ in range(ncopy)]
         scs = [sc.clone() for _ in range(ncopy)]
         Y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
-        ws = aria.workspace(aria.aria_workspace_bytes(M, K, N, aria.W8A8 if mode == "w8a8" else aria.W4A16))
+        ws = aria.workspace(aria.aria_workspace_bytes(M, K, N, aria.W8A8 if mode.startswith("w8a8") else aria.W4A16))
+
+        xq_sx = aria.aria_quantize_act_int8(X) if mode == "w8a8_gemm" else None
 
         def launch_all():
             for i in range(ncopy):
                 if mode == "w8a8":
                     aria.aria_linear_w8a8(X, wqs[i], scs[i], b, act, aria.BF16, ws=ws, out=Y)
+                elif mode == "w8a8_gemm":      # S2 + S3 alone, on already-quantised activations
+                    aria.aria_linear_w8a8_q(xq_sx[0], xq_sx[1], wqs[i], scs[i], b, act, aria.BF16, out=Y)
                 else:
                     aria.aria_linear_w4a16(X, wqs[i], scs[i], b, act, aria.BF16, ws=ws, out=Y)
         launch_all()
@@ -244,10 +252,15 @@ def per_linear_table(torch, aria, inputs, pk):
         ops = 2.0 * M * N * K
         abytes = M * K * 2 + wbytes + 2 * N + M * N * 2          # X + weights(+scales) + bias + Y
         tput = ops / (ms * 1e-3) / 1e12
-        peak_t = pk["bf16_burst"] * (NOMINAL_INT8_OVER_BF16 if mode == "w8a8" else 1.0)
+        i8 = mode.startswith("w8a8")
+        # int8: the MEASURED tensor peak (issue loop, burst); bf16: the driver-measured cuBLAS burst figure
+        peak_t = peak8 if i8 else pk["bf16_burst"]
+        if mode == "w8a8_gemm":
+            abytes = M * K + 4 * M + wbytes + 2 * N + M * N * 2  # Xq + sx instead of X
         t_roof = max(ops / (peak_t * 1e12), abytes / (pk["hbm_gbs"] * 1e9))
         out.append({"case": name, "mode": mode, "M": M, "K": K, "N": N, "us": round(ms * 1e3, 2),
-                    "tput": round(tput, 1), "unit": "TOPS" if mode == "w8a8" else "eff_TFLOPS",
+                    "tput": round(tput, 1), "unit": "TOPS" if i8 else "eff_TFLOPS",
+                    "frac_of_tensor_peak": round(tput / peak_t, 3),
                     "gbs": round(abytes / (ms * 1e-3) / 1e9, 1),
                     "bound": "tensor" if ops / (peak_t * 1e12) >= abytes / (pk["hbm_gbs"] * 1e9) else "hbm",
                     "roofline_frac": round(t_roof / (ms * 1e-3), 3)})
@@ -257,6 +270,9 @@ def per_linear_table(torch, aria, inputs, pk):
     bench_case("C2 out", "w8a8", 512, 1536, 1536, aria.ACT_NONE)
     bench_case("C3 up+gelu", "w8a8", 4096, 1536, 6144, aria.ACT_GELU_ERF)
     bench_case("C3 down", "w8a8", 4096, 6144, 1536, aria.ACT_NONE)
+    # north_star's large-M target is stated for the int8 GEMM: S2 + S3 alone on pre-quantised activations
+    bench_case("C3 up+gelu GEMM only", "w8a8_gemm", 4096, 1536, 6144, aria.ACT_GELU_ERF)
+    bench_case("C3 down GEMM only", "w8a8_gemm", 4096, 6144, 1536, aria.ACT_NONE)
     for M in inputs.C4_MS:
         for (K, N) in inputs.C4_SHAPES:
             bench_case(f"C4 M={M}", "w4a16", M, K, N, aria.ACT_NONE)
