@@ -31,8 +31,10 @@ sys.path.insert(0, ROOT)
 METRIC = "quantized DiT linear throughput: W8A8 int8 TOPS + W4A16 effective bf16 TFLOPS over one C5 denoising-step stack"
 UNIT = "Top/s"
 WORKLOAD = "C5: 24 blocks x (QKV 1536->4608, out 1536->1536, MLP 1536->6144->1536), M=2048, all-W8A8 then all-W4A16, CUDA-graph replay"
-W4A16_TRAFFIC = 15.05e6          # bytes per launch, ncu (updated with each profiles/ capture)
-W4A16_TRAFFIC_SRC = "profiles/r1c_w4a16_full.md"
+W4A16_TRAFFIC = 15.06e6          # bytes per launch, ncu (updated with each profiles/ capture)
+W4A16_TRAFFIC_SRC = "profiles/r2_w4a16_full.md"
+W8A8_TRAFFIC = 17.4e6            # bytes per launch, ncu
+W8A8_TRAFFIC_SRC = "profiles/r2_w8a8_full.md"
 NOMINAL_INT8_OVER_BF16 = 2.0     # B200_PROFILING.md: 4.5 POP/s int8 vs 2.25 PFLOP/s bf16, dense
 BURST_REGION_S = 1.0             # a timed region shorter than this runs at burst clocks: score against the burst peak
 
@@ -376,6 +378,46 @@ def next_rows(torch, aria, inputs, pk):
     return out
 
 
+def hbm_passes(torch, aria, inputs, pk):
+    """The HBM-bound passes around the GEMMs, each alone on distinct buffers totalling > 2 x L2 (HBM-cold), replayed
+    from one CUDA graph: S1 (aria_quantize_act_int8) and norm + S1 (aria_norm_quantize_act_int8) at the step's
+    shape, at C3's down-projection input and at a large token count.  Bytes are algorithmic: 2 in + 1 out per
+    element + 4 per row."""
+    out = []
+    for (M, K) in ((2048, 1536), (4096, 6144), (16384, 1536)):
+        nbuf = max(2, int(2 * 126e6 // (M * K * 2)) + 1)
+        xs = [torch.randn((M, K), device="cuda").to(torch.bfloat16) for _ in range(nbuf)]
+        xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+        sx = torch.empty((M,), dtype=torch.float32, device="cuda")
+        gm = torch.ones((K,), dtype=torch.float32, device="cuda")
+        bt = torch.zeros((K,), dtype=torch.float32, device="cuda")
+        L = aria.lib()
+        import ctypes
+        st = lambda: ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)   # noqa: E731
+
+        def s1_all():
+            for x in xs:
+                rc = L.aria_quantize_act_int8(x.data_ptr(), aria.BF16, M, K, xq.data_ptr(), sx.data_ptr(), st())
+                assert rc == 0
+
+        def nq_all():
+            for x in xs:
+                aria.aria_norm_quantize_act_int8(x, gm, bt, aria.NORM_LAYER, 1e-5, out=(xq, sx))
+        for name, fn in (("S1", s1_all), ("LayerNorm+S1", nq_all)):
+            fn()
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                fn()
+            g.replay()
+            ms = time_region(torch, g.replay, 5) / nbuf
+            nbytes = M * K * 3 + 4 * M
+            out.append({"pass": name, "M": M, "K": K, "us": round(ms * 1e3, 2), "gbs": round(nbytes / (ms * 1e-3) / 1e9, 1),
+                        "hbm_frac_measured": round(nbytes / (ms * 1e-3) / 1e9 / pk["hbm_gbs"], 3)})
+        del xs
+    return out
+
+
 def small_m_stream(torch, aria, inputs, pk, iters=20):
     """SURVEY S8(d) 'C5-shaped stack at M=32, W4A16': the weight-bound regime.  One plan
     (aria_stack_plan_*) = ONE persistent weight-streaming kernel over all 96 layers, captured in a CUDA
@@ -549,7 +591,7 @@ def run_ours(args):
                 "peak_source": src8,
                 "frac_of_2x_bf16_burst": ach / (pk["bf16_burst"] * NOMINAL_INT8_OVER_BF16),
                 "frac_of_nominal_4500": ach / 4500.0, "avg_launch_us": dur * 1e6, "launches": n_l,
-                "traffic": 12.64e6, "traffic_unit": "bytes/launch (ncu, profiles/r1c_w8a8_full.md)"}
+                "traffic": W8A8_TRAFFIC, "traffic_unit": f"bytes/launch (ncu, {W8A8_TRAFFIC_SRC})"}
 
     # ---- roofline of the DOMINANT kernel of the step: w4a16_gemm_kernel.  The W4A16 half of the step is 96
     # launches of that kernel and nothing else, so its average launch duration is t4 / 96 from the CUDA
@@ -584,10 +626,14 @@ def run_ours(args):
         cpu = {"value": ops / t / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"block 0's 4 linears at 1024 of the 2048 tokens, both modes, {t:.1f} s"}
     ops8, ops4 = st8.ops, st4.ops
-    table = small = nxt = None
+    table = small = nxt = hbm = None
     if world == 1 and not args.no_per_linear:
         table = per_linear_table(torch, aria, inputs, pk)
         small = small_m_stream(torch, aria, inputs, pk)
+        try:
+            hbm = hbm_passes(torch, aria, inputs, pk)
+        except Exception as ex:                  # noqa: BLE001
+            log(f"[bench] hbm_passes failed: {ex!r}")
         try:
             nxt = next_rows(torch, aria, inputs, pk)
         except Exception as ex:                  # noqa: BLE001
@@ -617,8 +663,10 @@ def run_ours(args):
                    "multi_gpu": "replicas only"},
         "roofline": roofline, "roofline_w8a8_gemm": roofline_w8a8, "tensor_peaks": tp, "sustained": sustained,
         "cpu_baseline": cpu, "e2e": e2e,
-        "gpu_launches": args.steps * (2 * n_l + n_l), "clocks": clocks, "per_linear": table,
-        "small_m": small, "next_rows": nxt,
+        # kernels of this library launched inside the timed region: per step 96 W4A16 GEMMs + 96 W8A8 GEMMs + the
+        # stand-alone S1 passes the W8A8 chain keeps (layer 0, and the rounding pass of every chained layer)
+        "gpu_launches": args.steps * (2 * n_l + 1 + sum(1 for s in st8.specs if s["in"] is None)), "clocks": clocks, "per_linear": table,
+        "small_m": small, "hbm_passes": hbm, "next_rows": nxt,
     }
     log("[bench] " + json.dumps({k: line[k] for k in ("value", "ms_per_step", "modes", "roofline", "roofline_w8a8_gemm",
                                                        "tensor_peaks", "sustained")}))
@@ -692,7 +740,8 @@ def main():
         from paper_2607_08526_b200 import binding as aria
         from paper_2607_08526_b200 import inputs
         aria.lib()
-        print(json.dumps({"next_rows": next_rows(torch, aria, inputs, peaks())}))
+        print(json.dumps({"next_rows": next_rows(torch, aria, inputs, peaks()),
+                          "hbm_passes": hbm_passes(torch, aria, inputs, peaks())}))
         return
     if args.per_linear_only:
         import torch
