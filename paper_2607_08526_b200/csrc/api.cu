@@ -268,6 +268,7 @@ int aria_gemm_i8_i32(const int8_t* Xq, const int8_t* Wq, int M, int N, int K, in
 __attribute__((visibility("default"))) void aria_debug_w4_profile(long long* buf) { w4_set_profile_buffer(buf); }
 __attribute__((visibility("default"))) void aria_debug_ws_profile(long long* buf) { ws_set_profile_buffer(buf); }
 __attribute__((visibility("default"))) void aria_debug_w8_profile(long long* buf) { w8_set_profile_buffer(buf); }
+__attribute__((visibility("default"))) void aria_debug_att_profile(long long* buf) { att_set_profile_buffer(buf); }
 #endif
 
 int aria_steer(void* H, int ht, int M, int D, const float* d, const float* strength, float hbar_norm, int op,

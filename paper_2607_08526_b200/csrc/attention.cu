@@ -49,7 +49,18 @@ struct AttParams {
     float* row_absmax;      // [B*S] or nullptr
     int S, H;
     float c;                // scale * log2(e)
+#ifdef ARIA_DEBUG
+    long long* prof;        // per-CTA role timings (debug builds), or nullptr
+#endif
 };
+
+#ifdef ARIA_DEBUG
+static long long* g_att_prof = nullptr;
+void att_set_profile_buffer(long long* p) { g_att_prof = p; }
+#define AT_TIMED(acc, stmt) do { const long long t_ = clock64(); stmt; acc += clock64() - t_; } while (0)
+#else
+#define AT_TIMED(acc, stmt) do { stmt; } while (0)
+#endif
 
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* m, int c0, int c1, int c2, uint32_t bar) {
     asm volatile(
@@ -142,10 +153,12 @@ attention_kernel(const __grid_constant__ CUtensorMap tmQKV, const AttParams p) {
         const uint64_t desc_hi = make_smem_desc_sw128(0);
         const uint64_t q_desc = desc_hi | ((sQ & 0x3FFFF) >> 4);
         const uint32_t s_tmem = tmem_base + AT_S_COL, p_tmem = tmem_base + AT_P_COL, o_tmem = tmem_base + AT_O_COL;
+        long long m_p = 0, m_v = 0, m_k = 0, m_s = 0;
+        const long long m_t0 = clock64();
         auto issue_pv = [&](int j) {
             const int st = j % AT_ST;
-            mbar_wait(pfull, j & 1);                             // P_j in tensor memory, O rescaled
-            mbar_wait(vfull0 + 8 * st, (j / AT_ST) & 1);
+            AT_TIMED(m_p, mbar_wait(pfull, j & 1));              // P_j in tensor memory, O rescaled
+            AT_TIMED(m_v, mbar_wait(vfull0 + 8 * st, (j / AT_ST) & 1));
             tc_fence_after();
             if (elect_one()) {
                 // V tile: 128 keys x 128 bytes; 8 keys = one 1024-byte swizzle atom, K = 16 keys = 2 atoms
@@ -162,8 +175,8 @@ attention_kernel(const __grid_constant__ CUtensorMap tmQKV, const AttParams p) {
         mbar_wait(qfull, 0);
         for (int j = 0; j < nkv; ++j) {
             const int st = j % AT_ST;
-            mbar_wait(kfull0 + 8 * st, (j / AT_ST) & 1);
-            if (j > 0) mbar_wait(sfree, (j - 1) & 1);            // S_{j-1} is in the softmax warps' registers
+            AT_TIMED(m_k, mbar_wait(kfull0 + 8 * st, (j / AT_ST) & 1));
+            if (j > 0) AT_TIMED(m_s, mbar_wait(sfree, (j - 1) & 1));   // S_{j-1} is in the softmax warps' registers
             tc_fence_after();
             if (elect_one()) {
                 const uint64_t k_desc = desc_hi | (((sK + st * AT_TILE) & 0x3FFFF) >> 4);
@@ -177,6 +190,14 @@ attention_kernel(const __grid_constant__ CUtensorMap tmQKV, const AttParams p) {
             if (j > 0) issue_pv(j - 1);
         }
         issue_pv(nkv - 1);
+#ifdef ARIA_DEBUG
+        if (p.prof && lane == 0) {
+            long long* q = p.prof + (static_cast<size_t>(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * 16;
+            q[0] = m_k; q[1] = m_s; q[2] = m_p; q[3] = m_v; q[4] = clock64() - m_t0;
+        }
+#else
+        (void)m_p; (void)m_v; (void)m_k; (void)m_s; (void)m_t0;
+#endif
     } else {
         // ------------------------------------------------------------ softmax + epilogue (warps 2..5)
         const int quarter = warp & 3;                            // tensor-memory lane quarter of this warp
@@ -186,13 +207,17 @@ attention_kernel(const __grid_constant__ CUtensorMap tmQKV, const AttParams p) {
                        o_addr = tmem_base + AT_O_COL + lane_off;
         const float c = p.c;
         float m = 0.0f, l = 0.0f;
+        long long s_w = 0, s_ld = 0, s_pv = 0, s_st = 0;
+        const long long s_t0 = clock64();
         for (int j = 0; j < nkv; ++j) {
-            mbar_wait(sfull, j & 1);
+            AT_TIMED(s_w, mbar_wait(sfull, j & 1));
+            const long long t_ld_ = clock64();
             tc_fence_after();
             uint32_t v[4][32];
 #pragma unroll
             for (int i = 0; i < 4; ++i) tmem_ld_32x32b_x32(s_addr + 32 * i, v[i]);
             tmem_wait_ld();
+            s_ld += clock64() - t_ld_;
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(sfree);
@@ -228,7 +253,7 @@ attention_kernel(const __grid_constant__ CUtensorMap tmQKV, const AttParams p) {
                 }
             const float sum = (sum4[0] + sum4[1]) + (sum4[2] + sum4[3]);
             if (j > 0) {
-                mbar_wait(pvdone, (j - 1) & 1);                  // P_{j-1} consumed, O up to date
+                AT_TIMED(s_pv, mbar_wait(pvdone, (j - 1) & 1));  // P_{j-1} consumed, O up to date
                 tc_fence_after();
                 if (__any_sync(0xffffffffu, move)) {             // rare after the first tiles
                     uint32_t o[2][32];
@@ -246,14 +271,24 @@ attention_kernel(const __grid_constant__ CUtensorMap tmQKV, const AttParams p) {
             }
             l += sum;
             m = m_new;
+            const long long t_st_ = clock64();
             tmem_st_32x32b_x32(p_addr, v[0]);
             tmem_st_32x32b_x32(p_addr + 32, v[1]);
             tmem_wait_st();
+            s_st += clock64() - t_st_;
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(pfull);
         }
-        mbar_wait(pvdone, (nkv - 1) & 1);
+        AT_TIMED(s_pv, mbar_wait(pvdone, (nkv - 1) & 1));
+#ifdef ARIA_DEBUG
+        if (p.prof && warp == 2 && lane == 0) {
+            long long* q = p.prof + (static_cast<size_t>(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * 16;
+            q[8] = s_w; q[9] = s_ld; q[10] = s_pv; q[11] = s_st; q[12] = clock64() - s_t0;
+        }
+#else
+        (void)s_w; (void)s_ld; (void)s_pv; (void)s_st; (void)s_t0;
+#endif
         tc_fence_after();
         uint32_t o[2][32];
         tmem_ld_32x32b_x32(o_addr, o[0]);
@@ -302,10 +337,18 @@ int launch_attention(const void* QKV, int B, int S, int H, float scale, void* O,
     p.row_absmax = row_absmax;
     p.S = S; p.H = H;
     p.c = scale * 1.4426950408889634f;
+#ifdef ARIA_DEBUG
+    p.prof = g_att_prof;
+#endif
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((S + AT_BM - 1) / AT_BM, H, B);
     cfg.blockDim = dim3(192);
     cfg.dynamicSmemBytes = AT_SMEM;
+    if (const char* e = dbg_env("ARIA_ATT_ONE_CTA")) {          // debug builds only: one CTA per SM (timing experiment)
+        (void)e;
+        cfg.dynamicSmemBytes = 120 * 1024;
+        cudaFuncSetAttribute(attention_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+    }
     cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;

@@ -106,6 +106,9 @@ int launch_norm_quant(const void* X, int xt, int M, int K, const float* gamma, c
 // ---- attention.cu: fused full self-attention on the [B*S, 3*H*64] bf16 output of the QKV projection (NEXT-2)
 int launch_attention(const void* QKV, int B, int S, int H, float scale, void* O, float* row_absmax, cudaStream_t st,
                      bool pdl);
+#ifdef ARIA_DEBUG
+void att_set_profile_buffer(long long* p);  // per-CTA role timings
+#endif
 
 // ---- peak.cu: measurement helper (tensor-pipe issue loop)
 int tensor_peak(int kind, int ctas, int iters, double seconds, double* out, cudaStream_t st);
