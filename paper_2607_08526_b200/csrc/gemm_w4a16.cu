@@ -436,8 +436,15 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap tmP, const __grid_constant
                 uint32_t w[32];
 #pragma unroll
                 for (int j = 0; j < 8; ++j) { w[4 * j] = o[j].x; w[4 * j + 1] = o[j].y; w[4 * j + 2] = o[j].z; w[4 * j + 3] = o[j].w; }
+#ifdef ARIA_DEBUG
+                if (p.dbg == 6) {            // timing experiment: no tensor-memory store (results are WRONG)
+                    if (w[0] == 0x12345678u && w[31] == 0x9abcdef0u) static_cast<uint32_t*>(p.Y)[0] = w[7];
+                } else
+#endif
+                {
                 tmem_st_32x32b_x32(tmem_base + Cfg::A_COL0 + ab * 32 + (static_cast<uint32_t>(q_ * 32) << 16), w);
                 tmem_wait_st();
+                }
                 tc_fence_before();
             } else {
                 const uint32_t rowb = sA + ab * Cfg::A_BYTES + rowoff_;
