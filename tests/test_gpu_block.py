@@ -265,3 +265,56 @@ def test_block_stack_every_stage_teacher_forced_and_graph_replay(aria, oracle):
     st.replay()
     torch.cuda.synchronize()
     assert torch.equal(st.h, eager)
+
+
+@pytest.mark.parametrize("B,S,H", [(1, 2304, 2), (5, 256, 1), (1, 4000, 1)])
+def test_attention_long_and_many_sequences(aria, oracle, B, S, H):
+    # more key tiles than the bench shape (barrier phases wrap many times), more sequences than CFG's two
+    _att_case(aria, oracle, B, S, H, tid=S % 11, sample_bh=[(0, 0), (B - 1, H - 1)])
+
+
+def test_block_stack_full_size_as_benched_sampled(aria, oracle):
+    """BlockStack at the size bench.py times (2 x 1024 tokens, d_model 1536, 24 heads), 2 blocks: every stage against
+    the oracle on sampled rows / heads, each stage fed the GPU's actual input (a row of a linear depends only on its
+    own input row; a head's attention only on its own columns of its own sequence)."""
+    from paper_2607_08526_b200.stack import BlockStack
+    st = BlockStack(B=2, S=1024, n_blocks=2, d_model=1536, keep_host=True)
+    st.run(tap=True)
+    torch.cuda.synchronize()
+    rows = np.array([0, 1, 511, 1023, 1024, 1500, 2047])
+    for t, hst in zip(st.taps, st.host):
+        f = lambda k, r=None: host_f32(t[k] if r is None else t[k][r])        # noqa: E731
+        ridx = torch.from_numpy(rows).cuda()
+        # LayerNorm + S1 (rows), QKV (rows)
+        src = f("src", ridx)
+        ref = oracle.norm_rows(src, hst["g1"], hst["b1"], 0, 1e-5)
+        xn = f("xn1", ridx)
+        check_bf16_out(host_bits16(t["xn1"][ridx]), ref, inputs.bf16_bits(oracle.round_out(ref, 1)), 2e-6, 0.01)
+        q, s = oracle.quant_int8_rows(xn)
+        assert np.array_equal(t["xq1"][ridx].cpu().numpy(), q) and np.array_equal(t["sx1"][ridx].cpu().numpy(), s)
+        wq, sw = oracle.quant_int8_rows(hst["qkv"]["W"])
+        y = oracle.epilogue_w8a8(oracle.gemm_i8(q, wq), s, sw, hst["qkv"]["b"].astype(np.float64))
+        assert rel_err(f("qkv", ridx), y) <= 2.0 ** -8
+        # attention on sampled (sequence, head) pairs, all queries
+        qkv3 = f("qkv").reshape(st.B, st.S, 3, st.H, 64)
+        att3 = f("att").reshape(st.B, st.S, st.H, 64)
+        for (b, h) in [(0, 0), (1, st.H - 1), (0, 7)]:
+            sub = np.ascontiguousarray(qkv3[b, :, :, h, :]).reshape(st.S, 192)
+            assert rel_err(att3[b, :, h, :], oracle.attention(sub, 1, st.S, 1, 64)) <= ATT_TOL
+        # fused absmax + rounding-only S1 of the attention output, out-projection
+        q, s = oracle.quant_int8_rows(f("att", ridx))
+        assert np.array_equal(t["xq2"][ridx].cpu().numpy(), q) and np.array_equal(t["sx2"][ridx].cpu().numpy(), s)
+        wq, sw = oracle.quant_int8_rows(hst["out"]["W"])
+        y = oracle.epilogue_w8a8(oracle.gemm_i8(q, wq), s, sw, hst["out"]["b"].astype(np.float64))
+        assert rel_err(f("h2", ridx), y) <= 2.0 ** -8
+        # LayerNorm 2 + S1, up + GELU, S1 + down
+        ref = oracle.norm_rows(f("h2", ridx), hst["g2"], hst["b2"], 0, 1e-5)
+        check_bf16_out(host_bits16(t["xn3"][ridx]), ref, inputs.bf16_bits(oracle.round_out(ref, 1)), 2e-6, 0.01)
+        q, s = oracle.quant_int8_rows(f("xn3", ridx))
+        assert np.array_equal(t["xq3"][ridx].cpu().numpy(), q) and np.array_equal(t["sx3"][ridx].cpu().numpy(), s)
+        wq, sw = oracle.quant_int8_rows(hst["up"]["W"])
+        y = oracle.epilogue_w8a8(oracle.gemm_i8(q, wq), s, sw, hst["up"]["b"].astype(np.float64), oracle.ACT_GELU_ERF)
+        assert rel_err(f("mid", ridx), y) <= 2.0 ** -8
+        wq, sw = oracle.quant_int8_rows(hst["down"]["W"])
+        r = oracle.linear_w8a8(f("mid", ridx), wq, sw, hst["down"]["b"].astype(np.float64))
+        assert rel_err(f("h", ridx), r["y"]) <= 2.0 ** -8
