@@ -284,12 +284,13 @@ int aria_steer(void* H, int ht, int M, int D, const float* d, const float* stren
 
 int aria_norm_quantize_act_int8(const void* X, int xt, int M, int K, const float* gamma, const float* beta, int norm,
                                 float eps, void* Xn, int8_t* Xq, float* x_scale, void* stream) {
-    int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
-    if (rc != ARIA_OK) return rc;
+    // argument validation first (it needs no device), the architecture check last
     if (!gamma) return ARIA_ERR_NULL;
     if (norm != ARIA_NORM_LAYER && norm != ARIA_NORM_RMS) return ARIA_ERR_DTYPE;
     if (!(eps >= 0.0f) || K > 24576) return ARIA_ERR_SHAPE;
     if (misaligned(gamma) || misaligned(beta) || misaligned(Xn)) return ARIA_ERR_ALIGN;
+    int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
+    if (rc != ARIA_OK) return rc;
     return launch_norm_quant(X, xt, M, K, gamma, beta, norm, eps, Xn, Xq, x_scale, static_cast<cudaStream_t>(stream), true);
 }
 
@@ -304,10 +305,10 @@ int aria_attention(const void* QKV, int B, int S, int H, int Dh, float scale, vo
 
 int aria_round_act_int8(const void* X, int xt, int M, int K, float* absmax, int clear, int8_t* Xq, float* x_scale,
                         void* stream) {
-    int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
-    if (rc != ARIA_OK) return rc;
     if (!absmax) return ARIA_ERR_NULL;
     if (reinterpret_cast<uintptr_t>(absmax) & 3u) return ARIA_ERR_ALIGN;
+    int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
+    if (rc != ARIA_OK) return rc;
     return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), true, absmax, clear ? absmax : nullptr);
 }
 

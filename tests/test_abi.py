@@ -50,6 +50,22 @@ def test_validation_errors_need_no_gpu():
     assert L.aria_linear_w8a8(p16, 1, 4, 64, p16, p16, 16, None, 0, 0, p16, 1, p16, 16, None) == -6       # ws too small
     assert L.aria_workspace_bytes(0, 64, 64, 0) == 0
     assert L.aria_workspace_bytes(128, 1536, 4608, 0) >= 128 * 1536 + 128 * 4
+    # round-2 entry points
+    st = None
+    assert L.aria_linear_w8a16(p16, 4, 64, p16, p16, 12, None, 0, p16, 1, None, 0, st) == -2             # N % 8
+    assert L.aria_linear_w8a16(None, 4, 64, p16, p16, 16, None, 0, p16, 1, None, 0, st) == -1            # NULL
+    assert L.aria_norm_quantize_act_int8(p16, 1, 4, 48, p16, None, 0, 1e-5, None, p16, p16, st) == -2    # K % 32
+    assert L.aria_norm_quantize_act_int8(p16, 1, 4, 64, None, None, 0, 1e-5, None, p16, p16, st) == -1   # gamma NULL
+    assert L.aria_norm_quantize_act_int8(p16, 1, 4, 64, p16, None, 5, 1e-5, None, p16, p16, st) == -4    # unknown norm
+    assert L.aria_norm_quantize_act_int8(p16, 1, 4, 64, p16, None, 0, -1.0, None, p16, p16, st) == -2    # eps < 0
+    assert L.aria_attention(p16, 1, 128, 2, 32, 0.125, p16, None, st) == -2                              # head_dim != 64
+    assert L.aria_attention(p16, 1, 128, 2, 64, -1.0, p16, None, st) == -2                               # scale <= 0
+    assert L.aria_attention(p16, 0, 128, 2, 64, 0.125, p16, None, st) == -2                              # B <= 0
+    assert L.aria_attention(p16 + 8, 1, 128, 2, 64, 0.125, p16, None, st) == -3                          # alignment
+    assert L.aria_round_act_int8(p16, 1, 4, 64, None, 0, p16, p16, st) == -1                             # absmax NULL
+    assert L.aria_steer(p16, 1, 4, 12, p16, p16, 1.0, 0, st) == -2                                       # D % 8
+    assert L.aria_steer(p16, 1, 4, 16, p16, p16, 1.0, 9, st) == -4                                       # unknown op
+    assert L.aria_tensor_peak(3, 1, 16, 0.0, None, st) == -1
 
 
 def test_tile_plans_reach_every_compiled_variant_on_148_sms():
