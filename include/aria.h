@@ -181,8 +181,9 @@ ARIA_API int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M
  * Co-residency.  The stream kernel's CTAs (and those of aria_linear_w4a16 with split-K) wait on
  * completion counters written by other CTAs of the same grid.  The stream kernel is therefore a
  * COOPERATIVE launch of at most one CTA per SM: if the device cannot hold the grid at once the launch
- * fails with ARIA_ERR_CUDA instead of deadlocking.  Do not run two plans, or a plan and a split-K
- * linear, concurrently on different streams of one device.
+ * fails with ARIA_ERR_CUDA instead of deadlocking, and so is every split-K launch of aria_linear_w4a16 /
+ * aria_linear_w8a16.  Do not run two plans, or a plan and a split-K linear, concurrently on different
+ * streams of one device (the second launch would fail, not hang).
  *
  * aria_stack_plan_fallback_fired: SYNCHRONOUS (copies one word from the device after the stream's work
  * has been synchronised by the caller); *fired = 0 if the last run stayed in the fp16 domain, else a

@@ -773,10 +773,21 @@ static int launch_w4(const void* X, int M, int K, const uint8_t* Wq4, int N, con
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
+    int na = 0;
+    if (p.splits > 1) {
+        // split-K units wait for one another (per-tile counters): a COOPERATIVE launch (grid <= #SMs, one CTA per SM)
+        // either has every CTA resident or fails with ARIA_ERR_CUDA -- it cannot deadlock when another tenant's
+        // kernel holds SMs.  Such a launch is not also a programmatic dependent.
+        at[0].id = cudaLaunchAttributeCooperative;
+        at[0].val.cooperative = 1;
+        na = 1;
+    } else if (pdl) {
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        na = 1;
+    }
     cfg.attrs = at;
-    cfg.numAttrs = pdl ? 1 : 0;
+    cfg.numAttrs = na;
     return cudaLaunchKernelEx(&cfg, kern, tmP, tmX, tmY, p) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
