@@ -24,8 +24,11 @@
 //               Epilogue: O / l -> bf16 -> 128 contiguous bytes per thread to global memory; optionally the
 //               per-token max |o| is reduced across heads with atomicMax (first half of a fused S1 for a
 //               W8A8 out-projection).
-// Tensor work per (query tile, key tile) is 512 cycles, the 16384 exponentials are 1024 cycles of the SM's
-// 16 MUFU lanes: the kernel is bound by the exponential unit, not by the tensor pipe or HBM.
+// Roofline: per (query tile, key tile) 640 cycles of tensor work (an N = 64 tcgen05.mma costs 48 cycles, not 32)
+// against 1024 cycles of the SM's 16 ex2 lanes -- the exponential unit is the kernel's ceiling.
+// Measured (debug-build role timings): 2990 cycles per key tile per CTA, of which ~650 are the
+// exponentials and ~560 barrier waits of the softmax warp; without exponentials at all the kernel is only 16 %
+// faster, so today it is bound by the per-tile chain of dependent phases, not by that ceiling.
 #include "internal.cuh"
 
 namespace aria {
