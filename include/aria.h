@@ -93,6 +93,31 @@ ARIA_API int aria_linear_w8a8(const void* X, int xt, int M, int K, const int8_t*
                      int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
                      size_t ws_bytes, void* stream);
 
+/* The same W8A8 linear for callers that CANNOT ALLOCATE device memory and so have no `ws` to pass:
+ *   - real-time threads (an audio callback of an on-device generator): cudaMalloc takes a
+ *     process-wide lock, may synchronise the device and has no latency bound, so they never call it;
+ *   - plug-ins inside a host or serving engine whose own pool already owns all GPU memory (cudaMalloc fails);
+ *   - code handed raw device pointers by another runtime, with no allocator to ask.
+ * The Xq / sx scratch is a fixed array of ARIA_STATIC_WS_BYTES inside the library's device image instead.  The
+ * call allocates nothing: no cudaMalloc / cudaFree, no allocating library routine.  X, Wq, w_scale, bias and Y
+ * are passed exactly as to aria_linear_w8a8 and the result is the same, bit for bit (same kernels, same launches).
+ *  - Limit: round_up(M*K, 256) + round_up(4*M, 256) <= ARIA_STATIC_WS_BYTES (16 MiB: up to M = 2048 tokens at
+ *    K = 6144, the largest linear of config C5).  A larger shape returns ARIA_ERR_WORKSPACE, nothing is enqueued
+ *    and Y is not touched; use aria_linear_w8a8 with your own workspace there.  aria_static_ws_bytes() returns
+ *    the limit of the library that is actually loaded.
+ *  - Cost: every GPU on which this entry point has been called keeps the 16 MiB until the process exits.
+ *  - First call on each device: looks up the array's device address (cudaGetSymbolAddress, which loads the
+ *    module on that device; the address differs per GPU and is cached per device ordinal).  Make that first
+ *    call with the device current and BEFORE starting any stream capture on it.
+ *  - One array per device, shared by every call and every stream: two calls whose kernels may overlap on
+ *    the GPU (different streams, no ordering between them) race on it and corrupt each other's codes.  Calls on
+ *    one stream, or ordered by events, are safe.  The array keeps the previous call's bytes; nothing in it needs
+ *    clearing, because S1 overwrites every code and scale the GEMM reads.                                       */
+#define ARIA_STATIC_WS_BYTES (16u << 20)
+ARIA_API int aria_linear_w8a8_static_ws(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
+                                        int N, const void* bias, int bt, int act, void* Y, int yt, void* stream);
+ARIA_API size_t aria_static_ws_bytes(void);
+
 /* S2+S3 only -- the same linear for activations that are ALREADY quantised (a producer that
  * emitted int8 codes, or a caller reusing one S1 pass for several linears of the same input):
  * Xq int8 [M,K] and x_scale fp32 [M] as produced by aria_quantize_act_int8.  No workspace.     */

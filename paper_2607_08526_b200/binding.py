@@ -54,6 +54,10 @@ def lib() -> ctypes.CDLL:
         L.aria_quantize_weights_int4.argtypes = [c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p]
         L.aria_linear_w8a8.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p,
                                        c_int, c_int, c_void_p, c_int, c_void_p, c_size_t, c_void_p]
+        L.aria_linear_w8a8_static_ws.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p,
+                                                 c_int, c_int, c_void_p, c_int, c_void_p]
+        L.aria_static_ws_bytes.restype = c_size_t
+        L.aria_static_ws_bytes.argtypes = []
         L.aria_linear_w8a8_q.argtypes = [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p,
                                          c_int, c_int, c_void_p, c_int, c_void_p]
         L.aria_linear_w4a16.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_int, c_int, c_void_p,
@@ -81,7 +85,7 @@ def lib() -> ctypes.CDLL:
         L.aria_stack_plan_destroy.restype = None
         for name in EXPORTS:
             if name not in ("aria_version", "aria_status_string", "aria_workspace_bytes",
-                            "aria_workspace_bytes_host", "aria_stack_plan_destroy"):
+                            "aria_workspace_bytes_host", "aria_stack_plan_destroy", "aria_static_ws_bytes"):
                 getattr(L, name).restype = c_int
         _lib = L
     return _lib
@@ -93,7 +97,8 @@ EXPORTS = ("aria_linear_w8a8_q", "aria_quantize_weights_int8", "aria_quantize_we
            "aria_status_string", "aria_gemm_i8_i32", "aria_version", "aria_stack_plan_create",
            "aria_stack_plan_run", "aria_stack_plan_is_streaming", "aria_stack_plan_destroy",
            "aria_stack_plan_fallback_fired", "aria_w8a8_tile_plan", "aria_w4a16_tile_plan", "aria_tensor_peak", "aria_linear_w8a16", "aria_steer",
-           "aria_norm_quantize_act_int8", "aria_attention", "aria_round_act_int8")
+           "aria_norm_quantize_act_int8", "aria_attention", "aria_round_act_int8", "aria_linear_w8a8_static_ws",
+           "aria_static_ws_bytes")
 
 
 def _check(rc: int, what: str):
@@ -176,6 +181,24 @@ def aria_linear_w8a8(X, Wq, w_scale, bias=None, act: int = ACT_NONE, yt: int = B
     _check(lib().aria_linear_w8a8(_ptr(X), _dt(X), M, K, _ptr(Wq), _ptr(w_scale), N, _ptr(bias),
                                   _dt(bias) if bias is not None else F32, act, _ptr(Y), yt, _ptr(ws),
                                   ws.numel(), _stream()), "aria_linear_w8a8")
+    return Y
+
+
+def aria_static_ws_bytes() -> int:
+    return int(lib().aria_static_ws_bytes())
+
+
+def aria_linear_w8a8_static_ws(X, Wq, w_scale, bias=None, act: int = ACT_NONE, yt: int = BF16, out=None):
+    """aria_linear_w8a8 for callers that cannot allocate a workspace (real-time threads, plug-ins inside an engine
+    that owns all GPU memory): the Xq / sx scratch is a fixed 16 MiB array inside the library, shared by all calls
+    on the device.  Shapes beyond aria_static_ws_bytes() raise (ARIA_ERR_WORKSPACE).  Pass `out` to avoid the one
+    allocation this Python wrapper would otherwise make for Y."""
+    M, K = X.shape
+    N = Wq.shape[0]
+    Y = out if out is not None else torch.empty((M, N), dtype=_out_dtype(yt), device=X.device)
+    _check(lib().aria_linear_w8a8_static_ws(_ptr(X), _dt(X), M, K, _ptr(Wq), _ptr(w_scale), N, _ptr(bias),
+                                            _dt(bias) if bias is not None else F32, act, _ptr(Y), yt, _stream()),
+           "aria_linear_w8a8_static_ws")
     return Y
 
 

@@ -18,7 +18,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libaria_b200.so")
-SOURCES = ["api.cu", "quant.cu", "tensormap.cu", "gemm_w8a8.cu", "gemm_w4a16.cu", "w4a16_stream.cu", "peak.cu", "steer.cu", "norm.cu", "attention.cu"]
+SOURCES = ["api.cu", "quant.cu", "tensormap.cu", "gemm_w8a8.cu", "gemm_w4a16.cu", "w4a16_stream.cu", "peak.cu", "steer.cu", "norm.cu", "attention.cu", "static_ws.cu"]
 HEADERS = ["internal.cuh", "ptx.cuh", "quant_dev.cuh", os.path.join("..", "..", "include", "aria.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
