@@ -1100,11 +1100,14 @@ int ws_plan_fallback_fired(const WsPlan* plan, int* fired) {
 }
 
 // The kernel's CTAs wait on one another (completion counters), so the whole grid must be co-resident:
-// a COOPERATIVE launch, which fails cleanly (instead of deadlocking) when the device cannot hold the grid
-// at once, e.g. because another tenant's kernel holds SMs.  `dependent`: the bf16 fallback launch, a
-// programmatic dependent of the fp16 launch before it (its launch latency hides behind that kernel).
+// a COOPERATIVE launch, which is either fully resident or not started (and fails cleanly when the grid
+// can never fit), instead of deadlocking on a CTA that has no SM, e.g. because another tenant's kernel
+// holds SMs.  This holds for BOTH launches of a plan: the bf16 fallback runs the same cross-CTA waits when
+// the fp16 launch left its domain, so it is cooperative too and follows the fp16 launch in plain stream
+// order (it is not a programmatic dependent: its griddepcontrol.wait is then a no-op, and the flag it
+// reads is complete when it starts).
 template <bool AF16, bool PROF>
-static int ws_launch(const WsPlan* plan, cudaStream_t st, bool dependent) {
+static int ws_launch(const WsPlan* plan, cudaStream_t st) {
     static std::atomic<uint64_t> attr_done{0};
     auto kern = w4a16_stream_kernel<AF16, PROF>;
     if (!ensure_dyn_smem(kern, WS_SMEM_BYTES, attr_done)) return ARIA_ERR_CUDA;
@@ -1114,30 +1117,27 @@ static int ws_launch(const WsPlan* plan, cudaStream_t st, bool dependent) {
     cfg.dynamicSmemBytes = WS_SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute at[1];
-    if (dependent) {
-        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        at[0].val.programmaticStreamSerializationAllowed = 1;
-    } else {
-        at[0].id = cudaLaunchAttributeCooperative;
-        at[0].val.cooperative = 1;
-    }
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, kern, plan->params) == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
 }
 
-static int ws_run_one(const WsPlan* plan, cudaStream_t st, bool dependent) {
+static int ws_run_one(const WsPlan* plan, cudaStream_t st) {
 #ifdef ARIA_DEBUG
     const bool prof = plan->params.prof != nullptr || (plan->params.dbg & 127) != 0;   // instrumented kernel
-    if (prof) return plan->a_f16 ? ws_launch<true, true>(plan, st, dependent) : ws_launch<false, true>(plan, st, dependent);
+    if (prof) return plan->a_f16 ? ws_launch<true, true>(plan, st) : ws_launch<false, true>(plan, st);
 #endif
-    return plan->a_f16 ? ws_launch<true, false>(plan, st, dependent) : ws_launch<false, false>(plan, st, dependent);
+    return plan->a_f16 ? ws_launch<true, false>(plan, st) : ws_launch<false, false>(plan, st);
 }
 
+// One step = a memset of the counters and flags, the stream kernel and, for fp16-operand plans, the
+// bf16 fallback kernel (which exits at once unless the first launch raised its domain flag).
 int ws_plan_run(const WsPlan* plan, cudaStream_t st) {
     if (cudaMemsetAsync(plan->d_done, 0, plan->done_bytes, st) != cudaSuccess) return ARIA_ERR_CUDA;
-    int rc = ws_run_one(plan, st, false);
-    if (rc == ARIA_OK && plan->fallback) rc = ws_run_one(plan->fallback, st, true);
+    int rc = ws_run_one(plan, st);
+    if (rc == ARIA_OK && plan->fallback) rc = ws_run_one(plan->fallback, st);
     return rc;
 }
 

@@ -332,3 +332,33 @@ def test_partial_overlap_of_an_earlier_output_takes_the_per_layer_path(aria, ora
     b, _ = _layer(aria, oracle, M, 256, 128, 95, 10)
     b["in"] = a["out"].view(-1)[M * N // 2:].view(M, 256)
     list(_run_plan(aria, [a, b], M, expect_stream=0))
+
+
+def test_fallback_launch_runs_correctly_while_another_kernel_holds_an_sm(aria, oracle):
+    """the fired bf16 fallback runs the same cross-CTA waits as the fp16 launch, so it must be a
+    cooperative launch too (all CTAs resident before any starts).  Here a long single-CTA kernel on another
+    stream holds one SM for ~0.2 s (well under the kernel's 2 s watchdog) while a plan whose input leaves the
+    fp16 domain runs: the result must be the exact-bf16 one, as in an undisturbed run."""
+    M, K, N = 32, 768, 256
+    x = inputs.normal_f32((M, K), 1.0, 95, 0)
+    x[3, 17] = 1.0e5
+    spec, host = _edge_layer(aria, oracle, M, K, N, 95, _edge_weights(N, K, 95), x)
+    layers = aria.make_layers([spec])
+    plan = aria.aria_stack_plan_create(layers, M, aria.W4A16, aria.BF16)
+    try:
+        assert aria.aria_stack_plan_is_streaming(plan) == 1
+        aria.aria_stack_plan_run(plan)
+        torch.cuda.synchronize()
+        quiet = host_bits16(spec["out"]).copy()
+        spec["out"].zero_()
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            torch.cuda._sleep(400_000_000)               # ~0.2 s on one SM
+        aria.aria_stack_plan_run(plan)                   # current stream: overlaps the sleeper
+        torch.cuda.synchronize()
+        assert aria.aria_stack_plan_fallback_fired(plan) != 0
+        busy = host_bits16(spec["out"]).copy()
+    finally:
+        aria.aria_stack_plan_destroy(plan)
+    assert np.array_equal(busy, quiet)
+    _check(oracle, host, host["x"], busy, 0)
