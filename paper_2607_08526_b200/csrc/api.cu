@@ -32,9 +32,10 @@ size_t w8_ws_bytes(int M, int K) { return up256(static_cast<size_t>(M) * K) + up
 
 // One W8A8 linear as two launches: the S1 kernel, then the GEMM as its programmatic dependent (the GEMM's
 // prologue -- barrier init, tensor-memory allocation, tensor-map prefetch -- overlaps the quantiser).
-// pdl_first: whether the S1 kernel itself may be a programmatic dependent of what precedes it on the stream
-// (only inside a chain this library enqueued: its kernels all execute griddepcontrol.wait before they touch
-// global memory, a foreign kernel gives no such guarantee).
+// pdl_first: whether the S1 kernel itself is a programmatic dependent of what precedes it on the stream.  The
+// rule is the one include/aria.h states under "Programmatic dependent launch": the stand-alone entry points
+// pass true (safe after every predecessor except a foreign programmatic dependent that never waits); layer 0
+// of aria_denoiser_linears passes false, so a captured step starts with a fully serialised launch.
 int linear_w8a8_impl(const void* X, int xt, int M, int K, const int8_t* Wq, const float* w_scale,
                      int N, const void* bias, int bt, int act, void* Y, int yt, void* ws,
                      cudaStream_t st, bool pdl_first, bool pdl) {
@@ -309,7 +310,8 @@ int aria_round_act_int8(const void* X, int xt, int M, int K, float* absmax, int 
     if (reinterpret_cast<uintptr_t>(absmax) & 3u) return ARIA_ERR_ALIGN;
     int rc = check_rows_args(X, xt, M, K, Xq, x_scale);
     if (rc != ARIA_OK) return rc;
-    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), true, absmax, clear ? absmax : nullptr);
+    return launch_quant_rows_i8(X, xt, M, K, Xq, x_scale, static_cast<cudaStream_t>(stream), true, absmax, clear ? absmax : nullptr,
+                                true);
 }
 
 int aria_tensor_peak(int kind, int ctas, int iters, double seconds, double* out, void* stream) {

@@ -35,9 +35,11 @@ inline bool ensure_dyn_smem(Kern kern, int bytes, std::atomic<uint64_t>& mask) {
 // ---- quant.cu
 // known_absmax: per-row max |x| already computed by the producing epilogue (fused S1): the pass
 // skips its reduction.  zero_absmax: a [R] buffer this pass zeroes (the buffer the GEMM that consumes
-// this pass's codes will atomicMax into).
+// this pass's codes will atomicMax into).  check_known: known_absmax comes from outside the library and may be
+// too small -- rows where it is are rounded by the clamping path (the other kernels check for free, always).
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl, const float* known_absmax = nullptr, float* zero_absmax = nullptr);
+                         bool pdl, const float* known_absmax = nullptr, float* zero_absmax = nullptr,
+                         bool check_known = false);
 int launch_quant_groups_i4(const void* W, int wt, int N, int K, uint8_t* q4, uint16_t* sg,
                            cudaStream_t st);
 

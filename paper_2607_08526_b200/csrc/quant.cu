@@ -47,8 +47,15 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
     const int nwarp = nthr >> 5;
     a = red[0];
     for (int w = 1; w < nwarp; ++w) a = fmaxf(a, red[w]);
-    // fused S1: the producing epilogue already reduced this row (same value, taken after the wait above)
-    if (known_absmax) asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(known_absmax + row) : "memory");
+    // fused S1: the producing epilogue already reduced this row (same value, taken after the wait above).
+    // `wrong`: the supplied maximum is below the row's own (a stale or foreign buffer) or not a number --
+    // the division-free rounding would wrap instead of saturating, so the row takes the clamping path.
+    bool wrong = false;
+    if (known_absmax) {
+        const float own = a;
+        asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(known_absmax + row) : "memory");
+        wrong = !(own <= a);
+    }
 
     const float s = a > 0.0f ? __fdiv_rn(a, 127.0f) : 1.0f;
     if (known_absmax && zero_absmax == known_absmax) __syncthreads();   // every thread has read it before it is cleared
@@ -63,7 +70,7 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
         const int idx = tid + i * nthr;
         if (idx < nvec) {
             uint2 o;
-            if (!f.ok || !quant8_fast(v[i], f, o)) o = quant8_i8(v[i], s);
+            if (!f.ok || wrong || !quant8_fast(v[i], f, o)) o = quant8_i8(v[i], s);
             *reinterpret_cast<uint2*>(q + 8 * idx) = o;
         }
     }
@@ -71,7 +78,7 @@ quant_rows_i8_kernel(const T* __restrict__ X, int K, int8_t* __restrict__ Xq,
         float t[8];
         load8<T>(x + 8 * idx, t);
         uint2 o;
-        if (!f.ok || !quant8_fast(t, f, o)) o = quant8_i8(t, s);
+        if (!f.ok || wrong || !quant8_fast(t, f, o)) o = quant8_i8(t, s);
         *reinterpret_cast<uint2*>(q + 8 * idx) = o;
     }
 }
@@ -105,8 +112,12 @@ quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restr
             a = absmax8(v, a);
         }
     }
+    bool wrong = false;   // this lane holds a value above the supplied maximum (or that is NaN): clamp, see above
     if (known_absmax) {   // fused S1: reduced by the producing epilogue (warp-uniform branch)
+        const float own = a;
         asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(known_absmax + row) : "memory");
+        wrong = !(own <= a);
+        __syncwarp();     // every lane has read absmax[row] before lane 0 may clear it below
     } else {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
@@ -124,7 +135,7 @@ quant_rows_i8_warp_kernel(const T* __restrict__ X, int R, int K, int8_t* __restr
             float v[8];
             unpack8(raw[i], v);
             uint2 o;
-            if (!f.ok || !quant8_fast(v, f, o)) o = quant8_i8(v, s);
+            if (!f.ok || wrong || !quant8_fast(v, f, o)) o = quant8_i8(v, s);
             *reinterpret_cast<uint2*>(q + 8 * idx) = o;
         }
     }
@@ -163,7 +174,7 @@ quant_groups_i4_kernel(const T* __restrict__ W, int64_t n_vec, uint8_t* __restri
 template <int VPT>
 __global__ void __launch_bounds__(256)
 quant_rows_bf16_kernel(const __nv_bfloat16* __restrict__ X, int R, int K, int tpr, int8_t* __restrict__ Xq,
-                       float* __restrict__ scale, const float* known_absmax, float* zero_absmax) {
+                       float* __restrict__ scale, const float* known_absmax, float* zero_absmax, int check_known) {
     __shared__ float red[8];
     pdl_wait_prior_grid();
     pdl_launch_dependents();
@@ -180,10 +191,22 @@ quant_rows_bf16_kernel(const __nv_bfloat16* __restrict__ X, int R, int K, int tp
         raw[i] = (live && idx < nvec) ? ld_global_v4(x + 8 * idx) : make_uint4(0, 0, 0, 0);
     }
     float a;
+    bool wrong = false;
     if (known_absmax) {            // fused S1: reduced by the producing epilogue
         a = 0.0f;
         if (live) asm volatile("ld.global.f32 %0, [%1];" : "=f"(a) : "l"(known_absmax + row) : "memory");
-        if (zero_absmax == known_absmax && tpr > 32) __syncthreads();   // all of the row's threads have read it
+        if (zero_absmax == known_absmax) {   // all of the row's threads have read it before thread 0 clears it
+            if (tpr > 32) __syncthreads();
+            else __syncwarp();
+        }
+        // check_known (a maximum supplied through the public aria_round_act_int8, not by this library's own
+        // epilogues): a thread holding a value above it, or a NaN maximum, takes the clamping path
+        if (check_known) {
+            uint32_t acc = 0;
+#pragma unroll
+            for (int i = 0; i < VPT; ++i) acc = absmax8_bf16(raw[i], acc);
+            wrong = !(absmax_bf16x2_to_f32(acc) <= a);
+        }
     } else {
         uint32_t acc = 0;
 #pragma unroll
@@ -211,7 +234,7 @@ quant_rows_bf16_kernel(const __nv_bfloat16* __restrict__ X, int R, int K, int tp
         const int idx = t + tpr * i;
         if (live && idx < nvec) {
             uint2 o;
-            if (!f.ok || !quant8_fast_bf16(raw[i], f, o)) {
+            if (!f.ok || wrong || !quant8_fast_bf16(raw[i], f, o)) {
                 float v[8];
                 Raw8<__nv_bfloat16> r8;
                 r8.a = raw[i];
@@ -233,7 +256,8 @@ static cudaError_t launch_warp_rows(const void* X, int R, int C, int8_t* q, floa
 }
 
 int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* s, cudaStream_t st,
-                         bool pdl, const float* known, float* zero) {
+                         bool pdl, const float* known, float* zero, bool check_known) {
+    const int ck = check_known ? 1 : 0;
     const int nvec = C / 8;
     if (xt == ARIA_BF16 && nvec <= 1024) {
         int tpr = 32;
@@ -251,10 +275,10 @@ int launch_quant_rows_i8(const void* X, int xt, int R, int C, int8_t* q, float* 
         cfg.numAttrs = pdl ? 1 : 0;
         const __nv_bfloat16* x = static_cast<const __nv_bfloat16*>(X);
         cudaError_t e;
-        if (vpt == 1) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<1>, x, R, C, tpr, q, s, known, zero);
-        else if (vpt == 2) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<2>, x, R, C, tpr, q, s, known, zero);
-        else if (vpt == 3) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<3>, x, R, C, tpr, q, s, known, zero);
-        else e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<4>, x, R, C, tpr, q, s, known, zero);
+        if (vpt == 1) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<1>, x, R, C, tpr, q, s, known, zero, ck);
+        else if (vpt == 2) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<2>, x, R, C, tpr, q, s, known, zero, ck);
+        else if (vpt == 3) e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<3>, x, R, C, tpr, q, s, known, zero, ck);
+        else e = cudaLaunchKernelEx(&cfg, quant_rows_bf16_kernel<4>, x, R, C, tpr, q, s, known, zero, ck);
         return e == cudaSuccess ? ARIA_OK : ARIA_ERR_CUDA;
     }
     {   // warp-per-row variants (fp32 rows, and bf16 rows wider than 8192 elements): rows up to 3072 elements (wider rows: one CTA per row, below; a 24-vector

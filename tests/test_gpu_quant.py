@@ -73,3 +73,41 @@ def test_weights_int4(aria, oracle, N, K):
     q4, s = aria.aria_quantize_weights_int4(dev_bf16(bits))
     torch.cuda.synchronize()
     assert np.array_equal(host_bits16(s), sg) and np.array_equal(q4.cpu().numpy(), packed)
+
+
+@pytest.mark.parametrize("dtype,M,K", [("bf16", 64, 1536), ("bf16", 40, 6144), ("bf16", 9, 9984), ("f32", 33, 1536),
+                                       ("f32", 5, 6144)])
+def test_round_act_with_a_too_small_absmax_saturates_instead_of_wrapping(aria, oracle, dtype, M, K):
+    """aria_round_act_int8 takes the row maximum from the caller.  With a maximum BELOW the row's own
+    (a stale buffer) the division-free rounding used to wrap (x/s = 130 -> code -126); aria.h promises the
+    clamp.  Expected value without retyping the formula: quantising with absmax a' saturates exactly the
+    elements above a', so it equals the oracle's S1 of the row clipped to +-a' (a' is a value of the row,
+    hence the clipped row's own maximum).  Rows with a correct maximum stay bit-identical to S1, a NaN
+    maximum means scale 1 with saturation, and clear=1 still zeroes the buffer.  All row-kernel variants."""
+    if dtype == "bf16":
+        bits, x = inputs.normal_bf16((M, K), 1.0, 52, M + K)
+        X = dev_bf16(bits)
+    else:
+        x = inputs.normal_f32((M, K), 1.0, 52, M + K)
+        X = dev_f32(x)
+    ax = np.abs(x)
+    amax = ax.max(axis=1).astype(np.float32)
+    small = np.sort(ax, axis=1)[:, -K // 16].astype(np.float32)   # 1/16 of each row lies above it
+    given = amax.copy()
+    given[0::2] = small[0::2]                                     # even rows: too small; odd rows: correct
+    clipped = np.clip(x, -given[:, None], given[:, None])
+    qo, so = oracle.quant_int8_rows(clipped)
+    buf = dev_f32(given)
+    q, s = aria.aria_round_act_int8(X, buf, clear=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(s.cpu().numpy().view(np.uint32), so.view(np.uint32))
+    assert np.array_equal(q.cpu().numpy(), qo)
+    assert int((q.cpu().numpy()[0::2] == 127).sum() + (q.cpu().numpy()[0::2] == -127).sum()) >= (M + 1) // 2 * (K // 16)
+    assert not buf.any()                                          # cleared after it was read
+    # NaN maximum: scale 1, codes clamp(rint(x), +-127) -- x scaled up so that saturation matters
+    big = (x * np.float32(64.0)).astype(np.float32)
+    Xb = dev_bf16(inputs.bf16_bits(big)) if dtype == "bf16" else dev_f32(big)
+    q, s = aria.aria_round_act_int8(Xb, torch.full((M,), float("nan"), device="cuda"))
+    torch.cuda.synchronize()
+    assert np.all(s.cpu().numpy() == 1.0)
+    assert np.array_equal(q.cpu().numpy(), np.clip(np.rint(big), -127, 127).astype(np.int8))
