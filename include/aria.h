@@ -21,6 +21,18 @@
  *  - `stream` is a cudaStream_t passed as void*.  Device entry points only ENQUEUE work on it:
  *    no host synchronisation, no allocation -- every one of them may be captured in a CUDA
  *    graph.  `_host` entry points copy and synchronise (see there).
+ *  - Programmatic dependent launch.  aria_quantize_act_int8, aria_linear_w8a8, aria_linear_w8a8_static_ws,
+ *    aria_linear_w8a8_q, aria_norm_quantize_act_int8, aria_round_act_int8 and aria_attention launch their
+ *    first kernel as a PROGRAMMATIC DEPENDENT of whatever precedes it on `stream` (its prologue overlaps
+ *    that kernel's tail); every kernel of this library executes griddepcontrol.wait -- which returns only when
+ *    the preceding kernel has completed and its writes are visible -- before it reads or writes global
+ *    memory.  This is ordinary stream order after any predecessor that was launched normally, and after
+ *    this library's own kernels.  The one predecessor it is NOT safe after: a foreign kernel that was itself
+ *    launched with the programmatic attribute and exits without cudaGridDependencySynchronize(): such a
+ *    kernel can finish before ITS predecessor, and the wait here covers only the immediate predecessor.
+ *    Put an event or a normally launched kernel in between in that case.  aria_quantize_weights_*,
+ *    aria_linear_w4a16, aria_linear_w8a16, aria_steer and the first kernel of aria_denoiser_linears /
+ *    aria_stack_plan_run are plain launches.
  *  - Return value: aria_status (0 = OK, negative = error).  On a validation error nothing is
  *    enqueued and no output is written.  Non-finite inputs are not checked (undefined).
  *  - Alignment: every data pointer must be 16-byte aligned.  K % 32 == 0, N % 8 == 0.
@@ -204,11 +216,12 @@ ARIA_API int aria_denoiser_linears(const aria_layer* layers, int n_layers, int M
  * ONE step at a time: do not run the same plan concurrently on two streams.
  *
  * Co-residency.  The stream kernel's CTAs (and those of aria_linear_w4a16 with split-K) wait on
- * completion counters written by other CTAs of the same grid.  The stream kernel is therefore a
- * COOPERATIVE launch of at most one CTA per SM: if the device cannot hold the grid at once the launch
- * fails with ARIA_ERR_CUDA instead of deadlocking, and so is every split-K launch of aria_linear_w4a16 /
- * aria_linear_w8a16.  Do not run two plans, or a plan and a split-K linear, concurrently on different
- * streams of one device (the second launch would fail, not hang).
+ * completion counters written by other CTAs of the same grid.  Every launch of the stream kernel -- the
+ * fp16 launch AND the bf16 fallback launch that follows it in stream order -- is therefore a COOPERATIVE
+ * launch of at most one CTA per SM, and so is every split-K launch of aria_linear_w4a16 /
+ * aria_linear_w8a16: the grid starts only when all of it is resident (SMs held by another kernel delay
+ * it, they cannot deadlock it), and a grid the device can never hold at once fails with ARIA_ERR_CUDA.
+ * One step of a streaming plan enqueues one memset and one (bf16 plans) or two (fp16 plans) kernels.
  *
  * aria_stack_plan_fallback_fired: SYNCHRONOUS (copies one word from the device after the stream's work
  * has been synchronised by the caller); *fired = 0 if the last run stayed in the fp16 domain, else a
@@ -291,7 +304,9 @@ ARIA_API int aria_attention(const void* QKV, int B, int S, int H, int Dh, float 
  * per-token max|x| is already known (reduced by the kernel that produced X, e.g. aria_attention), so the pass
  * only rounds:  x_scale = absmax / 127 (1 if 0), Xq = clamp(rint(x / x_scale), +-127).  Bit-identical to
  * aria_quantize_act_int8 when absmax[m] == max_k |X[m,k]|.  absmax: fp32 [M]; clear != 0 resets absmax[m] to 0
- * once it has been read, so the buffer is ready for the next producer without a memset in the captured step.  */
+ * once it has been read, so the buffer is ready for the next producer without a memset in the captured step.
+ * A wrong absmax[m] gives the scale it implies, never a wrapped code: values above it saturate at +-127 (the
+ * kernel compares what it holds against absmax[m]), and a NaN absmax[m] is treated as scale 1.               */
 ARIA_API int aria_round_act_int8(const void* X, int xt, int M, int K, float* absmax, int clear, int8_t* Xq,
                                  float* x_scale, void* stream);
 

@@ -7,12 +7,15 @@
 //   warp 1      MMA issuer (one thread): 4 x tcgen05.mma (K = 32 each) per k-block into one of two
 //               TMEM accumulators [128 lanes x BN columns]; tcgen05.commit frees the ring slot and,
 //               after the last k-block, signals `tmem_full`.
-//   warps 2..9  epilogue (two warps per TMEM lane quarter): tcgen05.ld 32 lanes x 32 columns ->
-//               registers -> x sx[m] x sw[n] + b[n] (scales/bias staged in smem per tile) -> GELU ->
-//               cast -> 64-byte-swizzled smem block -> TMA store.  Runs on accumulator `a` while the
-//               MMA warp fills accumulator `a^1`.
-// Tails: TMA zero-fills rows >= M / >= N and bytes >= K on load (zero codes add nothing) and clips
-// them on store.
+//   epilogue    8 warps, two per TMEM lane quarter (warp ids: see "Warp roles" below): tcgen05.ld 32 lanes
+//               x 32 columns, one chunk ahead -> registers -> x sx[m] x sw[n] + b[n] (scales / bias staged
+//               in smem per tile) -> GELU -> cast -> DIRECT 16- / 32-byte global stores, a thread owning one
+//               output row (round 2; the round-1 swizzled-smem + TMA-store epilogue is gone).  Runs on
+//               accumulator `a` while the MMA warp fills accumulator `a^1`; optionally reduces the
+//               per-token absmax of what it stores (fused S1) and runs the next layer's S1 as a side
+//               job while it waits for its first accumulator.
+// Tails: TMA zero-fills rows >= M / >= N and bytes >= K on load (zero codes add nothing); the stores are
+// predicated on row < M and column < N.
 #include <cstdio>
 #include <cstdlib>
 
