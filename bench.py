@@ -31,12 +31,28 @@ sys.path.insert(0, ROOT)
 METRIC = "quantized DiT linear throughput: W8A8 int8 TOPS + W4A16 effective bf16 TFLOPS over one C5 denoising-step stack"
 UNIT = "Top/s"
 WORKLOAD = "C5: 24 blocks x (QKV 1536->4608, out 1536->1536, MLP 1536->6144->1536), M=2048, all-W8A8 then all-W4A16, CUDA-graph replay"
-W4A16_TRAFFIC = 15.06e6          # bytes per launch, ncu (updated with each profiles/ capture)
-W4A16_TRAFFIC_SRC = "profiles/r2_w4a16_full.md"
-W8A8_TRAFFIC = 17.4e6            # bytes per launch, ncu
+W4A16_TRAFFIC_SRC = "profiles/r2_w4a16_full.md"   # ncu --set full summaries the `traffic` figures are read from
 W8A8_TRAFFIC_SRC = "profiles/r2_w8a8_full.md"
 NOMINAL_INT8_OVER_BF16 = 2.0     # B200_PROFILING.md: 4.5 POP/s int8 vs 2.25 PFLOP/s bf16, dense
 BURST_REGION_S = 1.0             # a timed region shorter than this runs at burst clocks: score against the burst peak
+
+
+def profile_traffic(rel_path: str):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, mean over the captured launches) read
+    from a committed ncu summary under profiles/ -- nothing typed in by hand.  None if the file or rows are missing."""
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    tot = {}
+    try:
+        for ln in open(os.path.join(ROOT, rel_path)):
+            c = [x.strip() for x in ln.strip().strip("|").split("|")]
+            if len(c) >= 3 and c[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and c[1] in unit:
+                tot[c[0]] = [float(v) * unit[c[1]] for v in c[2:]]
+    except OSError:
+        return None
+    if len(tot) != 2 or len(tot["dram__bytes_read.sum"]) != len(tot["dram__bytes_write.sum"]):
+        return None
+    per = [r + w for r, w in zip(tot["dram__bytes_read.sum"], tot["dram__bytes_write.sum"])]
+    return sum(per) / len(per)
 
 
 def log(*a):
@@ -611,7 +627,7 @@ def run_ours(args):
                 "peak_source": src8,
                 "frac_of_2x_bf16_burst": ach / (pk["bf16_burst"] * NOMINAL_INT8_OVER_BF16),
                 "frac_of_nominal_4500": ach / 4500.0, "avg_launch_us": dur * 1e6, "launches": n_l,
-                "traffic": W8A8_TRAFFIC, "traffic_unit": f"bytes/launch (ncu, {W8A8_TRAFFIC_SRC})"}
+                "traffic": profile_traffic(W8A8_TRAFFIC_SRC), "traffic_unit": f"bytes/launch, mean of the launches in {W8A8_TRAFFIC_SRC} (ncu, shared-input step: X is L2-resident there)"}
 
     # ---- roofline of the DOMINANT kernel of the step: w4a16_gemm_kernel.  The W4A16 half of the step is 96
     # launches of that kernel and nothing else, so its average launch duration is t4 / 96 from the CUDA
@@ -628,7 +644,7 @@ def run_ours(args):
                 "frac_of_issue_loop_peak": (ach4 / tp["bf16"]["burst" if burst else "sustained"]) if tp else None,
                 "avg_launch_us": dur4 * 1e6, "launches": n_l, "share_of_step": t4 / (t8 + t4),
                 "algorithmic_flops_per_launch": st4.ops / n_l,
-                "traffic": W4A16_TRAFFIC, "traffic_unit": f"bytes/launch (ncu, {W4A16_TRAFFIC_SRC})"}
+                "traffic": profile_traffic(W4A16_TRAFFIC_SRC), "traffic_unit": f"bytes/launch, mean of the launches in {W4A16_TRAFFIC_SRC} (ncu, shared-input step: X is L2-resident there)"}
 
     # ---- e2e: same step through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -658,6 +674,30 @@ def run_ours(args):
             nxt = next_rows(torch, aria, inputs, pk)
         except Exception as ex:                  # noqa: BLE001
             log(f"[bench] next_rows failed: {ex!r}")
+    # Reading R14 says every linear reads its OWN N(0,1) input.  The headline step above shares one input buffer per
+    # distinct K (three buffers, L2-resident); here the same step with 72 distinct external inputs (453 MB, HBM-cold
+    # on every replay), timed the same way.  Built after the headline so its memory and time cannot disturb it.
+    distinct = None
+    if world == 1 and not args.no_per_linear:
+        try:
+            d8 = LinearStack(aria.W8A8, M=M, shared_inputs=False)
+            d4 = LinearStack(aria.W4A16, M=M, shared_inputs=False)
+            d8.capture()
+            d4.capture()
+            for _ in range(3):
+                d8.replay()
+                d4.replay()
+            m8 = time_region(torch, d8.replay, args.steps)
+            m4 = time_region(torch, d4.replay, args.steps)
+            distinct = {"ms_w8a8": m8, "ms_w4a16": m4, "ms_per_step": m8 + m4,
+                        "value": (ops8 + ops4) / ((m8 + m4) * 1e-3) / 1e12, "unit": UNIT,
+                        "ratio_to_shared_inputs": (m8 + m4) / (t8 + t4),
+                        "what": "the C5 step with one N(0,1) input buffer per linear (72 external inputs, reading R14) "
+                                "instead of one per distinct K; each half timed over its own replays"}
+            del d8, d4
+            torch.cuda.empty_cache()
+        except Exception as ex:                  # noqa: BLE001
+            log(f"[bench] distinct-input step failed: {ex!r}")
     # last (they heat the part): the long replay of the same step, then the sustained tensor peaks
     sustained = None
     if world == 1 and not args.no_sustained:
@@ -686,7 +726,7 @@ def run_ours(args):
         # kernels of this library launched inside the timed region: per step 96 W4A16 GEMMs + 96 W8A8 GEMMs + the
         # stand-alone S1 passes the W8A8 chain keeps (layer 0, and the rounding pass of every chained layer)
         "gpu_launches": args.steps * (2 * n_l + 1 + sum(1 for s in st8.specs if s["in"] is None)), "clocks": clocks, "per_linear": table,
-        "small_m": small, "hbm_passes": hbm, "next_rows": nxt,
+        "small_m": small, "hbm_passes": hbm, "next_rows": nxt, "distinct_inputs": distinct,
     }
     log("[bench] " + json.dumps({k: line[k] for k in ("value", "ms_per_step", "modes", "roofline", "roofline_w8a8_gemm",
                                                        "tensor_peaks", "sustained")}))
