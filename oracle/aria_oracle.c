@@ -273,18 +273,10 @@ void oracle_epilogue_w8a8(const int64_t *acc, const float *sx, const float *sw, 
 /* W4A16 linear (config C4; readings R12):
  *   variant 0: w^ = bf16_rne(float(q) * float(sg))   (product exact in fp32)
  *   variant 1: w^ = q * sg  exactly (not rounded to bf16)
- *   variant 2: w^ = fp16_rne(float(q) * float(sg))   (reading R12b: the small-M
- *              weight-streaming path feeds the tensor core fp16 operands)
- *   variant 3: w^ = fp16_rne(float(q + 8) * float(sg)) - 8 * sg   (reading R12c: offset-binary
- *              dequantisation -- the unsigned code u = q + 8 is scaled and rounded to fp16, the
- *              zero point 8 * sg is subtracted exactly)
  *   y = sum_k (double)x[m,k] * (double)w^[n,k] + (double)b[n]  (fp64)
- * X is fp32 holding bf16 values exactly.  codes[N,K] int8, sg_bits[N,K/G]. */
-static double oracle_w4_offset_binary(int8_t q, float sg)
-{
-    float uprod = (float)(q + 8) * sg; /* exact: 4-bit x 11-bit */
-    return (double)oracle_fp16_bits_to_f32(oracle_f32_to_fp16_bits(uprod)) - 8.0 * (double)sg;
-}
+ * X is fp32 holding bf16 values exactly.  codes[N,K] int8, sg_bits[N,K/G].
+ * (Models of a kernel's operand FORMAT -- the former variants 2 and 3 -- are not definitions
+ * and live with the tests: tests/kernel_models.py.) */
 
 void oracle_linear_w4a16(const float *X, const int8_t *codes, const uint16_t *sg_bits,
                          const double *bias, int act, int variant, int64_t M, int64_t N,
@@ -299,10 +291,6 @@ void oracle_linear_w4a16(const float *X, const int8_t *codes, const uint16_t *sg
             float prod = (float)codes[n * K + k] * sg; /* exact: 3-bit x 11-bit */
             if (variant == 0)
                 wrow[k] = (double)oracle_bf16_bits_to_f32(oracle_f64_to_bf16_bits((double)prod));
-            else if (variant == 2)
-                wrow[k] = (double)oracle_fp16_bits_to_f32(oracle_f32_to_fp16_bits(prod));
-            else if (variant == 3)
-                wrow[k] = oracle_w4_offset_binary(codes[n * K + k], sg);
             else
                 wrow[k] = (double)prod;
         }
@@ -319,7 +307,7 @@ void oracle_linear_w4a16(const float *X, const int8_t *codes, const uint16_t *sg
     }
 }
 
-/* Dequantised weight matrix of variant 0/1/2/3 as fp64 [N,K] (for the pin that
+/* Dequantised weight matrix of variant 0/1 as fp64 [N,K] (for the pin that
  * reduces O4 to numpy.matmul). */
 void oracle_dequant_int4(const int8_t *codes, const uint16_t *sg_bits, int variant, int64_t N,
                          int64_t K, int G, double *What)
@@ -329,12 +317,8 @@ void oracle_dequant_int4(const int8_t *codes, const uint16_t *sg_bits, int varia
         for (int64_t k = 0; k < K; ++k) {
             float sg = oracle_fp16_bits_to_f32(sg_bits[n * ng + k / G]);
             float prod = (float)codes[n * K + k] * sg;
-            What[n * K + k] = variant == 3
-                                  ? oracle_w4_offset_binary(codes[n * K + k], sg)
-                              : variant == 0
+            What[n * K + k] = variant == 0
                                   ? (double)oracle_bf16_bits_to_f32(oracle_f64_to_bf16_bits(prod))
-                              : variant == 2
-                                  ? (double)oracle_fp16_bits_to_f32(oracle_f32_to_fp16_bits(prod))
                                   : (double)prod;
         }
 }

@@ -162,6 +162,7 @@ def unpack_int4(packed, K: int):
 
 
 def dequant_int4(codes, sg_bits, variant: int = 0, group: int = 32):
+    assert variant in (0, 1), "the oracle holds the definitions only (tests/kernel_models.py has the operand-format models)"
     codes = _c(codes, np.int8)
     sg_bits = _c(sg_bits, np.uint16)
     N, K = codes.shape
@@ -211,7 +212,8 @@ def linear_w8a8(X, Wq, sw, bias=None, act: int = ACT_NONE):
 # ------------------------------------------------------------------------ O4
 def linear_w4a16(X, codes, sg_bits, bias=None, act: int = ACT_NONE, variant: int = 0,
                  group: int = 32):
-    """O4: y fp64 [M,N].  X fp32 holding bf16 values; codes int8 [N,K]."""
+    """O4: y fp64 [M,N].  X fp32 holding bf16 values; codes int8 [N,K].  variant 0: w^ = bf16_rne(q sg); 1: w^ = q sg."""
+    assert variant in (0, 1), "the oracle holds the definitions only (tests/kernel_models.py has the operand-format models)"
     X = _c(X, np.float32)
     codes = _c(codes, np.int8)
     sg_bits = _c(sg_bits, np.uint16)

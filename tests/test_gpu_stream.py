@@ -2,7 +2,7 @@
 weight-streaming kernel (csrc/w4a16_stream.cu).  The ACCEPTANCE gate is north_star's: <= 2e-2 against
 the definition with w^ = bf16_rne(q*sg) (oracle variant 0) and with w^ = q*sg (variant 1), for EVERY
 input aria_linear_w4a16 accepts.  Inside its domain the kernel feeds the tensor core fp16 operands,
-w^ = fp16_rn((q+8)*sg) - 8*sg: oracle variants 2 and 3 restate that operand format and are a DIAGNOSTIC
+w^ = fp16_rn((q+8)*sg) - 8*sg: tests/kernel_models.py restates that operand format (indices 2 and 3 below) as a DIAGNOSTIC
 (R12c) -- the tight bf16-output gate of reading R9 is applied against the variant the run
 actually computed (3 in the fp16 domain, 0 after the bf16 fallback or for a bf16-operand plan), which
 pins down that the kernel does what it says, not that the definition moved."""
@@ -11,6 +11,7 @@ import pytest
 import torch
 
 from paper_2607_08526_b200 import inputs
+import kernel_models
 from aria_testutil import check_bf16_out, dev_bf16, dev_f32, host_bits16, host_f32, rel_err
 
 pytestmark = pytest.mark.gpu
@@ -67,7 +68,9 @@ def _run_plan(aria, specs, M, expect_stream=1, expect_fired=0):
 
 def _check(oracle, host, x, got_bits, variant):
     got = inputs.bf16_as_f32(got_bits)
-    refs = [oracle.linear_w4a16(x, host["codes"], host["sg"], host["b"], host["act"], variant=v) for v in (0, 1, 2, 3)]
+    refs = [oracle.linear_w4a16(x, host["codes"], host["sg"], host["b"], host["act"], variant=v) for v in (0, 1)]
+    refs += [kernel_models.linear_w4a16(x, host["codes"], host["sg"], host["b"], host["act"], m)      # diagnostics
+             for m in (kernel_models.FP16_OPERAND, kernel_models.OFFSET_BINARY)]
     for r in refs[:2]:                      # THE gate (north_star): variants 0 and 1
         assert rel_err(got, r) <= TOL
     if variant == 3:                        # diagnostics of the operand format (they follow from the gate's margin)

@@ -6,6 +6,7 @@ import json
 import math
 import os
 
+import kernel_models
 import ml_dtypes
 import numpy as np
 
@@ -156,17 +157,11 @@ def test_o4_reduces_to_numpy_matmul(oracle):
     W = inputs.normal_f32((40, 256), 0.02, 78, 1)
     b = inputs.normal_f32((40,), 0.01, 78, 2).astype(np.float64)
     codes, sg, packed = oracle.quant_int4_groups(W)
-    for variant in (0, 1, 2, 3):
-        # independent dequantisation: numpy fp16 decode, exact product, ml_dtypes bf16 rounding
-        # (variant 0) / numpy float16 rounding (variant 2, the fp16-operand reading R12b) / numpy
-        # float16 rounding of the UNSIGNED code's product minus the exact zero point (variant 3, R12c)
+    for variant in (0, 1):
+        # independent dequantisation: numpy fp16 decode, exact product, ml_dtypes bf16 rounding (variant 0)
         s = np.repeat(sg.view(np.float16).astype(np.float32), 32, axis=1)
         prod = codes.astype(np.float32) * s
-        uprod = (codes.astype(np.float32) + 8.0) * s
-        what = (prod.astype(ml_dtypes.bfloat16).astype(np.float64) if variant == 0 else
-                prod.astype(np.float16).astype(np.float64) if variant == 2 else
-                uprod.astype(np.float16).astype(np.float64) - 8.0 * s.astype(np.float64) if variant == 3 else
-                prod.astype(np.float64))
+        what = prod.astype(ml_dtypes.bfloat16).astype(np.float64) if variant == 0 else prod.astype(np.float64)
         assert np.array_equal(oracle.dequant_int4(codes, sg, variant), what)
         ref = X.astype(np.float64) @ what.T + b
         y = oracle.linear_w4a16(X, codes, sg, b, variant=variant)
@@ -175,15 +170,24 @@ def test_o4_reduces_to_numpy_matmul(oracle):
     y0 = oracle.linear_w4a16(X, codes, sg, variant=0)
     y1 = oracle.linear_w4a16(X, codes, sg, variant=1)
     assert 0 < np.abs(y0 - y1).max() < 2e-2 * np.abs(y1).max()
+    # the operand-format models of the stream kernel (tests/kernel_models.py; diagnostics, not definitions):
     # fp16 rounding of w^ (11 significant bits) sits 8x closer to the exact product than bf16 rounding
-    y2 = oracle.linear_w4a16(X, codes, sg, variant=2)
+    y2 = kernel_models.linear_w4a16(X, codes, sg, None, 0, kernel_models.FP16_OPERAND)
     assert 0 < np.abs(y2 - y1).max() < 0.25 * np.abs(y0 - y1).max()
-    # offset-binary fp16 rounding acts on u*sg (up to 15*sg): at most ~2x the error of variant 2
-    y3 = oracle.linear_w4a16(X, codes, sg, variant=3)
+    # offset-binary fp16 rounding acts on u*sg (up to 15*sg): at most ~2x the error of the fp16-operand model
+    y3 = kernel_models.linear_w4a16(X, codes, sg, None, 0, kernel_models.OFFSET_BINARY)
     assert 0 < np.abs(y3 - y1).max() < 0.5 * np.abs(y0 - y1).max()
+    # and the models rebuilt from the oracle's own (pinned) scalar fp16 conversions, element by element
+    sf = [[oracle.fp16_bits_to_f32(int(v)) for v in row] for row in sg]
+    for model, f in ((kernel_models.FP16_OPERAND, lambda q, s_: oracle.fp16_bits_to_f32(oracle.f32_to_fp16_bits(float(np.float32(q) * np.float32(s_))))),
+                     (kernel_models.OFFSET_BINARY, lambda q, s_: oracle.fp16_bits_to_f32(oracle.f32_to_fp16_bits(float(np.float32(q + 8) * np.float32(s_)))) - 8.0 * s_)):
+        w = kernel_models.dequant_int4(codes, sg, model)
+        for n in range(0, codes.shape[0], 7):
+            for k in range(0, codes.shape[1], 5):
+                assert w[n, k] == f(int(codes[n, k]), sf[n][k // 32])
 
 
-def test_o4_variant3_hand_values(oracle):
+def test_offset_binary_model_hand_values():
     # H2(iii) group (tests/golden/h2_int4.json): sg = 0x297C = 0.0428466796875, codes [2,-5,7,-1].
     # u*sg = [10, 3, 15, 7]*sg = [0.428466796875, 0.1285400390625, 0.6427001953125, 0.2999267578125];
     # fp16 spacing is 2^-12 in [0.25,0.5), 2^-13 in [0.125,0.25), 2^-11 in [0.5,1):
@@ -191,7 +195,7 @@ def test_o4_variant3_hand_values(oracle):
     #   0.6427001953125 = 1316.25*2^-11 -> 1316*2^-11 = 0.642578125; 0.2999267578125 = 1228.5*2^-12 -> tie to even 1228*2^-12 = 0.2998046875
     sg = np.zeros((1, 1), np.uint16); sg[0, 0] = 0x297C
     codes = np.zeros((1, 32), np.int8); codes[0, :4] = [2, -5, 7, -1]
-    w = oracle.dequant_int4(codes, sg, 3)[0]
+    w = kernel_models.dequant_int4(codes, sg, kernel_models.OFFSET_BINARY)[0]
     s = 0.0428466796875
     assert w[0] == 0.428466796875 - 8 * s and w[1] == 0.1285400390625 - 8 * s
     assert w[2] == 0.642578125 - 8 * s and w[3] == 0.2998046875 - 8 * s
