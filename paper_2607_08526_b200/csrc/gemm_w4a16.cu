@@ -40,19 +40,10 @@ constexpr int W4_EPI_WARP0 = 4;
 constexpr int W4_DEQ_WARP0 = 8;
 constexpr int W4_G = 3;         // dequantiser groups = A buffers
 
-// (A CTA-pair variant -- cta_group::2, 256 channels x TT tokens, half of X staged per CTA -- and an X
-// multicast variant were built and measured in round 1: the pair lost ~1.3k cycles per k-block on the
-// cross-CTA "A ready" hand-off, multicast changed nothing (3.79 vs 3.81 ms per C5 step).  Both removed.)
 // WB = weight bits: 4 (S4, int4 group-32 + fp16 group scales) or 8 (NEXT-1 "q8", int8 per-channel + fp32
 // scales).  The two formats share everything but the packed-tile geometry and the dequantiser arithmetic.
-// (CTA pairs -- tcgen05 cta_group::2, 256 channels x 192 tokens per pair, each CTA dequantising its own 128 rows into
-// its own tensor memory and staging half of X -- were built and measured TWICE.  Round 1, A in shared memory: the
-// cross-CTA "A ready" hand-off cost ~1.3k cycles per k-block.  Round 2, A in tensor memory (4 slots, 3 groups, 8 X
-// stages, merged barriers as below): correct -- every parity test passed -- and, once the peer's arrivals used
-// mbarrier.arrive.RELAXED.cluster (the releasing form blocks the issuing warp ~1400 cycles), exactly as fast as one
-// CTA per unit: 127.9 vs 120.6 us per C5 block at M = 2048.  Halving the X traffic buys nothing because neither shared
-// memory, nor the L2, nor the tensor pipe sets the k-block time: issuing a quarter of the MMAs, or loading no X at
-// all, left it unchanged, while skipping the dequantiser arithmetic cut it by 27 %.  Pairs removed.)
+// (CTA pairs and X multicast were built, parity-green and measured twice: no gain, removed -- the dequantiser
+// arithmetic, not X traffic or the tensor pipe, sets the k-block time.  DESIGN.md 9.)
 template <int TT, int WB = 4>
 struct W4Cfg {
     static constexpr int G = W4_G;
