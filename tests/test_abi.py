@@ -95,3 +95,14 @@ def test_product_library_reads_no_environment_variable_and_exports_no_debug_hook
     assert exported == _declared(), set(exported) ^ set(_declared())
     undefined = subprocess.run(["nm", "-D", "--undefined-only", path], capture_output=True, text=True).stdout
     assert "getenv" not in undefined.split()
+
+
+def test_bench_reads_its_ncu_traffic_figures_from_the_committed_profiles():
+    """bench.py's `roofline.traffic` is parsed from the profiles/ summaries it cites (no typed-in constants): the
+    files exist, parse, and give the per-launch DRAM bytes their own summary line states."""
+    import bench
+    w4 = bench.profile_traffic(bench.W4A16_TRAFFIC_SRC)
+    w8 = bench.profile_traffic(bench.W8A8_TRAFFIC_SRC)
+    assert w4 is not None and abs(w4 - 15.06e6) < 0.02e6      # "mean 15.06" MB in profiles/r2_w4a16_full.md
+    assert w8 is not None and abs(w8 - 17.39e6) < 0.02e6      # "mean 17.39" MB in profiles/r2_w8a8_full.md
+    assert bench.profile_traffic("profiles/does_not_exist.md") is None
