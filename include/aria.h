@@ -20,7 +20,9 @@
  *    aria_quantize_weights_* has completed on the stream (the paper's "releases the original").
  *  - `stream` is a cudaStream_t passed as void*.  Device entry points only ENQUEUE work on it:
  *    no host synchronisation, no allocation -- every one of them may be captured in a CUDA
- *    graph.  `_host` entry points copy and synchronise (see there).
+ *    graph.  `_host` entry points copy and synchronise (see there);
+ *    aria_linear_w8a8_static_ws has a one-time set-up on its first call per device and states
+ *    its own rules (this sentence says nothing about it).
  *  - Programmatic dependent launch.  aria_quantize_act_int8, aria_linear_w8a8, aria_linear_w8a8_static_ws,
  *    aria_linear_w8a8_q, aria_norm_quantize_act_int8, aria_round_act_int8 and aria_attention launch their
  *    first kernel as a PROGRAMMATIC DEPENDENT of whatever precedes it on `stream` (its prologue overlaps
